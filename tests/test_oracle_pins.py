@@ -1,0 +1,408 @@
+"""Pins of the CPU oracle (oracle/cavity_oracle.cpp) against what the paper and the mathematics fix.
+
+Nothing here touches the CUDA path.  P:n = /root/reference/PAPER.md line n; S8(c) = SURVEY.md section 8(c).
+Each pin is chosen so that a plausible mistake in the oracle (dropped term, wrong sign or index,
+transposed operand, wrong coefficient) fails it.  Both arithmetic modes are pinned.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import MODE_FMA, MODE_PLAIN
+
+MODES = [MODE_PLAIN, MODE_FMA]
+
+
+def grid(N):
+    k = np.arange(N + 1, dtype=np.float64) / N
+    X, Y = np.meshgrid(k, k)          # arrays [j, i]: X varies along i (columns), Y along j (rows)
+    return X, Y
+
+
+# --------------------------------------------------------------------------------------------
+# (a) manufactured Poisson solution psi = sin(pi x) sin(pi y)  (BASELINE.json self-test (a))
+# --------------------------------------------------------------------------------------------
+
+def lam_h(N, k, l):
+    """Eigenvalue of the 5-point -Laplacian for sin(k pi x) sin(l pi y) on the N-interval grid (textbook)."""
+    h = 1.0 / N
+    return (4.0 / h ** 2) * (math.sin(k * math.pi * h / 2) ** 2 + math.sin(l * math.pi * h / 2) ** 2)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_poisson_manufactured_second_order(mode):
+    errs = []
+    for N in (8, 16, 32, 64):
+        X, Y = grid(N)
+        exact = np.sin(np.pi * X) * np.sin(np.pi * Y)
+        omega = 2.0 * np.pi ** 2 * exact                     # -lap(psi) = omega  (eq 3)
+        beta = 2.0 / (1.0 + math.sin(math.pi / N))           # Young's optimal factor
+        psi = oracle.sor(N, beta, np.zeros_like(exact), omega, 40 * N, mode)
+        # exact DISCRETE solution: omega is an eigenvector of the 5-point operator
+        disc = omega / lam_h(N, 1, 1)
+        assert np.max(np.abs(psi - disc)) < 1e-13
+        errs.append(np.max(np.abs(psi - exact)))
+    ratios = [errs[k] / errs[k + 1] for k in range(3)]
+    for r in ratios:
+        assert 3.8 < r < 4.2, ratios                          # second-order decay
+    # leading error term: psi_h - psi = (2 pi^2 / lam_h - 1) ~ pi^2 h^2 / 12
+    assert abs(errs[-1] / (math.pi ** 2 / 64 ** 2 / 12) - 1.0) < 5e-3
+
+
+def test_poisson_eigenvalues_survey_values():
+    # SURVEY S8(c) pin table (closed form, printed there to 12 digits)
+    for N, v in ((8, 19.486839677111), (16, 19.675872867092), (32, 19.723359550682), (64, 19.735245534456),
+                 (128, 19.738217925560)):
+        assert abs(lam_h(N, 1, 1) - v) < 5e-12
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_poisson_mode_k2_l3(mode):
+    # a non-symmetric mode catches an x/y transposition or an anisotropic coefficient slip
+    N = 24
+    X, Y = grid(N)
+    omega = 3.0 * np.sin(2 * np.pi * X) * np.sin(3 * np.pi * Y)
+    psi = oracle.sor(N, 1.7, np.zeros_like(omega), omega, 1500, mode)
+    assert np.max(np.abs(psi - omega / lam_h(N, 2, 3))) < 1e-13
+
+
+# --------------------------------------------------------------------------------------------
+# (b) exactness of the discrete operators on quadratics  (self-test (b))
+# --------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("N", [8, 20])
+def test_rhs_exact_on_quadratics(mode, N):
+    X, Y = grid(N)
+    Re = 7.0
+    psi = X ** 2 - X * Y + 2.0 * Y ** 2
+    om = 3.0 * X ** 2 + Y ** 2 - X
+    psi_x, psi_y = 2.0 * X - Y, -X + 4.0 * Y
+    om_x, om_y = 6.0 * X - 1.0, 2.0 * Y
+    exact = -psi_y * om_x + psi_x * om_y + (1.0 / Re) * 8.0       # eq 4
+    L = oracle.rhs(N, Re, psi, om, mode)
+    I = (slice(1, N), slice(1, N))
+    assert np.max(np.abs(L[I] - exact[I])) < 2e-11
+    assert np.all(L[0, :] == 0) and np.all(L[:, 0] == 0)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_rhs_each_term_separately(mode):
+    # one term at a time, so a sign error in any single term shows
+    N = 10
+    X, Y = grid(N)
+    Z = np.zeros_like(X)
+    I = (slice(1, N), slice(1, N))
+    # u = psi_y = 1, omega = x      ->  L = -u omega_x = -1
+    assert np.allclose(oracle.rhs(N, 1e30, Y, X, mode)[I], -1.0, atol=1e-12)
+    # v = -psi_x = -1 (psi = x), omega = y  ->  L = -v omega_y = +1
+    assert np.allclose(oracle.rhs(N, 1e30, X, Y, mode)[I], 1.0, atol=1e-12)
+    # psi = 0, omega = x^2 + 3 y^2 -> L = nu * 8
+    assert np.allclose(oracle.rhs(N, 4.0, Z, X ** 2 + 3 * Y ** 2, mode)[I], 2.0, atol=1e-11)
+    # cross terms vanish: u = 1 with omega = y ; v = -1 with omega = x
+    assert np.allclose(oracle.rhs(N, 1e30, Y, Y, mode)[I], 0.0, atol=1e-12)
+    assert np.allclose(oracle.rhs(N, 1e30, X, X, mode)[I], 0.0, atol=1e-12)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_sor_fixed_point_on_quadratic(mode):
+    # the 5-point Laplacian is exact on quadratics: psi = x^2 - xy + 2y^2 has lap = 6, so with
+    # omega = -6 it is a fixed point of every sweep, whatever beta (walls carry the quadratic)
+    N = 12
+    X, Y = grid(N)
+    psi = X ** 2 - X * Y + 2.0 * Y ** 2
+    om = np.full_like(psi, -6.0)
+    for beta in (0.7, 1.0, 1.9):
+        out = oracle.sor(N, beta, psi, om, 3, mode)
+        assert np.max(np.abs(out - psi)) < 1e-14
+    # and a wrong right-hand side is NOT a fixed point
+    assert np.max(np.abs(oracle.sor(N, 1.0, psi, -om, 1, mode) - psi)) > 1e-3
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_sor_red_first_then_black(mode):
+    # G9: one sweep from psi = 0 with a point source at a red point (i + j even): red half-sweep
+    # sets it, black half-sweep spreads it to the four neighbours; a source at a black point
+    # reaches only itself in that sweep.
+    N, beta = 8, 1.5
+    h2 = 1.0 / N ** 2
+    om = np.zeros((N + 1, N + 1))
+    om[4, 4] = 1.0                                  # red
+    p = oracle.sor(N, beta, np.zeros_like(om), om, 1, mode)
+    c = beta * h2 / 4
+    assert abs(p[4, 4] - c) < 1e-18
+    for (j, i) in ((4, 3), (4, 5), (3, 4), (5, 4)):
+        assert abs(p[j, i] - beta * c / 4) < 1e-18
+    assert np.count_nonzero(p) == 5
+    om[:] = 0.0
+    om[4, 3] = 1.0                                  # black
+    p = oracle.sor(N, beta, np.zeros_like(om), om, 1, mode)
+    assert np.count_nonzero(p) == 1 and abs(p[4, 3] - c) < 1e-18
+
+
+# --------------------------------------------------------------------------------------------
+# Thom wall vorticity, eq 25
+# --------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("mode", MODES)
+def test_thom_exact_on_quadratic_wall_profile(mode):
+    N, U, a = 16, 1.0, 0.37
+    h = 1.0 / N
+    X, Y = grid(N)
+    w_in = np.full((N + 1, N + 1), 123.0)
+    # lid (j = N): s = 1 - y, psi = -U s + a s^2  => u(wall) = U, omega_wall = -psi_yy = -2a
+    s = 1.0 - Y
+    w = oracle.thom(N, U, -U * s + a * s ** 2, w_in, mode)
+    assert np.allclose(w[N, :], -2 * a, atol=1e-11)
+    # bottom (j = 0), left (i = 0), right (i = N): resting walls, psi = a s^2 => omega_wall = -2a
+    w = oracle.thom(N, U, a * Y ** 2, w_in, mode)
+    assert np.allclose(w[0, :], -2 * a, atol=1e-11)
+    w = oracle.thom(N, U, a * X ** 2, w_in, mode)
+    assert np.allclose(w[1:N, 0], -2 * a, atol=1e-11)
+    w = oracle.thom(N, U, a * (1 - X) ** 2, w_in, mode)
+    assert np.allclose(w[1:N, N], -2 * a, atol=1e-11)
+    # interior untouched
+    assert np.all(w[1:N, 1:N] == 123.0)
+    # G10 corners: psi = 0 -> bottom corners 0, top corners -2U/h
+    w = oracle.thom(N, U, np.zeros_like(X), w_in, mode)
+    assert w[0, 0] == 0 and w[0, N] == 0
+    assert abs(w[N, 0] + 2 * U / h) < 1e-12 and abs(w[N, N] + 2 * U / h) < 1e-12
+    assert np.all(w[N, :] == w[N, 0]) and np.all(w[1:N, 0] == 0) and np.all(w[1:N, N] == 0)
+
+
+# --------------------------------------------------------------------------------------------
+# (c) SSPRK(5,4) tableau, eq 9-13
+# --------------------------------------------------------------------------------------------
+
+C5 = 0.004477718303076      # z^5 coefficient of the stability polynomial (SURVEY S8(c) pin table)
+
+
+def R_poly(z):
+    return 1 + z + z ** 2 / 2 + z ** 3 / 6 + z ** 4 / 24 + C5 * z ** 5
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_ssprk_constant_preserved(mode):
+    # every stage's weights sum to 1: lambda = 0 leaves y unchanged (catches the G1 misprint)
+    # (the 15-digit decimals of eq 13 sum to 1 + 1e-15, hence the per-step allowance)
+    assert abs(oracle.ssprk54_scalar(0.0, 0.1, 1.0, 1, mode) - 1.0) < 2e-15
+    assert abs(oracle.ssprk54_scalar(0.0, 0.1, 1.0, 50, mode) - 1.0) < 1e-13
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_ssprk_stability_polynomial(mode):
+    # one step on y' = lambda y is a degree-5 polynomial in z = lambda dt; fourth order fixes its
+    # coefficients up to z^4 at 1/k!.  Recover them by interpolation at 6 nodes.
+    zs = np.array([-1.0, -0.6, -0.2, 0.2, 0.6, 1.0])
+    ys = np.array([oracle.ssprk54_scalar(z, 1.0, 1.0, 1, mode) for z in zs])
+    coef = np.linalg.solve(np.vander(zs, 6, increasing=True), ys)
+    for k in range(5):
+        assert abs(coef[k] - 1.0 / math.factorial(k)) < 1e-13, (k, coef)
+    assert abs(coef[5] - C5) < 1e-12
+    assert abs(coef[5] - 1.0 / 120) > 1e-3          # not fifth order
+    for z in (-2.5, -0.3, 0.7):
+        assert abs(oracle.ssprk54_scalar(z, 1.0, 1.0, 1, mode) - R_poly(z)) < 1e-13
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_ssprk_fourth_order_convergence(mode):
+    errs = []
+    for n in (8, 16, 32, 64, 128):
+        y = oracle.ssprk54_scalar(-1.0, 1.0 / n, 1.0, n, mode)
+        errs.append(abs(y - math.exp(-1.0)))
+    orders = [math.log2(errs[k] / errs[k + 1]) for k in range(4)]
+    assert all(3.9 < p < 4.2 for p in orders), orders
+    assert abs(orders[-1] - 4.0) < 0.02
+    assert abs(errs[-1] / 5.35e-12 - 1) < 0.05          # error 5.35e-12 at n = 128
+
+
+def test_printed_eq10_coefficient_is_a_misprint():
+    # G1: with the value printed at P:87 the stage-2 weights do not sum to 1
+    assert abs(0.444370493651235 + 0.555626506348765 - 1.0) > 2e-6
+    assert abs(0.444370493651235 + 0.555629506348765 - 1.0) < 1e-15
+
+
+# --------------------------------------------------------------------------------------------
+# whole step, linear part: psi = 0, U = 0, S = 0  => pure diffusion of a discrete eigenfunction,
+# omega^{n} = R(-nu lam_h dt)^n omega^0 exactly (pins stage wiring, dt, nu, the Thom ring and buffers)
+# --------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("mode", MODES)
+def test_step_diffusion_closed_form(mode):
+    N, Re, dt, nsteps = 16, 50.0, 2e-3, 7
+    X, Y = grid(N)
+    w0 = np.sin(2 * np.pi * X) * np.sin(np.pi * Y)
+    o = oracle.OracleCavity(N, Re, dt, 1.5, 0, mode)
+    o.set_lid(0.0)
+    o.set_fields(None, w0)
+    o.step(nsteps)
+    psi, w = o.get_fields()
+    z = -(1.0 / Re) * lam_h(N, 2, 1) * dt
+    assert np.all(psi == 0)
+    assert np.max(np.abs(w - R_poly(z) ** nsteps * w0)) < 1e-14
+    assert abs(o.diag()["t"] - nsteps * dt) < 1e-15 and o.diag()["step"] == nsteps
+
+
+# --------------------------------------------------------------------------------------------
+# (d) invariants and the SOR convergence rate (Young)
+# --------------------------------------------------------------------------------------------
+
+def rho_sor(N, beta):
+    rj = math.cos(math.pi / N)
+    bstar = 2.0 / (1.0 + math.sin(math.pi / N))
+    if beta >= bstar:
+        return beta - 1.0
+    return ((beta * rj + math.sqrt(beta ** 2 * rj ** 2 - 4 * (beta - 1))) / 2) ** 2
+
+
+@pytest.mark.parametrize("N,beta", [(32, 1.0), (32, 1.5), (32, 1.8), (64, 1.9)])
+def test_sor_rate_matches_young(N, beta):
+    rng = np.random.default_rng(5)
+    psi = np.zeros((N + 1, N + 1))
+    psi[1:N, 1:N] = rng.standard_normal((N - 1, N - 1))
+    om = np.zeros_like(psi)                              # homogeneous problem: psi -> 0
+    n0 = 40 * N // 10 * 10
+    psi = oracle.sor(N, beta, psi, om, n0)
+    a = np.max(np.abs(psi))
+    psi = oracle.sor(N, beta, psi, om, 100)
+    b = np.max(np.abs(psi))
+    assert abs((b / a) ** 0.01 - rho_sor(N, beta)) < 2e-4
+
+
+def test_sor_rate_survey_values():
+    # rho at the BASELINE configs
+    for N, beta, v in ((32, 1.8, 0.8888), (128, 1.95, 0.9642), (512, 1.99, 0.9900), (1024, 1.995, 0.9950)):
+        assert abs(rho_sor(N, beta) - v) < 1e-4
+
+
+def test_sor_overrelaxed_rate_geometric_mean():
+    N, beta = 32, 1.9                                    # > beta*: complex eigenvalues of modulus beta - 1
+    rng = np.random.default_rng(6)
+    psi = np.zeros((N + 1, N + 1))
+    psi[1:N, 1:N] = rng.standard_normal((N - 1, N - 1))
+    om = np.zeros_like(psi)
+    psi = oracle.sor(N, beta, psi, om, 100)
+    a = np.linalg.norm(psi)
+    psi = oracle.sor(N, beta, psi, om, 200)
+    b = np.linalg.norm(psi)
+    assert abs((b / a) ** (1 / 200) - 0.9) < 5e-3
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_walls_stay_zero_and_residual_bounded(mode):
+    from paper_0809_3098_b200 import workloads as W
+    wl = W.config(1)
+    psi0, w0 = W.initial_fields(wl)
+    o = oracle.OracleCavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage, mode)
+    o.set_fields(psi0 + 3.0, w0)                         # wall entries of psi must be ignored
+    res = []
+    for _ in range(5):
+        o.step(10)
+        psi, w = o.get_fields()
+        assert np.all(psi[0, :] == 0) and np.all(psi[-1, :] == 0) and np.all(psi[:, 0] == 0) and np.all(psi[:, -1] == 0)
+        assert np.all(np.isfinite(psi)) and np.all(np.isfinite(w))
+        res.append(o.diag()["res_inf"])
+    assert max(res) < 50.0
+    # frozen omega: each further block of S sweeps cuts the residual by about rho^S
+    r1 = o.poisson(wl.sweeps_per_stage)
+    r2 = o.poisson(wl.sweeps_per_stage)
+    r3 = o.poisson(wl.sweeps_per_stage)
+    assert r3 < r2 < r1
+    assert (r3 / r1) ** (1 / (2 * wl.sweeps_per_stage)) < rho_sor(wl.N, wl.sor_omega) + 0.02
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_rest_state_is_a_fixed_point_without_lid(mode):
+    o = oracle.OracleCavity(16, 100.0, 0.01, 1.7, 5, mode)
+    o.set_lid(0.0)
+    o.set_fields(None, np.zeros((17, 17)))
+    o.step(3)
+    psi, w = o.get_fields()
+    assert np.all(psi == 0) and np.all(w == 0)
+
+
+def test_primary_vortex_is_clockwise():
+    # qualitative only (no literature numbers are used): lid moving in +x drives psi < 0
+    from paper_0809_3098_b200 import workloads as W
+    wl = W.config(1)
+    o = oracle.OracleCavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage)
+    o.set_fields(*W.initial_fields(wl))
+    o.step(wl.steps)
+    psi, w = o.get_fields()
+    j, i = np.unravel_index(np.argmin(psi), psi.shape)
+    assert psi[j, i] < -0.05 and j > wl.N // 2           # centre in the upper half at Re = 100
+    d = o.diag()
+    assert d["kinetic_energy"] > 0 and d["enstrophy"] > 0 and d["res_inf"] < 1e-2
+
+
+# --------------------------------------------------------------------------------------------
+# (e) brute force: dense direct solve on the 9 x 9 grid
+# --------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("mode", MODES)
+def test_sor_converges_to_dense_direct_solve_9x9(mode):
+    N = 8
+    n = N - 1
+    rng = np.random.default_rng(11)
+    om = np.zeros((N + 1, N + 1))
+    om[1:N, 1:N] = rng.uniform(-1, 1, (n, n))
+    A = np.zeros((n * n, n * n))
+    for j in range(n):
+        for i in range(n):
+            r = j * n + i
+            A[r, r] = 4.0
+            if i > 0: A[r, r - 1] = -1.0
+            if i < n - 1: A[r, r + 1] = -1.0
+            if j > 0: A[r, r - n] = -1.0
+            if j < n - 1: A[r, r + n] = -1.0
+    direct = np.linalg.solve(A, (om[1:N, 1:N] / N ** 2).ravel()).reshape(n, n)
+    psi = oracle.sor(N, 1.4, np.zeros_like(om), om, 400, mode)
+    assert np.max(np.abs(psi[1:N, 1:N] - direct)) < 1e-15
+    assert np.all(psi[0, :] == 0) and np.all(psi[:, N] == 0)
+    # asymmetric source: catches an i/j transposition of the stored layout
+    om[:] = 0.0
+    om[2, 5] = 1.0                                       # j = 2, i = 5
+    direct = np.linalg.solve(A, (om[1:N, 1:N] / N ** 2).ravel()).reshape(n, n)
+    psi = oracle.sor(N, 1.4, np.zeros_like(om), om, 400, mode)
+    assert np.max(np.abs(psi[1:N, 1:N] - direct)) < 1e-16
+    assert np.unravel_index(np.argmax(psi), psi.shape) == (2, 5)
+
+
+# --------------------------------------------------------------------------------------------
+# the two arithmetic modes agree to rounding, and the diagnostics match their definitions
+# --------------------------------------------------------------------------------------------
+
+def test_modes_agree_to_rounding():
+    from paper_0809_3098_b200 import workloads as W
+    wl = W.config(1)
+    out = []
+    for mode in MODES:
+        o = oracle.OracleCavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage, mode)
+        o.set_fields(*W.initial_fields(wl))
+        o.step(wl.steps)
+        out.append(o.get_fields())
+    for a, b in zip(out[0], out[1]):
+        assert np.max(np.abs(a - b)) / np.max(np.abs(a)) < 1e-13     # ~1e-15 observed
+    assert not np.array_equal(out[0][0], out[1][0])                  # but they ARE different roundings
+
+
+def test_diagnostics_definitions():
+    N = 16
+    h = 1.0 / N
+    X, Y = grid(N)
+    psi = np.sin(np.pi * X) * np.sin(np.pi * Y)
+    om = lam_h(N, 1, 1) * psi                              # discrete residual = 0
+    o = oracle.OracleCavity(N, 100.0, 0.01, 1.5, 0)
+    o.set_fields(psi, om)
+    d = o.diag()
+    assert d["res_inf"] < 1e-12 and d["res_l2"] < 1e-12
+    I = (slice(1, N), slice(1, N))
+    u = (psi[2:, 1:N] - psi[:-2, 1:N]) / (2 * h)
+    v = -(psi[1:N, 2:] - psi[1:N, :-2]) / (2 * h)
+    assert abs(d["kinetic_energy"] - 0.5 * h * h * np.sum(u * u + v * v)) < 1e-14
+    assert abs(d["enstrophy"] - 0.5 * h * h * np.sum(om[I] ** 2)) < 1e-11
+    o.set_fields(psi, om + 2.0)                            # residual = 2 everywhere
+    d = o.diag()
+    assert abs(d["res_inf"] - 2.0) < 1e-11 and abs(d["res_l2"] - 2.0 * (N - 1) * h) < 1e-11
