@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the fp64 SSPRK(5,4) cavity step (arXiv 0809.3098) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+A "step" is one pass of the whole hot path over the workload: one SSPRK(5,4) time step = 5 x [S red-black SOR
+sweeps (a1), Thom wall vorticity (a2), transport RHS + stage combination (a3)] on the (N+1)^2 grid.
+The workload is BASELINE.json configs[3] (1025 x 1025, Re 10 000, S = 200, beta = 1.995): the one the metric's
+target is quoted on.  Metric: fp64 grid-point-stage updates per second, GPSU/s = 5 (N+1)^2 steps / time
+(Poisson sweeps included).
+
+One JSON line on stdout (rank 0).  Keys beyond the base contract:
+  roofline      the dominant kernel (the a1 sweep kernel), measured live with CUDA events around sweep-only
+                launches (cav_poisson): SURVEY.md S8(d) item 2 bytes (24 B per point-sweep, what a
+                one-pass-per-sweep streaming kernel must move) / average launch duration, against the measured
+                HBM copy peak of MEASURED_PEAKS.json.  Temporal blocking moves fewer bytes than that, so the
+                fraction may exceed 1; `alu` then gives the bound that is left (fp64 pipe utilisation).
+  cpu_baseline  the oracle (oracle/, single thread, as it stands) timed on this box on a bounded sample.
+  e2e           the same metric through the C ABI with HOST buffers every step (cav_set_fields from pinned
+                memory -> cav_step(1) -> cav_get_fields), copies inside the timed region.
+
+--impl reference times the CPU oracle instead (there is no reference implementation of the paper).
+N > 1: replicas only (one independent context per GPU, no data-path collective).
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 grid-point-stage updates/s (incl. Poisson sweeps)"
+UNIT = "GPSU/s"
+FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+SM_COUNT, FP64_LANES_PER_SM = 148, 64   # B200: 148 SMs x 64 fp64 lanes
+FP64_INSTR_PER_POINT_SWEEP = 5     # 3 DADD + 2 DFMA
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (default 4, the metric's)")
+    ap.add_argument("--engine", default="auto", choices=["auto", "stream", "resident"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", float(p.get("sm_max_mhz", 1965.0))
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)", 1965.0
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------------------------------------
+# the CPU oracle, timed (cpu_baseline leg and --impl reference)
+# ----------------------------------------------------------------------------------------------------------
+
+def oracle_sample_rate(wl, seconds_budget, nsamples=None):
+    """Times the oracle as it stands (single thread) on whole time steps of `wl`; returns (GPSU/s, description)."""
+    import oracle
+    from paper_0809_3098_b200 import workloads as W
+    o = oracle.OracleCavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage, oracle.MODE_PLAIN)
+    o.set_fields(*W.initial_fields(wl))
+    G = (wl.N + 1) ** 2
+    t0 = time.perf_counter()
+    o.step(1)
+    t1 = time.perf_counter() - t0
+    n = nsamples if nsamples is not None else max(1, min(20, int(seconds_budget / max(t1, 1e-9)) - 1))
+    t0 = time.perf_counter()
+    o.step(n)
+    dt = time.perf_counter() - t0
+    o.close()
+    return 5.0 * G * n / dt, "%d SSPRK(5,4) time steps of %s (after 1 untimed), %.1f s of one core" % (n, wl.name, dt)
+
+
+def run_reference(args, wl):
+    """--impl reference: the oracle on the host cores.  Each 'step' is a bounded sample of the workload: one whole
+    time step when K + W of them fit in ~170 s, else one RK-stage-equivalent (S sweeps + Thom via orc_poisson, then
+    the transport operator via orc_rhs) = (N+1)^2 grid-point-stage updates."""
+    import numpy as np
+    import oracle
+    from paper_0809_3098_b200 import workloads as W
+    K = args.steps if args.steps is not None else 20
+    Wm = args.warmup if args.warmup is not None else 3
+    G = (wl.N + 1) ** 2
+    o = oracle.OracleCavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage, oracle.MODE_PLAIN)
+    o.set_fields(*W.initial_fields(wl))
+    t0 = time.perf_counter()
+    o.poisson(wl.sweeps_per_stage)
+    psi, w = o.get_fields()
+    oracle.rhs(wl.N, wl.Re, psi, w)
+    t_stage = time.perf_counter() - t0
+    full = (K + Wm) * 5.0 * t_stage <= 170.0
+    units = 5.0 * G if full else 1.0 * G
+
+    def one():
+        if full:
+            o.step(1)
+        else:
+            o.poisson(wl.sweeps_per_stage)
+            p, ww = o.get_fields()
+            oracle.rhs(wl.N, wl.Re, p, ww)
+
+    for _ in range(Wm):
+        one()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        one()
+    dt = time.perf_counter() - t0
+    o.close()
+    value = units * K / dt
+    sample = ("one whole SSPRK(5,4) time step of %s per step" % wl.name) if full else \
+             ("one RK-stage-equivalent of %s per step (S=%d sweeps + Thom + transport operator = (N+1)^2 GPSU)"
+              % (wl.name, wl.sweeps_per_stage))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
+            "warmup": Wm, "ms_per_step": 1e3 * dt / K, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "grid": "%dx%d" % (wl.N + 1, wl.N + 1), "Re": wl.Re,
+                       "sweeps_per_stage": wl.sweeps_per_stage, "sor_omega": wl.sor_omega, "dt": wl.dt,
+                       "note": "no reference implementation of the paper exists; this arm is the CPU oracle"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------------------
+# our arm
+# ----------------------------------------------------------------------------------------------------------
+
+def run_ours(args, wl, rank, world, local_rank):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_0809_3098_b200 import binding, replicas
+    from paper_0809_3098_b200 import workloads as W
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    use_dist = world > 1
+    if use_dist:
+        dist.init_process_group("nccl", device_id=dev)
+    K = args.steps if args.steps is not None else 200
+    Wm = args.warmup if args.warmup is not None else 5
+    Wm = max(Wm, 3)
+
+    wl = replicas.replica_workload(wl, rank, world)
+    G = (wl.N + 1) ** 2
+    P = (wl.N - 1) ** 2
+    S = wl.sweeps_per_stage
+    cav = binding.Cavity(wl.N, wl.Re, wl.dt, wl.sor_omega, S, engine=args.engine)
+    psi0, w0 = W.initial_fields(wl)
+    cav.set_fields(psi0, w0)
+    if wl.poisson_sweeps:
+        cav.poisson(wl.poisson_sweeps, want_residual=False)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)       # > 126 MB of L2
+
+    def barrier():
+        if use_dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: K steps, L2 flushed (untimed) before each, CUDA events on the launch stream ----
+    for _ in range(Wm):
+        cav.step_async(1)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    l0 = cav.launch_count()
+    barrier()
+    for k in range(K):
+        flush.fill_(k & 0xFF)
+        ev[k][0].record()
+        cav.step_async(1)
+        ev[k][1].record()
+    barrier()
+    launches = cav.launch_count() - l0
+    clocks = sampler.stop()
+    per_step_ms = [a.elapsed_time(b) for a, b in ev]
+    t_local = sum(per_step_ms) * 1e-3
+    units_total, t_max = replicas.combine(5.0 * G * K, t_local, world, dist if use_dist else None, dev)
+    value = units_total / t_max
+
+    # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        hp = torch.empty((wl.N + 1, wl.N + 1), dtype=torch.float64).pin_memory()
+        hw = torch.empty((wl.N + 1, wl.N + 1), dtype=torch.float64).pin_memory()
+        hp_n, hw_n = hp.numpy(), hw.numpy()
+        cav.get_fields(hp_n, hw_n)
+        Ke = K
+        for _ in range(3):
+            cav.set_fields(hp_n, hw_n); cav.step(1); cav.get_fields(hp_n, hw_n)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(Ke):
+            cav.set_fields(hp_n, hw_n)          # H2D: psi and omega
+            cav.step(1)
+            cav.get_fields(hp_n, hw_n)          # D2H: psi and omega (the step's result)
+        torch.cuda.synchronize()
+        te = time.perf_counter() - t0
+        ue, tmax_e = replicas.combine(5.0 * G * Ke, te, world, dist if use_dist else None, dev)
+        e2e = {"value": ue / tmax_e, "unit": UNIT, "h2d_bytes_per_step": 2 * G * 8, "d2h_bytes_per_step": 2 * G * 8,
+               "ms_per_step": 1e3 * tmax_e / Ke, "api": "cav_set_fields(host) -> cav_step(1) -> cav_get_fields(host)"}
+
+    # ---- roofline of the dominant kernel (a1 sweeps), measured live: sweep-only launches via cav_poisson ----
+    hbm_gbs, peak_src, sm_max_mhz = measured_peaks()
+    nsw = 5 * S
+    for _ in range(2):
+        cav.poisson(nsw, want_residual=False)
+    reps, tsw, lsw = 5, 0.0, 0
+    for _ in range(reps):
+        flush.fill_(1)
+        l1 = cav.launch_count()
+        cav.poisson(nsw, want_residual=False)
+        tsw += cav.last_elapsed_ms() * 1e-3
+        lsw += cav.launch_count() - l1 - 2          # minus the scale and Thom launches
+    bytes_per_call = 24.0 * P * nsw                 # 24 B per point-sweep
+    achieved = bytes_per_call * reps / tsw / 1e9
+    sweep_share = (tsw / reps) / (statistics.mean(per_step_ms) * 1e-3)
+    sm_mhz = clocks.get("sm_mhz") or sm_max_mhz
+    fp64_rate = FP64_INSTR_PER_POINT_SWEEP * P * nsw * reps / tsw
+    fp64_peak_max = SM_COUNT * FP64_LANES_PER_SM * sm_max_mhz * 1e6
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
+                "traffic": None, "peak_source": peak_src, "kernel": "a1 sweep kernel(s), engine " + cav.describe(),
+                "bytes_model": "24 B per point-sweep x (N-1)^2 x sweeps (streaming-equivalent, SURVEY S8(d) item 2)",
+                "avg_launch_us": 1e6 * tsw / max(lsw, 1), "launches_per_step": lsw // reps,
+                "share_of_step": sweep_share,
+                "alu": {"bound": "alu", "achieved": fp64_rate / 1e12, "peak": fp64_peak_max / 1e12,
+                        "unit": "T fp64 instr/s", "frac": fp64_rate / fp64_peak_max,
+                        "model": "5 fp64 instr per point-sweep; peak = 148 SMs x 64 lanes x sm_max_mhz"}}
+    b0 = 24.0 * S + 33.6
+    hbm_equiv = value / max(world, 1) * b0 / 1e9
+    cav.close()
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": 1e3 * t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name if world == 1 else W.config(args.config).name + " (rank 0) + Table-1 Re replicas",
+                       "grid": "%dx%d" % (wl.N + 1, wl.N + 1), "Re": wl.Re, "sweeps_per_stage": S,
+                       "sor_omega": wl.sor_omega, "dt": wl.dt, "parallelism": "replicas x%d" % world,
+                       "l2": "flushed before every timed step (256 MiB write, outside the per-step CUDA events)",
+                       "timing": "sum of per-step CUDA-event times on the launch stream, max over ranks"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "hbm_streaming_equiv": {"bytes_per_gpsu": b0, "GBps_per_gpu": hbm_equiv, "frac_of_measured_peak": hbm_equiv / hbm_gbs,
+                                    "frac_of_8TBps_nominal": hbm_equiv / 8000.0,
+                                    "note": "BASELINE target: >= 0.70 of nominal for the full step at 1025^2"},
+            "ms_per_step_min": min(per_step_ms), "ms_per_step_median": statistics.median(per_step_ms)}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, sample = oracle_sample_rate(W.config(args.config), 15.0)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                                "host_cores": os.cpu_count()}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if use_dist:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_0809_3098_b200 import workloads as W
+    wl = W.config(args.config)
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, wl)
+        return
+    run_ours(args, wl, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

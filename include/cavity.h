@@ -1,0 +1,114 @@
+/* cavity.h — C ABI of libcavity.so: the fp64 SSPRK(5,4) time step of the 2-D vorticity /
+ * stream-function lid-driven cavity of arXiv 0809.3098 (Cardoso & Bicudo) on one B200 (sm_100a).
+ *
+ * P:n = /root/reference/PAPER.md line n;  S8 = SURVEY.md section 8;  Gk / Dk = the readings and
+ * departures listed in DESIGN.md ("Readings of the paper").
+ *
+ * The problem: unit square, uniform grid of (N+1) x (N+1) points, h = 1/N, grid index
+ * i = 0..N <-> x = i h, j = 0..N <-> y = j h, j = N is the lid moving at U = 1; psi = 0 on all four
+ * walls (eq 23-24); nu = 1/Re.
+ *
+ * One time step (eq 9-13) is five stages; stage k with input vorticity w_in = omega^(k-1):
+ *   (a1) S = sweeps_per_stage red-black SOR sweeps of the 5-point Poisson problem lap(psi) = -w_in,
+ *        warm-started from the current psi; red = (i + j) even first, then black (G9):
+ *          psi_ij <- psi_ij + beta ( (psi_W + psi_E + psi_S + psi_N + h^2 w_ij) / 4 - psi_ij )
+ *        (eq 15-21 P:114-138 reduced to the 5-point operator, D1-D3)
+ *   (a2) Thom wall vorticity of w_in from psi (eq 25): omega_wall = -2 psi_adjacent / h^2,
+ *        minus 2U/h on the lid; the top and bottom rows own the four corners (G10)
+ *   (a3) dL = dt L(psi, w_in) with eq 8 P:80 and eq 22, then the stage combination of eq 9-13.
+ *
+ * All entry points: host code, callable from any thread, but a context must not be used from two
+ * threads at once.  All array arguments are HOST pointers unless the name ends in _dev; fields are
+ * dense row-major (N+1) x (N+1) fp64 arrays, element k = j (N+1) + i.  Buffers are borrowed for the
+ * duration of the call only.  Every call returns CAV_OK (0) or a negative CAV_E* code; nothing
+ * throws across the ABI.  Device memory comes from PyTorch's CUDA caching allocator and all work is
+ * enqueued on the PyTorch current stream of the device that was current at cav_create; every call
+ * below is synchronous at return unless stated otherwise.  There is no CPU fallback: without a CUDA
+ * device cav_create returns CAV_ECUDA.
+ */
+#ifndef CAVITY_H
+#define CAVITY_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CAV_OK       0
+#define CAV_EINVAL  (-1)   /* bad argument */
+#define CAV_ENOMEM  (-2)   /* host or device allocation failed */
+#define CAV_ECUDA   (-3)   /* CUDA runtime error, or no usable device */
+#define CAV_ENOTSUP (-4)   /* requested engine cannot run this problem on this device */
+
+/* Sweep engines (all compute the same red-black SOR, bit for bit; they differ in how it is scheduled). */
+#define CAV_ENGINE_AUTO     0   /* pick by grid size (default) */
+#define CAV_ENGINE_STREAM   1   /* one kernel per colour half-sweep over global memory (the streaming baseline) */
+#define CAV_ENGINE_RESIDENT 2   /* persistent register/shared-memory resident tiles, temporal blocking */
+
+typedef struct cav_ctx cav_ctx;   /* opaque; owned by the library from cav_create to cav_destroy */
+
+typedef struct cav_diag {
+    double t;                /* simulated time = step * dt */
+    long long step;          /* time steps taken since cav_create / cav_set_fields */
+    double res_inf;          /* max |r_ij| over interior points, r = lap_h(psi) + omega   (S8(a) row a4) */
+    double res_l2;           /* sqrt(h^2 sum r^2) */
+    double kinetic_energy;   /* (1/2) h^2 sum (u^2 + v^2), u, v of eq 22 */
+    double enstrophy;        /* (1/2) h^2 sum omega^2 */
+} cav_diag;
+
+/* Allocates psi, omega and the stage buffers (zero-filled: fluid at rest) for an (N+1) x (N+1) grid.
+ * Re: Reynolds number (nu = 1/Re); dt: time step; sor_omega: relaxation factor beta in (0, 2);
+ * sweeps_per_stage: S >= 0 red-black sweeps per RK stage (D3).
+ * Errors: CAV_EINVAL (out null, N < 2, Re <= 0, dt <= 0, sor_omega outside (0, 2), S < 0, or any
+ * of them not finite); CAV_ENOMEM; CAV_ECUDA.  On error *out is NULL. */
+int cav_create(cav_ctx** out, int N, double Re, double dt, double sor_omega, int sweeps_per_stage);
+
+/* Frees everything.  NULL is a no-op. */
+void cav_destroy(cav_ctx* ctx);
+
+/* Loads the state from host arrays.  psi == NULL means psi <- 0.  Wall entries of psi are ignored and
+ * forced to 0 (eq 23-24, G5); wall entries of omega are stored as given (a2 overwrites them before
+ * first use).  Resets step and t to 0.  omega == NULL is CAV_EINVAL. */
+int cav_set_fields(cav_ctx* ctx, const double* psi, const double* omega);
+
+/* Copies the state into caller-owned host arrays of (N+1)^2 doubles (either may be NULL).  Pure.
+ * After a step: omega interior = omega^{n+1}; psi and the omega ring are those of stage 5 (G16). */
+int cav_get_fields(cav_ctx* ctx, double* psi_out, double* omega_out);
+
+/* Advances nsteps SSPRK(5,4) steps, each 5 x [a1 x S, a2, a3].  nsteps < 0: CAV_EINVAL; 0: no-op. */
+int cav_step(cav_ctx* ctx, int nsteps);
+
+/* As cav_step but returns after enqueueing on the context's stream (no host synchronisation). */
+int cav_step_async(cav_ctx* ctx, int nsteps);
+
+/* Blocks until all work enqueued for this context has finished. */
+int cav_sync(cav_ctx* ctx);
+
+/* nsweeps of a1 on the current (psi, omega), then one a2 so that the omega ring matches psi; writes
+ * the max-norm residual (row a4) to *res_inf_out if non-NULL.  Does not advance time. */
+int cav_poisson(cav_ctx* ctx, int nsweeps, double* res_inf_out);
+
+/* Runs the a4 reductions on the current state.  Pure. */
+int cav_get_diag(cav_ctx* ctx, cav_diag* out);
+
+/* Selects the sweep engine (CAV_ENGINE_*).  CAV_ENOTSUP if that engine cannot run this grid on this
+ * device.  The default is CAV_ENGINE_AUTO. */
+int cav_set_engine(cav_ctx* ctx, int engine);
+
+/* Describes the launch plan of the current engine in `buf` (NUL-terminated, truncated to len). */
+int cav_describe(cav_ctx* ctx, char* buf, int len);
+
+/* Number of kernel launches enqueued by this context since cav_create (for bench.py's gpu_launches). */
+long long cav_launch_count(cav_ctx* ctx);
+
+/* CUDA-event time in milliseconds of the most recent cav_step / cav_step_async / cav_poisson on the
+ * context's stream (events recorded around the enqueued work); blocks until that work has finished.
+ * Writes 0 if none has run. */
+int cav_last_elapsed_ms(cav_ctx* ctx, float* ms_out);
+
+/* Static string for an error code. */
+const char* cav_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CAVITY_H */

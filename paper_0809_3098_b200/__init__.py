@@ -9,6 +9,7 @@ from . import workloads  # noqa: F401
 
 def __getattr__(name):
     if name in ("Cavity", "binding"):
-        from . import binding
+        import importlib
+        binding = importlib.import_module(__name__ + ".binding")
         return binding if name == "binding" else binding.Cavity
     raise AttributeError(name)

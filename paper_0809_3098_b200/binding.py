@@ -1,0 +1,165 @@
+"""ctypes binding of libcavity.so (include/cavity.h).  Argument marshalling only: every step of the path
+runs in the CUDA kernels behind the C ABI.  There is no CPU fallback; a missing library or a missing
+CUDA device raises.
+
+`import torch` happens before the library is loaded: libcavity.so takes its device memory from PyTorch's
+caching allocator and enqueues on PyTorch's current stream.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+ENGINE_AUTO, ENGINE_STREAM, ENGINE_RESIDENT = 0, 1, 2
+_ENGINES = {"auto": ENGINE_AUTO, "stream": ENGINE_STREAM, "resident": ENGINE_RESIDENT}
+
+# every symbol include/cavity.h declares
+SYMBOLS = ("cav_create", "cav_destroy", "cav_set_fields", "cav_get_fields", "cav_step", "cav_step_async", "cav_sync",
+           "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_describe", "cav_launch_count",
+           "cav_last_elapsed_ms", "cav_strerror")
+
+_lib = None
+
+
+class CavDiag(C.Structure):
+    _fields_ = [("t", C.c_double), ("step", C.c_longlong), ("res_inf", C.c_double), ("res_l2", C.c_double),
+                ("kinetic_energy", C.c_double), ("enstrophy", C.c_double)]
+
+
+class CavityError(RuntimeError):
+    def __init__(self, what, code):
+        msg = lib().cav_strerror(code).decode() if _lib is not None else "?"
+        super().__init__("%s failed: %s (code %d)" % (what, msg, code))
+        self.code = code
+
+
+def lib_path():
+    return os.path.join(os.path.dirname(os.path.abspath(__file__)), "libcavity.so")
+
+
+def lib():
+    """Loads libcavity.so (building it first if the sources are newer).  Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    import torch  # noqa: F401  (loads libc10 / libc10_cuda, which libcavity.so links against)
+    path = lib_path()
+    if os.environ.get("CAVITY_NO_BUILD", "0") != "1":
+        from .build import build
+        path = build()
+    if not os.path.exists(path):
+        raise RuntimeError("libcavity.so is missing (%s); run python -m paper_0809_3098_b200.build" % path)
+    L = C.CDLL(path)
+    dp = C.POINTER(C.c_double)
+    L.cav_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.c_double, C.c_double, C.c_int]
+    L.cav_destroy.argtypes = [C.c_void_p]
+    L.cav_destroy.restype = None
+    L.cav_set_fields.argtypes = [C.c_void_p, dp, dp]
+    L.cav_get_fields.argtypes = [C.c_void_p, dp, dp]
+    L.cav_step.argtypes = [C.c_void_p, C.c_int]
+    L.cav_step_async.argtypes = [C.c_void_p, C.c_int]
+    L.cav_sync.argtypes = [C.c_void_p]
+    L.cav_poisson.argtypes = [C.c_void_p, C.c_int, dp]
+    L.cav_get_diag.argtypes = [C.c_void_p, C.POINTER(CavDiag)]
+    L.cav_set_engine.argtypes = [C.c_void_p, C.c_int]
+    L.cav_describe.argtypes = [C.c_void_p, C.c_char_p, C.c_int]
+    L.cav_launch_count.argtypes = [C.c_void_p]
+    L.cav_launch_count.restype = C.c_longlong
+    L.cav_last_elapsed_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+    L.cav_strerror.argtypes = [C.c_int]
+    L.cav_strerror.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _p(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double)) if a is not None else None
+
+
+def _chk(rc, what):
+    if rc != 0:
+        raise CavityError(what, rc)
+
+
+def _field(a, N, name):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if a.shape != (N + 1, N + 1):
+        raise ValueError("%s must have shape (N+1, N+1) = (%d, %d), row j = y index" % (name, N + 1, N + 1))
+    return a
+
+
+class Cavity:
+    """One cav_ctx.  Fields are numpy (N+1, N+1) float64 arrays indexed [j, i] (row N = lid)."""
+
+    def __init__(self, N, Re, dt, sor_omega, sweeps_per_stage, engine="auto"):
+        self.N = int(N)
+        self._h = C.c_void_p()
+        _chk(lib().cav_create(C.byref(self._h), int(N), float(Re), float(dt), float(sor_omega),
+                              int(sweeps_per_stage)), "cav_create")
+        if engine != "auto":
+            self.set_engine(engine)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().cav_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def set_engine(self, engine):
+        _chk(lib().cav_set_engine(self._h, _ENGINES[engine] if isinstance(engine, str) else int(engine)),
+             "cav_set_engine")
+
+    def set_fields(self, psi, omega):
+        psi = None if psi is None else _field(psi, self.N, "psi")
+        omega = _field(omega, self.N, "omega")
+        _chk(lib().cav_set_fields(self._h, _p(psi), _p(omega)), "cav_set_fields")
+
+    def get_fields(self, psi_out=None, omega_out=None):
+        psi = np.empty((self.N + 1, self.N + 1)) if psi_out is None else psi_out
+        w = np.empty((self.N + 1, self.N + 1)) if omega_out is None else omega_out
+        _chk(lib().cav_get_fields(self._h, _p(psi), _p(w)), "cav_get_fields")
+        return psi, w
+
+    def step(self, nsteps=1):
+        _chk(lib().cav_step(self._h, int(nsteps)), "cav_step")
+
+    def step_async(self, nsteps=1):
+        _chk(lib().cav_step_async(self._h, int(nsteps)), "cav_step_async")
+
+    def sync(self):
+        _chk(lib().cav_sync(self._h), "cav_sync")
+
+    def poisson(self, nsweeps, want_residual=True):
+        r = C.c_double()
+        _chk(lib().cav_poisson(self._h, int(nsweeps), C.byref(r) if want_residual else None), "cav_poisson")
+        return r.value if want_residual else None
+
+    def diag(self):
+        d = CavDiag()
+        _chk(lib().cav_get_diag(self._h, C.byref(d)), "cav_get_diag")
+        return {"t": d.t, "step": d.step, "res_inf": d.res_inf, "res_l2": d.res_l2,
+                "kinetic_energy": d.kinetic_energy, "enstrophy": d.enstrophy}
+
+    def describe(self):
+        buf = C.create_string_buffer(1024)
+        _chk(lib().cav_describe(self._h, buf, 1024), "cav_describe")
+        return buf.value.decode()
+
+    def launch_count(self):
+        return int(lib().cav_launch_count(self._h))
+
+    def last_elapsed_ms(self):
+        ms = C.c_float()
+        _chk(lib().cav_last_elapsed_ms(self._h, C.byref(ms)), "cav_last_elapsed_ms")
+        return float(ms.value)

@@ -1,0 +1,356 @@
+// cavity_api.cu — the C ABI of include/cavity.h: context, step scheduler, host <-> device copies.
+//
+// PyTorch is used for exactly two things (BASELINE.json north_star): device memory comes from its CUDA
+// caching allocator and work is enqueued on its current stream.  No ATen operator does any arithmetic;
+// every step of the path runs in the kernels of cavity_kernels.cu / cavity_resident.cu.
+// There is no CPU fallback: without a CUDA device cav_create fails with CAV_ECUDA.
+#include <c10/cuda/CUDACachingAllocator.h>
+#include <c10/cuda/CUDAStream.h>
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/cavity.h"
+#include "cavity_kernels.cuh"
+#include "cavity_resident.cuh"
+
+#define CAV_API extern "C" __attribute__((visibility("default")))
+
+struct cav_ctx {
+    int N = 0, S = 0, device = 0;
+    double Re = 0, dt = 0, beta = 0;
+    cavk::Params P{};
+    cudaStream_t st = nullptr;
+    void* slab = nullptr;            // one allocation from PyTorch's caching allocator
+    double* psi = nullptr;           // stream function
+    double* psi_alt = nullptr;       // second psi buffer (halo exchange of the resident engine)
+    double* q = nullptr;             // (beta/4) h^2 w_in, the scaled right-hand side of the current stage
+    double* w[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // omega^n (state), omega^(1..4)
+    double* T = nullptr;             // first three terms of eq 13
+    double* scratch = nullptr;       // diagnostics partials
+    double* out4 = nullptr;          // diagnostics result (device)
+    unsigned int* flags = nullptr;   // resident engine: per-tile round counters
+    size_t field_doubles = 0;
+    long long step = 0;
+    long long launches = 0;
+    int engine_req = CAV_ENGINE_AUTO;
+    int engine = CAV_ENGINE_STREAM;  // resolved
+    cavk::ResidentPlan plan{};       // valid if plan.ok
+    cudaGraphExec_t graph = nullptr; // one full time step of the current engine
+    long long graph_launches = 0;    // kernel launches inside `graph`
+    bool graph_tried = false;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool timed = false;
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+inline bool finite_pos(double x) { return std::isfinite(x) && x > 0.0; }
+
+cavk::Params make_params(int N, double Re, double dt, double beta) {
+    cavk::Params P;
+    const double U = 1.0;                    // lid speed
+    const double h = 1.0 / (double)N;        // uniform grid of the unit square
+    P.N = N;
+    P.pitch = ((N + 1) + 3) & ~3;
+    P.cb = 0.25 * beta;
+    P.cq = (0.25 * beta) * (h * h);
+    P.omb = 1.0 - beta;
+    P.i2h = 0.5 * (double)N;
+    P.ih2 = (double)N * (double)N;
+    P.nu = 1.0 / Re;
+    P.c2h2 = 2.0 * ((double)N * (double)N);
+    P.lid = 2.0 * U * (double)N;
+    P.dt = dt;
+    return P;
+}
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+#define CK(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { cudaGetLastError(); return CAV_ECUDA; } } while (0)
+#define LAUNCH(expr) do { int n_ = (expr); if (n_ < 0) { cudaGetLastError(); return CAV_ECUDA; } nl += n_; } while (0)
+
+void drop_graph(cav_ctx* c) {
+    if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }
+    c->graph_tried = false;
+    c->graph_launches = 0;
+}
+
+void resolve_engine(cav_ctx* c) {
+    int e = c->engine_req;
+    if (e == CAV_ENGINE_AUTO) e = c->plan.ok ? CAV_ENGINE_RESIDENT : CAV_ENGINE_STREAM;
+    if (e != c->engine) { c->engine = e; drop_graph(c); }
+}
+
+// a1: nsweeps red-black sweeps on psi with right-hand side q
+int enqueue_sweeps(cav_ctx* c, int nsweeps, long long& nl) {
+    if (nsweeps <= 0) return CAV_OK;
+    if (c->engine == CAV_ENGINE_RESIDENT) {
+        LAUNCH(cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi_alt, c->q, c->flags, nsweeps, c->st));
+    } else {
+        LAUNCH(cavk::stream_sweeps(c->P, c->psi, c->q, nsweeps, c->st));
+    }
+    return CAV_OK;
+}
+
+// one SSPRK(5,4) step: 5 x [scale, a1 x S, a2 + a3]
+int enqueue_step(cav_ctx* c, long long& nl) {
+    double* const* w = c->w;
+    const double* win[5] = {w[0], w[1], w[2], w[3], w[4]};
+    const double* a[5] = {nullptr, w[0], w[0], w[0], c->T};
+    const double* b[5] = {nullptr, nullptr, nullptr, w[2], nullptr};
+    double* wout[5] = {w[1], w[2], w[3], w[4], w[0]};
+    for (int k = 0; k < 5; ++k) {
+        LAUNCH(cavk::scale_rhs(c->P, win[k], c->q, c->st));
+        int rc = enqueue_sweeps(c, c->S, nl);
+        if (rc != CAV_OK) return rc;
+        LAUNCH(cavk::rk_stage(c->P, k + 1, c->psi, win[k], a[k], b[k], wout[k], c->T, c->st));
+    }
+    return CAV_OK;
+}
+
+// Capture one step into a CUDA graph (the stream engine launches 10 S + 10 kernels per step).
+void try_build_graph(cav_ctx* c) {
+    if (c->graph_tried) return;
+    c->graph_tried = true;
+    if (c->engine == CAV_ENGINE_RESIDENT) return;     // 10-odd launches per step: a graph buys nothing
+    cudaGraph_t g = nullptr;
+    if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return; }
+    long long nl = 0;
+    int rc = enqueue_step(c, nl);
+    cudaError_t e = cudaStreamEndCapture(c->st, &g);
+    if (rc != CAV_OK || e != cudaSuccess || !g) { cudaGetLastError(); if (g) cudaGraphDestroy(g); return; }
+    cudaGraphExec_t ge = nullptr;
+    if (cudaGraphInstantiate(&ge, g, 0) == cudaSuccess) { c->graph = ge; c->graph_launches = nl; }
+    else cudaGetLastError();
+    cudaGraphDestroy(g);
+}
+
+int step_impl(cav_ctx* c, int nsteps, bool sync) {
+    if (!c || nsteps < 0) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    if (nsteps == 0) return CAV_OK;
+    resolve_engine(c);
+    try_build_graph(c);
+    CK(cudaEventRecord(c->ev0, c->st));
+    for (int n = 0; n < nsteps; ++n) {
+        if (c->graph) {
+            CK(cudaGraphLaunch(c->graph, c->st));
+            c->launches += c->graph_launches;
+        } else {
+            long long nl = 0;
+            int rc = enqueue_step(c, nl);
+            c->launches += nl;
+            if (rc != CAV_OK) return rc;
+        }
+    }
+    CK(cudaEventRecord(c->ev1, c->st));
+    c->timed = true;
+    c->step += nsteps;
+    if (sync) CK(cudaStreamSynchronize(c->st));
+    return CAV_OK;
+}
+
+}  // namespace
+
+CAV_API int cav_create(cav_ctx** out, int N, double Re, double dt, double sor_omega, int sweeps_per_stage) {
+    if (!out) return CAV_EINVAL;
+    *out = nullptr;
+    if (N < 2 || N > 32766 || !finite_pos(Re) || !finite_pos(dt) || !std::isfinite(sor_omega) || !(sor_omega > 0.0) ||
+        !(sor_omega < 2.0) || sweeps_per_stage < 0)
+        return CAV_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return CAV_ECUDA; }
+    cav_ctx* c = new (std::nothrow) cav_ctx();
+    if (!c) return CAV_ENOMEM;
+    int rc = CAV_OK;
+    try {
+        if (cudaGetDevice(&c->device) != cudaSuccess) throw (int)CAV_ECUDA;
+        c->N = N; c->S = sweeps_per_stage; c->Re = Re; c->dt = dt; c->beta = sor_omega;
+        c->P = make_params(N, Re, dt, sor_omega);
+        c->st = c10::cuda::getCurrentCUDAStream(c->device).stream();
+        c->plan = cavk::resident_plan(c->P, c->device);
+
+        const size_t fd = align_up((size_t)c->P.pitch * (size_t)(N + 1), 32);   // doubles per field, 256 B multiple
+        c->field_doubles = fd;
+        const size_t nfields = 9;    // psi, psi_alt, q, w0..w4, T
+        const size_t scratch_d = align_up(4 * (size_t)cavk::diag_scratch_doubles(), 32);
+        const size_t flags_b = align_up(sizeof(unsigned int) * 4 * (size_t)(c->plan.ok ? c->plan.ntiles : 1) + 256, 256);
+        const size_t bytes = (nfields * fd + scratch_d + 32) * sizeof(double) + flags_b;
+        c->slab = c10::cuda::CUDACachingAllocator::raw_alloc_with_stream(bytes, c->st);
+        if (!c->slab) throw (int)CAV_ENOMEM;
+        if (cudaMemsetAsync(c->slab, 0, bytes, c->st) != cudaSuccess) throw (int)CAV_ECUDA;
+        double* p = (double*)c->slab;
+        c->psi = p; p += fd;
+        c->psi_alt = p; p += fd;
+        c->q = p; p += fd;
+        for (int k = 0; k < 5; ++k) { c->w[k] = p; p += fd; }
+        c->T = p; p += fd;
+        c->scratch = p; p += scratch_d;
+        c->out4 = p; p += 32;
+        c->flags = (unsigned int*)p;
+        if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) throw (int)CAV_ECUDA;
+        if (cudaStreamSynchronize(c->st) != cudaSuccess) throw (int)CAV_ECUDA;
+        resolve_engine(c);
+    } catch (int code) {
+        rc = code;
+    } catch (const std::bad_alloc&) {
+        rc = CAV_ENOMEM;
+    } catch (const std::exception& ex) {
+        // c10 reports out-of-memory and missing-driver conditions as exceptions
+        rc = (std::strstr(ex.what(), "out of memory") != nullptr) ? CAV_ENOMEM : CAV_ECUDA;
+    } catch (...) {
+        rc = CAV_ECUDA;
+    }
+    if (rc != CAV_OK) { cudaGetLastError(); cav_destroy(c); return rc; }
+    *out = c;
+    return CAV_OK;
+}
+
+CAV_API void cav_destroy(cav_ctx* c) {
+    if (!c) return;
+    {
+        DeviceGuard dg(c->device);
+        if (c->st || c->slab) cudaStreamSynchronize(c->st);
+        drop_graph(c);
+        if (c->ev0) cudaEventDestroy(c->ev0);
+        if (c->ev1) cudaEventDestroy(c->ev1);
+        if (c->slab) {
+            try { c10::cuda::CUDACachingAllocator::raw_delete(c->slab); } catch (...) {}
+        }
+        cudaGetLastError();
+    }
+    delete c;
+}
+
+CAV_API int cav_set_fields(cav_ctx* c, const double* psi, const double* omega) {
+    if (!c || !omega) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    const int N = c->N;
+    const size_t row = (size_t)(N + 1) * sizeof(double), dp = (size_t)c->P.pitch * sizeof(double);
+    long long nl = 0;
+    if (psi) CK(cudaMemcpy2DAsync(c->psi, dp, psi, row, row, N + 1, cudaMemcpyHostToDevice, c->st));
+    else CK(cudaMemsetAsync(c->psi, 0, c->field_doubles * sizeof(double), c->st));
+    LAUNCH(cavk::zero_ring(c->P, c->psi, c->st));                   // psi = 0 on the walls (eq 23-24)
+    CK(cudaMemcpy2DAsync(c->w[0], dp, omega, row, row, N + 1, cudaMemcpyHostToDevice, c->st));
+    c->launches += nl;
+    c->step = 0;
+    CK(cudaStreamSynchronize(c->st));
+    return CAV_OK;
+}
+
+CAV_API int cav_get_fields(cav_ctx* c, double* psi_out, double* omega_out) {
+    if (!c) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    const int N = c->N;
+    const size_t row = (size_t)(N + 1) * sizeof(double), dp = (size_t)c->P.pitch * sizeof(double);
+    if (psi_out) CK(cudaMemcpy2DAsync(psi_out, row, c->psi, dp, row, N + 1, cudaMemcpyDeviceToHost, c->st));
+    if (omega_out) CK(cudaMemcpy2DAsync(omega_out, row, c->w[0], dp, row, N + 1, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    return CAV_OK;
+}
+
+CAV_API int cav_step(cav_ctx* c, int nsteps) { return step_impl(c, nsteps, true); }
+CAV_API int cav_step_async(cav_ctx* c, int nsteps) { return step_impl(c, nsteps, false); }
+
+CAV_API int cav_sync(cav_ctx* c) {
+    if (!c) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    CK(cudaStreamSynchronize(c->st));
+    return CAV_OK;
+}
+
+CAV_API int cav_poisson(cav_ctx* c, int nsweeps, double* res_inf_out) {
+    if (!c || nsweeps < 0) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    resolve_engine(c);
+    long long nl = 0;
+    CK(cudaEventRecord(c->ev0, c->st));
+    LAUNCH(cavk::scale_rhs(c->P, c->w[0], c->q, c->st));
+    int rc = enqueue_sweeps(c, nsweeps, nl);
+    if (rc != CAV_OK) { c->launches += nl; return rc; }
+    LAUNCH(cavk::thom_ring(c->P, c->psi, c->w[0], c->st));
+    CK(cudaEventRecord(c->ev1, c->st));
+    c->timed = true;
+    double r = 0.0;
+    if (res_inf_out) {
+        LAUNCH(cavk::diagnostics(c->P, c->psi, c->w[0], c->scratch, c->out4, c->st));
+        CK(cudaMemcpyAsync(&r, c->out4, sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    }
+    c->launches += nl;
+    CK(cudaStreamSynchronize(c->st));
+    if (res_inf_out) *res_inf_out = r;
+    return CAV_OK;
+}
+
+CAV_API int cav_get_diag(cav_ctx* c, cav_diag* out) {
+    if (!c || !out) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    long long nl = 0;
+    double r[4] = {0, 0, 0, 0};
+    LAUNCH(cavk::diagnostics(c->P, c->psi, c->w[0], c->scratch, c->out4, c->st));
+    c->launches += nl;
+    CK(cudaMemcpyAsync(r, c->out4, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    out->t = (double)c->step * c->dt;
+    out->step = c->step;
+    out->res_inf = r[0]; out->res_l2 = r[1]; out->kinetic_energy = r[2]; out->enstrophy = r[3];
+    return CAV_OK;
+}
+
+CAV_API int cav_set_engine(cav_ctx* c, int engine) {
+    if (!c || engine < CAV_ENGINE_AUTO || engine > CAV_ENGINE_RESIDENT) return CAV_EINVAL;
+    if (engine == CAV_ENGINE_RESIDENT && !c->plan.ok) return CAV_ENOTSUP;
+    DeviceGuard dg(c->device);
+    CK(cudaStreamSynchronize(c->st));
+    c->engine_req = engine;
+    resolve_engine(c);
+    return CAV_OK;
+}
+
+CAV_API int cav_describe(cav_ctx* c, char* buf, int len) {
+    if (!c || !buf || len < 1) return CAV_EINVAL;
+    resolve_engine(c);
+    std::string s;
+    char tmp[512];
+    std::snprintf(tmp, sizeof tmp, "grid %dx%d pitch %d S %d engine %s", c->N + 1, c->N + 1, c->P.pitch, c->S,
+                  c->engine == CAV_ENGINE_RESIDENT ? "resident" : "stream");
+    s = tmp;
+    if (c->plan.ok) { cavk::resident_describe(c->plan, tmp, sizeof tmp); s += " | resident plan: "; s += tmp; }
+    else s += " | resident plan: unavailable";
+    std::snprintf(buf, (size_t)len, "%s", s.c_str());
+    return CAV_OK;
+}
+
+CAV_API long long cav_launch_count(cav_ctx* c) { return c ? c->launches : 0; }
+
+CAV_API int cav_last_elapsed_ms(cav_ctx* c, float* ms_out) {
+    if (!c || !ms_out) return CAV_EINVAL;
+    *ms_out = 0.0f;
+    if (!c->timed) return CAV_OK;
+    DeviceGuard dg(c->device);
+    CK(cudaEventSynchronize(c->ev1));
+    CK(cudaEventElapsedTime(ms_out, c->ev0, c->ev1));
+    return CAV_OK;
+}
+
+CAV_API const char* cav_strerror(int code) {
+    switch (code) {
+        case CAV_OK: return "ok";
+        case CAV_EINVAL: return "invalid argument";
+        case CAV_ENOMEM: return "out of memory";
+        case CAV_ECUDA: return "CUDA error or no usable CUDA device";
+        case CAV_ENOTSUP: return "engine not supported for this problem on this device";
+        default: return "unknown error";
+    }
+}

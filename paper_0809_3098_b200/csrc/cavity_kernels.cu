@@ -1,0 +1,265 @@
+// cavity_kernels.cu — support kernels (a2, a3, a4) and the streaming sweep engine (a1) for sm_100a.
+//
+// Build with -fmad=false: every fused multiply-add below is an explicit fma(), so the expression
+// association is exactly the one DESIGN.md "Canonical arithmetic" states (and tests compare bit for bit).
+// P:n = /root/reference/PAPER.md line n.
+#include "cavity_kernels.cuh"
+
+namespace cavk {
+
+namespace {
+
+// SSPRK(5,4) in Shu-Osher form, eq 9-13 P:85-108.  eq 9's constant is printed with 11 digits and eq 10's
+// second weight with a wrong digit (0.555626...); the values below are the 15-digit ones of the paper's
+// ref [23], which make every stage's weights sum to 1 (readings G1, G2).
+__device__ constexpr double RK1_C  = 0.391752226571890;
+__device__ constexpr double RK2_A0 = 0.444370493651235, RK2_A1 = 0.555629506348765, RK2_C = 0.368410593050371;
+__device__ constexpr double RK3_A0 = 0.620101851488403, RK3_A2 = 0.379898148511597, RK3_C = 0.251891774271694;
+__device__ constexpr double RK4_A0 = 0.178079954393132, RK4_A3 = 0.821920045606868, RK4_C = 0.544974750228521;
+__device__ constexpr double RK5_A2 = 0.517231671970585, RK5_A3 = 0.096059710526147, RK5_C3 = 0.063692468666290;
+__device__ constexpr double RK5_A4 = 0.386708617503269, RK5_C4 = 0.226007483236906;
+
+inline int cdiv(int a, int b) { return (a + b - 1) / b; }
+
+inline int launched(int n) {
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? n : -(int)e;
+}
+
+// ---- q = cq * w --------------------------------------------------------------------------------------
+__global__ void k_scale_rhs(int N, int pitch, double cq, const double* __restrict__ w, double* __restrict__ q) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i > N || j > N) return;
+    const size_t k = (size_t)j * pitch + i;
+    const bool interior = (i >= 1) & (i <= N - 1) & (j >= 1) & (j <= N - 1);
+    q[k] = interior ? cq * w[k] : 0.0;
+}
+
+// ---- a2: Thom ring, eq 25 P:161-169 ------------------------------------------------------------------
+__device__ __forceinline__ double thom_wall(double c2h2, double p_adj) { return -(c2h2 * p_adj); }
+__device__ __forceinline__ double thom_lid(double c2h2, double lid, double p_adj) { return -(c2h2 * p_adj) - lid; }
+
+__global__ void k_thom_ring(int N, int pitch, double c2h2, double lid, const double* __restrict__ psi,
+                            double* __restrict__ w) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t <= N) {                                    // bottom and top rows own the corners (G10)
+        w[t] = thom_wall(c2h2, psi[(size_t)pitch + t]);
+        w[(size_t)N * pitch + t] = thom_lid(c2h2, lid, psi[(size_t)(N - 1) * pitch + t]);
+    }
+    if (t >= 1 && t <= N - 1) {                      // side walls, j = 1..N-1
+        w[(size_t)t * pitch] = thom_wall(c2h2, psi[(size_t)t * pitch + 1]);
+        w[(size_t)t * pitch + N] = thom_wall(c2h2, psi[(size_t)t * pitch + N - 1]);
+    }
+}
+
+__global__ void k_zero_ring(int N, int pitch, double* __restrict__ psi) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t <= N) {
+        psi[t] = 0.0;
+        psi[(size_t)N * pitch + t] = 0.0;
+        psi[(size_t)t * pitch] = 0.0;
+        psi[(size_t)t * pitch + N] = 0.0;
+    }
+}
+
+// ---- a2 + a3: transport right-hand side and the stage combination ------------------------------------
+template <int K>
+__global__ void __launch_bounds__(256)
+k_rk_stage(Params P, const double* __restrict__ psi, const double* __restrict__ w_in, const double* __restrict__ a,
+           const double* __restrict__ b, double* __restrict__ w_out, double* __restrict__ t_out) {
+    const int N = P.N, pitch = P.pitch;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i > N || j > N) return;
+    const size_t k = (size_t)j * pitch + i;
+
+    if (j == 0) { w_out[k] = thom_wall(P.c2h2, psi[k + pitch]); return; }
+    if (j == N) { w_out[k] = thom_lid(P.c2h2, P.lid, psi[k - pitch]); return; }
+    if (i == 0) { w_out[k] = thom_wall(P.c2h2, psi[k + 1]); return; }
+    if (i == N) { w_out[k] = thom_wall(P.c2h2, psi[k - 1]); return; }
+
+    const double pW = psi[k - 1], pE = psi[k + 1], pS = psi[k - pitch], pN = psi[k + pitch];
+    const double w0 = w_in[k];
+    double wW, wE, wS, wN;
+    if (i == 1 || i == N - 1 || j == 1 || j == N - 1) {
+        // the wall value next to this point is Thom's formula applied to this point's own psi
+        const double p0 = psi[k];
+        wW = (i == 1) ? thom_wall(P.c2h2, p0) : w_in[k - 1];
+        wE = (i == N - 1) ? thom_wall(P.c2h2, p0) : w_in[k + 1];
+        wS = (j == 1) ? thom_wall(P.c2h2, p0) : w_in[k - pitch];
+        wN = (j == N - 1) ? thom_lid(P.c2h2, P.lid, p0) : w_in[k + pitch];
+    } else {
+        wW = w_in[k - 1]; wE = w_in[k + 1]; wS = w_in[k - pitch]; wN = w_in[k + pitch];
+    }
+    // eq 22: u = dpsi/dy, v = -dpsi/dx;  eq 8
+    const double u = (pN - pS) * P.i2h;
+    const double v = (pW - pE) * P.i2h;
+    const double wx = (wE - wW) * P.i2h;
+    const double wy = (wN - wS) * P.i2h;
+    const double lap = (((wW + wE) + (wS + wN)) - 4.0 * w0) * P.ih2;
+    const double L = fma(P.nu, lap, -fma(u, wx, v * wy));
+    const double dL = P.dt * L;
+
+    if (K == 1) {
+        w_out[k] = fma(RK1_C, dL, w0);                                              // eq 9
+    } else if (K == 2) {
+        w_out[k] = fma(RK2_C, dL, fma(RK2_A1, w0, RK2_A0 * a[k]));                  // eq 10 (w0 here is omega^(1))
+    } else if (K == 3) {
+        w_out[k] = fma(RK3_C, dL, fma(RK3_A2, w0, RK3_A0 * a[k]));                  // eq 11
+    } else if (K == 4) {
+        w_out[k] = fma(RK4_C, dL, fma(RK4_A3, w0, RK4_A0 * a[k]));                  // eq 12
+        t_out[k] = fma(RK5_C3, dL, fma(RK5_A3, w0, RK5_A2 * b[k]));                 // eq 13, first three terms
+    } else {
+        w_out[k] = fma(RK5_C4, dL, fma(RK5_A4, w0, a[k]));                          // eq 13, the rest (a = T)
+    }
+}
+
+// ---- a4: diagnostics ----------------------------------------------------------------------------------
+constexpr int DIAG_BLOCKS = 296;
+constexpr int DIAG_THREADS = 256;
+
+__device__ __forceinline__ double warp_sum(double v) {
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+    return v;
+}
+
+// block-level reduction of (max, sum, sum, sum); result valid in thread 0
+__device__ __forceinline__ void block_reduce4(double& m, double& s1, double& s2, double& s3) {
+    __shared__ double sh[4][DIAG_THREADS / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    m = warp_max(m); s1 = warp_sum(s1); s2 = warp_sum(s2); s3 = warp_sum(s3);
+    if (lane == 0) { sh[0][wid] = m; sh[1][wid] = s1; sh[2][wid] = s2; sh[3][wid] = s3; }
+    __syncthreads();
+    if (wid == 0) {
+        const int nw = blockDim.x >> 5;
+        m = lane < nw ? sh[0][lane] : 0.0;
+        s1 = lane < nw ? sh[1][lane] : 0.0;
+        s2 = lane < nw ? sh[2][lane] : 0.0;
+        s3 = lane < nw ? sh[3][lane] : 0.0;
+        m = warp_max(m); s1 = warp_sum(s1); s2 = warp_sum(s2); s3 = warp_sum(s3);
+    }
+}
+
+__global__ void __launch_bounds__(DIAG_THREADS)
+k_diag_partial(int N, int pitch, const double* __restrict__ psi, const double* __restrict__ w,
+               double* __restrict__ scratch) {
+    const double h = 1.0 / (double)N;
+    const double h2 = h * h, twoh = 2.0 * h;
+    const long long M = (long long)(N - 1) * (N - 1);
+    double m = 0.0, s_r2 = 0.0, s_ke = 0.0, s_en = 0.0;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < M; t += (long long)gridDim.x * blockDim.x) {
+        const int j = 1 + (int)(t / (N - 1)), i = 1 + (int)(t % (N - 1));
+        const size_t k = (size_t)j * pitch + i;
+        const double pW = psi[k - 1], pE = psi[k + 1], pS = psi[k - pitch], pN = psi[k + pitch], p = psi[k];
+        const double wv = w[k];
+        const double r = (pW + pE + pS + pN - 4.0 * p) / h2 + wv;       // S8(a) row a4
+        const double u = (pN - pS) / twoh;
+        const double v = -(pE - pW) / twoh;
+        m = fmax(m, fabs(r));
+        s_r2 = fma(r, r, s_r2);
+        s_ke += fma(u, u, v * v);
+        s_en = fma(wv, wv, s_en);
+    }
+    block_reduce4(m, s_r2, s_ke, s_en);
+    if (threadIdx.x == 0) {
+        scratch[0 * DIAG_BLOCKS + blockIdx.x] = m;
+        scratch[1 * DIAG_BLOCKS + blockIdx.x] = s_r2;
+        scratch[2 * DIAG_BLOCKS + blockIdx.x] = s_ke;
+        scratch[3 * DIAG_BLOCKS + blockIdx.x] = s_en;
+    }
+}
+
+// second stage: one block, fixed order (deterministic; no floating-point atomics anywhere)
+__global__ void __launch_bounds__(DIAG_THREADS)
+k_diag_final(int N, const double* __restrict__ scratch, double* __restrict__ out4) {
+    double m = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    for (int t = threadIdx.x; t < DIAG_BLOCKS; t += blockDim.x) {
+        m = fmax(m, scratch[t]);
+        s1 += scratch[DIAG_BLOCKS + t];
+        s2 += scratch[2 * DIAG_BLOCKS + t];
+        s3 += scratch[3 * DIAG_BLOCKS + t];
+    }
+    block_reduce4(m, s1, s2, s3);
+    if (threadIdx.x == 0) {
+        const double h = 1.0 / (double)N;
+        const double h2 = h * h;
+        out4[0] = m;
+        out4[1] = sqrt(h2 * s1);
+        out4[2] = 0.5 * h2 * s2;
+        out4[3] = 0.5 * h2 * s3;
+    }
+}
+
+// ---- a1, stream engine: one colour half-sweep over global memory --------------------------------------
+// eq 15-21 P:114-138 reduced to the 5-point operator (D1-D3):
+//   psi <- (1 - beta) psi + (beta/4) (psi_W + psi_E + psi_S + psi_N) + (beta/4) h^2 omega
+__global__ void __launch_bounds__(256)
+k_half_sweep(int N, int pitch, double cb, double omb, double* __restrict__ psi, const double* __restrict__ q,
+             int colour) {
+    const int j = 1 + blockIdx.y * blockDim.y + threadIdx.y;
+    if (j > N - 1) return;
+    const int i0 = (((1 + j) & 1) == colour) ? 1 : 2;
+    const int i = i0 + 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+    if (i > N - 1) return;
+    const size_t k = (size_t)j * pitch + i;
+    const double nb = (psi[k - 1] + psi[k + 1]) + (psi[k - pitch] + psi[k + pitch]);
+    psi[k] = fma(omb, psi[k], fma(cb, nb, q[k]));
+}
+
+}  // namespace
+
+int scale_rhs(const Params& P, const double* w, double* q, cudaStream_t st) {
+    dim3 b(32, 8), g(cdiv(P.N + 1, 32), cdiv(P.N + 1, 8));
+    k_scale_rhs<<<g, b, 0, st>>>(P.N, P.pitch, P.cq, w, q);
+    return launched(1);
+}
+
+int thom_ring(const Params& P, const double* psi, double* w, cudaStream_t st) {
+    k_thom_ring<<<cdiv(P.N + 1, 128), 128, 0, st>>>(P.N, P.pitch, P.c2h2, P.lid, psi, w);
+    return launched(1);
+}
+
+int zero_ring(const Params& P, double* psi, cudaStream_t st) {
+    k_zero_ring<<<cdiv(P.N + 1, 128), 128, 0, st>>>(P.N, P.pitch, psi);
+    return launched(1);
+}
+
+int rk_stage(const Params& P, int k, const double* psi, const double* w_in, const double* a, const double* b,
+             double* w_out, double* t_out, cudaStream_t st) {
+    dim3 bl(32, 8), g(cdiv(P.N + 1, 32), cdiv(P.N + 1, 8));
+    switch (k) {
+        case 1: k_rk_stage<1><<<g, bl, 0, st>>>(P, psi, w_in, a, b, w_out, t_out); break;
+        case 2: k_rk_stage<2><<<g, bl, 0, st>>>(P, psi, w_in, a, b, w_out, t_out); break;
+        case 3: k_rk_stage<3><<<g, bl, 0, st>>>(P, psi, w_in, a, b, w_out, t_out); break;
+        case 4: k_rk_stage<4><<<g, bl, 0, st>>>(P, psi, w_in, a, b, w_out, t_out); break;
+        case 5: k_rk_stage<5><<<g, bl, 0, st>>>(P, psi, w_in, a, b, w_out, t_out); break;
+        default: return -(int)cudaErrorInvalidValue;
+    }
+    return launched(1);
+}
+
+int diag_scratch_doubles() { return DIAG_BLOCKS; }
+
+int diagnostics(const Params& P, const double* psi, const double* w, double* scratch_dev, double* out4_dev,
+                cudaStream_t st) {
+    k_diag_partial<<<DIAG_BLOCKS, DIAG_THREADS, 0, st>>>(P.N, P.pitch, psi, w, scratch_dev);
+    k_diag_final<<<1, DIAG_THREADS, 0, st>>>(P.N, scratch_dev, out4_dev);
+    return launched(2);
+}
+
+int stream_sweeps(const Params& P, double* psi, const double* q, int nsweeps, cudaStream_t st) {
+    const int per_row = (P.N - 1 + 1) / 2;
+    dim3 b(64, 4), g(cdiv(per_row, 64), cdiv(P.N - 1, 4));
+    for (int s = 0; s < nsweeps; ++s) {
+        k_half_sweep<<<g, b, 0, st>>>(P.N, P.pitch, P.cb, P.omb, psi, q, 0);   // red = (i + j) even first (G9)
+        k_half_sweep<<<g, b, 0, st>>>(P.N, P.pitch, P.cb, P.omb, psi, q, 1);
+    }
+    return launched(2 * nsweeps);
+}
+
+}  // namespace cavk

@@ -1,0 +1,59 @@
+// cavity_kernels.cuh — launchers of the sm_100a kernels behind include/cavity.h.
+// Plain CUDA: no torch types.  Every launcher enqueues on `st` and returns the number of kernel
+// launches it made (negative = cudaError_t negated).
+//
+// P:n = /root/reference/PAPER.md line n.  Device layout of a field:
+// element (i, j) lives at  j * pitch + i,  pitch = (N + 1) rounded up to a multiple of 4 doubles, so that
+// every row starts on a 32-byte sector boundary; the base pointer is 256-byte aligned.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace cavk {
+
+// Constants of one problem, computed once on the host (cavity_api.cu: make_params).
+struct Params {
+    int N;          // intervals per side
+    int pitch;      // doubles per device row
+    double cb;      // beta / 4
+    double cq;      // (beta / 4) h^2                (scales omega into the sweep's right-hand side q)
+    double omb;     // 1 - beta
+    double i2h;     // 1 / (2h) = N / 2
+    double ih2;     // 1 / h^2 = N^2
+    double nu;      // 1 / Re
+    double c2h2;    // 2 / h^2                       (eq 25)
+    double lid;     // 2 U / h, U = 1                (eq 25, lid term)
+    double dt;
+};
+
+// ---- support kernels (both engines) ---------------------------------------------------------------
+// q_ij = cq * w_ij on interior points (the per-stage right-hand side of a1; constant over the S sweeps).
+int scale_rhs(const Params& P, const double* w, double* q, cudaStream_t st);
+
+// a2: Thom ring of w from psi (eq 25; corners owned by the top/bottom rows, G10).
+int thom_ring(const Params& P, const double* psi, double* w, cudaStream_t st);
+
+// a2 + a3 fused, stage k = 1..5 (eq 8, eq 22, eq 9-13).  The wall vorticity a near-wall
+// point needs is evaluated on the fly from psi by the same formula thom_ring uses; ring threads store it to
+// the ring of w_out.  Pointer roles per stage:
+//   k=1: w_in = w0                         -> w_out = w1
+//   k=2: w_in = w1, a = w0                 -> w_out = w2
+//   k=3: w_in = w2, a = w0                 -> w_out = w3
+//   k=4: w_in = w3, a = w0, b = w2         -> w_out = w4, t_out = T   (first three terms of eq 13)
+//   k=5: w_in = w4, a = T                  -> w_out = omega^{n+1} (may alias w0: only pointwise access to it)
+int rk_stage(const Params& P, int k, const double* psi, const double* w_in, const double* a, const double* b,
+             double* w_out, double* t_out, cudaStream_t st);
+
+// a4: res_inf, res_l2, kinetic energy, enstrophy -> out4_dev[0..3] (device).  scratch_dev must hold
+// 4 * diag_scratch_doubles() doubles.
+int diag_scratch_doubles();
+int diagnostics(const Params& P, const double* psi, const double* w, double* scratch_dev, double* out4_dev,
+                cudaStream_t st);
+
+// forces the wall ring of psi to +0.0 (cav_set_fields)
+int zero_ring(const Params& P, double* psi, cudaStream_t st);
+
+// ---- stream engine: one kernel per colour half-sweep ----------------------------------------------
+// nsweeps x (red half-sweep, black half-sweep) of a1 on psi in place, right-hand side q (already scaled).
+int stream_sweeps(const Params& P, double* psi, const double* q, int nsweeps, cudaStream_t st);
+
+}  // namespace cavk

@@ -1,0 +1,312 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle, element by
+element on the same seeded inputs.
+
+Two bars:
+  * the contract of BASELINE.json north_star: max-norm relative error <= 1e-10 in psi and omega against the
+    oracle's PLAIN mode (formulas as the paper prints them, no fused multiply-add);
+  * bit for bit against the oracle's FMA mode, which associates every expression the way the kernels do
+    (SURVEY.md Appendix A): a red-black sweep has no order dependence inside a colour, so tiling, temporal
+    blocking and thread order may not change a single bit.  Any difference is an indexing / halo / barrier bug.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from paper_0809_3098_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10          # BASELINE.json north_star: "max relative error of 1e-10 in psi and omega"
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.fixture(scope="module")
+def cav():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    from paper_0809_3098_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def orc():
+    import oracle
+    oracle.lib()
+    return oracle
+
+
+def relerr(a, b):
+    """max-norm relative error (reading G18): max |a - b| / max |b|."""
+    den = float(np.max(np.abs(b)))
+    return float(np.max(np.abs(a - b))) / (den if den > 0 else 1.0)
+
+
+def engines(cav, N):
+    """engines that can run this grid on this device"""
+    out = ["stream"]
+    c = cav.Cavity(N, 100.0, 1e-3, 1.5, 1)
+    try:
+        c.set_engine("resident")
+        out.append("resident")
+    except cav.CavityError:
+        pass
+    c.close()
+    return out
+
+
+def random_fields(N, seed, amp_psi=0.05, amp_w=3.0):
+    u = W.lcg_uniform(seed, 2 * (N + 1) * (N + 1)).reshape(2, N + 1, N + 1)
+    psi = amp_psi * (2.0 * u[0] - 1.0)
+    w = amp_w * (2.0 * u[1] - 1.0)
+    return psi, w
+
+
+def run_pair(cav, orc, N, Re, dt, beta, S, nsteps, psi0, w0, mode, engine, poisson=0):
+    g = cav.Cavity(N, Re, dt, beta, S, engine=engine)
+    o = orc.OracleCavity(N, Re, dt, beta, S, mode)
+    g.set_fields(psi0, w0)
+    o.set_fields(psi0, w0)
+    if poisson:
+        g.poisson(poisson)
+        o.poisson(poisson)
+    g.step(nsteps)
+    o.step(nsteps)
+    out = g.get_fields(), o.get_fields(), g.diag(), o.diag()
+    g.close()
+    o.close()
+    return out
+
+
+# ------------------------------------------------------------------------------------------------------
+# bit-exact against the FMA-mode oracle: many grid sizes (odd, even, not powers of two, tiny), random fields
+# ------------------------------------------------------------------------------------------------------
+
+SIZES = [2, 3, 4, 5, 8, 9, 17, 31, 32, 33, 64, 100, 127, 128, 129, 219, 257, 299]     # 219 / 299: the paper's 220^2 / 300^2 grids
+
+
+@pytest.mark.parametrize("N", SIZES)
+def test_step_bit_exact_fma_oracle(cav, orc, N):
+    psi0, w0 = random_fields(N, 1000 + N)
+    for S in (0, 1, 7):
+        nsteps = 2 if N > 150 else 3
+        for engine in engines(cav, N):
+            (gp, gw), (op, ow), _, _ = run_pair(cav, orc, N, 400.0, 0.4 / N, 1.7, S, nsteps, psi0, w0, orc.MODE_FMA,
+                                                engine)
+            assert np.array_equal(gp, op), (N, S, engine, np.max(np.abs(gp - op)))
+            assert np.array_equal(gw, ow), (N, S, engine, np.max(np.abs(gw - ow)))
+
+
+@pytest.mark.parametrize("N,nsweeps", [(2, 3), (7, 1), (33, 40), (130, 25), (257, 33), (300, 64), (513, 17)])
+def test_poisson_bit_exact_fma_oracle(cav, orc, N, nsweeps):
+    psi0, w0 = random_fields(N, 77 + N)
+    for engine in engines(cav, N):
+        g = cav.Cavity(N, 100.0, 1e-3, 1.93, 5, engine=engine)
+        o = orc.OracleCavity(N, 100.0, 1e-3, 1.93, 5, orc.MODE_FMA)
+        g.set_fields(psi0, w0)
+        o.set_fields(psi0, w0)
+        rg = g.poisson(nsweeps)
+        ro = o.poisson(nsweeps)
+        gp, gw = g.get_fields()
+        op, ow = o.get_fields()
+        assert np.array_equal(gp, op), (N, engine)
+        assert np.array_equal(gw, ow), (N, engine)          # the Thom ring after cav_poisson
+        assert abs(rg - ro) <= 1e-9 * max(1.0, abs(ro))
+        g.close()
+        o.close()
+
+
+def test_config1_full_length_bit_exact_and_contract(cav, orc):
+    wl = W.config(1)
+    psi0, w0 = W.initial_fields(wl)
+    for engine in engines(cav, wl.N):
+        (gp, gw), (op, ow), _, _ = run_pair(cav, orc, wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage, wl.steps,
+                                            psi0, w0, orc.MODE_FMA, engine)
+        assert np.array_equal(gp, op) and np.array_equal(gw, ow), engine
+        (gp, gw), (op, ow), gd, od = run_pair(cav, orc, wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage,
+                                              wl.steps, psi0, w0, orc.MODE_PLAIN, engine)
+        assert relerr(gp, op) <= TOL and relerr(gw, ow) <= TOL, (engine, relerr(gp, op), relerr(gw, ow))
+        I = (slice(1, wl.N), slice(1, wl.N))
+        assert relerr(gw[I], ow[I]) <= TOL
+        for key in ("res_inf", "res_l2", "kinetic_energy", "enstrophy"):
+            assert abs(gd[key] - od[key]) <= 1e-9 * abs(od[key]), key
+        assert gd["step"] == od["step"] == wl.steps and abs(gd["t"] - od["t"]) < 1e-12
+
+
+def test_config2_contract_full_length(cav, orc):
+    # 2000 steps of the 129 x 129 grid: the oracle needs ~40 s of one host core
+    wl = W.config(2)
+    psi0, w0 = W.initial_fields(wl)
+    o = orc.OracleCavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage, orc.MODE_PLAIN)
+    o.set_fields(psi0, w0)
+    gs = {e: cav.Cavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage, engine=e) for e in engines(cav, wl.N)}
+    for g in gs.values():
+        g.set_fields(psi0, w0)
+    done = 0
+    for cp in (1, 10, 100, 1000, 2000):
+        o.step(cp - done)
+        op, ow = o.get_fields()
+        for e, g in gs.items():
+            g.step(cp - done)
+            gp, gw = g.get_fields()
+            assert relerr(gp, op) <= TOL and relerr(gw, ow) <= TOL, (e, cp, relerr(gp, op), relerr(gw, ow))
+        done = cp
+    for g in gs.values():
+        g.close()
+    o.close()
+
+
+# ------------------------------------------------------------------------------------------------------
+# full-size configs in the launch configuration bench.py times, against stored oracle values
+# (tests/golden/cfgK.json, written by tests/golden/make_golden.py from oracle/ only): sampled points and a4.
+# ------------------------------------------------------------------------------------------------------
+
+def check_against_golden(cav, k, engine, max_step=None):
+    path = os.path.join(GOLDEN, "cfg%d.json" % k)
+    if not os.path.exists(path):
+        pytest.skip("tests/golden/cfg%d.json has not been generated" % k)
+    gold = json.load(open(path))
+    wl = W.config(k)
+    assert gold["N"] == wl.N and gold["seed"] == wl.seed and gold["sweeps_per_stage"] == wl.sweeps_per_stage
+    g = cav.Cavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage, engine=engine)
+    g.set_fields(*W.initial_fields(wl))
+    done = 0
+    checked = 0
+    for cp in gold["checkpoints"]:
+        if cp["label"] == "poisson":
+            g.poisson(wl.poisson_sweeps)
+        else:
+            if max_step is not None and cp["step"] > max_step:
+                break
+            g.step(cp["step"] - done)
+            done = cp["step"]
+        psi, w = g.get_fields()
+        s = np.array(cp["sample_index"])
+        ps, ws = psi[np.ix_(s, s)], w[np.ix_(s, s)]
+        ep = np.max(np.abs(ps - np.array(cp["psi"]))) / cp["psi_absmax"]
+        ew = np.max(np.abs(ws - np.array(cp["omega"]))) / cp["omega_absmax"]
+        inner = slice(1, len(s) - 1)
+        ewi = np.max(np.abs(ws[inner, inner] - np.array(cp["omega"])[inner, inner])) / cp["omega_absmax_interior"]
+        assert ep <= TOL and ew <= TOL and ewi <= TOL, (k, engine, cp["label"], ep, ew, ewi)
+        d = g.diag()
+        for key in ("kinetic_energy", "enstrophy", "res_l2", "res_inf"):
+            assert abs(d[key] - cp[key]) <= 1e-8 * abs(cp[key]), (k, engine, cp["label"], key, d[key], cp[key])
+        assert abs(np.max(np.abs(psi)) - cp["psi_absmax"]) <= TOL * cp["psi_absmax"]
+        assert abs(np.min(psi) - cp["psi_min"]) <= TOL * cp["psi_absmax"]
+        # invariants that hold at any size: psi is exactly 0 on the walls
+        assert not psi[0].any() and not psi[-1].any() and not psi[:, 0].any() and not psi[:, -1].any()
+        checked += 1
+    g.close()
+    assert checked > 0
+
+
+@pytest.mark.parametrize("k", [2, 3, 4, 5])
+def test_full_size_configs_against_golden(cav, k):
+    eng = engines(cav, W.config(k).N)
+    # the default (auto) engine is the one bench.py times; the streaming engine is checked on the early checkpoints
+    check_against_golden(cav, k, "auto")
+    if len(eng) > 1:
+        check_against_golden(cav, k, "stream", max_step=10)
+
+
+@pytest.mark.parametrize("N,S,nsteps", [(1024, 200, 2), (512, 100, 3), (1000, 37, 2), (219, 50, 4)])
+def test_engines_agree_bit_for_bit_at_full_size(cav, N, S, nsteps):
+    eng = engines(cav, N)
+    if len(eng) < 2:
+        pytest.skip("only one engine can run this grid")
+    psi0, w0 = random_fields(N, 4242 + N)
+    res = []
+    for e in eng:
+        g = cav.Cavity(N, 5000.0, 0.5 / N, 1.99, S, engine=e)
+        g.set_fields(psi0, w0)
+        g.step(nsteps)
+        res.append(g.get_fields())
+        g.close()
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
+
+
+# ------------------------------------------------------------------------------------------------------
+# properties and edge cases
+# ------------------------------------------------------------------------------------------------------
+
+def test_poisson_manufactured_solution_on_gpu(cav):
+    # omega = 2 pi^2 sin(pi x) sin(pi y): the exact DISCRETE solution is omega / lambda_h (closed form)
+    import math
+    for N in (16, 64, 200):
+        k = np.arange(N + 1) / N
+        X, Y = np.meshgrid(k, k)
+        exact = np.sin(np.pi * X) * np.sin(np.pi * Y)
+        omega = 2.0 * np.pi ** 2 * exact
+        lam = (4.0 * N * N) * 2.0 * math.sin(math.pi / (2 * N)) ** 2
+        beta = 2.0 / (1.0 + math.sin(math.pi / N))
+        for engine in engines(cav, N):
+            g = cav.Cavity(N, 100.0, 1e-3, beta, 1, engine=engine)
+            g.set_fields(None, omega)
+            res = g.poisson(40 * N)
+            psi, _ = g.get_fields()
+            assert np.max(np.abs(psi - omega / lam)) < 1e-12, (N, engine)
+            assert res < 1e-8
+            g.close()
+
+
+def test_edge_cases(cav):
+    g = cav.Cavity(8, 10.0, 0.01, 1.5, 3)
+    psi0, w0 = random_fields(8, 5)
+    g.set_fields(psi0, w0)
+    p1, w1 = g.get_fields()
+    assert not p1[0].any() and not p1[-1].any() and not p1[:, 0].any() and not p1[:, -1].any()   # walls forced to 0
+    assert np.array_equal(p1[1:-1, 1:-1], psi0[1:-1, 1:-1]) and np.array_equal(w1, w0)            # ring of omega kept
+    g.step(0)                                             # no-op
+    p2, w2 = g.get_fields()
+    assert np.array_equal(p1, p2) and np.array_equal(w1, w2)
+    assert g.diag()["step"] == 0
+    with pytest.raises(cav.CavityError):
+        g.step(-1)
+    with pytest.raises(cav.CavityError):
+        g.poisson(-1)
+    assert cav.lib().cav_set_fields(g._h, None, None) == -1          # omega == NULL is CAV_EINVAL
+    g.step(2)
+    assert g.diag()["step"] == 2 and g.launch_count() > 0
+    g.set_fields(None, w0)                                # psi == NULL -> 0, counters reset
+    p3, _ = g.get_fields()
+    assert not p3.any() and g.diag()["step"] == 0
+    assert "grid 9x9" in g.describe()
+    g.close()
+    g.close()                                             # idempotent
+
+
+def test_lid_drives_the_flow_and_walls_stay_zero(cav):
+    # from rest, the only forcing is the lid term of eq 25: the primary vortex is clockwise (psi < 0)
+    g = cav.Cavity(64, 100.0, 0.2 / 64, 1.9, 30)
+    g.set_fields(None, np.zeros((65, 65)))
+    g.step(50)
+    psi, w = g.get_fields()
+    assert psi.min() < -1e-3 and abs(psi.max()) < 1e-3
+    assert np.all(w[-1, :] < 0) and w[-1, 32] < -2.0 * 64 * 0.5          # lid ring ~ -2U/h + ...
+    assert not psi[0].any() and not psi[-1].any() and not psi[:, 0].any() and not psi[:, -1].any()
+    assert np.isfinite(psi).all() and np.isfinite(w).all()
+    g.close()
+
+
+def test_two_contexts_are_independent(cav):
+    a = cav.Cavity(32, 100.0, 0.0156, 1.8, 20)
+    b = cav.Cavity(40, 300.0, 0.01, 1.7, 5)
+    pa, wa = random_fields(32, 1)
+    pb, wb = random_fields(40, 2)
+    a.set_fields(pa, wa)
+    b.set_fields(pb, wb)
+    a.step_async(3)
+    b.step_async(3)
+    a.sync()
+    b.sync()
+    ra = a.get_fields()
+    a2 = cav.Cavity(32, 100.0, 0.0156, 1.8, 20)
+    a2.set_fields(pa, wa)
+    a2.step(3)
+    r2 = a2.get_fields()
+    assert np.array_equal(ra[0], r2[0]) and np.array_equal(ra[1], r2[1])
+    assert a.last_elapsed_ms() > 0
+    for c in (a, b, a2):
+        c.close()
