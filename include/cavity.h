@@ -22,7 +22,8 @@
  * dense row-major (N+1) x (N+1) fp64 arrays, element k = j (N+1) + i.  Buffers are borrowed for the
  * duration of the call only.  Every call returns CAV_OK (0) or a negative CAV_E* code; nothing
  * throws across the ABI.  Device memory comes from PyTorch's CUDA caching allocator and all work is
- * enqueued on the PyTorch current stream of the device that was current at cav_create; every call
+ * enqueued on the PyTorch current stream of the device that was current at cav_create (the caller must
+ * have initialised PyTorch's CUDA state first: torch.cuda.init(); the Python binding does); every call
  * below is synchronous at return unless stated otherwise.  There is no CPU fallback: without a CUDA
  * device cav_create returns CAV_ECUDA.
  */
@@ -93,6 +94,12 @@ int cav_get_diag(cav_ctx* ctx, cav_diag* out);
 /* Selects the sweep engine (CAV_ENGINE_*).  CAV_ENOTSUP if that engine cannot run this grid on this
  * device.  The default is CAV_ENGINE_AUTO. */
 int cav_set_engine(cav_ctx* ctx, int engine);
+
+/* Resident engine only: forces T, the number of sweeps between two halo exchanges (even, 2..16; the halo is 2T
+ * points deep), and re-plans the tiling for it; 0 restores the planner's own choice.  The result of every
+ * other call is unchanged bit for bit; this is a tuning / testing knob.  CAV_ENOTSUP if no plan exists for that T
+ * (the previous plan is kept). */
+int cav_set_sweeps_per_exchange(cav_ctx* ctx, int sweeps_per_exchange);
 
 /* Describes the launch plan of the current engine in `buf` (NUL-terminated, truncated to len). */
 int cav_describe(cav_ctx* ctx, char* buf, int len);

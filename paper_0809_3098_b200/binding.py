@@ -15,7 +15,7 @@ _ENGINES = {"auto": ENGINE_AUTO, "stream": ENGINE_STREAM, "resident": ENGINE_RES
 
 # every symbol include/cavity.h declares
 SYMBOLS = ("cav_create", "cav_destroy", "cav_set_fields", "cav_get_fields", "cav_step", "cav_step_async", "cav_sync",
-           "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_describe", "cav_launch_count",
+           "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_set_sweeps_per_exchange", "cav_describe", "cav_launch_count",
            "cav_last_elapsed_ms", "cav_strerror")
 
 _lib = None
@@ -62,6 +62,7 @@ def lib():
     L.cav_poisson.argtypes = [C.c_void_p, C.c_int, dp]
     L.cav_get_diag.argtypes = [C.c_void_p, C.POINTER(CavDiag)]
     L.cav_set_engine.argtypes = [C.c_void_p, C.c_int]
+    L.cav_set_sweeps_per_exchange.argtypes = [C.c_void_p, C.c_int]
     L.cav_describe.argtypes = [C.c_void_p, C.c_char_p, C.c_int]
     L.cav_launch_count.argtypes = [C.c_void_p]
     L.cav_launch_count.restype = C.c_longlong
@@ -91,13 +92,19 @@ def _field(a, N, name):
 class Cavity:
     """One cav_ctx.  Fields are numpy (N+1, N+1) float64 arrays indexed [j, i] (row N = lid)."""
 
-    def __init__(self, N, Re, dt, sor_omega, sweeps_per_stage, engine="auto"):
+    def __init__(self, N, Re, dt, sor_omega, sweeps_per_stage, engine="auto", resident_T=0):
         self.N = int(N)
         self._h = C.c_void_p()
+        L = lib()
+        import torch
+        if torch.cuda.is_available():
+            torch.cuda.init()          # libcavity.so allocates through PyTorch's caching allocator
         _chk(lib().cav_create(C.byref(self._h), int(N), float(Re), float(dt), float(sor_omega),
                               int(sweeps_per_stage)), "cav_create")
         if engine != "auto":
             self.set_engine(engine)
+        if resident_T:
+            self.set_resident_T(resident_T)
 
     def close(self):
         if getattr(self, "_h", None):
@@ -119,6 +126,9 @@ class Cavity:
     def set_engine(self, engine):
         _chk(lib().cav_set_engine(self._h, _ENGINES[engine] if isinstance(engine, str) else int(engine)),
              "cav_set_engine")
+
+    def set_resident_T(self, T):
+        _chk(lib().cav_set_sweeps_per_exchange(self._h, int(T)), "cav_set_sweeps_per_exchange")
 
     def set_fields(self, psi, omega):
         psi = None if psi is None else _field(psi, self.N, "psi")

@@ -27,13 +27,16 @@ struct cav_ctx {
     cudaStream_t st = nullptr;
     void* slab = nullptr;            // one allocation from PyTorch's caching allocator
     double* psi = nullptr;           // stream function
-    double* psi_alt = nullptr;       // second psi buffer (halo exchange of the resident engine)
+    double* xa = nullptr;            // resident engine: exchange field of even rounds
+    double* xb = nullptr;            // resident engine: exchange field of odd rounds
     double* q = nullptr;             // (beta/4) h^2 w_in, the scaled right-hand side of the current stage
     double* w[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // omega^n (state), omega^(1..4)
     double* T = nullptr;             // first three terms of eq 13
     double* scratch = nullptr;       // diagnostics partials
     double* out4 = nullptr;          // diagnostics result (device)
-    unsigned int* flags = nullptr;   // resident engine: per-tile round counters
+    unsigned int* flags = nullptr;   // resident engine: per-tile event counters + the error word
+    unsigned int epoch = 0;          // resident engine: flag epoch (host side)
+    int flag_words = 0;              // words allocated behind `flags`
     size_t field_doubles = 0;
     long long step = 0;
     long long launches = 0;
@@ -92,18 +95,28 @@ void resolve_engine(cav_ctx* c) {
     if (e != c->engine) { c->engine = e; drop_graph(c); }
 }
 
-// a1: nsweeps red-black sweeps on psi with right-hand side q
-int enqueue_sweeps(cav_ctx* c, int nsweeps, long long& nl) {
+// a1: nsweeps red-black sweeps on psi with right-hand side w_in
+int enqueue_sweeps(cav_ctx* c, const double* w_in, int nsweeps, long long& nl) {
     if (nsweeps <= 0) return CAV_OK;
     if (c->engine == CAV_ENGINE_RESIDENT) {
-        LAUNCH(cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi_alt, c->q, c->flags, nsweeps, c->st));
+        LAUNCH(cavk::resident_sweeps(c->P, c->plan, c->psi, c->xa, c->xb, w_in, c->flags, &c->epoch, nsweeps, c->st));
     } else {
+        LAUNCH(cavk::scale_rhs(c->P, w_in, c->q, c->st));
         LAUNCH(cavk::stream_sweeps(c->P, c->psi, c->q, nsweeps, c->st));
     }
     return CAV_OK;
 }
 
-// one SSPRK(5,4) step: 5 x [scale, a1 x S, a2 + a3]
+// the resident engine's tiles give up (and say so) instead of spinning forever on a neighbour that never arrives
+int check_resident_error(cav_ctx* c) {
+    if (!c->plan.ok || !c->flags) return CAV_OK;
+    unsigned int e = 0;
+    if (cudaMemcpyAsync(&e, c->flags + cavk::resident_error_word_index(c->plan), sizeof e, cudaMemcpyDeviceToHost, c->st) != cudaSuccess ||
+        cudaStreamSynchronize(c->st) != cudaSuccess) { cudaGetLastError(); return CAV_ECUDA; }
+    return e ? CAV_ECUDA : CAV_OK;
+}
+
+// one SSPRK(5,4) step: 5 x [a1 x S, a2 + a3]
 int enqueue_step(cav_ctx* c, long long& nl) {
     double* const* w = c->w;
     const double* win[5] = {w[0], w[1], w[2], w[3], w[4]};
@@ -111,8 +124,7 @@ int enqueue_step(cav_ctx* c, long long& nl) {
     const double* b[5] = {nullptr, nullptr, nullptr, w[2], nullptr};
     double* wout[5] = {w[1], w[2], w[3], w[4], w[0]};
     for (int k = 0; k < 5; ++k) {
-        LAUNCH(cavk::scale_rhs(c->P, win[k], c->q, c->st));
-        int rc = enqueue_sweeps(c, c->S, nl);
+        int rc = enqueue_sweeps(c, win[k], c->S, nl);
         if (rc != CAV_OK) return rc;
         LAUNCH(cavk::rk_stage(c->P, k + 1, c->psi, win[k], a[k], b[k], wout[k], c->T, c->st));
     }
@@ -157,7 +169,10 @@ int step_impl(cav_ctx* c, int nsteps, bool sync) {
     CK(cudaEventRecord(c->ev1, c->st));
     c->timed = true;
     c->step += nsteps;
-    if (sync) CK(cudaStreamSynchronize(c->st));
+    if (sync) {
+        CK(cudaStreamSynchronize(c->st));
+        if (c->engine == CAV_ENGINE_RESIDENT) return check_resident_error(c);
+    }
     return CAV_OK;
 }
 
@@ -183,16 +198,19 @@ CAV_API int cav_create(cav_ctx** out, int N, double Re, double dt, double sor_om
 
         const size_t fd = align_up((size_t)c->P.pitch * (size_t)(N + 1), 32);   // doubles per field, 256 B multiple
         c->field_doubles = fd;
-        const size_t nfields = 9;    // psi, psi_alt, q, w0..w4, T
+        const size_t nfields = 10;   // psi, xa, xb, q, w0..w4, T
         const size_t scratch_d = align_up(4 * (size_t)cavk::diag_scratch_doubles(), 32);
-        const size_t flags_b = align_up(sizeof(unsigned int) * 4 * (size_t)(c->plan.ok ? c->plan.ntiles : 1) + 256, 256);
+        c->flag_words = 1024;        // >= tiles + 1 of any plan (a plan never has more tiles than SMs)
+        if (cavk::resident_flag_words(c->plan) > c->flag_words) c->plan.ok = false;
+        const size_t flags_b = align_up(sizeof(unsigned int) * (size_t)c->flag_words, 256);
         const size_t bytes = (nfields * fd + scratch_d + 32) * sizeof(double) + flags_b;
         c->slab = c10::cuda::CUDACachingAllocator::raw_alloc_with_stream(bytes, c->st);
         if (!c->slab) throw (int)CAV_ENOMEM;
         if (cudaMemsetAsync(c->slab, 0, bytes, c->st) != cudaSuccess) throw (int)CAV_ECUDA;
         double* p = (double*)c->slab;
         c->psi = p; p += fd;
-        c->psi_alt = p; p += fd;
+        c->xa = p; p += fd;
+        c->xb = p; p += fd;
         c->q = p; p += fd;
         for (int k = 0; k < 5; ++k) { c->w[k] = p; p += fd; }
         c->T = p; p += fd;
@@ -267,7 +285,7 @@ CAV_API int cav_sync(cav_ctx* c) {
     if (!c) return CAV_EINVAL;
     DeviceGuard dg(c->device);
     CK(cudaStreamSynchronize(c->st));
-    return CAV_OK;
+    return check_resident_error(c);
 }
 
 CAV_API int cav_poisson(cav_ctx* c, int nsweeps, double* res_inf_out) {
@@ -276,8 +294,7 @@ CAV_API int cav_poisson(cav_ctx* c, int nsweeps, double* res_inf_out) {
     resolve_engine(c);
     long long nl = 0;
     CK(cudaEventRecord(c->ev0, c->st));
-    LAUNCH(cavk::scale_rhs(c->P, c->w[0], c->q, c->st));
-    int rc = enqueue_sweeps(c, nsweeps, nl);
+    int rc = enqueue_sweeps(c, c->w[0], nsweeps, nl);
     if (rc != CAV_OK) { c->launches += nl; return rc; }
     LAUNCH(cavk::thom_ring(c->P, c->psi, c->w[0], c->st));
     CK(cudaEventRecord(c->ev1, c->st));
@@ -290,6 +307,7 @@ CAV_API int cav_poisson(cav_ctx* c, int nsweeps, double* res_inf_out) {
     c->launches += nl;
     CK(cudaStreamSynchronize(c->st));
     if (res_inf_out) *res_inf_out = r;
+    if (c->engine == CAV_ENGINE_RESIDENT) return check_resident_error(c);
     return CAV_OK;
 }
 
@@ -315,6 +333,16 @@ CAV_API int cav_set_engine(cav_ctx* c, int engine) {
     CK(cudaStreamSynchronize(c->st));
     c->engine_req = engine;
     resolve_engine(c);
+    return CAV_OK;
+}
+
+CAV_API int cav_set_sweeps_per_exchange(cav_ctx* c, int sweeps_per_exchange) {
+    if (!c || sweeps_per_exchange < 0) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    CK(cudaStreamSynchronize(c->st));
+    cavk::ResidentPlan pl = cavk::resident_plan(c->P, c->device, sweeps_per_exchange);
+    if (!pl.ok || cavk::resident_flag_words(pl) > c->flag_words) return CAV_ENOTSUP;
+    c->plan = pl;
     return CAV_OK;
 }
 
