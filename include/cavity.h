@@ -96,10 +96,18 @@ int cav_get_diag(cav_ctx* ctx, cav_diag* out);
 int cav_set_engine(cav_ctx* ctx, int engine);
 
 /* Resident engine only: forces T, the number of sweeps between two halo exchanges (even, 2..16; the halo is 2T
- * points deep), and re-plans the tiling for it; 0 restores the planner's own choice.  The result of every
- * other call is unchanged bit for bit; this is a tuning / testing knob.  CAV_ENOTSUP if no plan exists for that T
- * (the previous plan is kept). */
-int cav_set_sweeps_per_exchange(cav_ctx* ctx, int sweeps_per_exchange);
+ * points deep; 0 = the planner's own choice) and / or the micro-tile variant (index, -1 = the planner's choice),
+ * and re-plans the tiling.  The result of every other call is unchanged bit for bit; this is a tuning / testing
+ * knob.  CAV_ENOTSUP if no such plan exists (the previous plan is kept). */
+int cav_set_resident_plan(cav_ctx* ctx, int sweeps_per_exchange, int variant);
+
+/* Profiling aid, resident engine only: runs nsweeps of a1 on the current (psi, omega) like cav_poisson (without the
+ * a2 pass) and returns, for every tile, SM-clock stamps at the phase boundaries: stamps_out is a HOST array of
+ * ntiles x slots_per_tile; slot 0 = kernel start, 1 = inputs loaded, then for exchange round r: 2 + 4r = sweeps done,
+ * 3 + 4r = border strips posted, 4 + 4r = neighbours arrived, 5 + 4r = halo reloaded.  Unused slots are 0; stamps of
+ * different tiles come from different SM clocks.  *ntiles_out (if non-NULL) receives the tile count; call once with
+ * the capacity of a plan's tile count (at most 1023).  CAV_ENOTSUP if the engine in use is not the resident one. */
+int cav_trace_sweeps(cav_ctx* ctx, int nsweeps, long long* stamps_out, int slots_per_tile, int* ntiles_out);
 
 /* Describes the launch plan of the current engine in `buf` (NUL-terminated, truncated to len). */
 int cav_describe(cav_ctx* ctx, char* buf, int len);

@@ -15,7 +15,7 @@ _ENGINES = {"auto": ENGINE_AUTO, "stream": ENGINE_STREAM, "resident": ENGINE_RES
 
 # every symbol include/cavity.h declares
 SYMBOLS = ("cav_create", "cav_destroy", "cav_set_fields", "cav_get_fields", "cav_step", "cav_step_async", "cav_sync",
-           "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_set_sweeps_per_exchange", "cav_describe", "cav_launch_count",
+           "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_set_resident_plan", "cav_trace_sweeps", "cav_describe", "cav_launch_count",
            "cav_last_elapsed_ms", "cav_strerror")
 
 _lib = None
@@ -62,7 +62,8 @@ def lib():
     L.cav_poisson.argtypes = [C.c_void_p, C.c_int, dp]
     L.cav_get_diag.argtypes = [C.c_void_p, C.POINTER(CavDiag)]
     L.cav_set_engine.argtypes = [C.c_void_p, C.c_int]
-    L.cav_set_sweeps_per_exchange.argtypes = [C.c_void_p, C.c_int]
+    L.cav_set_resident_plan.argtypes = [C.c_void_p, C.c_int, C.c_int]
+    L.cav_trace_sweeps.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_longlong), C.c_int, C.POINTER(C.c_int)]
     L.cav_describe.argtypes = [C.c_void_p, C.c_char_p, C.c_int]
     L.cav_launch_count.argtypes = [C.c_void_p]
     L.cav_launch_count.restype = C.c_longlong
@@ -127,8 +128,16 @@ class Cavity:
         _chk(lib().cav_set_engine(self._h, _ENGINES[engine] if isinstance(engine, str) else int(engine)),
              "cav_set_engine")
 
-    def set_resident_T(self, T):
-        _chk(lib().cav_set_sweeps_per_exchange(self._h, int(T)), "cav_set_sweeps_per_exchange")
+    def set_resident_T(self, T, variant=-1):
+        _chk(lib().cav_set_resident_plan(self._h, int(T), int(variant)), "cav_set_resident_plan")
+
+    def trace_sweeps(self, nsweeps, slots_per_tile=64):
+        """(ntiles, slots) int64 array of SM-clock stamps (see include/cavity.h: cav_trace_sweeps)."""
+        out = np.zeros((1024, slots_per_tile), dtype=np.int64)
+        nt = C.c_int()
+        _chk(lib().cav_trace_sweeps(self._h, int(nsweeps), out.ctypes.data_as(C.POINTER(C.c_longlong)),
+                                    int(slots_per_tile), C.byref(nt)), "cav_trace_sweeps")
+        return out[:nt.value]
 
     def set_fields(self, psi, omega):
         psi = None if psi is None else _field(psi, self.N, "psi")

@@ -336,14 +336,38 @@ CAV_API int cav_set_engine(cav_ctx* c, int engine) {
     return CAV_OK;
 }
 
-CAV_API int cav_set_sweeps_per_exchange(cav_ctx* c, int sweeps_per_exchange) {
-    if (!c || sweeps_per_exchange < 0) return CAV_EINVAL;
+CAV_API int cav_set_resident_plan(cav_ctx* c, int sweeps_per_exchange, int variant) {
+    if (!c || sweeps_per_exchange < 0 || variant >= cavk::resident_variants()) return CAV_EINVAL;
     DeviceGuard dg(c->device);
     CK(cudaStreamSynchronize(c->st));
-    cavk::ResidentPlan pl = cavk::resident_plan(c->P, c->device, sweeps_per_exchange);
+    cavk::ResidentPlan pl = cavk::resident_plan(c->P, c->device, sweeps_per_exchange, variant < 0 ? -1 : variant);
     if (!pl.ok || cavk::resident_flag_words(pl) > c->flag_words) return CAV_ENOTSUP;
     c->plan = pl;
     return CAV_OK;
+}
+
+CAV_API int cav_trace_sweeps(cav_ctx* c, int nsweeps, long long* stamps_out, int slots_per_tile, int* ntiles_out) {
+    if (!c || nsweeps < 1 || !stamps_out || slots_per_tile < 2) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    resolve_engine(c);
+    if (c->engine != CAV_ENGINE_RESIDENT) return CAV_ENOTSUP;
+    const size_t n = (size_t)c->plan.ntiles * (size_t)slots_per_tile;
+    long long* dev = nullptr;
+    try { dev = (long long*)c10::cuda::CUDACachingAllocator::raw_alloc_with_stream(n * sizeof(long long), c->st); }
+    catch (...) { return CAV_ENOMEM; }
+    int rc = CAV_OK;
+    if (cudaMemsetAsync(dev, 0, n * sizeof(long long), c->st) != cudaSuccess) rc = CAV_ECUDA;
+    if (rc == CAV_OK) {
+        int nl = cavk::resident_sweeps(c->P, c->plan, c->psi, c->xa, c->xb, c->w[0], c->flags, &c->epoch, nsweeps, c->st,
+                                       dev, slots_per_tile);
+        if (nl < 0) rc = CAV_ECUDA; else c->launches += nl;
+    }
+    if (rc == CAV_OK && (cudaMemcpyAsync(stamps_out, dev, n * sizeof(long long), cudaMemcpyDeviceToHost, c->st) != cudaSuccess ||
+                         cudaStreamSynchronize(c->st) != cudaSuccess)) rc = CAV_ECUDA;
+    if (rc != CAV_OK) cudaGetLastError();
+    try { c10::cuda::CUDACachingAllocator::raw_delete(dev); } catch (...) {}
+    if (ntiles_out) *ntiles_out = c->plan.ntiles;
+    return rc == CAV_OK ? check_resident_error(c) : rc;
 }
 
 CAV_API int cav_describe(cav_ctx* c, char* buf, int len) {

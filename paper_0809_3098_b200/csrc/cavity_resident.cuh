@@ -25,8 +25,10 @@ struct ResidentPlan {
     int sm_count = 0;
 };
 
-// T_override > 0 forces the sweeps per round (tests use it to exercise short and ragged rounds).
-ResidentPlan resident_plan(const Params& P, int device, int T_override = 0);
+// T_override > 0 forces the sweeps per round (tests use it to exercise short and ragged rounds);
+// variant_override >= 0 forces the micro-tile shape (index into the compiled variants).
+ResidentPlan resident_plan(const Params& P, int device, int T_override = 0, int variant_override = -1);
+int resident_variants();
 void resident_describe(const ResidentPlan& plan, char* buf, int len);
 
 // Flag words the engine needs (per tile, plus the error word); the caller zero-fills them once.
@@ -35,9 +37,12 @@ int resident_flag_words(const ResidentPlan& plan);
 // nsweeps red-black sweeps of a1 on psi in place with right-hand side cq * w (w = the stage's input vorticity,
 // scaled on the fly exactly as scale_rhs does).  xa, xb: two exchange fields of the same layout as psi.
 // flags: resident_flag_words() words; *epoch is the host-side flag epoch, advanced by this call.
+// trace_dev (profiling only): device array of ntiles x trace_cap clock64 stamps, slot 0 = start, 1 = inputs loaded,
+// then per round r: 2 + 4r computed, 3 + 4r strips posted, 4 + 4r neighbours arrived, 5 + 4r halo reloaded.
 // Returns the number of kernel launches (1), or a negative cudaError_t.
 int resident_sweeps(const Params& P, const ResidentPlan& plan, double* psi, double* xa, double* xb, const double* w,
-                    unsigned int* flags, unsigned int* epoch, int nsweeps, cudaStream_t st);
+                    unsigned int* flags, unsigned int* epoch, int nsweeps, cudaStream_t st,
+                    long long* trace_dev = nullptr, int trace_cap = 0);
 
 // 0 if no tile ever timed out waiting for a neighbour (checked by the API after synchronising).
 int resident_error_word_index(const ResidentPlan& plan);
