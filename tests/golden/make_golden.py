@@ -65,16 +65,22 @@ def run(k):
     if wl.poisson_sweeps:
         o.poisson(wl.poisson_sweeps)
         out["checkpoints"].append(snapshot(o, wl.N, "poisson"))
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "cfg%d.json" % k)
+
+    def write():
+        # rewritten after every checkpoint: an interrupted run leaves a valid file with the checkpoints reached so far
+        out["oracle_wall_seconds"] = round(time.time() - t0, 1)
+        with open(path + ".tmp.%d" % os.getpid(), "w") as f:
+            json.dump(out, f, indent=1)
+        os.replace(path + ".tmp.%d" % os.getpid(), path)
+
     done = 0
     for cp in CHECKPOINTS[k]:
         o.step(cp - done)
         done = cp
         out["checkpoints"].append(snapshot(o, wl.N, "step%d" % cp))
         print("cfg%d step %d  %.1f s" % (k, cp, time.time() - t0), flush=True)
-    out["oracle_wall_seconds"] = round(time.time() - t0, 1)
-    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "cfg%d.json" % k)
-    with open(path, "w") as f:
-        json.dump(out, f, indent=1)
+        write()
     print("wrote", path)
 
 

@@ -1,0 +1,58 @@
+"""Multi-GPU host logic (replicas only): which workload a rank runs and how per-rank timings
+combine into the whole-job figure.  World size 2 over gloo on CPU; no kernel is involved."""
+import os
+import socket
+
+import pytest
+
+from paper_0809_3098_b200 import replicas
+from paper_0809_3098_b200 import workloads as W
+
+
+def test_replica_workloads_same_grid_distinct_reynolds():
+    base = W.config(4)
+    ws = [replicas.replica_workload(base, r, 8) for r in range(8)]
+    assert ws[0] is base
+    for r, w in enumerate(ws):
+        assert (w.N, w.dt, w.sweeps_per_stage, w.sor_omega) == (base.N, base.dt, base.sweeps_per_stage, base.sor_omega)
+        assert w.Re in replicas.TABLE1_RE                      # Table 1 of the paper
+        if r:
+            assert w.Re != base.Re and w.seed != base.seed
+    assert len({w.seed for w in ws}) == 8
+    assert replicas.replica_workload(base, 3, 1) is base
+
+
+def test_combine_single_rank_is_identity():
+    assert replicas.combine(10.0, 2.0, 1) == (10.0, 2.0)
+
+
+def _worker(rank, world, port, q):
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        # rank r processed 100 (r + 1) units in (1 + r) seconds: the job did 300 units in max = 2 s
+        u, t = replicas.combine(100.0 * (rank + 1), 1.0 + rank, world, dist, torch.device("cpu"))
+        q.put((rank, u, t))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(120)
+def test_combine_world_size_2_gloo():
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    ps = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    got = sorted(q.get(timeout=90) for _ in ps)
+    for p in ps:
+        p.join(30)
+        assert p.exitcode == 0
+    assert got == [(0, 300.0, 2.0), (1, 300.0, 2.0)]
