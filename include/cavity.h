@@ -102,10 +102,10 @@ int cav_set_engine(cav_ctx* ctx, int engine);
 int cav_set_resident_plan(cav_ctx* ctx, int sweeps_per_exchange, int variant);
 
 /* Profiling aid, resident engine only: runs nsweeps of a1 on the current (psi, omega) like cav_poisson (without the
- * a2 pass) and returns, for every tile, SM-clock stamps at the phase boundaries: stamps_out is a HOST array of
+ * a2 pass) and returns, for every tile, %globaltimer stamps (ns, one clock for all tiles) at the phase boundaries: stamps_out is a HOST array of
  * ntiles x slots_per_tile; slot 0 = kernel start, 1 = inputs loaded, then for exchange round r: 2 + 4r = sweeps done,
- * 3 + 4r = border strips posted, 4 + 4r = neighbours arrived, 5 + 4r = halo reloaded.  Unused slots are 0; stamps of
- * different tiles come from different SM clocks.  *ntiles_out (if non-NULL) receives the tile count; call once with
+ * 3 + 4r = border strips stored, 4 + 4r = ring received from the neighbours, 5 + 4r = edges republished.  Unused slots are 0;
+ * *ntiles_out (if non-NULL) receives the tile count; call once with
  * the capacity of a plan's tile count (at most 1023).  CAV_ENOTSUP if the engine in use is not the resident one. */
 int cav_trace_sweeps(cav_ctx* ctx, int nsweeps, long long* stamps_out, int slots_per_tile, int* ntiles_out);
 

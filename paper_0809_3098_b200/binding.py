@@ -105,7 +105,7 @@ class Cavity:
         if engine != "auto":
             self.set_engine(engine)
         if resident_T:
-            self.set_resident_T(resident_T)
+            self.set_resident_plan(resident_T)
 
     def close(self):
         if getattr(self, "_h", None):
@@ -128,11 +128,11 @@ class Cavity:
         _chk(lib().cav_set_engine(self._h, _ENGINES[engine] if isinstance(engine, str) else int(engine)),
              "cav_set_engine")
 
-    def set_resident_T(self, T, variant=-1):
+    def set_resident_plan(self, T=0, variant=-1):
         _chk(lib().cav_set_resident_plan(self._h, int(T), int(variant)), "cav_set_resident_plan")
 
     def trace_sweeps(self, nsweeps, slots_per_tile=64):
-        """(ntiles, slots) int64 array of SM-clock stamps (see include/cavity.h: cav_trace_sweeps)."""
+        """(ntiles, slots) int64 array of %globaltimer stamps in ns (see include/cavity.h: cav_trace_sweeps)."""
         out = np.zeros((1024, slots_per_tile), dtype=np.int64)
         nt = C.c_int()
         _chk(lib().cav_trace_sweeps(self._h, int(nsweeps), out.ctypes.data_as(C.POINTER(C.c_longlong)),

@@ -13,6 +13,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
 
 #include "../../include/cavity.h"
 #include "cavity_kernels.cuh"
@@ -26,17 +27,17 @@ struct cav_ctx {
     cavk::Params P{};
     cudaStream_t st = nullptr;
     void* slab = nullptr;            // one allocation from PyTorch's caching allocator
-    double* psi = nullptr;           // stream function
-    double* xa = nullptr;            // resident engine: exchange field of even rounds
-    double* xb = nullptr;            // resident engine: exchange field of odd rounds
+    double* psi = nullptr;           // stream function (current)
+    double* psi2 = nullptr;          // resident engine: the field the next sweep launch writes (then swapped with psi)
+    double* xa = nullptr;            // resident engine: exchange buffer of even rounds (16-byte units, 2 fields long)
+    double* xb = nullptr;            // resident engine: exchange buffer of odd rounds
     double* q = nullptr;             // (beta/4) h^2 w_in, the scaled right-hand side of the current stage
     double* w[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // omega^n (state), omega^(1..4)
     double* T = nullptr;             // first three terms of eq 13
     double* scratch = nullptr;       // diagnostics partials
     double* out4 = nullptr;          // diagnostics result (device)
-    unsigned int* flags = nullptr;   // resident engine: per-tile event counters + the error word
-    unsigned int epoch = 0;          // resident engine: flag epoch (host side)
-    int flag_words = 0;              // words allocated behind `flags`
+    unsigned int* err_word = nullptr;// resident engine: device error word (a tile gave up waiting for a neighbour)
+    unsigned int epoch = 0;          // resident engine: tag epoch (host side)
     size_t field_doubles = 0;
     long long step = 0;
     long long launches = 0;
@@ -99,7 +100,8 @@ void resolve_engine(cav_ctx* c) {
 int enqueue_sweeps(cav_ctx* c, const double* w_in, int nsweeps, long long& nl) {
     if (nsweeps <= 0) return CAV_OK;
     if (c->engine == CAV_ENGINE_RESIDENT) {
-        LAUNCH(cavk::resident_sweeps(c->P, c->plan, c->psi, c->xa, c->xb, w_in, c->flags, &c->epoch, nsweeps, c->st));
+        LAUNCH(cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, w_in, c->err_word, &c->epoch, nsweeps, c->st));
+        std::swap(c->psi, c->psi2);
     } else {
         LAUNCH(cavk::scale_rhs(c->P, w_in, c->q, c->st));
         LAUNCH(cavk::stream_sweeps(c->P, c->psi, c->q, nsweeps, c->st));
@@ -109,9 +111,9 @@ int enqueue_sweeps(cav_ctx* c, const double* w_in, int nsweeps, long long& nl) {
 
 // the resident engine's tiles give up (and say so) instead of spinning forever on a neighbour that never arrives
 int check_resident_error(cav_ctx* c) {
-    if (!c->plan.ok || !c->flags) return CAV_OK;
+    if (!c->plan.ok || !c->err_word) return CAV_OK;
     unsigned int e = 0;
-    if (cudaMemcpyAsync(&e, c->flags + cavk::resident_error_word_index(c->plan), sizeof e, cudaMemcpyDeviceToHost, c->st) != cudaSuccess ||
+    if (cudaMemcpyAsync(&e, c->err_word, sizeof e, cudaMemcpyDeviceToHost, c->st) != cudaSuccess ||
         cudaStreamSynchronize(c->st) != cudaSuccess) { cudaGetLastError(); return CAV_ECUDA; }
     return e ? CAV_ECUDA : CAV_OK;
 }
@@ -198,25 +200,25 @@ CAV_API int cav_create(cav_ctx** out, int N, double Re, double dt, double sor_om
 
         const size_t fd = align_up((size_t)c->P.pitch * (size_t)(N + 1), 32);   // doubles per field, 256 B multiple
         c->field_doubles = fd;
-        const size_t nfields = 10;   // psi, xa, xb, q, w0..w4, T
+        const size_t xd = cavk::resident_exchange_doubles(fd);
+        const size_t nfields = 9;    // psi, psi2, q, w0..w4, T  (+ the two exchange buffers)
         const size_t scratch_d = align_up(4 * (size_t)cavk::diag_scratch_doubles(), 32);
-        c->flag_words = 1024;        // >= tiles + 1 of any plan (a plan never has more tiles than SMs)
-        if (cavk::resident_flag_words(c->plan) > c->flag_words) c->plan.ok = false;
-        const size_t flags_b = align_up(sizeof(unsigned int) * (size_t)c->flag_words, 256);
-        const size_t bytes = (nfields * fd + scratch_d + 32) * sizeof(double) + flags_b;
+        const size_t flags_b = 256;
+        const size_t bytes = (nfields * fd + 2 * xd + scratch_d + 32) * sizeof(double) + flags_b;
         c->slab = c10::cuda::CUDACachingAllocator::raw_alloc_with_stream(bytes, c->st);
         if (!c->slab) throw (int)CAV_ENOMEM;
         if (cudaMemsetAsync(c->slab, 0, bytes, c->st) != cudaSuccess) throw (int)CAV_ECUDA;
         double* p = (double*)c->slab;
         c->psi = p; p += fd;
-        c->xa = p; p += fd;
-        c->xb = p; p += fd;
+        c->psi2 = p; p += fd;
+        c->xa = p; p += xd;
+        c->xb = p; p += xd;
         c->q = p; p += fd;
         for (int k = 0; k < 5; ++k) { c->w[k] = p; p += fd; }
         c->T = p; p += fd;
         c->scratch = p; p += scratch_d;
         c->out4 = p; p += 32;
-        c->flags = (unsigned int*)p;
+        c->err_word = (unsigned int*)p;
         if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) throw (int)CAV_ECUDA;
         if (cudaStreamSynchronize(c->st) != cudaSuccess) throw (int)CAV_ECUDA;
         resolve_engine(c);
@@ -341,7 +343,7 @@ CAV_API int cav_set_resident_plan(cav_ctx* c, int sweeps_per_exchange, int varia
     DeviceGuard dg(c->device);
     CK(cudaStreamSynchronize(c->st));
     cavk::ResidentPlan pl = cavk::resident_plan(c->P, c->device, sweeps_per_exchange, variant < 0 ? -1 : variant);
-    if (!pl.ok || cavk::resident_flag_words(pl) > c->flag_words) return CAV_ENOTSUP;
+    if (!pl.ok) return CAV_ENOTSUP;
     c->plan = pl;
     return CAV_OK;
 }
@@ -358,9 +360,9 @@ CAV_API int cav_trace_sweeps(cav_ctx* c, int nsweeps, long long* stamps_out, int
     int rc = CAV_OK;
     if (cudaMemsetAsync(dev, 0, n * sizeof(long long), c->st) != cudaSuccess) rc = CAV_ECUDA;
     if (rc == CAV_OK) {
-        int nl = cavk::resident_sweeps(c->P, c->plan, c->psi, c->xa, c->xb, c->w[0], c->flags, &c->epoch, nsweeps, c->st,
-                                       dev, slots_per_tile);
-        if (nl < 0) rc = CAV_ECUDA; else c->launches += nl;
+        int nl = cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, c->w[0], c->err_word, &c->epoch, nsweeps,
+                                       c->st, dev, slots_per_tile);
+        if (nl < 0) rc = CAV_ECUDA; else { c->launches += nl; std::swap(c->psi, c->psi2); }
     }
     if (rc == CAV_OK && (cudaMemcpyAsync(stamps_out, dev, n * sizeof(long long), cudaMemcpyDeviceToHost, c->st) != cudaSuccess ||
                          cudaStreamSynchronize(c->st) != cudaSuccess)) rc = CAV_ECUDA;

@@ -1,4 +1,4 @@
-// cavity_resident.cu — the resident sweep engine (a1) for sm_100a.  DESIGN.md "Resident engine".
+// cavity_resident.cu — the resident sweep engine (a1) for sm_100a.  DESIGN.md section 6.
 //
 // What it computes is exactly S red-black SOR sweeps of the 5-point Poisson problem (eq 15-21 P:114-138 reduced,
 // DESIGN.md D1-D3), red = (i + j) even first (G9), with the arithmetic of DESIGN.md "Canonical arithmetic":
@@ -12,12 +12,30 @@
 // psi AND q in registers for the whole call; a warp spans 32 C points of R rows.  Threads exchange only the
 // perimeter of their micro-tile: left / right columns by warp shuffle, bottom / top rows through shared memory
 // (edge arrays laid out so that every access is unit-stride over the lanes), one __syncthreads per colour half-sweep.
+//
+// Walls cost nothing inside the sweeps.  The origin of an edge tile is shifted so that the wall column x = 0 is the LAST
+// column of a lane (x = N: the FIRST column of a lane) and the wall row y = 0 the LAST row of a warp (y = N: the FIRST row
+// of a warp).  Such a lane / warp owns no interior point; what it computes is never used: the adjacent lane substitutes
+// 0 for what the shuffle brings (the select that the tile edge needs anyway), and the warp never publishes that edge row,
+// so the shared-memory slot keeps the +0.0 it was initialised with (eq 23-24: psi = 0 on the walls).  A tile
+// whose origin parity is odd sweeps its local colour 1 first.  Walls that cannot be aligned (both walls of one direction in
+// the same tile: small grids) fall back to a bit mask of points that are put back to +0.0 after every half-sweep.
+//
 // Every T sweeps (2T half-sweeps, each of which invalidates one more ring of the halo) the CTAs refresh their
-// halos through L2: write the 2T-wide border strips of the core to an exchange field, release a per-tile flag,
-// acquire the flags of the up to 8 neighbours, reload the halo (ld.global.cg: L1 is not coherent).  Two
-// exchange fields alternate, so a tile can run at most one round ahead of a neighbour without a hazard.
-// Points on a wall are forced back to +0.0 after every half-sweep by the (few) threads that own any; points
-// outside the walls have only zero inputs and therefore stay +0.0 by themselves.
+// halos through L2 WITHOUT any fence, flag or barrier between CTAs: the validity tag travels inside the data.
+// A point is exchanged as one 16-byte unit {lo32(psi), tag, hi32(psi), tag} written by one st.v4.b32; each 8-byte half is
+// a single-copy-atomic access carrying its own tag, so a reader that finds both tags equal to the tag of the round it waits
+// for holds the two halves of that round's value, however the stores of the sender were ordered or torn.  Tags are unique
+// per round and per launch (a host-side epoch).  Two exchange buffers alternate by round parity: a tile can write round
+// r + 1 only after it has received round r from every neighbour, and a neighbour posts round r only after it has consumed
+// round r - 1, so the buffer a tile overwrites is never still being read.
+// The exchange is cooperative and coalesced: owners put the border-strip values into a shared-memory staging array, then
+// ALL threads of the CTA store the strip units (consecutive threads = consecutive x) and fetch the ring units the same
+// way (a few units per thread, all in flight together; a unit that does not carry the tag yet is polled), and the owners
+// pick the ring values up from the staging array.  Which unit a thread moves is precomputed once per launch into
+// shared-memory tables.
+// The kernel reads psi_in and writes psi_out (the API ping-pongs two fields), so no tile ever overwrites input a
+// neighbour has not loaded yet.
 #include "cavity_resident.cuh"
 
 #include <algorithm>
@@ -27,67 +45,113 @@ namespace cavk {
 
 namespace {
 
-constexpr long long SPIN_TIMEOUT_CYCLES = 4000000000LL;   // ~2 s: a neighbour that never arrives is a bug, not a wait
+constexpr long long SPIN_TIMEOUT_CYCLES = 4000000000LL;   // ~2 s: a neighbour whose data never arrives is a bug, not a wait
+constexpr unsigned int NO_UNIT = 0xffffffffu;
 
 struct ResArgs {
     int N, pitch;
     double cb, omb, cq;
     const double* w;        // stage input vorticity; q = cq * w on interior points
-    double* psi;            // in / out
-    double* x0;             // exchange field of even rounds
-    double* x1;             // exchange field of odd rounds
-    unsigned int* flags;    // one word per tile (monotonic event counter) ...
-    unsigned int* err;      // ... and the error word
-    unsigned int base;      // flag epoch of this launch
+    const double* psi_in;   // stream function before the sweeps
+    double* psi_out;        // ... and after (a different field)
+    uint4* x0;              // exchange buffer of even rounds: one 16-byte unit per grid point, same (pitch) indexing as a field
+    uint4* x1;              // exchange buffer of odd rounds
+    unsigned int* err;      // error word: set if a tile gave up waiting for a neighbour
+    unsigned int base;      // tag epoch of this launch: round r is tagged base + 1 + r
     int nsweeps, T, halo, CW, CH, ntx, nty;
-    long long* trace;       // profiling only (cav_trace_sweeps): per tile, clock64 at the phase boundaries; else null
+    int ns_per, nr_per;     // table entries per thread: strip units to store / ring units to fetch
+    long long* trace;       // profiling only (cav_trace_sweeps): per tile, %globaltimer at the phase boundaries; else null
     int trace_cap;          // slots per tile
 };
 
-__device__ __forceinline__ unsigned int ld_relaxed(const unsigned int* p) {
-    unsigned int v;
-    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+// Geometry of tile (bi, bj): owned core, origin of the thread grid, wall alignment.  Shared by the planner (host) and the
+// kernel so that both agree on what fits.
+struct TileGeom {
+    int cx0, cx1, cy0, cy1;        // core [cx0, cx1) x [cy0, cy1)
+    int ox, oy;                    // grid coordinates of local point (0, 0)
+    bool left_al, right_al, bot_al, top_al;   // wall isolated in a lane / warp that owns no interior point
+    bool fits;                     // the W x H thread grid covers core + halo (clipped to the grid) and the aligned walls
+};
+
+__host__ __device__ inline TileGeom tile_geom(int N, int CW, int CH, int halo, int ntx, int nty, int bi, int bj, int C, int R,
+                                              int W, int H) {
+    TileGeom g;
+    g.cx0 = bi * CW; g.cy0 = bj * CH;
+    g.cx1 = g.cx0 + CW < N + 1 ? g.cx0 + CW : N + 1;
+    g.cy1 = g.cy0 + CH < N + 1 ? g.cy0 + CH : N + 1;
+    g.left_al = bi == 0;
+    g.right_al = bi == ntx - 1 && ntx > 1;
+    g.bot_al = bj == 0;
+    g.top_al = bj == nty - 1 && nty > 1;
+    if (g.left_al) g.ox = -(C - 1);                                   // x = 0 is column C - 1 of lane 0
+    else if (g.right_al) g.ox = g.cx0 - halo - (C - (N - g.cx0 + halo) % C) % C;      // (N - ox) % C == 0
+    else g.ox = g.cx0 - halo;
+    if (g.bot_al) g.oy = -(R - 1);                                    // y = 0 is row R - 1 of warp 0
+    else if (g.top_al) g.oy = g.cy0 - halo - (R - (N - g.cy0 + halo) % R) % R;        // (N - oy) % R == 0
+    else g.oy = g.cy0 - halo;
+    const int xneed = (g.cx1 + halo < N + 1 ? g.cx1 + halo : N + 1);  // one past the last column the tile must hold
+    const int yneed = (g.cy1 + halo < N + 1 ? g.cy1 + halo : N + 1);
+    g.fits = g.ox + W >= xneed && g.oy + H >= yneed;
+    return g;
+}
+
+// One exchanged point: {lo32, tag, hi32, tag}.  Each aligned 8-byte half is single-copy atomic and self-validating.
+__device__ __forceinline__ void st_unit(uint4* p, double v, unsigned int tag) {
+    const unsigned int lo = (unsigned int)__double2loint(v), hi = (unsigned int)__double2hiint(v);
+    asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(lo), "r"(tag), "r"(hi), "r"(tag) : "memory");
+}
+__device__ __forceinline__ uint4 ld_unit(const uint4* p) {
+    uint4 v;
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void st_release(unsigned int* p, unsigned int v) {
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+__device__ __forceinline__ bool unit_ok(const uint4& v, unsigned int tag) { return v.y == tag && v.w == tag; }
+__device__ __forceinline__ double unit_value(const uint4& v) { return __hiloint2double((int)v.z, (int)v.x); }
+
+__device__ __forceinline__ long long globaltimer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return (long long)t;
+}
+__device__ __forceinline__ void mark(const ResArgs& a, int slot) {
+    if (a.trace != nullptr && threadIdx.x == 0 && threadIdx.y == 0 && slot < a.trace_cap)
+        a.trace[(size_t)(blockIdx.y * a.ntx + blockIdx.x) * a.trace_cap + slot] = globaltimer_ns();
+}
+// An integer zero the compiler cannot see through: values computed from special registers + opaque_zero() are
+// recomputed where they are used instead of being kept live across the sweep loop (which would push q into local memory).
+__device__ __forceinline__ int opaque_zero() {
+    int z = 0;
+    asm volatile("" : "+r"(z));
+    return z;
 }
 
-// All threads' earlier global stores -> visible to whoever acquires flag >= v.
-__device__ __forceinline__ void post(unsigned int* flag, unsigned int v) {
-    __syncthreads();
-    if (threadIdx.x == 0 && threadIdx.y == 0) st_release(flag, v);     // release = fence + store: cumulative over the barrier
-}
+// Per-thread flags of the sweep (one register): what the lane / warp must NOT take from / give to its neighbours.
+constexpr unsigned int FL_ZERO_LEFT = 1u;     // the left neighbour column is a wall or the tile edge: use 0
+constexpr unsigned int FL_ZERO_RIGHT = 2u;    // same on the right
+constexpr unsigned int FL_PUB_BOTTOM = 4u;    // publish the bottom row of the micro-tile to the warp below
+constexpr unsigned int FL_PUB_TOP = 8u;       // publish the top row to the warp above
 
-// Waits until each existing neighbour tile has posted event >= v.  Threads 0..7 of warp 0 take one direction each.
-__device__ __forceinline__ void wait_neighbours(const ResArgs& a, int bi, int bj, unsigned int v) {
-    if (threadIdx.y == 0 && threadIdx.x < 8) {
-        const int d = threadIdx.x < 4 ? threadIdx.x : threadIdx.x + 1;     // 0..8 without the centre (4)
-        const int ni = bi + d % 3 - 1, nj = bj + d / 3 - 1;
-        if (ni >= 0 && ni < a.ntx && nj >= 0 && nj < a.nty && *(volatile unsigned int*)a.err == 0u) {
-            const unsigned int* f = a.flags + (nj * a.ntx + ni);
-            const long long t0 = clock64();
-            while ((int)(ld_relaxed(f) - v) < 0) {
-                if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) { atomicExch(a.err, 1u); break; }
-            }
-        }
-        __threadfence();      // one acquire fence after the relaxed polls; the barrier extends it to the CTA
-    }
-    __syncthreads();
-}
-
-// One colour half-sweep on the register micro-tile.  K = colour being updated; local point (ci, rj) has colour
-// (ci + rj) & 1 because every tile origin is even in x and y and C, R are even (resident_plan guarantees it).
+// One colour half-sweep on the register micro-tile.  K = LOCAL colour being updated: local point (ci, rj) has local colour
+// (ci + rj) & 1 (C, R even); the kernel maps the global colour to the local one through the parity of the tile origin.
 // Left / right neighbours live in the adjacent lanes and come by warp shuffle (no barrier, no shared memory);
 // the rows above / below live in the adjacent warps and come through the sB / sT edge arrays.
-// wallmask: bit rj * C + ci set = that point lies ON a wall and is put back to +0.0 after the update
-// (eq 23-24).  Points outside the walls need nothing: all their inputs are 0, so they stay +0.0.
-template <int C, int R, int K>
+// wallmask: bit rj * C + ci set = that point lies ON a wall that could not be isolated by alignment and is put back to
+// +0.0 after the update (eq 23-24).
+template <int C, int R, int K, bool FIX, int TOPOFF>
 __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[R][C], const double cb, const double omb,
-                                           double* __restrict__ sB, double* __restrict__ sT, const unsigned int wallmask,
-                                           const int lane) {
-    // sB / sT point at [warp][0][lane] of the bottom / top edge arrays (stride 32 per ci, C * 32 per warp)
-    double Lnb[R], Rnb[R], Bnb[C], Tnb[C];
+                                           double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl) {
+    // sB / sT point at [warp][0][lane] of the bottom / top edge arrays (stride 32 per ci, C * 32 per warp);
+    // the top array starts TOPOFF doubles after the bottom one (a compile-time distance: one address register)
+    // q of the two middle rows of the micro-tile lives in shared memory, in two more arrays of the same shape 2 TOPOFF and
+    // 3 TOPOFF after the bottom edge array (same address register): 16 registers fewer held across the whole kernel.
+    double* const sT = sB + TOPOFF;
+    constexpr int Q0 = R / 2 - 1;
+    double Lnb[R], Rnb[R], Bnb[C], Tnb[C], qs[2][C];
+#pragma unroll
+    for (int ci = 0; ci < C; ++ci) {
+        if (((ci + Q0) & 1) == K) qs[0][ci] = sB[2 * TOPOFF + ci * 32];
+        if (((ci + Q0 + 1) & 1) == K) qs[1][ci] = sB[3 * TOPOFF + ci * 32];
+    }
 #pragma unroll
     for (int ci = 0; ci < C; ++ci) {
         if ((ci & 1) == K) Bnb[ci] = sT[ci * 32];                          // top row of the warp below (slot warp)
@@ -95,13 +159,13 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
     }
 #pragma unroll
     for (int rj = 0; rj < R; ++rj) {
-        if ((rj & 1) == K) {                                               // right edge of lane - 1; nothing left of lane 0
+        if ((rj & 1) == K) {                                               // right edge of lane - 1
             const double v = __shfl_up_sync(0xffffffffu, p[rj][C - 1], 1);
-            Lnb[rj] = lane == 0 ? 0.0 : v;
+            Lnb[rj] = (fl & FL_ZERO_LEFT) ? 0.0 : v;
         }
-        if (((C - 1 + rj) & 1) == K) {                                     // left edge of lane + 1; nothing right of lane 31
+        if (((C - 1 + rj) & 1) == K) {                                     // left edge of lane + 1
             const double v = __shfl_down_sync(0xffffffffu, p[rj][0], 1);
-            Rnb[rj] = lane == 31 ? 0.0 : v;
+            Rnb[rj] = (fl & FL_ZERO_RIGHT) ? 0.0 : v;
         }
     }
 #pragma unroll
@@ -114,12 +178,13 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
             const double pS = rj > 0 ? p[rj - 1][ci] : Bnb[ci];
             const double pN = rj < R - 1 ? p[rj + 1][ci] : Tnb[ci];
             const double nb = (pW + pE) + (pS + pN);
-            p[rj][ci] = fma(omb, p[rj][ci], fma(cb, nb, q[rj][ci]));
+            const double qv = (rj == Q0 || rj == Q0 + 1) ? qs[rj - Q0][ci] : q[rj][ci];
+            p[rj][ci] = fma(omb, p[rj][ci], fma(cb, nb, qv));
         }
     }
-    unsigned int wm = wallmask;
-    asm volatile("" : "+r"(wm));      // opaque: keeps the bit tests from being hoisted into live registers
-    if (wm) {
+    unsigned int wm = FIX ? wallmask : 0u;
+    if (FIX) asm volatile("" : "+r"(wm));      // opaque: keeps the bit tests from being hoisted into live registers
+    if (FIX && wm) {
 #pragma unroll
         for (int ci = 0; ci < C; ++ci) {
             unsigned int colbits = 0;                                      // the points of column ci with colour K
@@ -136,161 +201,334 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
     // publish the updated points of the bottom and top rows
 #pragma unroll
     for (int ci = 0; ci < C; ++ci) {
-        if ((ci & 1) == K) sB[ci * 32] = p[0][ci];
-        if (((ci + R - 1) & 1) == K) sT[C * 32 + ci * 32] = p[R - 1][ci];
+        if ((ci & 1) == K && (fl & FL_PUB_BOTTOM)) sB[ci * 32] = p[0][ci];
+        if (((ci + R - 1) & 1) == K && (fl & FL_PUB_TOP)) sT[C * 32 + ci * 32] = p[R - 1][ci];
     }
     __syncthreads();
 }
 
-template <int C, int R>
-__device__ __forceinline__ void publish_all(const double (&p)[R][C], double* __restrict__ sB, double* __restrict__ sT) {
+template <int C, int R, int TOPOFF>
+__device__ __forceinline__ void publish_all(const double (&p)[R][C], double* __restrict__ sB, const unsigned int fl) {
+    double* const sT = sB + TOPOFF;
 #pragma unroll
-    for (int ci = 0; ci < C; ++ci) { sB[ci * 32] = p[0][ci]; sT[C * 32 + ci * 32] = p[R - 1][ci]; }
+    for (int ci = 0; ci < C; ++ci) {
+        if (fl & FL_PUB_BOTTOM) sB[ci * 32] = p[0][ci];
+        if (fl & FL_PUB_TOP) sT[C * 32 + ci * 32] = p[R - 1][ci];
+    }
     __syncthreads();
 }
 
-__device__ __forceinline__ void load4(const double* __restrict__ g, double (&v)[4], bool cg) {
-    const double2* g2 = reinterpret_cast<const double2*>(g);
-    double2 a, b;
-    if (cg) { a = __ldcg(g2); b = __ldcg(g2 + 1); } else { a = g2[0]; b = g2[1]; }
-    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+// ---- the points a tile sends (border strips of its core) and receives (its ring): four disjoint rectangles each ----
+struct Rect { int x0, x1, y0, y1; };                     // [x0, x1) x [y0, y1)
+struct Region { Rect r[4]; };
+__host__ __device__ inline int imax(int a, int b) { return a > b ? a : b; }
+__host__ __device__ inline int imin(int a, int b) { return a < b ? a : b; }
+__host__ __device__ inline int rect_count(const Rect& r) {
+    const int w = r.x1 - r.x0, h = r.y1 - r.y0;
+    return (w > 0 && h > 0) ? w * h : 0;
 }
-__device__ __forceinline__ void store4(double* __restrict__ g, const double (&v)[4]) {
-    double2* g2 = reinterpret_cast<double2*>(g);
-    g2[0] = make_double2(v[0], v[1]);
-    g2[1] = make_double2(v[2], v[3]);
+__device__ __forceinline__ bool region_has(const Region& g, int x, int y) {
+    bool in = false;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) in = in || (x >= g.r[k].x0 && x < g.r[k].x1 && y >= g.r[k].y0 && y < g.r[k].y1);
+    return in;
+}
+// u-th point of the region (row-major inside each rectangle, rectangles in order); false if u is past the end
+__device__ __forceinline__ bool region_point(const Region& g, int u, int& x, int& y) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int n = rect_count(g.r[k]);
+        if (u < n) {
+            const int w = g.r[k].x1 - g.r[k].x0;
+            y = g.r[k].y0 + u / w;
+            x = g.r[k].x0 + u % w;
+            return true;
+        }
+        u -= n;
+    }
+    return false;
+}
+// Interior points of the core within `halo` of a core edge that has a neighbour tile behind it (walls are never sent).
+__host__ __device__ inline Region send_region(const TileGeom& t, int N, int halo, int bi, int bj, int ntx, int nty) {
+    const int X0 = imax(t.cx0, 1), X1 = imin(t.cx1, N), Y0 = imax(t.cy0, 1), Y1 = imin(t.cy1, N);
+    const int hb = bj > 0 ? halo : 0, ht = bj < nty - 1 ? halo : 0, wl = bi > 0 ? halo : 0, wr = bi < ntx - 1 ? halo : 0;
+    const int yB = imin(Y0 + hb, Y1), yT = imax(Y1 - ht, yB), xL = imin(X0 + wl, X1), xR = imax(X1 - wr, xL);
+    Region g;
+    g.r[0] = Rect{X0, X1, Y0, yB};
+    g.r[1] = Rect{X0, X1, yT, Y1};
+    g.r[2] = Rect{X0, xL, yB, yT};
+    g.r[3] = Rect{xR, X1, yB, yT};
+    return g;
+}
+// Interior points within `halo` of the core, outside it (the ring).
+__host__ __device__ inline Region recv_region(const TileGeom& t, int N, int halo) {
+    const int xlo = imax(t.cx0 - halo, 1), xhi = imin(t.cx1 + halo, N), ylo = imax(t.cy0 - halo, 1), yhi = imin(t.cy1 + halo, N);
+    const int yc0 = imax(t.cy0, ylo), yc1 = imin(t.cy1, yhi), xc0 = imax(t.cx0, xlo), xc1 = imin(t.cx1, xhi);
+    Region g;
+    g.r[0] = Rect{xlo, xhi, ylo, yc0};
+    g.r[1] = Rect{xlo, xhi, yc1, yhi};
+    g.r[2] = Rect{xlo, xc0, yc0, yc1};
+    g.r[3] = Rect{xc1, xhi, yc0, yc1};
+    return g;
 }
 
-__device__ __forceinline__ void mark(const ResArgs& a, int tile, int slot) {
-    if (a.trace != nullptr && threadIdx.x == 0 && threadIdx.y == 0 && slot < a.trace_cap)
-        a.trace[(size_t)tile * a.trace_cap + slot] = clock64();
+// Shared-memory layout (doubles unless said otherwise), nthreads = 32 nwarps:
+//   edges   4 (MAXW + 1) C 32            bottom / top rows of the micro-tiles, q of the two middle rows (sized for MAXW warps)
+//   stage   R C (nthreads + 4)           one slot per thread and micro-tile point, [point][thread] (+4: the 4 points of a chunk fall in different banks)
+//   tabS    ns_per nthreads uint2        {unit offset in the exchange buffer, staging slot} of the strip units this thread stores
+//   tabR    nr_per nthreads uint2        same for the ring units this thread fetches
+//   masks   2 nthreads u32               bit k: point k of this thread's micro-tile is in the send region / in the ring
+__host__ __device__ inline size_t smem_layout_bytes(int C, int R, int maxw, int warps, int ns_per, int nr_per) {
+    const size_t nth = 32 * (size_t)warps;
+    return 8 * (4 * (size_t)(maxw + 1) * C * 32 + (size_t)R * C * (nth + 4) + (size_t)(ns_per + nr_per) * nth) + 4 * 2 * nth;
 }
 
 // MAXW = most warps per CTA this variant is launched with: 65536 / (32 MAXW) registers per thread are available.
-template <int C, int R, int MAXW>
+template <int C, int R, int MAXW, bool FIX>
 __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const ResArgs a) {
-    static_assert(C == 4, "vector loads below assume 4 consecutive x-points per thread");
-    static_assert(R % 2 == 0 && R * C <= 32, "R must be even and the micro-tile must fit the 32-bit wall mask");
-    extern __shared__ double sm[];
+    constexpr int TOPOFF = (MAXW + 1) * C * 32;
+    static_assert(C % 2 == 0 && R % 2 == 0 && R * C <= 32, "even micro-tile that fits the 32-bit point masks");
+    extern __shared__ __align__(16) double sm[];
     const int lane = threadIdx.x, warp = threadIdx.y, nwarps = blockDim.y;
     const int tid = warp * 32 + lane, nthreads = nwarps * 32;
     const int N = a.N, pitch = a.pitch;
-
-    // edge arrays; the slots no thread ever writes (warp -1, warp nwarps) stay 0
-    double* const sBa = sm;                                   // [nwarps + 1][C][32]  bottom row of warp at [warp]
-    double* const sTa = sBa + (nwarps + 1) * C * 32;          // [nwarps + 1][C][32]  top row of warp at [warp + 1]
-    const int smem_doubles = 2 * (nwarps + 1) * C * 32;
-    for (int k = tid; k < smem_doubles; k += nthreads) sm[k] = 0.0;
-    double* const sB = sBa + warp * C * 32 + lane;
-    double* const sT = sTa + warp * C * 32 + lane;
-
     const int bi = blockIdx.x, bj = blockIdx.y;
-    const int cx0 = bi * a.CW, cy0 = bj * a.CH;
-    const int cx1 = min(cx0 + a.CW, N + 1), cy1 = min(cy0 + a.CH, N + 1);
-    const int gx0 = cx0 - a.halo + lane * C;       // multiple of 4: 32-byte aligned in every device row
-    const int gy0 = cy0 - a.halo + warp * R;       // even
-    const bool x_in = gx0 >= 0 && gx0 <= N;        // chunk [gx0, gx0 + 4) lies inside the padded device row
-    const bool x_core = gx0 >= cx0 && gx0 < cx1;
+    mark(a, 0);
 
-    const int tile = bj * a.ntx + bi;
-    mark(a, tile, 0);
+    // edge arrays; the slots no thread ever writes (warp -1, warp nwarps, unpublished wall rows) stay +0.0
+    constexpr int edge_doubles = 4 * TOPOFF;       // bottom edges, top edges, q of middle row 0, q of middle row 1
+    for (int k = tid; k < edge_doubles; k += nthreads) sm[k] = 0.0;
+    double* const sB = sm + warp * C * 32 + lane;      // [MAXW + 1][C][32] bottom row of warp at [warp]; top rows TOPOFF further, at [warp + 1]
+
+    const TileGeom t = tile_geom(N, a.CW, a.CH, a.halo, a.ntx, a.nty, bi, bj, C, R, 32 * C, nwarps * R);
+    const int gx0_ = t.ox + lane * C, gy0_ = t.oy + warp * R;
+    const bool odd_origin = ((t.ox + t.oy) & 1) != 0;          // local colour = global colour ^ odd_origin
+
+    unsigned int fl = FL_PUB_BOTTOM | FL_PUB_TOP;
+    {
+        const int lzl = t.left_al ? 1 : 0;                                     // lane 0 holds x = -(C-1) .. 0
+        const int lzr = t.right_al ? (N - t.ox) / C - 1 : 31;                  // lane (N - ox) / C holds x = N .. N + C - 1
+        if (lane == lzl) fl |= FL_ZERO_LEFT;
+        if (lane == lzr) fl |= FL_ZERO_RIGHT;
+        if (t.bot_al && warp == 0) fl &= ~FL_PUB_TOP;                          // warp 0 holds y = -(R-1) .. 0
+        if (t.top_al && warp == (N - t.oy) / R) fl &= ~FL_PUB_BOTTOM;          // that warp holds y = N .. N + R - 1
+    }
+
+    // ---- exchange tables and masks (multi-tile plans only) ----
+    const bool multi = a.ntx * a.nty > 1;
+    if (multi) {
+        double* const stage_ = sm + edge_doubles;
+        uint2* const tabS = reinterpret_cast<uint2*>(stage_ + R * C * (nthreads + 4));
+        uint2* const tabR = tabS + a.ns_per * nthreads;
+        unsigned int* const masks = reinterpret_cast<unsigned int*>(tabR + a.nr_per * nthreads);
+        const Region gs = send_region(t, N, a.halo, bi, bj, a.ntx, a.nty), gr = recv_region(t, N, a.halo);
+        for (int i = 0; i < a.ns_per + a.nr_per; ++i) {
+            const bool snd = i < a.ns_per;
+            const int u = (snd ? i : i - a.ns_per) * nthreads + tid;
+            int x = 0, y = 0;
+            uint2 e = make_uint2(NO_UNIT, 0u);
+            if (region_point(snd ? gs : gr, u, x, y)) {
+                const int lx = x - t.ox, ly = y - t.oy;                        // owner: lane lx / C, warp ly / R
+                e.x = (unsigned int)(y * pitch + x);                           // < 2^31: N <= 32766
+                e.y = (unsigned int)(((ly % R) * C + lx % C) * (nthreads + 4) + (ly / R) * 32 + lx / C);
+            }
+            (snd ? tabS : tabR)[(snd ? i : i - a.ns_per) * nthreads + tid] = e;
+        }
+        unsigned int smask = 0, rmask = 0;
+#pragma unroll
+        for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+            for (int ci = 0; ci < C; ++ci) {
+                if (region_has(gs, gx0_ + ci, gy0_ + rj)) smask |= 1u << (rj * C + ci);
+                if (region_has(gr, gx0_ + ci, gy0_ + rj)) rmask |= 1u << (rj * C + ci);
+            }
+        masks[tid] = smask;
+        masks[nthreads + tid] = rmask;
+    }
+
+    // ---- load the micro-tile ----
     double p[R][C], q[R][C];
-    unsigned int wallmask = 0;            // points ON a wall (psi = 0 there, eq 23-24)
+    unsigned int wallmask = 0;            // wall points that alignment could not isolate (psi = 0 there, eq 23-24)
 #pragma unroll
     for (int rj = 0; rj < R; ++rj) {
-        const int gy = gy0 + rj;
-        const bool in = x_in && gy >= 0 && gy <= N;
-        double pv[4] = {0.0, 0.0, 0.0, 0.0}, wv[4] = {0.0, 0.0, 0.0, 0.0};
-        if (in) {
-            load4(a.psi + (size_t)gy * pitch + gx0, pv, false);
-            load4(a.w + (size_t)gy * pitch + gx0, wv, false);
-        }
 #pragma unroll
         for (int ci = 0; ci < C; ++ci) {
-            const int gx = gx0 + ci;
+            const int gx = gx0_ + ci, gy = gy0_ + rj;
             const bool upd = gx >= 1 && gx <= N - 1 && gy >= 1 && gy <= N - 1;
-            p[rj][ci] = upd ? pv[ci] : 0.0;
-            q[rj][ci] = upd ? a.cq * wv[ci] : 0.0;
+            p[rj][ci] = upd ? a.psi_in[(size_t)gy * pitch + gx] : 0.0;
+            q[rj][ci] = upd ? a.cq * a.w[(size_t)gy * pitch + gx] : 0.0;
             const bool wall = gx >= 0 && gx <= N && gy >= 0 && gy <= N && !upd;
-            if (wall) wallmask |= 1u << (rj * C + ci);
+            const bool isolated = (gx == 0 && t.left_al) || (gx == N && t.right_al) || (gy == 0 && t.bot_al) || (gy == N && t.top_al);
+            if (FIX && wall && !isolated) wallmask |= 1u << (rj * C + ci);
         }
     }
-    __syncthreads();                      // the zero fill of the edge arrays is complete
-    publish_all<C, R>(p, sB, sT);
-
-    const bool multi = a.ntx * a.nty > 1;
-    unsigned int ev = a.base + 1;
-    if (multi) post(a.flags + tile, ev);  // event base + 1: this tile has read its inputs from psi
-    mark(a, tile, 1);
+    __syncthreads();                      // the zero fill of the edge arrays and the tables are complete
+#pragma unroll
+    for (int ci = 0; ci < C; ++ci) {      // q of the two middle rows moves to shared memory (read back by this thread only)
+        sB[2 * TOPOFF + ci * 32] = q[R / 2 - 1][ci];
+        sB[3 * TOPOFF + ci * 32] = q[R / 2][ci];
+    }
+    publish_all<C, R, TOPOFF>(p, sB, fl);
+    mark(a, 1);
 
     const int T = a.T;
     const int nrounds = (a.nsweeps + T - 1) / T;
     for (int r = 0; r < nrounds; ++r) {
         const int ns = min(T, a.nsweeps - r * T);
-        for (int s = 0; s < ns; ++s) {
-            half_sweep<C, R, 0>(p, q, a.cb, a.omb, sB, sT, wallmask, lane);     // red = (i + j) even first (G9)
-            half_sweep<C, R, 1>(p, q, a.cb, a.omb, sB, sT, wallmask, lane);
+        if (odd_origin) {
+            for (int s = 0; s < ns; ++s) {                                    // red = (i + j) even first (G9): local colour 1 here
+                half_sweep<C, R, 1, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
+                half_sweep<C, R, 0, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
+            }
+        } else {
+            for (int s = 0; s < ns; ++s) {
+                half_sweep<C, R, 0, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
+                half_sweep<C, R, 1, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
+            }
         }
-        mark(a, tile, 2 + 4 * r);
+        mark(a, 2 + 4 * r);
         if (r == nrounds - 1) break;
-        // ---- halo exchange through L2 ----
-        double* const xb = (r & 1) ? a.x1 : a.x0;
+
+        // ---- halo exchange through L2: tagged data, no fence, no flag ----
+        // Opaque copies: everything derived from them is recomputed here every round instead of being hoisted out of
+        // the round loop, where it would stay live across the sweeps and push q into local memory.
+        const int z = opaque_zero();
+        const int tid_o = ((int)threadIdx.y + z) * 32 + (int)threadIdx.x, nth_o = ((int)blockDim.y + z) * 32;
+        double* const stage = sm + edge_doubles;
+        const uint2* const tabS = reinterpret_cast<const uint2*>(stage + R * C * (nth_o + 4));
+        const uint2* const tabR = tabS + a.ns_per * nth_o;
+        const unsigned int* const masks = reinterpret_cast<const unsigned int*>(tabR + a.nr_per * nth_o);
+        uint4* const xb = (r & 1) ? a.x1 : a.x0;
+        const unsigned int tag = a.base + 1u + (unsigned int)r;
+
+        {   // owners stage the strip values, then all threads store strip units, consecutive threads = consecutive x
+            const unsigned int smask = masks[tid_o];
 #pragma unroll
-        for (int rj = 0; rj < R; ++rj) {
-            const int gy = gy0 + rj;
-            if (x_core && gy >= cy0 && gy < cy1) {
-                const bool strip = gy < cy0 + a.halo || gy >= cy1 - a.halo || gx0 < cx0 + a.halo || gx0 + C > cx1 - a.halo;
-                if (strip) store4(xb + (size_t)gy * pitch + gx0, p[rj]);
+            for (int k = 0; k < R * C; ++k)
+                if ((smask >> k) & 1u) stage[k * (nth_o + 4) + tid_o] = p[k / C][k % C];
+            __syncthreads();
+            for (int i = 0; i < a.ns_per; ++i) {
+                const uint2 e = tabS[i * nth_o + tid_o];
+                if (e.x != NO_UNIT) st_unit(xb + e.x, stage[e.y], tag);
             }
         }
-        ev += 1;
-        post(a.flags + tile, ev);
-        mark(a, tile, 3 + 4 * r);
-        wait_neighbours(a, bi, bj, ev);
-        mark(a, tile, 4 + 4 * r);
-        // Reload the ring.  What arrives is final as it stands: the owners keep wall points and the padding columns at +0.0.
-        // Loads go straight into the micro-tile registers, so all of a thread's rows are in flight together.
+        mark(a, 3 + 4 * r);
+        // All threads fetch ring units (4 in flight per thread), validate, and stage the values for their owners.
+        // While some unit of the warp does not carry the tag yet, ONE lane polls one such unit (2 100 pollers on the whole
+        // chip: waiting tiles do not load L2), then every lane fetches its missing units again.
+        for (int i0 = 0; i0 < a.nr_per; i0 += 4) {
+            uint2 e[4];
+            uint4 v[4];
+            unsigned int bad = 0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) e[j] = i0 + j < a.nr_per ? tabR[(i0 + j) * nth_o + tid_o] : make_uint2(NO_UNIT, 0u);
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (e[j].x != NO_UNIT) v[j] = ld_unit(xb + e[j].x);
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (e[j].x != NO_UNIT && !unit_ok(v[j], tag)) bad |= 1u << j;
+            unsigned int waiting = __ballot_sync(0xffffffffu, bad != 0u);
+            if (waiting) {
+                const long long t0 = clock64();
+                while (waiting) {
+                    int giveup = 0;
+                    if ((int)threadIdx.x == __ffs((int)waiting) - 1) {
+                        unsigned int off = e[3].x;                     // the first missing unit of this lane
+                        if (bad & 4u) off = e[2].x;
+                        if (bad & 2u) off = e[1].x;
+                        if (bad & 1u) off = e[0].x;
+                        while (!unit_ok(ld_unit(xb + off), tag)) {
+                            if (*(volatile unsigned int*)a.err != 0u) { giveup = 1; break; }      // some tile gave up: do not wait again
+                            if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) { atomicExch(a.err, 1u); giveup = 1; break; }
+                        }
+                    }
+                    if (__any_sync(0xffffffffu, giveup)) break;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        if ((bad >> j) & 1u) {
+                            v[j] = ld_unit(xb + e[j].x);
+                            if (unit_ok(v[j], tag)) bad &= ~(1u << j);
+                        }
+                    waiting = __ballot_sync(0xffffffffu, bad != 0u);
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (e[j].x != NO_UNIT) stage[e[j].y] = unit_value(v[j]);
+        }
+        __syncthreads();
         {
-            const bool xr = x_in && gx0 >= cx0 - a.halo && gx0 < cx1 + a.halo;
+            const unsigned int rmask = masks[nth_o + tid_o];
 #pragma unroll
-            for (int rj = 0; rj < R; ++rj) {
-                const int gy = gy0 + rj;
-                const bool core = x_core && gy >= cy0 && gy < cy1;
-                const bool ring = xr && !core && gy >= 0 && gy <= N && gy >= cy0 - a.halo && gy < cy1 + a.halo;
-                if (ring) load4(xb + (size_t)gy * pitch + gx0, p[rj], true);
-            }
+            for (int k = 0; k < R * C; ++k)
+                if ((rmask >> k) & 1u) p[k / C][k % C] = stage[k * (nth_o + 4) + tid_o];
         }
-        publish_all<C, R>(p, sB, sT);
-        mark(a, tile, 5 + 4 * r);
+        mark(a, 4 + 4 * r);
+        publish_all<C, R, TOPOFF>(p, sB, fl);
+        mark(a, 5 + 4 * r);
     }
 
-    // every neighbour has read its halo of the INPUT psi before this tile overwrites its core
-    if (multi) wait_neighbours(a, bi, bj, a.base + 1);
+    // ---- store the core (walls are exactly +0.0); the geometry is recomputed, not kept live across the sweeps ----
+    {
+        const int z = opaque_zero();
+        const int nw = (int)blockDim.y + z;
+        const TileGeom te = tile_geom(a.N + z, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R,
+                                      32 * C, nw * R);
+        const int ex0 = te.ox + ((int)threadIdx.x + z) * C, ey0 = te.oy + ((int)threadIdx.y + z) * R, Ne = a.N + z;
 #pragma unroll
-    for (int rj = 0; rj < R; ++rj) {
-        const int gy = gy0 + rj;
-        if (x_core && gy >= cy0 && gy < cy1) store4(a.psi + (size_t)gy * pitch + gx0, p[rj]);
+        for (int rj = 0; rj < R; ++rj) {
+#pragma unroll
+            for (int ci = 0; ci < C; ++ci) {
+                const int gx = ex0 + ci, gy = ey0 + rj;
+                const bool upd = gx >= 1 && gx <= Ne - 1 && gy >= 1 && gy <= Ne - 1;
+                if (gx >= te.cx0 && gx < te.cx1 && gy >= te.cy0 && gy < te.cy1)
+                    a.psi_out[(size_t)gy * a.pitch + gx] = upd ? p[rj][ci] : 0.0;
+            }
+        }
     }
 }
 
 // ---- compiled variants ------------------------------------------------------------------------------
 struct Variant {
     int C, R, maxw;
-    const void* fn;
+    const void* fn;        // every wall isolated by alignment (the plans of large grids)
+    const void* fn_fix;    // with the wall-mask fix-up (a tile that holds both walls of one direction)
 };
 const Variant VARIANTS[] = {
-    {4, 8, 12, (const void*)k_resident<4, 8, 12>},     // 32 points per thread, up to 170 registers
-    {4, 6, 16, (const void*)k_resident<4, 6, 16>},     // 24 points per thread, up to 128 registers
+    {4, 8, 12, (const void*)k_resident<4, 8, 12, false>, (const void*)k_resident<4, 8, 12, true>},     // 32 points per thread, up to 170 registers
+    {4, 6, 16, (const void*)k_resident<4, 6, 16, false>, (const void*)k_resident<4, 6, 16, true>},     // 24 points per thread, up to 128 registers
 };
 constexpr int NVARIANTS = sizeof(VARIANTS) / sizeof(VARIANTS[0]);
 
-int smem_bytes_for(int C, int R, int warps) {
-    (void)R;
-    return (int)sizeof(double) * (2 * (warps + 1) * C * 32);
-}
-
 inline int cdiv(int a, int b) { return (a + b - 1) / b; }
 inline int round_up(int a, int m) { return cdiv(a, m) * m; }
+
+int region_total(const Region& g) { return rect_count(g.r[0]) + rect_count(g.r[1]) + rect_count(g.r[2]) + rect_count(g.r[3]); }
+
+// Checks that every tile of the candidate fits its thread grid and counts the exchange units per thread.
+bool finish_plan(ResidentPlan& pl, int N, int max_smem) {
+    const int W = 32 * pl.C, H = pl.warps * pl.R, nth = 32 * pl.warps;
+    int smax = 0, rmax = 0;
+    for (int bj = 0; bj < pl.nty; ++bj)
+        for (int bi = 0; bi < pl.ntx; ++bi) {
+            const TileGeom t = tile_geom(N, pl.CW, pl.CH, pl.halo, pl.ntx, pl.nty, bi, bj, pl.C, pl.R, W, H);
+            if (!t.fits) return false;
+            if (pl.ntiles > 1) {
+                smax = std::max(smax, region_total(send_region(t, N, pl.halo, bi, bj, pl.ntx, pl.nty)));
+                rmax = std::max(rmax, region_total(recv_region(t, N, pl.halo)));
+            }
+        }
+    pl.ns_per = cdiv(smax, nth);
+    pl.nr_per = cdiv(rmax, nth);
+    const int maxw = VARIANTS[pl.variant].maxw;
+    const size_t smem = pl.ntiles > 1 ? smem_layout_bytes(pl.C, pl.R, maxw, pl.warps, pl.ns_per, pl.nr_per)
+                                      : 8 * (size_t)(4 * (maxw + 1) * pl.C * 32);
+    pl.fixup = pl.ntx == 1 || pl.nty == 1;
+    if (smem > (size_t)max_smem) return false;
+    pl.smem_bytes = (int)smem;
+    return true;
+}
 
 }  // namespace
 
@@ -310,30 +548,29 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
         const Variant& v = VARIANTS[vi];
         cudaFuncAttributes fa;
         if (cudaFuncGetAttributes(&fa, v.fn) != cudaSuccess) { cudaGetLastError(); continue; }
+        cudaFuncAttributes fb;
+        if (cudaFuncGetAttributes(&fb, v.fn_fix) != cudaSuccess) { cudaGetLastError(); continue; }
+        fa.numRegs = std::max(fa.numRegs, fb.numRegs);
+        fa.maxThreadsPerBlock = std::min(fa.maxThreadsPerBlock, fb.maxThreadsPerBlock);
         const int max_warps = std::min(v.maxw, std::min(fa.maxThreadsPerBlock / 32, (int)(prop.regsPerBlock / (32 * std::max(fa.numRegs, 1)))));
         const int W = 32 * v.C;                  // tile width in points
         for (int warps = 1; warps <= max_warps; ++warps) {
             const int H = warps * v.R;           // tile height in points
-            const int smem = smem_bytes_for(v.C, v.R, warps);
-            if (smem > (int)prop.sharedMemPerBlockOptin) continue;
+            ResidentPlan c;
+            c.ok = true; c.variant = vi; c.C = v.C; c.R = v.R; c.warps = warps; c.regs = fa.numRegs; c.sm_count = sms;
             // single tile: the whole grid in one CTA, no exchange at all
-            if (G <= W && G <= H) {
+            if (G + v.C - 1 <= W && G + v.R - 1 <= H) {
                 const double cost = (double)H * W * 0.11 + 150.0;
-                if (cost < best_cost) {
-                    best_cost = cost;
-                    best = ResidentPlan{};
-                    best.ok = true; best.variant = vi; best.C = v.C; best.R = v.R; best.warps = warps;
-                    best.T = 1 << 30; best.halo = 0; best.CW = round_up(G, v.C); best.CH = round_up(G, 2);
-                    best.ntx = best.nty = best.ntiles = 1; best.smem_bytes = smem; best.regs = fa.numRegs; best.sm_count = sms;
-                }
+                c.T = 1 << 30; c.halo = 0; c.CW = round_up(G, v.C); c.CH = round_up(G, 2); c.ntx = c.nty = c.ntiles = 1;
+                if (cost < best_cost && finish_plan(c, P.N, (int)prop.sharedMemPerBlockOptin)) { best_cost = cost; best = c; }
                 continue;
             }
-            for (int T = 2; T <= 16; T += 2) {   // halo = 2T must be a multiple of C = 4 (chunks never straddle the core edge)
+            for (int T = 2; T <= 16; T += 2) {   // halo = 2T, a multiple of C = 4
                 if (T_override > 0 && T != T_override) continue;
                 const int halo = 2 * T;
                 // x: either one tile column without an x-halo, or columns of CW <= W - 2 halo
                 int CW, ntx;
-                if (G + halo <= W) { CW = round_up(G, v.C); ntx = 1; }          // origin is -halo: [0, G) must still fit
+                if (G + v.C - 1 <= W) { CW = round_up(G, v.C); ntx = 1; }
                 else {
                     const int cwmax = W - 2 * halo;
                     if (cwmax < halo || cwmax < v.C) continue;
@@ -341,10 +578,12 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
                     CW = round_up(cdiv(G, ntx), v.C);
                     if (CW > cwmax) continue;
                     ntx = cdiv(G, CW);
-                    if (G - (ntx - 1) * CW < halo || CW < halo) continue;     // the halo must come from adjacent tiles only
+                    // the halo must come from adjacent tiles only, and must not reach a wall through an edge tile (only an
+                // edge tile isolates the wall; elsewhere nothing keeps a wall point inside the thread grid at 0)
+                if (G - (ntx - 1) * CW <= halo || CW <= halo) continue;
                 }
                 int CH, nty;
-                if (G + halo <= H) { CH = round_up(G, 2); nty = 1; }
+                if (G + v.R - 1 <= H) { CH = round_up(G, 2); nty = 1; }
                 else {
                     const int chmax = H - 2 * halo;
                     if (chmax < halo || chmax < 2) continue;
@@ -352,30 +591,25 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
                     CH = round_up(cdiv(G, nty), 2);
                     if (CH > chmax) continue;
                     nty = cdiv(G, CH);
-                    if (G - (nty - 1) * CH < halo || CH < halo) continue;
+                    if (G - (nty - 1) * CH <= halo || CH <= halo) continue;
                 }
-                if (ntx * nty > sms) continue;
-                // cost per sweep in SM cycles: shared-memory-bound compute of the whole tile + two barriers + exchange / T
+                if (ntx * nty > sms || ntx * nty < 2) continue;
+                // cost per sweep in SM cycles: compute of the whole tile + two barriers + exchange / T
                 const double cost = (double)H * W * 0.11 + 150.0 + 3000.0 / T;
-                if (cost < best_cost) {
-                    best_cost = cost;
-                    best = ResidentPlan{};
-                    best.ok = true; best.variant = vi; best.C = v.C; best.R = v.R; best.warps = warps;
-                    best.T = T; best.halo = halo; best.CW = CW; best.CH = CH; best.ntx = ntx; best.nty = nty;
-                    best.ntiles = ntx * nty; best.smem_bytes = smem; best.regs = fa.numRegs; best.sm_count = sms;
-                }
+                c.T = T; c.halo = halo; c.CW = CW; c.CH = CH; c.ntx = ntx; c.nty = nty; c.ntiles = ntx * nty;
+                if (cost < best_cost && finish_plan(c, P.N, (int)prop.sharedMemPerBlockOptin)) { best_cost = cost; best = c; }
             }
         }
     }
     if (best.ok) {
-        const Variant& v = VARIANTS[best.variant];
-        if (cudaFuncSetAttribute(v.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin) != cudaSuccess) {
+        const void* fn = best.fixup ? VARIANTS[best.variant].fn_fix : VARIANTS[best.variant].fn;
+        if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin) != cudaSuccess) {
             cudaGetLastError();
             best.ok = false;
             return best;
         }
         int per_sm = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, v.fn, 32 * best.warps, best.smem_bytes) != cudaSuccess ||
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 32 * best.warps, best.smem_bytes) != cudaSuccess ||
             per_sm * sms < best.ntiles) {
             cudaGetLastError();
             best.ok = false;
@@ -392,34 +626,34 @@ void resident_describe(const ResidentPlan& pl, char* buf, int len) {
     else
         std::snprintf(buf, (size_t)len,
                       "%dx%d tiles of %dx%d core + halo %d, T=%d sweeps per exchange, %d warps x (%dx%d micro-tiles), "
-                      "%d regs, %d B smem, %d SMs",
-                      pl.ntx, pl.nty, pl.CW, pl.CH, pl.halo, pl.T, pl.warps, pl.C, pl.R, pl.regs, pl.smem_bytes, pl.sm_count);
+                      "%d+%d exchange units per thread, %d regs, %d B smem, %d SMs",
+                      pl.ntx, pl.nty, pl.CW, pl.CH, pl.halo, pl.T, pl.warps, pl.C, pl.R, pl.ns_per, pl.nr_per, pl.regs,
+                      pl.smem_bytes, pl.sm_count);
 }
 
 int resident_variants() { return NVARIANTS; }
 
-int resident_flag_words(const ResidentPlan& plan) { return (plan.ok ? plan.ntiles : 0) + 1; }
-int resident_error_word_index(const ResidentPlan& plan) { return plan.ok ? plan.ntiles : 0; }
-
-int resident_sweeps(const Params& P, const ResidentPlan& pl, double* psi, double* xa, double* xb, const double* w,
-                    unsigned int* flags, unsigned int* epoch, int nsweeps, cudaStream_t st, long long* trace_dev,
-                    int trace_cap) {
+int resident_sweeps(const Params& P, const ResidentPlan& pl, const double* psi_in, double* psi_out, void* xa, void* xb,
+                    const double* w, unsigned int* err_word, unsigned int* epoch, int nsweeps, cudaStream_t st,
+                    long long* trace_dev, int trace_cap) {
     if (!pl.ok) return -(int)cudaErrorNotSupported;
-    if (nsweeps <= 0) return 0;
+    if (nsweeps <= 0 || psi_in == psi_out) return -(int)cudaErrorInvalidValue;
     ResArgs a;
     a.N = P.N; a.pitch = P.pitch; a.cb = P.cb; a.omb = P.omb; a.cq = P.cq;
-    a.w = w; a.psi = psi; a.x0 = xa; a.x1 = xb;
-    a.flags = flags; a.err = flags + resident_error_word_index(pl);
+    a.w = w; a.psi_in = psi_in; a.psi_out = psi_out; a.x0 = (uint4*)xa; a.x1 = (uint4*)xb;
+    a.err = err_word;
     a.base = *epoch;
     a.nsweeps = nsweeps;
     a.T = pl.ntiles == 1 ? nsweeps : pl.T;
     a.halo = pl.halo; a.CW = pl.CW; a.CH = pl.CH; a.ntx = pl.ntx; a.nty = pl.nty;
+    a.ns_per = pl.ns_per; a.nr_per = pl.nr_per;
     a.trace = trace_dev; a.trace_cap = trace_cap;
     const int nrounds = (nsweeps + a.T - 1) / a.T;
-    *epoch += (unsigned int)nrounds + 1u;           // events base + 1 .. base + nrounds are used by this launch
+    *epoch += (unsigned int)nrounds;                // tags base + 1 .. base + nrounds - 1 are used by this launch
     void* args[] = {&a};
     const dim3 grid(pl.ntx, pl.nty), block(32, pl.warps);
-    const cudaError_t e = cudaLaunchCooperativeKernel(VARIANTS[pl.variant].fn, grid, block, args, (size_t)pl.smem_bytes, st);
+    const void* fn = pl.fixup ? VARIANTS[pl.variant].fn_fix : VARIANTS[pl.variant].fn;
+    const cudaError_t e = cudaLaunchCooperativeKernel(fn, grid, block, args, (size_t)pl.smem_bytes, st);
     if (e != cudaSuccess) { cudaGetLastError(); return -(int)e; }
     return 1;
 }

@@ -1,6 +1,6 @@
 // cavity_resident.cuh — the resident sweep engine (a1): one persistent CTA per tile, psi and the scaled
 // right-hand side held in registers for all S sweeps of a stage, temporal blocking with a 2T-deep halo that
-// is refreshed through L2 every T sweeps under neighbour-flag synchronisation.
+// is refreshed through L2 every T sweeps as self-validating tagged data (no fence, flag or grid barrier).
 // See DESIGN.md "Resident engine".  Plain CUDA: no torch types.
 #pragma once
 #include <cuda_runtime.h>
@@ -20,6 +20,8 @@ struct ResidentPlan {
     int CW = 0, CH = 0;   // core (owned) points per tile in x and y; tile (bi, bj) owns [bi CW, (bi+1) CW) x [bj CH, (bj+1) CH)
     int ntx = 0, nty = 0; // tiles in x and y
     int ntiles = 0;
+    int ns_per = 0, nr_per = 0;   // exchange units each thread stores / fetches per round (0 for a single tile)
+    bool fixup = false;           // some tile holds both walls of one direction: the kernel variant with the wall-mask fix-up
     int smem_bytes = 0;
     int regs = 0;         // registers per thread of the chosen variant (as compiled)
     int sm_count = 0;
@@ -31,20 +33,18 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override = 0, int 
 int resident_variants();
 void resident_describe(const ResidentPlan& plan, char* buf, int len);
 
-// Flag words the engine needs (per tile, plus the error word); the caller zero-fills them once.
-int resident_flag_words(const ResidentPlan& plan);
+// Doubles behind ONE exchange buffer (the engine needs two): a 16-byte unit per point of a pitch x (N+1) field.
+inline size_t resident_exchange_doubles(size_t field_doubles) { return 2 * field_doubles; }
 
-// nsweeps red-black sweeps of a1 on psi in place with right-hand side cq * w (w = the stage's input vorticity,
-// scaled on the fly exactly as scale_rhs does).  xa, xb: two exchange fields of the same layout as psi.
-// flags: resident_flag_words() words; *epoch is the host-side flag epoch, advanced by this call.
-// trace_dev (profiling only): device array of ntiles x trace_cap clock64 stamps, slot 0 = start, 1 = inputs loaded,
-// then per round r: 2 + 4r computed, 3 + 4r strips posted, 4 + 4r neighbours arrived, 5 + 4r halo reloaded.
+// nsweeps red-black sweeps of a1: reads psi_in, writes psi_out (two different fields), right-hand side cq * w (w = the
+// stage's input vorticity, scaled on the fly exactly as scale_rhs does).  xa, xb: the two exchange buffers (zero-filled once
+// by the caller).  err_word: one device word, zero-filled once; non-zero afterwards = a tile gave up waiting for a neighbour.
+// *epoch is the host-side tag epoch, advanced by this call (tags are unique per round and per launch).
+// trace_dev (profiling only): device array of ntiles x trace_cap %globaltimer stamps (ns), slot 0 = start, 1 = inputs loaded,
+// then per round r: 2 + 4r sweeps done, 3 + 4r border strips stored, 4 + 4r ring received, 5 + 4r edges republished.
 // Returns the number of kernel launches (1), or a negative cudaError_t.
-int resident_sweeps(const Params& P, const ResidentPlan& plan, double* psi, double* xa, double* xb, const double* w,
-                    unsigned int* flags, unsigned int* epoch, int nsweeps, cudaStream_t st,
+int resident_sweeps(const Params& P, const ResidentPlan& plan, const double* psi_in, double* psi_out, void* xa, void* xb,
+                    const double* w, unsigned int* err_word, unsigned int* epoch, int nsweeps, cudaStream_t st,
                     long long* trace_dev = nullptr, int trace_cap = 0);
-
-// 0 if no tile ever timed out waiting for a neighbour (checked by the API after synchronising).
-int resident_error_word_index(const ResidentPlan& plan);
 
 }  // namespace cavk

@@ -109,7 +109,7 @@ def test_resident_engine_forced_exchange_period_bit_exact(cav, orc, N, S, T):
     psi0, w0 = random_fields(N, 31337 + N + S)
     g = cav.Cavity(N, 800.0, 0.4 / N, 1.9, S, engine="resident")
     try:
-        g.set_resident_T(T)
+        g.set_resident_plan(T)
     except cav.CavityError:
         g.close()
         pytest.skip("no resident plan with T=%d for N=%d" % (T, N))
@@ -223,8 +223,13 @@ def check_against_golden(cav, k, engine, max_step=None):
         ewi = np.max(np.abs(ws[inner, inner] - np.array(cp["omega"])[inner, inner])) / cp["omega_absmax_interior"]
         assert ep <= TOL and ew <= TOL and ewi <= TOL, (k, engine, cp["label"], ep, ew, ewi)
         d = g.diag()
+        # The residual r = lap_h(psi) + omega carries a rounding error of a few eps * 4 max|psi| / h^2 per point however it
+        # is evaluated; after config 5's 10 000 Poisson-only sweeps the residual IS that floor (1.7e-10), so there the FMA
+        # kernels and the plain oracle agree only to that absolute level (tolerance).
+        floor = 64.0 * np.finfo(np.float64).eps * 4.0 * cp["psi_absmax"] * wl.N * wl.N
         for key in ("kinetic_energy", "enstrophy", "res_l2", "res_inf"):
-            assert abs(d[key] - cp[key]) <= 1e-8 * abs(cp[key]), (k, engine, cp["label"], key, d[key], cp[key])
+            atol = floor if key.startswith("res_") else 0.0
+            assert abs(d[key] - cp[key]) <= 1e-8 * abs(cp[key]) + atol, (k, engine, cp["label"], key, d[key], cp[key])
         assert abs(np.max(np.abs(psi)) - cp["psi_absmax"]) <= TOL * cp["psi_absmax"]
         assert abs(np.min(psi) - cp["psi_min"]) <= TOL * cp["psi_absmax"]
         # invariants that hold at any size: psi is exactly 0 on the walls
