@@ -42,6 +42,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
               "-D_GLIBCXX_USE_CXX11_ABI=1"] + ARCH
     if verbose:
         common += ["-Xptxas", "-v"]
+    common += os.environ.get("CAV_NVCC_FLAGS", "").split()      # tuning experiments (e.g. -DCAV_RECV_BATCH=8)
     for s in SOURCES:
         o = os.path.join(CSRC, s[:-3] + ".o")
         cmd = common + ["-I", inc, "-c", os.path.join(CSRC, s), "-o", o]

@@ -36,6 +36,7 @@ struct cav_ctx {
     double* T = nullptr;             // first three terms of eq 13
     double* scratch = nullptr;       // diagnostics partials
     double* out4 = nullptr;          // diagnostics result (device)
+    void* tables = nullptr;          // resident engine: per-plan exchange tables (own allocation, rebuilt on re-plan)
     unsigned int* err_word = nullptr;// resident engine: device error word (a tile gave up waiting for a neighbour)
     unsigned int epoch = 0;          // resident engine: tag epoch (host side)
     size_t field_doubles = 0;
@@ -90,6 +91,18 @@ void drop_graph(cav_ctx* c) {
     c->graph_launches = 0;
 }
 
+// (re)builds the exchange tables of c->plan; on failure the plan is marked unusable
+void build_plan_tables(cav_ctx* c) {
+    if (c->tables) { try { c10::cuda::CUDACachingAllocator::raw_delete(c->tables); } catch (...) {} c->tables = nullptr; }
+    const size_t nb = cavk::resident_table_bytes(c->plan);
+    if (!c->plan.ok || nb == 0) return;
+    try { c->tables = c10::cuda::CUDACachingAllocator::raw_alloc_with_stream(nb, c->st); } catch (...) { c->tables = nullptr; }
+    if (!c->tables) { c->plan.ok = false; return; }
+    const int nl = cavk::resident_build_tables(c->P, c->plan, c->tables, c->st);
+    if (nl < 0 || cudaStreamSynchronize(c->st) != cudaSuccess) { cudaGetLastError(); c->plan.ok = false; return; }
+    c->launches += nl;
+}
+
 void resolve_engine(cav_ctx* c) {
     int e = c->engine_req;
     if (e == CAV_ENGINE_AUTO) e = c->plan.ok ? CAV_ENGINE_RESIDENT : CAV_ENGINE_STREAM;
@@ -100,7 +113,7 @@ void resolve_engine(cav_ctx* c) {
 int enqueue_sweeps(cav_ctx* c, const double* w_in, int nsweeps, long long& nl) {
     if (nsweeps <= 0) return CAV_OK;
     if (c->engine == CAV_ENGINE_RESIDENT) {
-        LAUNCH(cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, w_in, c->err_word, &c->epoch, nsweeps, c->st));
+        LAUNCH(cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, c->tables, w_in, c->err_word, &c->epoch, nsweeps, c->st));
         std::swap(c->psi, c->psi2);
     } else {
         LAUNCH(cavk::scale_rhs(c->P, w_in, c->q, c->st));
@@ -221,6 +234,7 @@ CAV_API int cav_create(cav_ctx** out, int N, double Re, double dt, double sor_om
         c->err_word = (unsigned int*)p;
         if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) throw (int)CAV_ECUDA;
         if (cudaStreamSynchronize(c->st) != cudaSuccess) throw (int)CAV_ECUDA;
+        build_plan_tables(c);
         resolve_engine(c);
     } catch (int code) {
         rc = code;
@@ -247,6 +261,9 @@ CAV_API void cav_destroy(cav_ctx* c) {
         if (c->ev1) cudaEventDestroy(c->ev1);
         if (c->slab) {
             try { c10::cuda::CUDACachingAllocator::raw_delete(c->slab); } catch (...) {}
+        }
+        if (c->tables) {
+            try { c10::cuda::CUDACachingAllocator::raw_delete(c->tables); } catch (...) {}
         }
         cudaGetLastError();
     }
@@ -344,7 +361,10 @@ CAV_API int cav_set_resident_plan(cav_ctx* c, int sweeps_per_exchange, int varia
     CK(cudaStreamSynchronize(c->st));
     cavk::ResidentPlan pl = cavk::resident_plan(c->P, c->device, sweeps_per_exchange, variant < 0 ? -1 : variant);
     if (!pl.ok) return CAV_ENOTSUP;
+    const cavk::ResidentPlan old = c->plan;
     c->plan = pl;
+    build_plan_tables(c);
+    if (!c->plan.ok) { c->plan = old; build_plan_tables(c); resolve_engine(c); return CAV_ENOMEM; }
     return CAV_OK;
 }
 
@@ -360,7 +380,7 @@ CAV_API int cav_trace_sweeps(cav_ctx* c, int nsweeps, long long* stamps_out, int
     int rc = CAV_OK;
     if (cudaMemsetAsync(dev, 0, n * sizeof(long long), c->st) != cudaSuccess) rc = CAV_ECUDA;
     if (rc == CAV_OK) {
-        int nl = cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, c->w[0], c->err_word, &c->epoch, nsweeps,
+        int nl = cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, c->tables, c->w[0], c->err_word, &c->epoch, nsweeps,
                                        c->st, dev, slots_per_tile);
         if (nl < 0) rc = CAV_ECUDA; else { c->launches += nl; std::swap(c->psi, c->psi2); }
     }

@@ -47,6 +47,12 @@ namespace {
 
 constexpr long long SPIN_TIMEOUT_CYCLES = 4000000000LL;   // ~2 s: a neighbour whose data never arrives is a bug, not a wait
 constexpr unsigned int NO_UNIT = 0xffffffffu;
+#ifndef CAV_QROWS
+#define CAV_QROWS 2             // rows of the micro-tile whose q lives in shared memory instead of registers
+#endif
+#ifndef CAV_RECV_BATCH
+#define CAV_RECV_BATCH 4        // ring units a thread keeps in flight at a time (4 registers each)
+#endif
 
 struct ResArgs {
     int N, pitch;
@@ -60,6 +66,7 @@ struct ResArgs {
     unsigned int base;      // tag epoch of this launch: round r is tagged base + 1 + r
     int nsweeps, T, halo, CW, CH, ntx, nty;
     int ns_per, nr_per;     // table entries per thread: strip units to store / ring units to fetch
+    const uint4* tables;    // per-plan exchange tables, one block per tile (k_build_tables)
     long long* trace;       // profiling only (cav_trace_sweeps): per tile, %globaltimer at the phase boundaries; else null
     int trace_cap;          // slots per tile
 };
@@ -145,12 +152,13 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
     // q of the two middle rows of the micro-tile lives in shared memory, in two more arrays of the same shape 2 TOPOFF and
     // 3 TOPOFF after the bottom edge array (same address register): 16 registers fewer held across the whole kernel.
     double* const sT = sB + TOPOFF;
-    constexpr int Q0 = R / 2 - 1;
-    double Lnb[R], Rnb[R], Bnb[C], Tnb[C], qs[2][C];
+    constexpr int QR = CAV_QROWS, Q0 = (R - QR) / 2;
+    double Lnb[R], Rnb[R], Bnb[C], Tnb[C], qs[QR][C];
 #pragma unroll
     for (int ci = 0; ci < C; ++ci) {
-        if (((ci + Q0) & 1) == K) qs[0][ci] = sB[2 * TOPOFF + ci * 32];
-        if (((ci + Q0 + 1) & 1) == K) qs[1][ci] = sB[3 * TOPOFF + ci * 32];
+#pragma unroll
+        for (int k = 0; k < QR; ++k)
+            if (((ci + Q0 + k) & 1) == K) qs[k][ci] = sB[(2 + k) * TOPOFF + ci * 32];
     }
 #pragma unroll
     for (int ci = 0; ci < C; ++ci) {
@@ -178,7 +186,7 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
             const double pS = rj > 0 ? p[rj - 1][ci] : Bnb[ci];
             const double pN = rj < R - 1 ? p[rj + 1][ci] : Tnb[ci];
             const double nb = (pW + pE) + (pS + pN);
-            const double qv = (rj == Q0 || rj == Q0 + 1) ? qs[rj - Q0][ci] : q[rj][ci];
+            const double qv = (rj >= Q0 && rj < Q0 + QR) ? qs[rj - Q0 < 0 ? 0 : (rj - Q0 >= QR ? QR - 1 : rj - Q0)][ci] : q[rj][ci];
             p[rj][ci] = fma(omb, p[rj][ci], fma(cb, nb, qv));
         }
     }
@@ -272,20 +280,101 @@ __host__ __device__ inline Region recv_region(const TileGeom& t, int N, int halo
     return g;
 }
 
+__host__ __device__ inline size_t xtab_bytes(int nth, int ns_per, int nr_per) {
+    return (4 + 2) * (size_t)(ns_per + nr_per) * nth + 4 * 2 * (size_t)nth;      // a multiple of 64
+}
 // Shared-memory layout (doubles unless said otherwise), nthreads = 32 nwarps:
 //   edges   4 (MAXW + 1) C 32            bottom / top rows of the micro-tiles, q of the two middle rows (sized for MAXW warps)
 //   stage   R C (nthreads + 4)           one slot per thread and micro-tile point, [point][thread] (+4: the 4 points of a chunk fall in different banks)
-//   tabS    ns_per nthreads uint2        {unit offset in the exchange buffer, staging slot} of the strip units this thread stores
-//   tabR    nr_per nthreads uint2        same for the ring units this thread fetches
+//   offS    ns_per nthreads u32          unit offset in the exchange buffer of the strip units this thread stores (NO_UNIT: none)
+//   offR    nr_per nthreads u32          same for the ring units this thread fetches
 //   masks   2 nthreads u32               bit k: point k of this thread's micro-tile is in the send region / in the ring
+//   slotS   ns_per nthreads u16          staging slot of each of those units
+//   slotR   nr_per nthreads u16
 __host__ __device__ inline size_t smem_layout_bytes(int C, int R, int maxw, int warps, int ns_per, int nr_per) {
     const size_t nth = 32 * (size_t)warps;
-    return 8 * (4 * (size_t)(maxw + 1) * C * 32 + (size_t)R * C * (nth + 4) + (size_t)(ns_per + nr_per) * nth) + 4 * 2 * nth;
+    return 8 * ((2 + CAV_QROWS) * (size_t)(maxw + 1) * C * 32 + (size_t)R * C * (nth + 4)) + xtab_bytes((int)nth, ns_per, nr_per);
+}
+
+// Global <-> micro-tile transfers of one warp, coalesced: the warp moves rows of 32 C consecutive doubles (lane = x), and a
+// per-warp shared-memory buffer of R rows x 32 C doubles transposes between that and the C-consecutive-points-per-lane
+// layout of the registers.  Points that are not interior (walls, outside, row padding) read as +0.0.
+template <int C, int R>
+__device__ __forceinline__ void warp_load_tile(double (&v)[R][C], const double* __restrict__ g, const int x0w, const int y0,
+                                               const int N, const int pitch, double* __restrict__ wbuf, const int lane) {
+#pragma unroll
+    for (int rj = 0; rj < R; ++rj) {
+        const int gy = y0 + rj;
+#pragma unroll
+        for (int j = 0; j < C; ++j) {
+            const int gx = x0w + j * 32 + lane;
+            const bool upd = gx >= 1 && gx <= N - 1 && gy >= 1 && gy <= N - 1;
+            wbuf[rj * (32 * C) + j * 32 + lane] = upd ? g[(size_t)gy * pitch + gx] : 0.0;
+        }
+    }
+    __syncwarp();
+#pragma unroll
+    for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+        for (int ci = 0; ci < C; ci += 2) {
+            const double2 d = *reinterpret_cast<const double2*>(wbuf + rj * (32 * C) + lane * C + ci);
+            v[rj][ci] = d.x; v[rj][ci + 1] = d.y;
+        }
+    __syncwarp();
+}
+
+struct XTab {
+    unsigned int *offS, *offR, *masks;
+    unsigned short *slotS, *slotR;
+};
+__device__ __forceinline__ XTab xtab(void* base, int nth, int ns_per, int nr_per) {
+    XTab t;
+    t.offS = reinterpret_cast<unsigned int*>(base);
+    t.offR = t.offS + ns_per * nth;
+    t.masks = t.offR + nr_per * nth;
+    t.slotS = reinterpret_cast<unsigned short*>(t.masks + 2 * nth);
+    t.slotR = t.slotS + ns_per * nth;
+    return t;
+}
+
+// Builds, once per plan, the exchange tables of every tile in global memory (one block of xtab_bytes per tile, in the
+// layout the sweep kernel copies to shared memory at launch): which exchange unit each thread stores / fetches and which
+// staging slot it belongs to, and each thread's masks of micro-tile points that are sent / received.
+template <int C, int R>
+__global__ void k_build_tables(const ResArgs a, unsigned char* __restrict__ out) {
+    const int lane = threadIdx.x, warp = threadIdx.y, nwarps = blockDim.y;
+    const int tid = warp * 32 + lane, nthreads = nwarps * 32;
+    const int N = a.N, bi = blockIdx.x, bj = blockIdx.y;
+    const TileGeom t = tile_geom(N, a.CW, a.CH, a.halo, a.ntx, a.nty, bi, bj, C, R, 32 * C, nwarps * R);
+    const int gx0 = t.ox + lane * C, gy0 = t.oy + warp * R;
+    const XTab xt = xtab(out + (size_t)(bj * a.ntx + bi) * xtab_bytes(nthreads, a.ns_per, a.nr_per), nthreads, a.ns_per, a.nr_per);
+    const Region gs = send_region(t, N, a.halo, bi, bj, a.ntx, a.nty), gr = recv_region(t, N, a.halo);
+    for (int i = 0; i < a.ns_per + a.nr_per; ++i) {
+        const bool snd = i < a.ns_per;
+        const int u = (snd ? i : i - a.ns_per) * nthreads + tid;
+        int x = 0, y = 0;
+        uint2 e = make_uint2(NO_UNIT, 0u);
+        if (region_point(snd ? gs : gr, u, x, y)) {
+            const int lx = x - t.ox, ly = y - t.oy;                        // owner: lane lx / C, warp ly / R
+            e.x = (unsigned int)(y * a.pitch + x);                         // < 2^31: N <= 32766
+            e.y = (unsigned int)(((ly % R) * C + lx % C) * (nthreads + 4) + (ly / R) * 32 + lx / C);
+        }
+        (snd ? xt.offS : xt.offR)[(snd ? i : i - a.ns_per) * nthreads + tid] = e.x;
+        (snd ? xt.slotS : xt.slotR)[(snd ? i : i - a.ns_per) * nthreads + tid] = (unsigned short)e.y;
+    }
+    unsigned int smask = 0, rmask = 0;
+    for (int k = 0; k < R * C; ++k) {
+        if (region_has(gs, gx0 + k % C, gy0 + k / C)) smask |= 1u << k;
+        if (region_has(gr, gx0 + k % C, gy0 + k / C)) rmask |= 1u << k;
+    }
+    xt.masks[tid] = smask;
+    xt.masks[nthreads + tid] = rmask;
 }
 
 // MAXW = most warps per CTA this variant is launched with: 65536 / (32 MAXW) registers per thread are available.
-template <int C, int R, int MAXW, bool FIX>
-__global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const ResArgs a) {
+// PERSM = CTAs per SM the variant is built for (two half-size CTAs per SM hide each other's exchange and barrier latency).
+template <int C, int R, int MAXW, int PERSM, bool FIX>
+__global__ void __launch_bounds__(32 * MAXW, PERSM) k_resident(const ResArgs a) {
     constexpr int TOPOFF = (MAXW + 1) * C * 32;
     static_assert(C % 2 == 0 && R % 2 == 0 && R * C <= 32, "even micro-tile that fits the 32-bit point masks");
     extern __shared__ __align__(16) double sm[];
@@ -296,7 +385,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const ResArgs a) {
     mark(a, 0);
 
     // edge arrays; the slots no thread ever writes (warp -1, warp nwarps, unpublished wall rows) stay +0.0
-    constexpr int edge_doubles = 4 * TOPOFF;       // bottom edges, top edges, q of middle row 0, q of middle row 1
+    constexpr int edge_doubles = (2 + CAV_QROWS) * TOPOFF;       // bottom edges, top edges, q of the CAV_QROWS middle rows
     for (int k = tid; k < edge_doubles; k += nthreads) sm[k] = 0.0;
     double* const sB = sm + warp * C * 32 + lane;      // [MAXW + 1][C][32] bottom row of warp at [warp]; top rows TOPOFF further, at [warp + 1]
 
@@ -314,59 +403,41 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const ResArgs a) {
         if (t.top_al && warp == (N - t.oy) / R) fl &= ~FL_PUB_BOTTOM;          // that warp holds y = N .. N + R - 1
     }
 
-    // ---- exchange tables and masks (multi-tile plans only) ----
-    const bool multi = a.ntx * a.nty > 1;
-    if (multi) {
-        double* const stage_ = sm + edge_doubles;
-        uint2* const tabS = reinterpret_cast<uint2*>(stage_ + R * C * (nthreads + 4));
-        uint2* const tabR = tabS + a.ns_per * nthreads;
-        unsigned int* const masks = reinterpret_cast<unsigned int*>(tabR + a.nr_per * nthreads);
-        const Region gs = send_region(t, N, a.halo, bi, bj, a.ntx, a.nty), gr = recv_region(t, N, a.halo);
-        for (int i = 0; i < a.ns_per + a.nr_per; ++i) {
-            const bool snd = i < a.ns_per;
-            const int u = (snd ? i : i - a.ns_per) * nthreads + tid;
-            int x = 0, y = 0;
-            uint2 e = make_uint2(NO_UNIT, 0u);
-            if (region_point(snd ? gs : gr, u, x, y)) {
-                const int lx = x - t.ox, ly = y - t.oy;                        // owner: lane lx / C, warp ly / R
-                e.x = (unsigned int)(y * pitch + x);                           // < 2^31: N <= 32766
-                e.y = (unsigned int)(((ly % R) * C + lx % C) * (nthreads + 4) + (ly / R) * 32 + lx / C);
-            }
-            (snd ? tabS : tabR)[(snd ? i : i - a.ns_per) * nthreads + tid] = e;
-        }
-        unsigned int smask = 0, rmask = 0;
-#pragma unroll
-        for (int rj = 0; rj < R; ++rj)
-#pragma unroll
-            for (int ci = 0; ci < C; ++ci) {
-                if (region_has(gs, gx0_ + ci, gy0_ + rj)) smask |= 1u << (rj * C + ci);
-                if (region_has(gr, gx0_ + ci, gy0_ + rj)) rmask |= 1u << (rj * C + ci);
-            }
-        masks[tid] = smask;
-        masks[nthreads + tid] = rmask;
+    // ---- exchange tables and masks (multi-tile plans only): copied from the per-plan tables in global memory ----
+    if (a.ntx * a.nty > 1) {
+        const int n16 = (int)(xtab_bytes(nthreads, a.ns_per, a.nr_per) / 16);
+        const uint4* const src = a.tables + (size_t)(bj * a.ntx + bi) * n16;
+        uint4* const dst = reinterpret_cast<uint4*>(sm + edge_doubles + R * C * (nthreads + 4));
+        for (int k = tid; k < n16; k += nthreads) dst[k] = src[k];
     }
 
     // ---- load the micro-tile ----
     double p[R][C], q[R][C];
     unsigned int wallmask = 0;            // wall points that alignment could not isolate (psi = 0 there, eq 23-24)
+    {
+        double* const wbuf = sm + edge_doubles + warp * (R * 32 * C);         // inside the staging array, which is idle now
+        warp_load_tile<C, R>(p, a.psi_in, t.ox, gy0_, N, pitch, wbuf, lane);
+        warp_load_tile<C, R>(q, a.w, t.ox, gy0_, N, pitch, wbuf, lane);
+    }
 #pragma unroll
-    for (int rj = 0; rj < R; ++rj) {
+    for (int rj = 0; rj < R; ++rj)
 #pragma unroll
-        for (int ci = 0; ci < C; ++ci) {
-            const int gx = gx0_ + ci, gy = gy0_ + rj;
+        for (int ci = 0; ci < C; ++ci) q[rj][ci] = a.cq * q[rj][ci];          // +0.0 where the point is not interior
+    if (FIX) {
+#pragma unroll 1
+        for (int k = 0; k < R * C; ++k) {
+            const int gx = gx0_ + k % C, gy = gy0_ + k / C;
             const bool upd = gx >= 1 && gx <= N - 1 && gy >= 1 && gy <= N - 1;
-            p[rj][ci] = upd ? a.psi_in[(size_t)gy * pitch + gx] : 0.0;
-            q[rj][ci] = upd ? a.cq * a.w[(size_t)gy * pitch + gx] : 0.0;
             const bool wall = gx >= 0 && gx <= N && gy >= 0 && gy <= N && !upd;
             const bool isolated = (gx == 0 && t.left_al) || (gx == N && t.right_al) || (gy == 0 && t.bot_al) || (gy == N && t.top_al);
-            if (FIX && wall && !isolated) wallmask |= 1u << (rj * C + ci);
+            if (wall && !isolated) wallmask |= 1u << k;
         }
     }
     __syncthreads();                      // the zero fill of the edge arrays and the tables are complete
 #pragma unroll
     for (int ci = 0; ci < C; ++ci) {      // q of the two middle rows moves to shared memory (read back by this thread only)
-        sB[2 * TOPOFF + ci * 32] = q[R / 2 - 1][ci];
-        sB[3 * TOPOFF + ci * 32] = q[R / 2][ci];
+#pragma unroll
+        for (int k = 0; k < CAV_QROWS; ++k) sB[(2 + k) * TOPOFF + ci * 32] = q[(R - CAV_QROWS) / 2 + k][ci];
     }
     publish_all<C, R, TOPOFF>(p, sB, fl);
     mark(a, 1);
@@ -395,9 +466,8 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const ResArgs a) {
         const int z = opaque_zero();
         const int tid_o = ((int)threadIdx.y + z) * 32 + (int)threadIdx.x, nth_o = ((int)blockDim.y + z) * 32;
         double* const stage = sm + edge_doubles;
-        const uint2* const tabS = reinterpret_cast<const uint2*>(stage + R * C * (nth_o + 4));
-        const uint2* const tabR = tabS + a.ns_per * nth_o;
-        const unsigned int* const masks = reinterpret_cast<const unsigned int*>(tabR + a.nr_per * nth_o);
+        const XTab xt = xtab(stage + R * C * (nth_o + 4), nth_o, a.ns_per, a.nr_per);
+        const unsigned int* const masks = xt.masks;
         uint4* const xb = (r & 1) ? a.x1 : a.x0;
         const unsigned int tag = a.base + 1u + (unsigned int)r;
 
@@ -408,25 +478,28 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const ResArgs a) {
                 if ((smask >> k) & 1u) stage[k * (nth_o + 4) + tid_o] = p[k / C][k % C];
             __syncthreads();
             for (int i = 0; i < a.ns_per; ++i) {
-                const uint2 e = tabS[i * nth_o + tid_o];
-                if (e.x != NO_UNIT) st_unit(xb + e.x, stage[e.y], tag);
+                const unsigned int off = xt.offS[i * nth_o + tid_o];
+                if (off != NO_UNIT) st_unit(xb + off, stage[xt.slotS[i * nth_o + tid_o]], tag);
             }
         }
         mark(a, 3 + 4 * r);
         // All threads fetch ring units (4 in flight per thread), validate, and stage the values for their owners.
         // While some unit of the warp does not carry the tag yet, ONE lane polls one such unit (2 100 pollers on the whole
         // chip: waiting tiles do not load L2), then every lane fetches its missing units again.
-        for (int i0 = 0; i0 < a.nr_per; i0 += 4) {
-            uint2 e[4];
-            uint4 v[4];
+        constexpr int NB = CAV_RECV_BATCH;
+        for (int i0 = 0; i0 < a.nr_per; i0 += NB) {
+            uint2 e[NB];
+            uint4 v[NB];
             unsigned int bad = 0;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) e[j] = i0 + j < a.nr_per ? tabR[(i0 + j) * nth_o + tid_o] : make_uint2(NO_UNIT, 0u);
+            for (int j = 0; j < NB; ++j)
+                e[j] = i0 + j < a.nr_per ? make_uint2(xt.offR[(i0 + j) * nth_o + tid_o], xt.slotR[(i0 + j) * nth_o + tid_o])
+                                         : make_uint2(NO_UNIT, 0u);
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
+            for (int j = 0; j < NB; ++j)
                 if (e[j].x != NO_UNIT) v[j] = ld_unit(xb + e[j].x);
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
+            for (int j = 0; j < NB; ++j)
                 if (e[j].x != NO_UNIT && !unit_ok(v[j], tag)) bad |= 1u << j;
             unsigned int waiting = __ballot_sync(0xffffffffu, bad != 0u);
             if (waiting) {
@@ -434,10 +507,10 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const ResArgs a) {
                 while (waiting) {
                     int giveup = 0;
                     if ((int)threadIdx.x == __ffs((int)waiting) - 1) {
-                        unsigned int off = e[3].x;                     // the first missing unit of this lane
-                        if (bad & 4u) off = e[2].x;
-                        if (bad & 2u) off = e[1].x;
-                        if (bad & 1u) off = e[0].x;
+                        unsigned int off = e[NB - 1].x;                // the first missing unit of this lane
+#pragma unroll
+                        for (int j = NB - 2; j >= 0; --j)
+                            if ((bad >> j) & 1u) off = e[j].x;
                         while (!unit_ok(ld_unit(xb + off), tag)) {
                             if (*(volatile unsigned int*)a.err != 0u) { giveup = 1; break; }      // some tile gave up: do not wait again
                             if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) { atomicExch(a.err, 1u); giveup = 1; break; }
@@ -445,7 +518,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const ResArgs a) {
                     }
                     if (__any_sync(0xffffffffu, giveup)) break;
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
+                    for (int j = 0; j < NB; ++j)
                         if ((bad >> j) & 1u) {
                             v[j] = ld_unit(xb + e[j].x);
                             if (unit_ok(v[j], tag)) bad &= ~(1u << j);
@@ -454,7 +527,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const ResArgs a) {
                 }
             }
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
+            for (int j = 0; j < NB; ++j)
                 if (e[j].x != NO_UNIT) stage[e[j].y] = unit_value(v[j]);
         }
         __syncthreads();
@@ -475,15 +548,29 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const ResArgs a) {
         const int nw = (int)blockDim.y + z;
         const TileGeom te = tile_geom(a.N + z, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R,
                                       32 * C, nw * R);
-        const int ex0 = te.ox + ((int)threadIdx.x + z) * C, ey0 = te.oy + ((int)threadIdx.y + z) * R, Ne = a.N + z;
+        const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
+        const int ex0 = te.ox + ln * C, ey0 = te.oy + wp * R, Ne = a.N + z;
+        double* const wbuf = sm + (2 + CAV_QROWS) * TOPOFF + wp * (R * 32 * C);     // the staging array is idle again
+#pragma unroll
+        for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+            for (int ci = 0; ci < C; ci += 2) {
+                const int gy = ey0 + rj;
+                const bool rowi = gy >= 1 && gy <= Ne - 1;
+                double2 d;
+                d.x = (rowi && ex0 + ci >= 1 && ex0 + ci <= Ne - 1) ? p[rj][ci] : 0.0;
+                d.y = (rowi && ex0 + ci + 1 >= 1 && ex0 + ci + 1 <= Ne - 1) ? p[rj][ci + 1] : 0.0;
+                *reinterpret_cast<double2*>(wbuf + rj * (32 * C) + ln * C + ci) = d;
+            }
+        __syncwarp();
 #pragma unroll
         for (int rj = 0; rj < R; ++rj) {
+            const int gy = ey0 + rj;
 #pragma unroll
-            for (int ci = 0; ci < C; ++ci) {
-                const int gx = ex0 + ci, gy = ey0 + rj;
-                const bool upd = gx >= 1 && gx <= Ne - 1 && gy >= 1 && gy <= Ne - 1;
+            for (int j = 0; j < C; ++j) {
+                const int gx = te.ox + j * 32 + ln;
                 if (gx >= te.cx0 && gx < te.cx1 && gy >= te.cy0 && gy < te.cy1)
-                    a.psi_out[(size_t)gy * a.pitch + gx] = upd ? p[rj][ci] : 0.0;
+                    a.psi_out[(size_t)gy * a.pitch + gx] = wbuf[rj * (32 * C) + j * 32 + ln];
             }
         }
     }
@@ -491,18 +578,19 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const ResArgs a) {
 
 // ---- compiled variants ------------------------------------------------------------------------------
 struct Variant {
-    int C, R, maxw;
+    int C, R, maxw, persm;
     const void* fn;        // every wall isolated by alignment (the plans of large grids)
     const void* fn_fix;    // with the wall-mask fix-up (a tile that holds both walls of one direction)
 };
 const Variant VARIANTS[] = {
-    {4, 8, 12, (const void*)k_resident<4, 8, 12, false>, (const void*)k_resident<4, 8, 12, true>},     // 32 points per thread, up to 170 registers
-    {4, 6, 16, (const void*)k_resident<4, 6, 16, false>, (const void*)k_resident<4, 6, 16, true>},     // 24 points per thread, up to 128 registers
+    // one CTA of up to 16 warps per SM (also the single-tile plans of small grids)
+    {4, 6, 16, 1, (const void*)k_resident<4, 6, 16, 1, false>, (const void*)k_resident<4, 6, 16, 1, true>},
+    // two CTAs of up to 8 warps per SM: while one exchanges its halo or sits in a barrier, the other computes
+    {4, 6, 8, 2, (const void*)k_resident<4, 6, 8, 2, false>, (const void*)k_resident<4, 6, 8, 2, true>},
 };
 constexpr int NVARIANTS = sizeof(VARIANTS) / sizeof(VARIANTS[0]);
 
 inline int cdiv(int a, int b) { return (a + b - 1) / b; }
-inline int round_up(int a, int m) { return cdiv(a, m) * m; }
 
 int region_total(const Region& g) { return rect_count(g.r[0]) + rect_count(g.r[1]) + rect_count(g.r[2]) + rect_count(g.r[3]); }
 
@@ -523,11 +611,24 @@ bool finish_plan(ResidentPlan& pl, int N, int max_smem) {
     pl.nr_per = cdiv(rmax, nth);
     const int maxw = VARIANTS[pl.variant].maxw;
     const size_t smem = pl.ntiles > 1 ? smem_layout_bytes(pl.C, pl.R, maxw, pl.warps, pl.ns_per, pl.nr_per)
-                                      : 8 * (size_t)(4 * (maxw + 1) * pl.C * 32);
+                                      : 8 * (size_t)((2 + CAV_QROWS) * (maxw + 1) * pl.C * 32 + pl.R * pl.C * (nth + 4));
     pl.fixup = pl.ntx == 1 || pl.nty == 1;
     if (smem > (size_t)max_smem) return false;
     pl.smem_bytes = (int)smem;
     return true;
+}
+
+// One direction of the tiling: G points, thread grid of L points, halo h.  false if no uniform core size works.
+bool split(int G, int L, int lead, int h, int& core, int& n) {
+    if (G + lead <= L) { core = G; n = 1; return true; }       // one tile holds both walls (lead = alignment slack of the first wall)
+    const int cmax = L - 2 * h;
+    if (cmax <= h) return false;
+    n = cdiv(G, cmax);
+    core = cdiv(G, n);
+    n = cdiv(G, core);
+    // the halo must come from adjacent tiles only, and must not reach a wall through an edge tile (only an
+    // edge tile isolates the wall; elsewhere nothing keeps a wall point inside the thread grid at 0)
+    return core > h && G - (n - 1) * core > h;
 }
 
 }  // namespace
@@ -546,58 +647,41 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
     for (int vi = 0; vi < NVARIANTS; ++vi) {
         if (variant_override >= 0 && vi != variant_override) continue;
         const Variant& v = VARIANTS[vi];
-        cudaFuncAttributes fa;
-        if (cudaFuncGetAttributes(&fa, v.fn) != cudaSuccess) { cudaGetLastError(); continue; }
-        cudaFuncAttributes fb;
-        if (cudaFuncGetAttributes(&fb, v.fn_fix) != cudaSuccess) { cudaGetLastError(); continue; }
-        fa.numRegs = std::max(fa.numRegs, fb.numRegs);
-        fa.maxThreadsPerBlock = std::min(fa.maxThreadsPerBlock, fb.maxThreadsPerBlock);
-        const int max_warps = std::min(v.maxw, std::min(fa.maxThreadsPerBlock / 32, (int)(prop.regsPerBlock / (32 * std::max(fa.numRegs, 1)))));
+        cudaFuncAttributes fa, fb;
+        if (cudaFuncGetAttributes(&fa, v.fn) != cudaSuccess || cudaFuncGetAttributes(&fb, v.fn_fix) != cudaSuccess) { cudaGetLastError(); continue; }
+        const int regs = std::max(fa.numRegs, fb.numRegs);
+        const int max_threads = std::min(fa.maxThreadsPerBlock, fb.maxThreadsPerBlock);
+        const int max_warps = std::min(v.maxw, std::min(max_threads / 32, (int)(prop.regsPerBlock / (32 * std::max(regs, 1)))));
         const int W = 32 * v.C;                  // tile width in points
+        const int smem_cap = std::min((int)prop.sharedMemPerBlockOptin,
+                                      (int)(prop.sharedMemPerMultiprocessor / v.persm) - (int)prop.reservedSharedMemPerBlock);
         for (int warps = 1; warps <= max_warps; ++warps) {
             const int H = warps * v.R;           // tile height in points
             ResidentPlan c;
-            c.ok = true; c.variant = vi; c.C = v.C; c.R = v.R; c.warps = warps; c.regs = fa.numRegs; c.sm_count = sms;
+            c.ok = true; c.variant = vi; c.C = v.C; c.R = v.R; c.warps = warps; c.regs = regs; c.sm_count = sms; c.per_sm = v.persm;
             // single tile: the whole grid in one CTA, no exchange at all
             if (G + v.C - 1 <= W && G + v.R - 1 <= H) {
-                const double cost = (double)H * W * 0.11 + 150.0;
-                c.T = 1 << 30; c.halo = 0; c.CW = round_up(G, v.C); c.CH = round_up(G, 2); c.ntx = c.nty = c.ntiles = 1;
-                if (cost < best_cost && finish_plan(c, P.N, (int)prop.sharedMemPerBlockOptin)) { best_cost = cost; best = c; }
+                if (v.persm != 1) continue;
+                const double cost = (double)H * W * 0.135 + 150.0;
+                c.T = 1 << 30; c.halo = 0; c.CW = G; c.CH = G; c.ntx = c.nty = c.ntiles = 1;
+                if (cost < best_cost && finish_plan(c, P.N, smem_cap)) { best_cost = cost; best = c; }
                 continue;
             }
-            for (int T = 2; T <= 16; T += 2) {   // halo = 2T, a multiple of C = 4
+            for (int T = 1; T <= 8; ++T) {
                 if (T_override > 0 && T != T_override) continue;
                 const int halo = 2 * T;
-                // x: either one tile column without an x-halo, or columns of CW <= W - 2 halo
-                int CW, ntx;
-                if (G + v.C - 1 <= W) { CW = round_up(G, v.C); ntx = 1; }
-                else {
-                    const int cwmax = W - 2 * halo;
-                    if (cwmax < halo || cwmax < v.C) continue;
-                    ntx = cdiv(G, cwmax);
-                    CW = round_up(cdiv(G, ntx), v.C);
-                    if (CW > cwmax) continue;
-                    ntx = cdiv(G, CW);
-                    // the halo must come from adjacent tiles only, and must not reach a wall through an edge tile (only an
-                // edge tile isolates the wall; elsewhere nothing keeps a wall point inside the thread grid at 0)
-                if (G - (ntx - 1) * CW <= halo || CW <= halo) continue;
-                }
-                int CH, nty;
-                if (G + v.R - 1 <= H) { CH = round_up(G, 2); nty = 1; }
-                else {
-                    const int chmax = H - 2 * halo;
-                    if (chmax < halo || chmax < 2) continue;
-                    nty = cdiv(G, chmax);
-                    CH = round_up(cdiv(G, nty), 2);
-                    if (CH > chmax) continue;
-                    nty = cdiv(G, CH);
-                    if (G - (nty - 1) * CH <= halo || CH <= halo) continue;
-                }
-                if (ntx * nty > sms || ntx * nty < 2) continue;
-                // cost per sweep in SM cycles: compute of the whole tile + two barriers + exchange / T
-                const double cost = (double)H * W * 0.11 + 150.0 + 3000.0 / T;
-                c.T = T; c.halo = halo; c.CW = CW; c.CH = CH; c.ntx = ntx; c.nty = nty; c.ntiles = ntx * nty;
-                if (cost < best_cost && finish_plan(c, P.N, (int)prop.sharedMemPerBlockOptin)) { best_cost = cost; best = c; }
+                int CW, ntx, CH, nty;
+                if (!split(G, W, v.C - 1, halo, CW, ntx) || !split(G, H, v.R - 1, halo, CH, nty)) continue;
+                const int ntiles = ntx * nty;
+                if (ntiles < 2 || ntiles > v.persm * sms) continue;
+                // Cost per sweep in SM cycles, calibrated on B200 at 1025^2 (profiles/): 0.135 cycles per point of the thread
+                // grid(s) an SM holds (the CTAs of an SM share its fp64 pipe), plus one exchange per T sweeps whose cost is
+                // mostly latency (staging, store burst, L2 round trips) and grows with the halo depth.  Two CTAs per SM were
+                // measured NOT to hide each other's exchange (1.95 vs 1.67 us per sweep), so they get no discount.
+                const int ctas = cdiv(ntiles, sms);
+                const double cost = ctas * (double)H * W * 0.135 + (5000.0 + 600.0 * T) / T;
+                c.T = T; c.halo = halo; c.CW = CW; c.CH = CH; c.ntx = ntx; c.nty = nty; c.ntiles = ntiles;
+                if (cost < best_cost && finish_plan(c, P.N, smem_cap)) { best_cost = cost; best = c; }
             }
         }
     }
@@ -626,19 +710,37 @@ void resident_describe(const ResidentPlan& pl, char* buf, int len) {
     else
         std::snprintf(buf, (size_t)len,
                       "%dx%d tiles of %dx%d core + halo %d, T=%d sweeps per exchange, %d warps x (%dx%d micro-tiles), "
-                      "%d+%d exchange units per thread, %d regs, %d B smem, %d SMs",
+                      "%d+%d exchange units per thread, %d regs, %d B smem, up to %d CTAs per SM on %d SMs",
                       pl.ntx, pl.nty, pl.CW, pl.CH, pl.halo, pl.T, pl.warps, pl.C, pl.R, pl.ns_per, pl.nr_per, pl.regs,
-                      pl.smem_bytes, pl.sm_count);
+                      pl.smem_bytes, pl.per_sm, pl.sm_count);
 }
 
 int resident_variants() { return NVARIANTS; }
 
+size_t resident_table_bytes(const ResidentPlan& pl) {
+    return (pl.ok && pl.ntiles > 1) ? (size_t)pl.ntiles * xtab_bytes(32 * pl.warps, pl.ns_per, pl.nr_per) : 0;
+}
+
+int resident_build_tables(const Params& P, const ResidentPlan& pl, void* tables_dev, cudaStream_t st) {
+    if (!pl.ok || pl.ntiles <= 1) return 0;
+    ResArgs a{};
+    a.N = P.N; a.pitch = P.pitch;
+    a.halo = pl.halo; a.CW = pl.CW; a.CH = pl.CH; a.ntx = pl.ntx; a.nty = pl.nty;
+    a.ns_per = pl.ns_per; a.nr_per = pl.nr_per;
+    const dim3 grid(pl.ntx, pl.nty), block(32, pl.warps);
+    if (pl.C == 4 && pl.R == 6) k_build_tables<4, 6><<<grid, block, 0, st>>>(a, (unsigned char*)tables_dev);
+    else return -(int)cudaErrorNotSupported;
+    const cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? 1 : -(int)e;
+}
+
 int resident_sweeps(const Params& P, const ResidentPlan& pl, const double* psi_in, double* psi_out, void* xa, void* xb,
-                    const double* w, unsigned int* err_word, unsigned int* epoch, int nsweeps, cudaStream_t st,
-                    long long* trace_dev, int trace_cap) {
+                    const void* tables, const double* w, unsigned int* err_word, unsigned int* epoch, int nsweeps,
+                    cudaStream_t st, long long* trace_dev, int trace_cap) {
     if (!pl.ok) return -(int)cudaErrorNotSupported;
-    if (nsweeps <= 0 || psi_in == psi_out) return -(int)cudaErrorInvalidValue;
+    if (nsweeps <= 0 || psi_in == psi_out || (pl.ntiles > 1 && !tables)) return -(int)cudaErrorInvalidValue;
     ResArgs a;
+    a.tables = (const uint4*)tables;
     a.N = P.N; a.pitch = P.pitch; a.cb = P.cb; a.omb = P.omb; a.cq = P.cq;
     a.w = w; a.psi_in = psi_in; a.psi_out = psi_out; a.x0 = (uint4*)xa; a.x1 = (uint4*)xb;
     a.err = err_word;

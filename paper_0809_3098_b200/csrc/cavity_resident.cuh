@@ -25,9 +25,10 @@ struct ResidentPlan {
     int smem_bytes = 0;
     int regs = 0;         // registers per thread of the chosen variant (as compiled)
     int sm_count = 0;
+    int per_sm = 1;       // CTAs per SM the chosen kernel variant is built for
 };
 
-// T_override > 0 forces the sweeps per round (tests use it to exercise short and ragged rounds);
+// T_override > 0 forces the sweeps per round (1..8; tests use it to exercise short and ragged rounds);
 // variant_override >= 0 forces the micro-tile shape (index into the compiled variants).
 ResidentPlan resident_plan(const Params& P, int device, int T_override = 0, int variant_override = -1);
 int resident_variants();
@@ -36,15 +37,20 @@ void resident_describe(const ResidentPlan& plan, char* buf, int len);
 // Doubles behind ONE exchange buffer (the engine needs two): a 16-byte unit per point of a pitch x (N+1) field.
 inline size_t resident_exchange_doubles(size_t field_doubles) { return 2 * field_doubles; }
 
+// Per-plan exchange tables (device memory, built once per plan): their size, and the kernel that fills them.
+size_t resident_table_bytes(const ResidentPlan& plan);
+int resident_build_tables(const Params& P, const ResidentPlan& plan, void* tables_dev, cudaStream_t st);
+
 // nsweeps red-black sweeps of a1: reads psi_in, writes psi_out (two different fields), right-hand side cq * w (w = the
 // stage's input vorticity, scaled on the fly exactly as scale_rhs does).  xa, xb: the two exchange buffers (zero-filled once
-// by the caller).  err_word: one device word, zero-filled once; non-zero afterwards = a tile gave up waiting for a neighbour.
+// by the caller).  tables: what resident_build_tables wrote for this plan (may be null for a single-tile plan).
+// err_word: one device word, zero-filled once; non-zero afterwards = a tile gave up waiting for a neighbour.
 // *epoch is the host-side tag epoch, advanced by this call (tags are unique per round and per launch).
 // trace_dev (profiling only): device array of ntiles x trace_cap %globaltimer stamps (ns), slot 0 = start, 1 = inputs loaded,
 // then per round r: 2 + 4r sweeps done, 3 + 4r border strips stored, 4 + 4r ring received, 5 + 4r edges republished.
 // Returns the number of kernel launches (1), or a negative cudaError_t.
 int resident_sweeps(const Params& P, const ResidentPlan& plan, const double* psi_in, double* psi_out, void* xa, void* xb,
-                    const double* w, unsigned int* err_word, unsigned int* epoch, int nsweeps, cudaStream_t st,
-                    long long* trace_dev = nullptr, int trace_cap = 0);
+                    const void* tables, const double* w, unsigned int* err_word, unsigned int* epoch, int nsweeps,
+                    cudaStream_t st, long long* trace_dev = nullptr, int trace_cap = 0);
 
 }  // namespace cavk
