@@ -115,9 +115,9 @@ int cav_describe(cav_ctx* ctx, char* buf, int len);
 /* Number of kernel launches enqueued by this context since cav_create (for bench.py's gpu_launches). */
 long long cav_launch_count(cav_ctx* ctx);
 
-/* CUDA-event time in milliseconds of the most recent cav_step / cav_step_async / cav_poisson on the
- * context's stream (events recorded around the enqueued work); blocks until that work has finished.
- * Writes 0 if none has run. */
+/* CUDA-event time in milliseconds of the most recent cav_step / cav_step_async (the whole call) or cav_poisson (its a1
+ * sweeps alone, without the a2 pass and the residual) on the context's stream (events recorded around the enqueued
+ * work); blocks until that work has finished.  Writes 0 if none has run. */
 int cav_last_elapsed_ms(cav_ctx* ctx, float* ms_out);
 
 /* Static string for an error code. */

@@ -51,7 +51,7 @@ constexpr unsigned int NO_UNIT = 0xffffffffu;
 #define CAV_QROWS 2             // rows of the micro-tile whose q lives in shared memory instead of registers
 #endif
 #ifndef CAV_RECV_BATCH
-#define CAV_RECV_BATCH 4        // ring units a thread keeps in flight at a time (4 registers each)
+#define CAV_RECV_BATCH 2        // ring units a thread keeps in flight at a time (4 registers each; more than 2 makes ptxas spill around the exchange, which costs more than the extra L2 round trips: profiles/)
 #endif
 
 struct ResArgs {
