@@ -12,6 +12,7 @@ from .build import build
 
 MODE_PLAIN = 0
 MODE_FMA = 1
+SWEEP_REDBLACK, SWEEP_JACOBI = 0, 1
 
 _lib = None
 
@@ -39,6 +40,11 @@ def lib():
         L.orc_rhs.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, dp]
         L.orc_thom.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp]
         L.orc_sor.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, C.c_int]
+        L.orc_set_sweep.argtypes = [C.c_void_p, C.c_int]
+        L.orc_jacobi.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, C.c_int]
+        L.orc_step_res.argtypes = [C.c_void_p, dp, dp]
+        L.orc_run_to_steady.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int), dp, dp,
+                                        C.POINTER(C.c_int)]
         L.orc_ssprk54_scalar.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int, C.c_int]
         L.orc_ssprk54_scalar.restype = C.c_double
         _lib = L
@@ -82,6 +88,22 @@ class OracleCavity:
             self.close()
         except Exception:
             pass
+
+    def set_sweep(self, kind):
+        """SWEEP_REDBLACK (default) or SWEEP_JACOBI."""
+        _chk(lib().orc_set_sweep(self._h, kind), "orc_set_sweep")
+
+    def step_res(self):
+        """One time step; returns (RES_psi, RES_omega) of that step (eq 26-27)."""
+        rp, rw = C.c_double(), C.c_double()
+        _chk(lib().orc_step_res(self._h, C.byref(rp), C.byref(rw)), "orc_step_res")
+        return rp.value, rw.value
+
+    def run_to_steady(self, max_steps, check_every, tol_psi, tol_omega):
+        n, conv, rp, rw = C.c_int(), C.c_int(), C.c_double(), C.c_double()
+        _chk(lib().orc_run_to_steady(self._h, max_steps, check_every, tol_psi, tol_omega, C.byref(n), C.byref(rp),
+                                     C.byref(rw), C.byref(conv)), "orc_run_to_steady")
+        return {"steps": n.value, "res_psi": rp.value, "res_omega": rw.value, "converged": bool(conv.value)}
 
     def set_lid(self, U):
         _chk(lib().orc_set_lid(self._h, U), "orc_set_lid")
@@ -130,6 +152,13 @@ def sor(N, beta, psi, omega, nsweeps, mode=MODE_PLAIN):
     p = _field(psi, N, "psi").copy()
     omega = _field(omega, N, "omega")
     _chk(lib().orc_sor(N, beta, mode, _p(p), _p(omega), nsweeps), "orc_sor")
+    return p
+
+
+def jacobi(N, beta, psi, omega, nsweeps, mode=MODE_PLAIN):
+    p = _field(psi, N, "psi").copy()
+    omega = _field(omega, N, "omega")
+    _chk(lib().orc_jacobi(N, beta, mode, _p(p), _p(omega), nsweeps), "orc_jacobi")
     return p
 
 

@@ -52,6 +52,7 @@
 
 enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2 };
 enum { ORC_MODE_PLAIN = 0, ORC_MODE_FMA = 1 };
+enum { ORC_SWEEP_REDBLACK = 0, ORC_SWEEP_JACOBI = 1 };   // (a1) variants: red-black SOR (default) / damped Jacobi (NEXT-3)
 
 struct orc_diag {
     double t;
@@ -66,6 +67,7 @@ struct orc_ctx {
     int N;            // intervals per side; N+1 points per side
     int S;            // SOR sweeps per stage
     int mode;
+    int sweep;        // ORC_SWEEP_*
     double Re, dt, beta, U;
     double t;
     long long step;
@@ -140,6 +142,33 @@ void sor_sweeps(int N, int mode, double beta, std::vector<double>& psi, const st
         sor_half_sweep(N, mode, beta, psi, w, 0);   // red first (G9)
         sor_half_sweep(N, mode, beta, psi, w, 1);   // then black
     }
+}
+
+// ---- (a1, NEXT-3 variant) damped Jacobi sweeps ------------------------------------------------
+// BASELINE.json north_star allows "red-black SOR (or Jacobi)"; every interior point is relaxed from the
+// OLD values only,  psi_new = psi + beta ( (psi_W + psi_E + psi_S + psi_N + h^2 w) / 4 - psi ),  i.e. eq 15 P:116 without the
+// "use new values when available" of P:114.  The point formula is the one of the red-black sweep (sor_point_*); only the
+// data it reads differs (a second buffer).
+void jacobi_sweeps(int N, int mode, double beta, std::vector<double>& psi, const std::vector<double>& w, int nsweeps) {
+    const double h = 1.0 / (double)N;
+    std::vector<double> old(psi.size());
+    for (int s = 0; s < nsweeps; ++s) {
+        old = psi;
+        for (int j = 1; j <= N - 1; ++j) {
+            for (int i = 1; i <= N - 1; ++i) {
+                const double pW = old[idx(N, i - 1, j)], pE = old[idx(N, i + 1, j)];
+                const double pS = old[idx(N, i, j - 1)], pN = old[idx(N, i, j + 1)];
+                const double p = old[idx(N, i, j)], wij = w[idx(N, i, j)];
+                psi[idx(N, i, j)] = (mode == ORC_MODE_FMA) ? sor_point_fma(pW, pE, pS, pN, p, wij, beta, N)
+                                                            : sor_point_plain(pW, pE, pS, pN, p, wij, beta, h, h);
+            }
+        }
+    }
+}
+
+void poisson_sweeps(const orc_ctx* c, std::vector<double>& psi, const std::vector<double>& w, int nsweeps) {
+    if (c->sweep == ORC_SWEEP_JACOBI) jacobi_sweeps(c->N, c->mode, c->beta, psi, w, nsweeps);
+    else sor_sweeps(c->N, c->mode, c->beta, psi, w, nsweeps);
 }
 
 // ---- (a2) Thom wall vorticity, eq 25 P:161-169 ----------------------------------------------
@@ -238,7 +267,7 @@ void one_step(orc_ctx* c) {
 
     for (int k = 1; k <= 5; ++k) {
         std::vector<double>& win = (k == 1) ? w0 : (k == 2) ? c->w1 : (k == 3) ? c->w2 : (k == 4) ? c->w3 : c->w4;
-        sor_sweeps(N, m, c->beta, c->psi, win, c->S);          // (a1)
+        poisson_sweeps(c, c->psi, win, c->S);                   // (a1)
         thom(N, m, c->U, c->psi, win);                          // (a2)
         for (int j = 1; j <= N - 1; ++j) {                      // (a3)
             for (int i = 1; i <= N - 1; ++i) {
@@ -303,7 +332,7 @@ ORC_API int orc_create(orc_ctx** out, int N, double Re, double dt, double sor_om
     if (!c) return ORC_ENOMEM;
     try {
         const size_t G = (size_t)(N + 1) * (size_t)(N + 1);
-        c->N = N; c->S = sweeps_per_stage; c->mode = ORC_MODE_PLAIN;
+        c->N = N; c->S = sweeps_per_stage; c->mode = ORC_MODE_PLAIN; c->sweep = ORC_SWEEP_REDBLACK;
         c->Re = Re; c->dt = dt; c->beta = sor_omega; c->U = 1.0;   // P:190 U_wall = 1
         c->t = 0.0; c->step = 0;
         c->psi.assign(G, 0.0); c->w.assign(G, 0.0);
@@ -318,6 +347,12 @@ ORC_API void orc_destroy(orc_ctx* c) { delete c; }
 ORC_API int orc_set_mode(orc_ctx* c, int mode) {
     if (!c || (mode != ORC_MODE_PLAIN && mode != ORC_MODE_FMA)) return ORC_EINVAL;
     c->mode = mode;
+    return ORC_OK;
+}
+
+ORC_API int orc_set_sweep(orc_ctx* c, int kind) {
+    if (!c || (kind != ORC_SWEEP_REDBLACK && kind != ORC_SWEEP_JACOBI)) return ORC_EINVAL;
+    c->sweep = kind;
     return ORC_OK;
 }
 
@@ -359,7 +394,7 @@ ORC_API int orc_step(orc_ctx* c, int nsteps) {
 // nsweeps of (a1) on the current (psi, omega), then one (a2); max-norm residual if asked.
 ORC_API int orc_poisson(orc_ctx* c, int nsweeps, double* res_inf_out) {
     if (!c || nsweeps < 0) return ORC_EINVAL;
-    sor_sweeps(c->N, c->mode, c->beta, c->psi, c->w, nsweeps);
+    poisson_sweeps(c, c->psi, c->w, nsweeps);
     thom(c->N, c->mode, c->U, c->psi, c->w);
     if (res_inf_out) { orc_diag d; diagnostics(c, &d); *res_inf_out = d.res_inf; }
     return ORC_OK;
@@ -401,6 +436,60 @@ ORC_API int orc_sor(int N, double beta, int mode, double* psi, const double* ome
     std::vector<double> p(psi, psi + G), w(omega, omega + G);
     sor_sweeps(N, mode, beta, p, w, nsweeps);
     std::memcpy(psi, p.data(), G * sizeof(double));
+    return ORC_OK;
+}
+
+// nsweeps damped-Jacobi sweeps on psi (in place; walls taken as given) with right-hand side omega.
+ORC_API int orc_jacobi(int N, double beta, int mode, double* psi, const double* omega, int nsweeps) {
+    if (N < 2 || !psi || !omega || nsweeps < 0) return ORC_EINVAL;
+    const size_t G = (size_t)(N + 1) * (size_t)(N + 1);
+    std::vector<double> p(psi, psi + G), w(omega, omega + G);
+    jacobi_sweeps(N, mode, beta, p, w, nsweeps);
+    std::memcpy(psi, p.data(), G * sizeof(double));
+    return ORC_OK;
+}
+
+// NEXT-2: one time step and the paper's steady-state monitors of that step, eq 26-27 P:196-202:
+//   RES_psi = (1/N) sum_ij |psi^{n+1}_ij - psi^n_ij|,  RES_omega likewise, sums over ALL grid points, and N = n_x = n_y
+// the number of points per side, i.e. c->N + 1 here (reading G17: the literal divisor, not N^2).
+// psi^n / psi^{n+1} are the states orc_get_fields returns before / after the step (G16).  Sums in long double.
+ORC_API int orc_step_res(orc_ctx* c, double* res_psi_out, double* res_omega_out) {
+    if (!c) return ORC_EINVAL;
+    const std::vector<double> p0 = c->psi, w0 = c->w;
+    one_step(c);
+    long double sp = 0.0L, sw = 0.0L;
+    for (size_t k = 0; k < p0.size(); ++k) {
+        sp += (long double)std::fabs(c->psi[k] - p0[k]);
+        sw += (long double)std::fabs(c->w[k] - w0[k]);
+    }
+    const long double npts = (long double)(c->N + 1);
+    if (res_psi_out) *res_psi_out = (double)(sp / npts);
+    if (res_omega_out) *res_omega_out = (double)(sw / npts);
+    return ORC_OK;
+}
+
+// NEXT-2 driver: steps until RES_psi < tol_psi and RES_omega < tol_omega (the paper's stopping rule), checking the
+// monitors on every check_every-th step, for at most max_steps steps.  Returns the steps taken in *steps_out and the
+// monitors of the last checked step; *converged_out = 1 if the rule was met.
+ORC_API int orc_run_to_steady(orc_ctx* c, int max_steps, int check_every, double tol_psi, double tol_omega, int* steps_out,
+                              double* res_psi_out, double* res_omega_out, int* converged_out) {
+    if (!c || max_steps < 0 || check_every < 1) return ORC_EINVAL;
+    double rp = 0.0, rw = 0.0;
+    int n = 0, conv = 0;
+    while (n < max_steps) {
+        if ((n + 1) % check_every == 0) {
+            orc_step_res(c, &rp, &rw);
+            ++n;
+            if (rp < tol_psi && rw < tol_omega) { conv = 1; break; }
+        } else {
+            one_step(c);
+            ++n;
+        }
+    }
+    if (steps_out) *steps_out = n;
+    if (res_psi_out) *res_psi_out = rp;
+    if (res_omega_out) *res_omega_out = rw;
+    if (converged_out) *converged_out = conv;
     return ORC_OK;
 }
 

@@ -406,3 +406,116 @@ def test_diagnostics_definitions():
     o.set_fields(psi, om + 2.0)                            # residual = 2 everywhere
     d = o.diag()
     assert abs(d["res_inf"] - 2.0) < 1e-11 and abs(d["res_l2"] - 2.0 * (N - 1) * h) < 1e-11
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-3: damped Jacobi sweeps.  A discrete eigenmode sin(k pi x) sin(l pi y) of the homogeneous problem is damped by
+# exactly g = 1 - beta (1 - (cos k pi h + cos l pi h) / 2) per sweep (closed form); with a right-hand side the
+# iteration converges to the same discrete solution A / lam_h as SOR does.
+# --------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("k,l,beta", [(1, 1, 1.0), (3, 2, 0.8), (5, 7, 0.5), (1, 15, 1.0)])
+def test_jacobi_damping_factor_closed_form(mode, k, l, beta):
+    N, n = 16, 9
+    X, Y = grid(N)
+    e = np.sin(k * np.pi * X) * np.sin(l * np.pi * Y)
+    g = 1.0 - beta * (1.0 - 0.5 * (math.cos(k * math.pi / N) + math.cos(l * math.pi / N)))
+    out = oracle.jacobi(N, beta, e, np.zeros_like(e), n, mode)
+    assert np.max(np.abs(out - g ** n * e)) < 1e-14
+    # walls are never touched
+    assert np.array_equal(out[0], e[0]) and np.array_equal(out[-1], e[-1]) and np.array_equal(out[:, 0], e[:, 0])
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_jacobi_reads_old_values_only(mode):
+    # one sweep on a delta: only the four neighbours and the point itself change, by beta/4 and (1 - beta)
+    N, beta = 8, 0.7
+    p = np.zeros((N + 1, N + 1)); p[4, 4] = 1.0
+    out = oracle.jacobi(N, beta, p, np.zeros_like(p), 1, mode)
+    exp = np.zeros_like(p); exp[4, 4] = 1.0 - beta
+    for dj, di in ((1, 0), (-1, 0), (0, 1), (0, -1)):
+        exp[4 + dj, 4 + di] = 0.25 * beta
+    assert np.max(np.abs(out - exp)) < 1e-16
+    # whereas the red-black sweep lets the black neighbours see the NEW red value
+    rb = oracle.sor(N, beta, p, np.zeros_like(p), 1, mode)
+    assert abs(rb[4, 5] - 0.25 * beta * (1.0 - beta)) < 1e-16
+
+
+def test_jacobi_converges_to_discrete_solution():
+    N, A = 16, 3.0
+    X, Y = grid(N)
+    w = A * np.sin(np.pi * X) * np.sin(2 * np.pi * Y)
+    psi = oracle.jacobi(N, 1.0, np.zeros_like(w), w, 4000)
+    assert np.max(np.abs(psi - w / lam_h(N, 1, 2))) < 1e-13
+
+
+def test_step_with_jacobi_sweeps_differs_from_red_black_but_both_run():
+    N = 16
+    X, Y = grid(N)
+    w0 = np.sin(np.pi * X) * np.sin(np.pi * Y)
+    res = []
+    for kind in (oracle.SWEEP_REDBLACK, oracle.SWEEP_JACOBI):
+        o = oracle.OracleCavity(N, 100.0, 1e-2, 0.9, 30)
+        o.set_sweep(kind)
+        o.set_fields(None, w0)
+        o.step(3)
+        res.append(o.get_fields())
+        o.close()
+    assert np.max(np.abs(res[0][0] - res[1][0])) > 1e-6          # different iterations, different iterates
+    assert np.max(np.abs(res[0][0] - res[1][0])) < 1e-2          # ... of the same Poisson problem
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-2: the paper's steady-state monitors, eq 26-27, divisor = points per side (G17).
+# Closed form through a whole step: pure diffusion of an eigenmode (psi = 0, no lid, no sweeps) changes omega by
+# (R(z) - 1) omega^n, so RES_omega = |R(z) - 1| sum|omega^n| / (N + 1) and RES_psi = 0.
+# --------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("mode", MODES)
+def test_res_monitors_closed_form_diffusion(mode):
+    N, Re, dt = 16, 50.0, 2e-3
+    X, Y = grid(N)
+    w0 = np.sin(2 * np.pi * X) * np.sin(np.pi * Y)
+    o = oracle.OracleCavity(N, Re, dt, 1.5, 0, mode)
+    o.set_lid(0.0)
+    o.set_fields(None, w0)
+    z = -(1.0 / Re) * lam_h(N, 2, 1) * dt
+    wn = w0.copy()
+    for _ in range(3):
+        rp, rw = o.step_res()
+        assert rp == 0.0
+        assert abs(rw - abs(R_poly(z) - 1.0) * np.sum(np.abs(wn)) / (N + 1)) < 1e-13
+        wn = R_poly(z) * wn
+    o.close()
+
+
+def test_res_monitors_count_every_grid_point_including_the_ring():
+    # with the lid on, the first step changes the wall vorticity from 0 to -2U/h on the N + 1 lid points: RES_omega
+    # must contain that jump (sum over ALL (i, j)), and RES_psi the sum over the interior change of psi
+    N = 8
+    o = oracle.OracleCavity(N, 100.0, 1e-3, 1.0, 5)
+    z = np.zeros((N + 1, N + 1))
+    o.set_fields(None, z)
+    rp, rw = o.step_res()
+    psi, w = o.get_fields()
+    assert abs(rw - np.sum(np.abs(w)) / (N + 1)) < 1e-12 and abs(rp - np.sum(np.abs(psi)) / (N + 1)) < 1e-15
+    assert rw >= (N + 1) * (2.0 * N) / (N + 1) - 1e-9          # at least the lid jump 2U/h on N + 1 points
+    o.close()
+
+
+def test_run_to_steady_stops_by_the_papers_rule():
+    N = 8
+    o = oracle.OracleCavity(N, 10.0, 2e-3, 1.5, 10)
+    o.set_fields(None, np.zeros((N + 1, N + 1)))
+    r = o.run_to_steady(20000, 10, 1e-9, 1e-7)
+    assert r["converged"] and r["steps"] % 10 == 0 and r["res_psi"] < 1e-9 and r["res_omega"] < 1e-7
+    # the step before the last check did not satisfy the rule with room to spare: one more monitored step is smaller still
+    rp, rw = o.step_res()
+    assert rp < 1e-9 and rw < 1e-7
+    # and a run that is cut short reports it
+    o2 = oracle.OracleCavity(N, 10.0, 2e-3, 1.5, 10)
+    o2.set_fields(None, np.zeros((N + 1, N + 1)))
+    r2 = o2.run_to_steady(50, 10, 1e-9, 1e-7)
+    assert not r2["converged"] and r2["steps"] == 50
+    o.close(); o2.close()
