@@ -45,6 +45,10 @@ extern "C" {
 #define CAV_ENGINE_STREAM   1   /* one kernel per colour half-sweep over global memory (the streaming baseline) */
 #define CAV_ENGINE_RESIDENT 2   /* persistent register/shared-memory resident tiles, temporal blocking */
 
+/* a1 variants (BASELINE.json north_star: "red-black SOR (or Jacobi)"). */
+#define CAV_SWEEP_REDBLACK  0   /* red-black SOR, red = (i + j) even first (default; the timed path) */
+#define CAV_SWEEP_JACOBI    1   /* damped Jacobi: every interior point from the OLD values only */
+
 typedef struct cav_ctx cav_ctx;   /* opaque; owned by the library from cav_create to cav_destroy */
 
 typedef struct cav_diag {
@@ -55,6 +59,14 @@ typedef struct cav_diag {
     double kinetic_energy;   /* (1/2) h^2 sum (u^2 + v^2), u, v of eq 22 */
     double enstrophy;        /* (1/2) h^2 sum omega^2 */
 } cav_diag;
+
+/* Result of cav_run_to_steady. */
+typedef struct cav_monitor {
+    int steps;               /* time steps taken by the call */
+    int converged;           /* 1 if RES_psi < tol_psi and RES_omega < tol_omega at the last monitored step */
+    double res_psi;          /* eq 26 P:198 of the last monitored step */
+    double res_omega;        /* eq 27 */
+} cav_monitor;
 
 /* Allocates psi, omega and the stage buffers (zero-filled: fluid at rest) for an (N+1) x (N+1) grid.
  * Re: Reynolds number (nu = 1/Re); dt: time step; sor_omega: relaxation factor beta in (0, 2);
@@ -87,6 +99,23 @@ int cav_sync(cav_ctx* ctx);
 /* nsweeps of a1 on the current (psi, omega), then one a2 so that the omega ring matches psi; writes
  * the max-norm residual (row a4) to *res_inf_out if non-NULL.  Does not advance time. */
 int cav_poisson(cav_ctx* ctx, int nsweeps, double* res_inf_out);
+
+/* Selects the a1 variant (CAV_SWEEP_*) used by cav_step and cav_poisson from now on.  With CAV_SWEEP_JACOBI sor_omega is the
+ * damping factor: psi_new = psi + beta ((psi_W + psi_E + psi_S + psi_N + h^2 w) / 4 - psi), all from the previous sweep's
+ * values (it converges for beta <= 1; nothing is checked).  The Jacobi sweeps run as one kernel per sweep over global
+ * memory whatever the engine. */
+int cav_set_sweep(cav_ctx* ctx, int kind);
+
+/* One time step, and the paper's steady-state monitors of that step (eq 26-27):
+ *   RES_psi = (1 / n) sum_ij |psi^{n+1}_ij - psi^n_ij|,  RES_omega likewise with omega,
+ * sums over ALL (N+1)^2 grid points, n = N + 1 = the points per side (the paper's literal divisor; reading G17);
+ * psi^n, psi^{n+1} are what cav_get_fields returns before / after the step (G16).  Either pointer may be NULL. */
+int cav_step_res(cav_ctx* ctx, double* res_psi_out, double* res_omega_out);
+
+/* The paper's run-to-steady-state rule: steps until RES_psi < tol_psi and RES_omega < tol_omega, evaluating the
+ * monitors on every check_every-th step of the call (>= 1), for at most max_steps steps.  *out reports the steps taken,
+ * whether the rule was met, and the monitors of the last monitored step (0 if none was).  CAV_EINVAL on bad arguments. */
+int cav_run_to_steady(cav_ctx* ctx, int max_steps, int check_every, double tol_psi, double tol_omega, cav_monitor* out);
 
 /* Runs the a4 reductions on the current state.  Pure. */
 int cav_get_diag(cav_ctx* ctx, cav_diag* out);

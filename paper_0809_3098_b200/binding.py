@@ -16,7 +16,10 @@ _ENGINES = {"auto": ENGINE_AUTO, "stream": ENGINE_STREAM, "resident": ENGINE_RES
 # every symbol include/cavity.h declares
 SYMBOLS = ("cav_create", "cav_destroy", "cav_set_fields", "cav_get_fields", "cav_step", "cav_step_async", "cav_sync",
            "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_set_resident_plan", "cav_trace_sweeps", "cav_describe", "cav_launch_count",
-           "cav_last_elapsed_ms", "cav_strerror")
+           "cav_last_elapsed_ms", "cav_strerror", "cav_set_sweep", "cav_step_res", "cav_run_to_steady")
+
+SWEEP_REDBLACK, SWEEP_JACOBI = 0, 1
+_SWEEPS = {"redblack": SWEEP_REDBLACK, "jacobi": SWEEP_JACOBI}
 
 _lib = None
 
@@ -24,6 +27,10 @@ _lib = None
 class CavDiag(C.Structure):
     _fields_ = [("t", C.c_double), ("step", C.c_longlong), ("res_inf", C.c_double), ("res_l2", C.c_double),
                 ("kinetic_energy", C.c_double), ("enstrophy", C.c_double)]
+
+
+class CavMonitor(C.Structure):
+    _fields_ = [("steps", C.c_int), ("converged", C.c_int), ("res_psi", C.c_double), ("res_omega", C.c_double)]
 
 
 class CavityError(RuntimeError):
@@ -68,6 +75,9 @@ def lib():
     L.cav_launch_count.argtypes = [C.c_void_p]
     L.cav_launch_count.restype = C.c_longlong
     L.cav_last_elapsed_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+    L.cav_set_sweep.argtypes = [C.c_void_p, C.c_int]
+    L.cav_step_res.argtypes = [C.c_void_p, dp, dp]
+    L.cav_run_to_steady.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(CavMonitor)]
     L.cav_strerror.argtypes = [C.c_int]
     L.cav_strerror.restype = C.c_char_p
     _lib = L
@@ -127,6 +137,22 @@ class Cavity:
     def set_engine(self, engine):
         _chk(lib().cav_set_engine(self._h, _ENGINES[engine] if isinstance(engine, str) else int(engine)),
              "cav_set_engine")
+
+    def set_sweep(self, kind):
+        """'redblack' (default) or 'jacobi' (or the CAV_SWEEP_* integer)."""
+        _chk(lib().cav_set_sweep(self._h, _SWEEPS[kind] if isinstance(kind, str) else int(kind)), "cav_set_sweep")
+
+    def step_res(self):
+        """One time step; returns (RES_psi, RES_omega) of that step (eq 26-27 of the paper)."""
+        rp, rw = C.c_double(), C.c_double()
+        _chk(lib().cav_step_res(self._h, C.byref(rp), C.byref(rw)), "cav_step_res")
+        return rp.value, rw.value
+
+    def run_to_steady(self, max_steps, check_every, tol_psi, tol_omega):
+        m = CavMonitor()
+        _chk(lib().cav_run_to_steady(self._h, int(max_steps), int(check_every), float(tol_psi), float(tol_omega),
+                                     C.byref(m)), "cav_run_to_steady")
+        return {"steps": m.steps, "converged": bool(m.converged), "res_psi": m.res_psi, "res_omega": m.res_omega}
 
     def set_resident_plan(self, T=0, variant=-1):
         _chk(lib().cav_set_resident_plan(self._h, int(T), int(variant)), "cav_set_resident_plan")

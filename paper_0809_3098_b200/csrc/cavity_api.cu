@@ -8,6 +8,7 @@
 #include <c10/cuda/CUDAStream.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -34,6 +35,9 @@ struct cav_ctx {
     double* q = nullptr;             // (beta/4) h^2 w_in, the scaled right-hand side of the current stage
     double* w[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // omega^n (state), omega^(1..4)
     double* T = nullptr;             // first three terms of eq 13
+    double* psi_prev = nullptr;      // NEXT-2 monitors: psi and omega before the monitored step
+    double* w_prev = nullptr;
+    int sweep = CAV_SWEEP_REDBLACK;  // a1 variant
     double* scratch = nullptr;       // diagnostics partials
     double* out4 = nullptr;          // diagnostics result (device)
     void* tables = nullptr;          // resident engine: per-plan exchange tables (own allocation, rebuilt on re-plan)
@@ -112,7 +116,10 @@ void resolve_engine(cav_ctx* c) {
 // a1: nsweeps red-black sweeps on psi with right-hand side w_in
 int enqueue_sweeps(cav_ctx* c, const double* w_in, int nsweeps, long long& nl) {
     if (nsweeps <= 0) return CAV_OK;
-    if (c->engine == CAV_ENGINE_RESIDENT) {
+    if (c->sweep == CAV_SWEEP_JACOBI) {
+        LAUNCH(cavk::scale_rhs(c->P, w_in, c->q, c->st));
+        LAUNCH(cavk::jacobi_sweeps(c->P, c->psi, c->psi2, c->q, nsweeps, c->st));
+    } else if (c->engine == CAV_ENGINE_RESIDENT) {
         LAUNCH(cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, c->tables, w_in, c->err_word, &c->epoch, nsweeps, c->st));
         std::swap(c->psi, c->psi2);
     } else {
@@ -150,7 +157,7 @@ int enqueue_step(cav_ctx* c, long long& nl) {
 void try_build_graph(cav_ctx* c) {
     if (c->graph_tried) return;
     c->graph_tried = true;
-    if (c->engine == CAV_ENGINE_RESIDENT) return;     // 10-odd launches per step: a graph buys nothing
+    if (c->engine == CAV_ENGINE_RESIDENT && c->sweep == CAV_SWEEP_REDBLACK) return;     // 10 launches per step: a graph buys nothing
     cudaGraph_t g = nullptr;
     if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return; }
     long long nl = 0;
@@ -214,7 +221,7 @@ CAV_API int cav_create(cav_ctx** out, int N, double Re, double dt, double sor_om
         const size_t fd = align_up((size_t)c->P.pitch * (size_t)(N + 1), 32);   // doubles per field, 256 B multiple
         c->field_doubles = fd;
         const size_t xd = cavk::resident_exchange_doubles(fd);
-        const size_t nfields = 9;    // psi, psi2, q, w0..w4, T  (+ the two exchange buffers)
+        const size_t nfields = 11;   // psi, psi2, q, w0..w4, T, psi_prev, w_prev  (+ the two exchange buffers)
         const size_t scratch_d = align_up(4 * (size_t)cavk::diag_scratch_doubles(), 32);
         const size_t flags_b = 256;
         const size_t bytes = (nfields * fd + 2 * xd + scratch_d + 32) * sizeof(double) + flags_b;
@@ -229,6 +236,8 @@ CAV_API int cav_create(cav_ctx** out, int N, double Re, double dt, double sor_om
         c->q = p; p += fd;
         for (int k = 0; k < 5; ++k) { c->w[k] = p; p += fd; }
         c->T = p; p += fd;
+        c->psi_prev = p; p += fd;
+        c->w_prev = p; p += fd;
         c->scratch = p; p += scratch_d;
         c->out4 = p; p += 32;
         c->err_word = (unsigned int*)p;
@@ -342,6 +351,58 @@ CAV_API int cav_get_diag(cav_ctx* c, cav_diag* out) {
     out->t = (double)c->step * c->dt;
     out->step = c->step;
     out->res_inf = r[0]; out->res_l2 = r[1]; out->kinetic_energy = r[2]; out->enstrophy = r[3];
+    return CAV_OK;
+}
+
+CAV_API int cav_set_sweep(cav_ctx* c, int kind) {
+    if (!c || (kind != CAV_SWEEP_REDBLACK && kind != CAV_SWEEP_JACOBI)) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    CK(cudaStreamSynchronize(c->st));
+    if (kind != c->sweep) { c->sweep = kind; drop_graph(c); }
+    return CAV_OK;
+}
+
+CAV_API int cav_step_res(cav_ctx* c, double* res_psi_out, double* res_omega_out) {
+    if (!c) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    const size_t nb = c->field_doubles * sizeof(double);
+    CK(cudaMemcpyAsync(c->psi_prev, c->psi, nb, cudaMemcpyDeviceToDevice, c->st));
+    CK(cudaMemcpyAsync(c->w_prev, c->w[0], nb, cudaMemcpyDeviceToDevice, c->st));
+    int rc = step_impl(c, 1, false);
+    if (rc != CAV_OK) return rc;
+    long long nl = 0;
+    double r[2] = {0.0, 0.0};
+    LAUNCH(cavk::res_monitors(c->P, c->psi, c->psi_prev, c->w[0], c->w_prev, c->scratch, c->out4 + 8, c->st));
+    c->launches += nl;
+    CK(cudaMemcpyAsync(r, c->out4 + 8, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    if (res_psi_out) *res_psi_out = r[0];
+    if (res_omega_out) *res_omega_out = r[1];
+    if (c->engine == CAV_ENGINE_RESIDENT) return check_resident_error(c);
+    return CAV_OK;
+}
+
+CAV_API int cav_run_to_steady(cav_ctx* c, int max_steps, int check_every, double tol_psi, double tol_omega, cav_monitor* out) {
+    if (!c || max_steps < 0 || check_every < 1 || !out) return CAV_EINVAL;
+    out->steps = 0; out->converged = 0; out->res_psi = 0.0; out->res_omega = 0.0;
+    int n = 0;
+    while (n < max_steps) {
+        const int plain = std::min(check_every - 1, max_steps - n);      // steps before the next monitored one
+        if (plain > 0) {
+            const int rc = step_impl(c, plain, false);
+            if (rc != CAV_OK) return rc;
+            n += plain;
+        }
+        if (n >= max_steps) break;
+        const int rc = cav_step_res(c, &out->res_psi, &out->res_omega);    // step n + 1 is a multiple of check_every
+        if (rc != CAV_OK) return rc;
+        ++n;
+        if (out->res_psi < tol_psi && out->res_omega < tol_omega) { out->converged = 1; break; }
+    }
+    out->steps = n;
+    DeviceGuard dg(c->device);
+    CK(cudaStreamSynchronize(c->st));
+    if (c->engine == CAV_ENGINE_RESIDENT) return check_resident_error(c);
     return CAV_OK;
 }
 

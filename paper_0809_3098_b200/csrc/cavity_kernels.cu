@@ -211,7 +211,72 @@ k_half_sweep(int N, int pitch, double cb, double omb, double* __restrict__ psi, 
     psi[k] = fma(omb, psi[k], fma(cb, nb, q[k]));
 }
 
+// ---- a1, NEXT-3 variant: one damped-Jacobi sweep, old values only -------------------
+// Same point formula as the red-black sweep, read from psi_in, written to psi_out (walls of psi_out are +0.0 already).
+__global__ void __launch_bounds__(256)
+k_jacobi_sweep(int N, int pitch, double cb, double omb, const double* __restrict__ psi_in, const double* __restrict__ q,
+               double* __restrict__ psi_out) {
+    const int i = 1 + blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = 1 + blockIdx.y * blockDim.y + threadIdx.y;
+    if (i > N - 1 || j > N - 1) return;
+    const size_t k = (size_t)j * pitch + i;
+    const double nb = (psi_in[k - 1] + psi_in[k + 1]) + (psi_in[k - pitch] + psi_in[k + pitch]);
+    psi_out[k] = fma(omb, psi_in[k], fma(cb, nb, q[k]));
+}
+
+// ---- NEXT-2: RES_psi, RES_omega of eq 26-27: sum over ALL grid points of |new - old| ---------
+__global__ void __launch_bounds__(DIAG_THREADS)
+k_res_partial(int N, int pitch, const double* __restrict__ p1, const double* __restrict__ p0, const double* __restrict__ w1,
+              const double* __restrict__ w0, double* __restrict__ scratch) {
+    const long long M = (long long)(N + 1) * (N + 1);
+    double m = 0.0, sp = 0.0, sw = 0.0, unused = 0.0;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < M; t += (long long)gridDim.x * blockDim.x) {
+        const size_t k = (size_t)(t / (N + 1)) * pitch + (size_t)(t % (N + 1));
+        sp += fabs(p1[k] - p0[k]);
+        sw += fabs(w1[k] - w0[k]);
+    }
+    block_reduce4(m, sp, sw, unused);
+    if (threadIdx.x == 0) {
+        scratch[DIAG_BLOCKS + blockIdx.x] = sp;
+        scratch[2 * DIAG_BLOCKS + blockIdx.x] = sw;
+    }
+}
+
+__global__ void __launch_bounds__(DIAG_THREADS)
+k_res_final(int N, const double* __restrict__ scratch, double* __restrict__ out2) {
+    double m = 0.0, sp = 0.0, sw = 0.0, unused = 0.0;
+    for (int t = threadIdx.x; t < DIAG_BLOCKS; t += blockDim.x) {
+        sp += scratch[DIAG_BLOCKS + t];
+        sw += scratch[2 * DIAG_BLOCKS + t];
+    }
+    block_reduce4(m, sp, sw, unused);
+    if (threadIdx.x == 0) {
+        const double npts = (double)(N + 1);     // the paper's divisor: N = n_x = n_y points per side (reading G17)
+        out2[0] = sp / npts;
+        out2[1] = sw / npts;
+    }
+}
+
 }  // namespace
+
+int jacobi_sweeps(const Params& P, double* psi, double* psi_tmp, const double* q, int nsweeps, cudaStream_t st) {
+    dim3 b(64, 4), g(cdiv(P.N - 1, 64), cdiv(P.N - 1, 4));
+    double *in = psi, *out = psi_tmp;
+    for (int s = 0; s < nsweeps; ++s) {
+        k_jacobi_sweep<<<g, b, 0, st>>>(P.N, P.pitch, P.cb, P.omb, in, q, out);
+        double* t = in; in = out; out = t;
+    }
+    if (in != psi && cudaMemcpyAsync(psi, in, (size_t)P.pitch * (P.N + 1) * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        return -(int)cudaGetLastError();
+    return launched(nsweeps);
+}
+
+int res_monitors(const Params& P, const double* psi_new, const double* psi_old, const double* w_new, const double* w_old,
+                 double* scratch_dev, double* out2_dev, cudaStream_t st) {
+    k_res_partial<<<DIAG_BLOCKS, DIAG_THREADS, 0, st>>>(P.N, P.pitch, psi_new, psi_old, w_new, w_old, scratch_dev);
+    k_res_final<<<1, DIAG_THREADS, 0, st>>>(P.N, scratch_dev, out2_dev);
+    return launched(2);
+}
 
 int scale_rhs(const Params& P, const double* w, double* q, cudaStream_t st) {
     dim3 b(32, 8), g(cdiv(P.N + 1, 32), cdiv(P.N + 1, 8));

@@ -56,4 +56,15 @@ int zero_ring(const Params& P, double* psi, cudaStream_t st);
 // nsweeps x (red half-sweep, black half-sweep) of a1 on psi in place, right-hand side q (already scaled).
 int stream_sweeps(const Params& P, double* psi, const double* q, int nsweeps, cudaStream_t st);
 
+// ---- NEXT-3: damped-Jacobi sweeps ------------------------------------------------
+// nsweeps sweeps of psi_new = fma(1 - beta, psi, fma(beta / 4, nb, q)) from OLD values only; the result is in psi
+// (psi_tmp is a second field whose wall ring is +0.0; it is clobbered).
+int jacobi_sweeps(const Params& P, double* psi, double* psi_tmp, const double* q, int nsweeps, cudaStream_t st);
+
+// ---- NEXT-2: the paper's steady-state monitors (eq 26-27) ----------------------------------
+// out2_dev[0] = RES_psi = (1 / (N + 1)) sum |psi_new - psi_old|, out2_dev[1] = RES_omega likewise, over all grid points.
+// scratch_dev: as for diagnostics().
+int res_monitors(const Params& P, const double* psi_new, const double* psi_old, const double* w_new, const double* w_old,
+                 double* scratch_dev, double* out2_dev, cudaStream_t st);
+
 }  // namespace cavk
