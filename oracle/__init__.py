@@ -12,7 +12,7 @@ from .build import build
 
 MODE_PLAIN = 0
 MODE_FMA = 1
-SWEEP_REDBLACK, SWEEP_JACOBI = 0, 1
+SWEEP_REDBLACK, SWEEP_JACOBI, SWEEP_COMPACT9 = 0, 1, 2
 
 _lib = None
 
@@ -42,6 +42,7 @@ def lib():
         L.orc_sor.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, C.c_int]
         L.orc_set_sweep.argtypes = [C.c_void_p, C.c_int]
         L.orc_jacobi.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, C.c_int]
+        L.orc_compact.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, C.c_int]
         L.orc_step_res.argtypes = [C.c_void_p, dp, dp]
         L.orc_run_to_steady.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int), dp, dp,
                                         C.POINTER(C.c_int)]
@@ -90,7 +91,7 @@ class OracleCavity:
             pass
 
     def set_sweep(self, kind):
-        """SWEEP_REDBLACK (default) or SWEEP_JACOBI."""
+        """SWEEP_REDBLACK (default), SWEEP_JACOBI or SWEEP_COMPACT9."""
         _chk(lib().orc_set_sweep(self._h, kind), "orc_set_sweep")
 
     def step_res(self):
@@ -159,6 +160,14 @@ def jacobi(N, beta, psi, omega, nsweeps, mode=MODE_PLAIN):
     p = _field(psi, N, "psi").copy()
     omega = _field(omega, N, "omega")
     _chk(lib().orc_jacobi(N, beta, mode, _p(p), _p(omega), nsweeps), "orc_jacobi")
+    return p
+
+
+def compact(N, beta, psi, omega, nsweeps, mode=MODE_PLAIN):
+    """Four-colour sweeps of the paper's 4th-order compact operator (eq 14-21)."""
+    p = _field(psi, N, "psi").copy()
+    omega = _field(omega, N, "omega")
+    _chk(lib().orc_compact(N, beta, mode, _p(p), _p(omega), nsweeps), "orc_compact")
     return p
 
 

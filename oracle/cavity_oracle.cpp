@@ -52,7 +52,9 @@
 
 enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2 };
 enum { ORC_MODE_PLAIN = 0, ORC_MODE_FMA = 1 };
-enum { ORC_SWEEP_REDBLACK = 0, ORC_SWEEP_JACOBI = 1 };   // (a1) variants: red-black SOR (default) / damped Jacobi (NEXT-3)
+// (a1) variants: red-black SOR of the 5-point operator (default) / damped Jacobi (NEXT-3) / the paper's own 4th-order
+// compact 9-point operator relaxed in four colours (NEXT-1)
+enum { ORC_SWEEP_REDBLACK = 0, ORC_SWEEP_JACOBI = 1, ORC_SWEEP_COMPACT9 = 2 };
 
 struct orc_diag {
     double t;
@@ -166,8 +168,55 @@ void jacobi_sweeps(int N, int mode, double beta, std::vector<double>& psi, const
     }
 }
 
+// ---- (a1, NEXT-1 variant) the paper's fourth-order compact operator, eq 14-21 P:110-138 --------
+// eq 15:  psi <- (3/5) (beta / a) (A + B + C) + (1 - beta) psi,  with (eq 16-21, dx = dy = h, a = b + c, b = c = 1/h^2)
+//   A = b (psi_E + psi_W) + c (psi_N + psi_S)
+//   B = (1/12) (w_E + w_N + 8 w_0 + w_W + w_S)                      (reads the wall ring of omega next to a wall)
+//   C = (a/12) (psi_NE - 2 psi_N + psi_NW - 2 psi_E - 2 psi_W + psi_SE - 2 psi_S + psi_SW)
+// (eq 17 is printed twice and the tags (17)/(18) are displaced, G3; C is the expression printed above tag (18).)
+// ORDER (reading, N1): the paper relaxes lexicographically, "use the new values when they become available"
+// (P:114); its superscripts in eq 18 fit no single order (G3).  A 9-point stencil decouples under FOUR colours
+// (i mod 2, j mod 2), so both sides sweep colour (0,0), then (1,0), (0,1), (1,1), each from the latest values: inside a
+// colour no point reads another point of that colour, so the result does not depend on the order inside a colour.
+inline double compact_point_plain(const std::vector<double>& psi, const std::vector<double>& w, int N, int i, int j,
+                                  double beta) {
+    const double dx = 1.0 / (double)N, dy = 1.0 / (double)N;
+    const double b = 1.0 / (dx * dx), c = 1.0 / (dy * dy), a = b + c;
+    const double A = b * (psi[idx(N, i + 1, j)] + psi[idx(N, i - 1, j)]) + c * (psi[idx(N, i, j + 1)] + psi[idx(N, i, j - 1)]);
+    const double B = (1.0 / 12.0) * (w[idx(N, i + 1, j)] + w[idx(N, i, j + 1)] + 8.0 * w[idx(N, i, j)] + w[idx(N, i - 1, j)] +
+                                     w[idx(N, i, j - 1)]);
+    const double C = (1.0 / 12.0) * a *
+                     (psi[idx(N, i + 1, j + 1)] - 2.0 * psi[idx(N, i, j + 1)] + psi[idx(N, i - 1, j + 1)] - 2.0 * psi[idx(N, i + 1, j)] -
+                      2.0 * psi[idx(N, i - 1, j)] + psi[idx(N, i + 1, j - 1)] - 2.0 * psi[idx(N, i, j - 1)] + psi[idx(N, i - 1, j - 1)]);
+    return (3.0 / 5.0) * (beta / a) * (A + B + C) + (1.0 - beta) * psi[idx(N, i, j)];
+}
+// The same update collected as  psi <- (1 - beta) psi + 0.2 beta S_edge + 0.05 beta S_corner + (0.025 beta h^2) (S_edge(w) + 8 w_0)
+// with the association DESIGN.md "Canonical arithmetic" states for the kernels.
+inline double compact_point_fma(const std::vector<double>& psi, const std::vector<double>& w, int N, int i, int j,
+                                double beta) {
+    const double h = 1.0 / (double)N;
+    const double c1 = 0.2 * beta, c2 = 0.05 * beta, c3 = (0.025 * beta) * (h * h), omb = 1.0 - beta;
+    const double se = (psi[idx(N, i - 1, j)] + psi[idx(N, i + 1, j)]) + (psi[idx(N, i, j - 1)] + psi[idx(N, i, j + 1)]);
+    const double sc = (psi[idx(N, i - 1, j - 1)] + psi[idx(N, i + 1, j - 1)]) + (psi[idx(N, i - 1, j + 1)] + psi[idx(N, i + 1, j + 1)]);
+    const double sw = ((w[idx(N, i - 1, j)] + w[idx(N, i + 1, j)]) + (w[idx(N, i, j - 1)] + w[idx(N, i, j + 1)])) + 8.0 * w[idx(N, i, j)];
+    const double qB = c3 * sw;
+    return std::fma(omb, psi[idx(N, i, j)], std::fma(c1, se, std::fma(c2, sc, qB)));
+}
+
+void compact_sweeps(int N, int mode, double beta, std::vector<double>& psi, const std::vector<double>& w, int nsweeps) {
+    for (int s = 0; s < nsweeps; ++s)
+        for (int colour = 0; colour < 4; ++colour)               // (i mod 2, j mod 2) = (0,0), (1,0), (0,1), (1,1)
+            for (int j = 1; j <= N - 1; ++j)
+                for (int i = 1; i <= N - 1; ++i) {
+                    if ((i & 1) + 2 * (j & 1) != colour) continue;
+                    psi[idx(N, i, j)] = (mode == ORC_MODE_FMA) ? compact_point_fma(psi, w, N, i, j, beta)
+                                                                : compact_point_plain(psi, w, N, i, j, beta);
+                }
+}
+
 void poisson_sweeps(const orc_ctx* c, std::vector<double>& psi, const std::vector<double>& w, int nsweeps) {
-    if (c->sweep == ORC_SWEEP_JACOBI) jacobi_sweeps(c->N, c->mode, c->beta, psi, w, nsweeps);
+    if (c->sweep == ORC_SWEEP_COMPACT9) compact_sweeps(c->N, c->mode, c->beta, psi, w, nsweeps);
+    else if (c->sweep == ORC_SWEEP_JACOBI) jacobi_sweeps(c->N, c->mode, c->beta, psi, w, nsweeps);
     else sor_sweeps(c->N, c->mode, c->beta, psi, w, nsweeps);
 }
 
@@ -269,6 +318,14 @@ void one_step(orc_ctx* c) {
         std::vector<double>& win = (k == 1) ? w0 : (k == 2) ? c->w1 : (k == 3) ? c->w2 : (k == 4) ? c->w3 : c->w4;
         poisson_sweeps(c, c->psi, win, c->S);                   // (a1)
         thom(N, m, c->U, c->psi, win);                          // (a2)
+        if (k <= 4) {
+            // The stage output carries the wall vorticity just computed.  Nothing on the 5-point path ever reads it (a2 of
+            // the next stage overwrites it first); the compact operator's B (eq 17) does, during the next stage's sweeps:
+            // "the most recent wall vorticity" (reading N2; the paper is silent).
+            std::vector<double>& wout = (k == 1) ? c->w1 : (k == 2) ? c->w2 : (k == 3) ? c->w3 : c->w4;
+            for (int i = 0; i <= N; ++i) { wout[idx(N, i, 0)] = win[idx(N, i, 0)]; wout[idx(N, i, N)] = win[idx(N, i, N)]; }
+            for (int j = 1; j <= N - 1; ++j) { wout[idx(N, 0, j)] = win[idx(N, 0, j)]; wout[idx(N, N, j)] = win[idx(N, N, j)]; }
+        }
         for (int j = 1; j <= N - 1; ++j) {                      // (a3)
             for (int i = 1; i <= N - 1; ++i) {
                 const size_t p = idx(N, i, j);
@@ -351,7 +408,7 @@ ORC_API int orc_set_mode(orc_ctx* c, int mode) {
 }
 
 ORC_API int orc_set_sweep(orc_ctx* c, int kind) {
-    if (!c || (kind != ORC_SWEEP_REDBLACK && kind != ORC_SWEEP_JACOBI)) return ORC_EINVAL;
+    if (!c || kind < ORC_SWEEP_REDBLACK || kind > ORC_SWEEP_COMPACT9) return ORC_EINVAL;
     c->sweep = kind;
     return ORC_OK;
 }
@@ -445,6 +502,16 @@ ORC_API int orc_jacobi(int N, double beta, int mode, double* psi, const double* 
     const size_t G = (size_t)(N + 1) * (size_t)(N + 1);
     std::vector<double> p(psi, psi + G), w(omega, omega + G);
     jacobi_sweeps(N, mode, beta, p, w, nsweeps);
+    std::memcpy(psi, p.data(), G * sizeof(double));
+    return ORC_OK;
+}
+
+// nsweeps four-colour sweeps of the paper's compact operator on psi (in place; walls taken as given), RHS omega incl. its ring.
+ORC_API int orc_compact(int N, double beta, int mode, double* psi, const double* omega, int nsweeps) {
+    if (N < 2 || !psi || !omega || nsweeps < 0) return ORC_EINVAL;
+    const size_t G = (size_t)(N + 1) * (size_t)(N + 1);
+    std::vector<double> p(psi, psi + G), w(omega, omega + G);
+    compact_sweeps(N, mode, beta, p, w, nsweeps);
     std::memcpy(psi, p.data(), G * sizeof(double));
     return ORC_OK;
 }

@@ -519,3 +519,106 @@ def test_run_to_steady_stops_by_the_papers_rule():
     r2 = o2.run_to_steady(50, 10, 1e-9, 1e-7)
     assert not r2["converged"] and r2["steps"] == 50
     o.close(); o2.close()
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-1: the paper's own Poisson operator, the fourth-order compact 9-point scheme of eq 14-21, relaxed in
+# four colours.  Pins: (i) closed-form discrete solution for a sine mode and its FOURTH-order error decay;
+# (ii) a polynomial of degree 4 with omega = -lap(psi) is an exact fixed point (the scheme's truncation error has
+# sixth derivatives); (iii) brute force: dense solve of the assembled 9-point system on 9 x 9 with a random omega
+# INCLUDING its wall ring (eq 17 reads it); (iv) the colour order (hand-computed delta response).
+# --------------------------------------------------------------------------------------------
+
+def compact_ratio(N, k, l):
+    """psi / omega of the converged compact scheme for sin(k pi x) sin(l pi y)."""
+    h = 1.0 / N
+    cx, cy = math.cos(k * math.pi * h), math.cos(l * math.pi * h)
+    return h * h * (2.0 * (cx + cy) + 8.0) / 12.0 / (10.0 / 3.0 - (4.0 / 3.0) * (cx + cy) - (2.0 / 3.0) * cx * cy)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_compact_closed_form_and_fourth_order(mode):
+    errs = []
+    for N in (8, 16, 32):
+        X, Y = grid(N)
+        w = np.sin(np.pi * X) * np.sin(2 * np.pi * Y)
+        psi = oracle.compact(N, 1.0, np.zeros_like(w), w, 60 * N, mode)      # Gauss-Seidel-like: converges
+        assert np.max(np.abs(psi - compact_ratio(N, 1, 2) * w)) < 2e-13, N
+        errs.append(abs(compact_ratio(N, 1, 2) - 1.0 / (5.0 * np.pi ** 2)))
+    assert 14.0 < errs[0] / errs[1] < 17.5 and 15.0 < errs[1] / errs[2] < 16.5          # ratio 16 per halving: 4th order
+    # the 5-point operator of the hot path is only 2nd order on the same mode
+    assert 3.8 < abs(1 / lam_h(8, 1, 2) - 1 / (5 * np.pi ** 2)) / abs(1 / lam_h(16, 1, 2) - 1 / (5 * np.pi ** 2)) < 4.2
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_compact_exact_on_quartic(mode):
+    N = 12
+    X, Y = grid(N)
+    psi = X ** 4 - 3 * X ** 2 * Y ** 2 + X * Y ** 3 + 2 * Y ** 4 - X + 0.5
+    w = -((12 * X ** 2 - 6 * Y ** 2) + (-6 * X ** 2 + 6 * X * Y + 24 * Y ** 2))          # -(psi_xx + psi_yy)
+    out = oracle.compact(N, 1.0, psi, w, 3, mode)
+    assert np.max(np.abs(out - psi)) < 5e-14
+    # ... which the 5-point operator is not (error h^2/12 (psi_xxxx + psi_yyyy) = O(1e-2) here)
+    assert np.max(np.abs(oracle.sor(N, 1.0, psi, w, 3, mode) - psi)) > 1e-5
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_compact_converges_to_dense_direct_solve_9x9(mode):
+    N = 8
+    h = 1.0 / N
+    rng = np.random.default_rng(11)
+    w = rng.uniform(-1, 1, (N + 1, N + 1))                     # ring included: B of eq 17 reads it next to the walls
+    n = N - 1
+    A = np.zeros((n * n, n * n)); b = np.zeros(n * n)
+    ix = lambda i, j: (j - 1) * n + (i - 1)
+    for j in range(1, N):
+        for i in range(1, N):
+            r = ix(i, j)
+            A[r, r] = 10.0 / 3.0
+            for di, dj, c in ((1, 0, 2 / 3), (-1, 0, 2 / 3), (0, 1, 2 / 3), (0, -1, 2 / 3),
+                              (1, 1, 1 / 6), (-1, 1, 1 / 6), (1, -1, 1 / 6), (-1, -1, 1 / 6)):
+                ii, jj = i + di, j + dj
+                if 1 <= ii <= N - 1 and 1 <= jj <= N - 1:
+                    A[r, ix(ii, jj)] -= c
+            b[r] = h * h * (w[j, i + 1] + w[j, i - 1] + w[j + 1, i] + w[j - 1, i] + 8.0 * w[j, i]) / 12.0
+    ref = np.zeros((N + 1, N + 1)); ref[1:N, 1:N] = np.linalg.solve(A, b).reshape(n, n)
+    psi = oracle.compact(N, 1.2, np.zeros_like(w), w, 400, mode)
+    assert np.max(np.abs(psi - ref)) < 1e-14
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_compact_four_colour_order(mode):
+    # delta at (4,4) = colour (0,0), beta = 1, omega = 0, one sweep.  Colour (0,0) first: the delta itself -> 0 (all its
+    # neighbours are 0), its same-colour points stay 0.  Then (1,0): (3,4),(5,4) see only zeros -> 0.  So ONE sweep wipes
+    # a delta that sits on the first colour; a delta on the LAST colour (5,5) spreads to all 8 neighbours first.
+    N = 8
+    p = np.zeros((N + 1, N + 1)); p[4, 4] = 1.0
+    out = oracle.compact(N, 1.0, p, np.zeros_like(p), 1, mode)
+    assert not out.any()
+    p = np.zeros((N + 1, N + 1)); p[5, 5] = 1.0
+    out = oracle.compact(N, 1.0, p, np.zeros_like(p), 1, mode)
+    assert abs(out[4, 4] - 0.05) < 1e-16                        # colour (0,0): corner weight 1/20
+    # colour (1,0) point (i=5, j=4): edge neighbour (5,5) = 1 (old), edge neighbours (4,4) and (6,4) new = 0.05 each
+    assert abs(out[4, 5] - (0.2 * (1.0 + 0.05 + 0.05))) < 1e-16
+    # and finally the delta itself, colour (1,1), from its 8 new neighbours only
+    edges = out[4, 5] + out[6, 5] + out[5, 4] + out[5, 6]
+    corners = out[4, 4] + out[4, 6] + out[6, 4] + out[6, 6]
+    assert abs(out[5, 5] - (0.2 * edges + 0.05 * corners)) < 1e-15
+
+
+def test_step_with_compact_operator_uses_the_latest_wall_vorticity():
+    # stage k >= 2 must read, in B of eq 17, the ring Thom wrote at the end of stage k - 1 (reading N2): with the lid on
+    # and one step from rest the lid ring -2U/h enters psi through the top interior row already in stage 2
+    N = 8
+    o = oracle.OracleCavity(N, 100.0, 1e-3, 1.0, 3)
+    o.set_sweep(oracle.SWEEP_COMPACT9)
+    o.set_fields(None, np.zeros((N + 1, N + 1)))
+    o.step(1)
+    psi, w = o.get_fields()
+    assert psi[N - 1, 1:N].max() < 0.0                          # clockwise: psi < 0 under the lid
+    # the 5-point path from the same state moves psi only through the interior omega: much smaller after one step
+    o5 = oracle.OracleCavity(N, 100.0, 1e-3, 1.0, 3)
+    o5.set_fields(None, np.zeros((N + 1, N + 1)))
+    o5.step(1)
+    assert np.abs(psi).max() > 5 * np.abs(o5.get_fields()[0]).max()
+    o.close(); o5.close()
