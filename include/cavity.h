@@ -48,6 +48,8 @@ extern "C" {
 /* a1 variants (BASELINE.json north_star: "red-black SOR (or Jacobi)"). */
 #define CAV_SWEEP_REDBLACK  0   /* red-black SOR, red = (i + j) even first (default; the timed path) */
 #define CAV_SWEEP_JACOBI    1   /* damped Jacobi: every interior point from the OLD values only */
+#define CAV_SWEEP_COMPACT9  2   /* the paper's own operator: 4th-order compact 9-point scheme, eq 14-21, relaxed in
+                                   four colours (i mod 2, j mod 2) = (0,0), (1,0), (0,1), (1,1) (reading N1) */
 
 typedef struct cav_ctx cav_ctx;   /* opaque; owned by the library from cav_create to cav_destroy */
 
@@ -102,8 +104,11 @@ int cav_poisson(cav_ctx* ctx, int nsweeps, double* res_inf_out);
 
 /* Selects the a1 variant (CAV_SWEEP_*) used by cav_step and cav_poisson from now on.  With CAV_SWEEP_JACOBI sor_omega is the
  * damping factor: psi_new = psi + beta ((psi_W + psi_E + psi_S + psi_N + h^2 w) / 4 - psi), all from the previous sweep's
- * values (it converges for beta <= 1; nothing is checked).  The Jacobi sweeps run as one kernel per sweep over global
- * memory whatever the engine. */
+ * values (it converges for beta <= 1; nothing is checked).  With CAV_SWEEP_COMPACT9 a sweep is eq 15 of the paper,
+ *   psi <- (3/5)(beta/a)(A + B + C) + (1 - beta) psi,  A, B, C of eq 16-18, a = 2/h^2,
+ * whose B reads omega on the walls: the stage input carries the wall vorticity a2 computed in the previous stage (for the
+ * first stage after cav_set_fields: the ring as given; reading N2).  Both variants run as kernels over global
+ * memory whatever the engine (one per Jacobi sweep, four per compact sweep). */
 int cav_set_sweep(cav_ctx* ctx, int kind);
 
 /* One time step, and the paper's steady-state monitors of that step (eq 26-27):

@@ -18,8 +18,8 @@ SYMBOLS = ("cav_create", "cav_destroy", "cav_set_fields", "cav_get_fields", "cav
            "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_set_resident_plan", "cav_trace_sweeps", "cav_describe", "cav_launch_count",
            "cav_last_elapsed_ms", "cav_strerror", "cav_set_sweep", "cav_step_res", "cav_run_to_steady")
 
-SWEEP_REDBLACK, SWEEP_JACOBI = 0, 1
-_SWEEPS = {"redblack": SWEEP_REDBLACK, "jacobi": SWEEP_JACOBI}
+SWEEP_REDBLACK, SWEEP_JACOBI, SWEEP_COMPACT9 = 0, 1, 2
+_SWEEPS = {"redblack": SWEEP_REDBLACK, "jacobi": SWEEP_JACOBI, "compact9": SWEEP_COMPACT9}
 
 _lib = None
 
@@ -139,7 +139,7 @@ class Cavity:
              "cav_set_engine")
 
     def set_sweep(self, kind):
-        """'redblack' (default) or 'jacobi' (or the CAV_SWEEP_* integer)."""
+        """'redblack' (default), 'jacobi' or 'compact9' (or the CAV_SWEEP_* integer)."""
         _chk(lib().cav_set_sweep(self._h, _SWEEPS[kind] if isinstance(kind, str) else int(kind)), "cav_set_sweep")
 
     def step_res(self):

@@ -81,6 +81,9 @@ cavk::Params make_params(int N, double Re, double dt, double beta) {
     P.c2h2 = 2.0 * ((double)N * (double)N);
     P.lid = 2.0 * U * (double)N;
     P.dt = dt;
+    P.c9e = 0.2 * beta;
+    P.c9c = 0.05 * beta;
+    P.c9q = (0.025 * beta) * (h * h);
     return P;
 }
 
@@ -116,7 +119,10 @@ void resolve_engine(cav_ctx* c) {
 // a1: nsweeps red-black sweeps on psi with right-hand side w_in
 int enqueue_sweeps(cav_ctx* c, const double* w_in, int nsweeps, long long& nl) {
     if (nsweeps <= 0) return CAV_OK;
-    if (c->sweep == CAV_SWEEP_JACOBI) {
+    if (c->sweep == CAV_SWEEP_COMPACT9) {
+        LAUNCH(cavk::compact_rhs(c->P, w_in, c->q, c->st));
+        LAUNCH(cavk::compact_sweeps(c->P, c->psi, c->q, nsweeps, c->st));
+    } else if (c->sweep == CAV_SWEEP_JACOBI) {
         LAUNCH(cavk::scale_rhs(c->P, w_in, c->q, c->st));
         LAUNCH(cavk::jacobi_sweeps(c->P, c->psi, c->psi2, c->q, nsweeps, c->st));
     } else if (c->engine == CAV_ENGINE_RESIDENT) {
@@ -355,7 +361,7 @@ CAV_API int cav_get_diag(cav_ctx* c, cav_diag* out) {
 }
 
 CAV_API int cav_set_sweep(cav_ctx* c, int kind) {
-    if (!c || (kind != CAV_SWEEP_REDBLACK && kind != CAV_SWEEP_JACOBI)) return CAV_EINVAL;
+    if (!c || kind < CAV_SWEEP_REDBLACK || kind > CAV_SWEEP_COMPACT9) return CAV_EINVAL;
     DeviceGuard dg(c->device);
     CK(cudaStreamSynchronize(c->st));
     if (kind != c->sweep) { c->sweep = kind; drop_graph(c); }

@@ -224,6 +224,34 @@ k_jacobi_sweep(int N, int pitch, double cb, double omb, const double* __restrict
     psi_out[k] = fma(omb, psi_in[k], fma(cb, nb, q[k]));
 }
 
+// ---- a1, NEXT-1 variant: the paper's 4th-order compact 9-point operator, eq 14-21, four colours ----
+// eq 15 collected (dx = dy = h):  psi <- (1 - beta) psi + 0.2 beta S_edge(psi) + 0.05 beta S_corner(psi) + qB,
+// qB = (0.025 beta h^2) (S_edge(w) + 8 w_0)  = (3/5)(beta/a) B of eq 17; B reads the wall ring of w next to a wall.
+__global__ void __launch_bounds__(256)
+k_compact_rhs(int N, int pitch, double c9q, const double* __restrict__ w, double* __restrict__ qB) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i > N || j > N) return;
+    const size_t k = (size_t)j * pitch + i;
+    const bool interior = (i >= 1) & (i <= N - 1) & (j >= 1) & (j <= N - 1);
+    double v = 0.0;
+    if (interior) v = c9q * (((w[k - 1] + w[k + 1]) + (w[k - pitch] + w[k + pitch])) + 8.0 * w[k]);
+    qB[k] = v;
+}
+
+// one colour (i mod 2, j mod 2) = (colour & 1, colour >> 1) of a sweep; inside a colour no point reads another one of it
+__global__ void __launch_bounds__(256)
+k_compact_colour(int N, int pitch, double c9e, double c9c, double omb, double* __restrict__ psi, const double* __restrict__ qB,
+                 int colour) {
+    const int i = ((colour & 1) ? 1 : 2) + 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+    const int j = ((colour >> 1) ? 1 : 2) + 2 * (blockIdx.y * blockDim.y + threadIdx.y);
+    if (i > N - 1 || j > N - 1) return;
+    const size_t k = (size_t)j * pitch + i;
+    const double se = (psi[k - 1] + psi[k + 1]) + (psi[k - pitch] + psi[k + pitch]);
+    const double sc = (psi[k - pitch - 1] + psi[k - pitch + 1]) + (psi[k + pitch - 1] + psi[k + pitch + 1]);
+    psi[k] = fma(omb, psi[k], fma(c9e, se, fma(c9c, sc, qB[k])));
+}
+
 // ---- NEXT-2: RES_psi, RES_omega of eq 26-27: sum over ALL grid points of |new - old| ---------
 __global__ void __launch_bounds__(DIAG_THREADS)
 k_res_partial(int N, int pitch, const double* __restrict__ p1, const double* __restrict__ p0, const double* __restrict__ w1,
@@ -269,6 +297,21 @@ int jacobi_sweeps(const Params& P, double* psi, double* psi_tmp, const double* q
     if (in != psi && cudaMemcpyAsync(psi, in, (size_t)P.pitch * (P.N + 1) * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
         return -(int)cudaGetLastError();
     return launched(nsweeps);
+}
+
+int compact_rhs(const Params& P, const double* w, double* qB, cudaStream_t st) {
+    dim3 b(32, 8), g(cdiv(P.N + 1, 32), cdiv(P.N + 1, 8));
+    k_compact_rhs<<<g, b, 0, st>>>(P.N, P.pitch, P.c9q, w, qB);
+    return launched(1);
+}
+
+int compact_sweeps(const Params& P, double* psi, const double* qB, int nsweeps, cudaStream_t st) {
+    const int half = P.N / 2 + 1;
+    dim3 b(64, 4), g(cdiv(half, 64), cdiv(half, 4));
+    for (int s = 0; s < nsweeps; ++s)
+        for (int colour = 0; colour < 4; ++colour)             // (0,0), (1,0), (0,1), (1,1): reading N1
+            k_compact_colour<<<g, b, 0, st>>>(P.N, P.pitch, P.c9e, P.c9c, P.omb, psi, qB, colour);
+    return launched(4 * nsweeps);
 }
 
 int res_monitors(const Params& P, const double* psi_new, const double* psi_old, const double* w_new, const double* w_old,

@@ -23,6 +23,9 @@ struct Params {
     double c2h2;    // 2 / h^2                       (eq 25)
     double lid;     // 2 U / h, U = 1                (eq 25, lid term)
     double dt;
+    double c9e;     // 0.2 beta                      (NEXT-1 compact operator: weight of the four edge neighbours)
+    double c9c;     // 0.05 beta                     (weight of the four corner neighbours)
+    double c9q;     // (0.025 beta) h^2              (scales S_edge(w) + 8 w_0 into the sweep's right-hand side)
 };
 
 // ---- support kernels (both engines) ---------------------------------------------------------------
@@ -60,6 +63,12 @@ int stream_sweeps(const Params& P, double* psi, const double* q, int nsweeps, cu
 // nsweeps sweeps of psi_new = fma(1 - beta, psi, fma(beta / 4, nb, q)) from OLD values only; the result is in psi
 // (psi_tmp is a second field whose wall ring is +0.0; it is clobbered).
 int jacobi_sweeps(const Params& P, double* psi, double* psi_tmp, const double* q, int nsweeps, cudaStream_t st);
+
+// ---- NEXT-1: the paper's 4th-order compact 9-point operator (eq 14-21), four-colour SOR ------
+// qB = c9q (S_edge(w) + 8 w_0) on interior points (reads the wall ring of w), 0 elsewhere.
+int compact_rhs(const Params& P, const double* w, double* qB, cudaStream_t st);
+// nsweeps x four colour passes of psi <- fma(1 - beta, psi, fma(c9e, S_edge, fma(c9c, S_corner, qB))) in place.
+int compact_sweeps(const Params& P, double* psi, const double* qB, int nsweeps, cudaStream_t st);
 
 // ---- NEXT-2: the paper's steady-state monitors (eq 26-27) ----------------------------------
 // out2_dev[0] = RES_psi = (1 / (N + 1)) sum |psi_new - psi_old|, out2_dev[1] = RES_omega likewise, over all grid points.

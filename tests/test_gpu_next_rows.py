@@ -146,3 +146,62 @@ def test_run_to_steady_matches_oracle_driver(cav, orc):
     r2 = g2.run_to_steady(30, 7, 1e-9, 1e-7)
     assert not r2["converged"] and r2["steps"] == 30 and g2.diag()["step"] == 30
     g.close(); o.close(); g2.close()
+
+
+# ---- NEXT-1: the paper's 4th-order compact 9-point operator, four colours ----------------------------------
+
+@pytest.mark.parametrize("N,S,beta", [(2, 3, 1.0), (3, 2, 0.8), (8, 5, 1.2), (33, 12, 1.5), (64, 9, 0.6), (129, 6, 1.7), (300, 4, 1.0), (513, 3, 1.3)])
+def test_compact9_step_bit_exact_and_contract(cav, orc, N, S, beta):
+    psi0, w0 = random_fields(N, 2468 + N)            # omega's ring is random too: stage 1 reads it as given (reading N2)
+    for mode in (orc.MODE_FMA, orc.MODE_PLAIN):
+        g = cav.Cavity(N, 400.0, 0.4 / N, beta, S)
+        g.set_sweep("compact9")
+        o = orc.OracleCavity(N, 400.0, 0.4 / N, beta, S, mode)
+        o.set_sweep(orc.SWEEP_COMPACT9)
+        g.set_fields(psi0, w0); o.set_fields(psi0, w0)
+        g.poisson(S + 2); o.poisson(S + 2)
+        g.step(3); o.step(3)
+        (gp, gw), (op, ow) = g.get_fields(), o.get_fields()
+        if mode == orc.MODE_FMA:
+            assert np.array_equal(gp, op) and np.array_equal(gw, ow), (N, S)
+        else:
+            assert relerr(gp, op) <= TOL and relerr(gw, ow) <= TOL, (N, relerr(gp, op), relerr(gw, ow))
+        assert not gp[0].any() and not gp[-1].any() and not gp[:, 0].any() and not gp[:, -1].any()
+        g.close(); o.close()
+
+
+def test_compact9_fourth_order_on_gpu(cav):
+    # closed form, no oracle: converged psi / omega for sin(pi x) sin(2 pi y), and its error against the continuum
+    # 1 / (5 pi^2) falls by 16 per halving of h
+    errs = []
+    for N in (16, 32, 64):
+        h = 1.0 / N
+        x = np.arange(N + 1) * h
+        w = np.outer(np.sin(2 * np.pi * x), np.sin(np.pi * x))
+        cx, cy = math.cos(math.pi * h), math.cos(2 * math.pi * h)
+        ratio = h * h * (2.0 * (cx + cy) + 8.0) / 12.0 / (10.0 / 3.0 - (4.0 / 3.0) * (cx + cy) - (2.0 / 3.0) * cx * cy)
+        g = cav.Cavity(N, 100.0, 1e-3, 1.7, 1)
+        g.set_sweep("compact9")
+        wi = w.copy(); wi[0] = wi[-1] = 0.0; wi[:, 0] = wi[:, -1] = 0.0      # sin vanishes on the walls up to rounding
+        g.set_fields(None, wi)
+        g.poisson(40 * N)
+        psi, _ = g.get_fields()
+        assert np.max(np.abs(psi - ratio * wi)) < 1e-13, N
+        errs.append(abs(ratio - 1.0 / (5.0 * np.pi ** 2)))
+        g.close()
+    assert 15.0 < errs[0] / errs[1] < 16.5 and 15.5 < errs[1] / errs[2] < 16.5
+
+
+def test_compact9_config1_contract_and_cavity_physics(cav, orc):
+    # BASELINE config 1's grid and step count with the paper's operator and an under-relaxed beta in the paper's range
+    wl = W.config(1)
+    psi0, w0 = W.initial_fields(wl)
+    g = cav.Cavity(wl.N, wl.Re, wl.dt, 0.8, wl.sweeps_per_stage)
+    o = orc.OracleCavity(wl.N, wl.Re, wl.dt, 0.8, wl.sweeps_per_stage, orc.MODE_PLAIN)
+    g.set_sweep("compact9"); o.set_sweep(orc.SWEEP_COMPACT9)
+    g.set_fields(psi0, w0); o.set_fields(psi0, w0)
+    g.step(wl.steps); o.step(wl.steps)
+    (gp, gw), (op, ow) = g.get_fields(), o.get_fields()
+    assert relerr(gp, op) <= TOL and relerr(gw, ow) <= TOL
+    assert gp.min() < -0.05 and np.isfinite(gw).all()
+    g.close(); o.close()
