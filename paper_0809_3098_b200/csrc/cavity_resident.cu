@@ -272,11 +272,13 @@ __host__ __device__ inline Region send_region(const TileGeom& t, int N, int halo
 __host__ __device__ inline Region recv_region(const TileGeom& t, int N, int halo) {
     const int xlo = imax(t.cx0 - halo, 1), xhi = imin(t.cx1 + halo, N), ylo = imax(t.cy0 - halo, 1), yhi = imin(t.cy1 + halo, N);
     const int yc0 = imax(t.cy0, ylo), yc1 = imin(t.cy1, yhi), xc0 = imax(t.cx0, xlo), xc1 = imin(t.cx1, xhi);
+    // Order = the order in which the neighbours STORE these points (send_region: bottom strip, top strip, left, right), so
+    // that what was stored first is fetched first: the ring above comes from the northern tile's bottom strip, etc.
     Region g;
-    g.r[0] = Rect{xlo, xhi, ylo, yc0};
-    g.r[1] = Rect{xlo, xhi, yc1, yhi};
-    g.r[2] = Rect{xlo, xc0, yc0, yc1};
-    g.r[3] = Rect{xc1, xhi, yc0, yc1};
+    g.r[0] = Rect{xlo, xhi, yc1, yhi};      // ring above   <- bottom strips of the tiles above
+    g.r[1] = Rect{xlo, xhi, ylo, yc0};      // ring below   <- top strips of the tiles below
+    g.r[2] = Rect{xc1, xhi, yc0, yc1};      // ring right   <- left strip of the tile to the right
+    g.r[3] = Rect{xlo, xc0, yc0, yc1};      // ring left    <- right strip of the tile to the left
     return g;
 }
 
