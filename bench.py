@@ -42,8 +42,8 @@ SM_COUNT, FP64_LANES_PER_SM = 148, 64   # B200: 148 SMs x 64 fp64 lanes (DESIGN.
 FP64_INSTR_PER_POINT_SWEEP = 5     # 3 DADD + 2 DFMA
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE k_resident launch (200 sweeps at 1025^2) from the ncu --set full capture
 # summarised in profiles/ (cold L2 under ncu: psi and omega are read once, the result stays in L2)
-NCU_DRAM_BYTES_PER_LAUNCH = 26.9e6
-NCU_DRAM_SOURCE = "profiles/r1b_resident_tagged.md (ncu --set full, one launch of 200 sweeps)"
+NCU_DRAM_BYTES_PER_LAUNCH = 26.6e6
+NCU_DRAM_SOURCE = "profiles/r1c_final.md (ncu --set full, one launch of 200 sweeps)"
 
 
 def parse():
