@@ -143,6 +143,10 @@ int cav_set_resident_plan(cav_ctx* ctx, int sweeps_per_exchange, int variant);
  * the capacity of a plan's tile count (at most 1023).  CAV_ENOTSUP if the engine in use is not the resident one. */
 int cav_trace_sweeps(cav_ctx* ctx, int nsweeps, long long* stamps_out, int slots_per_tile, int* ntiles_out);
 
+/* Testing aid, resident engine: sets the host-side tag epoch of the halo exchange (tags are epoch + round, unique per round
+ * and launch; near 2^32 the library clears the exchange buffers and restarts the epoch at 0: this call lets a test get there). */
+int cav_debug_set_epoch(cav_ctx* ctx, unsigned int epoch);
+
 /* Describes the launch plan of the current engine in `buf` (NUL-terminated, truncated to len). */
 int cav_describe(cav_ctx* ctx, char* buf, int len);
 

@@ -16,7 +16,7 @@ _ENGINES = {"auto": ENGINE_AUTO, "stream": ENGINE_STREAM, "resident": ENGINE_RES
 # every symbol include/cavity.h declares
 SYMBOLS = ("cav_create", "cav_destroy", "cav_set_fields", "cav_get_fields", "cav_step", "cav_step_async", "cav_sync",
            "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_set_resident_plan", "cav_trace_sweeps", "cav_describe", "cav_launch_count",
-           "cav_last_elapsed_ms", "cav_strerror", "cav_set_sweep", "cav_step_res", "cav_run_to_steady")
+           "cav_last_elapsed_ms", "cav_strerror", "cav_set_sweep", "cav_step_res", "cav_run_to_steady", "cav_debug_set_epoch")
 
 SWEEP_REDBLACK, SWEEP_JACOBI, SWEEP_COMPACT9 = 0, 1, 2
 _SWEEPS = {"redblack": SWEEP_REDBLACK, "jacobi": SWEEP_JACOBI, "compact9": SWEEP_COMPACT9}
@@ -78,6 +78,7 @@ def lib():
     L.cav_set_sweep.argtypes = [C.c_void_p, C.c_int]
     L.cav_step_res.argtypes = [C.c_void_p, dp, dp]
     L.cav_run_to_steady.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(CavMonitor)]
+    L.cav_debug_set_epoch.argtypes = [C.c_void_p, C.c_uint]
     L.cav_strerror.argtypes = [C.c_int]
     L.cav_strerror.restype = C.c_char_p
     _lib = L
@@ -153,6 +154,9 @@ class Cavity:
         _chk(lib().cav_run_to_steady(self._h, int(max_steps), int(check_every), float(tol_psi), float(tol_omega),
                                      C.byref(m)), "cav_run_to_steady")
         return {"steps": m.steps, "converged": bool(m.converged), "res_psi": m.res_psi, "res_omega": m.res_omega}
+
+    def debug_set_epoch(self, epoch):
+        _chk(lib().cav_debug_set_epoch(self._h, int(epoch) & 0xFFFFFFFF), "cav_debug_set_epoch")
 
     def set_resident_plan(self, T=0, variant=-1):
         _chk(lib().cav_set_resident_plan(self._h, int(T), int(variant)), "cav_set_resident_plan")

@@ -126,6 +126,16 @@ int enqueue_sweeps(cav_ctx* c, const double* w_in, int nsweeps, long long& nl) {
         LAUNCH(cavk::scale_rhs(c->P, w_in, c->q, c->st));
         LAUNCH(cavk::jacobi_sweeps(c->P, c->psi, c->psi2, c->q, nsweeps, c->st));
     } else if (c->engine == CAV_ENGINE_RESIDENT) {
+        if (c->epoch > 0xF0000000u) {
+            // Tags are 32-bit and must never repeat while an older unit with the same tag can still sit in an exchange
+            // buffer: long before the epoch wraps, clear the buffers (tag 0 = never valid) and start over.
+            const size_t xb_bytes = cavk::resident_exchange_doubles(c->field_doubles) * sizeof(double);
+            if (cudaMemsetAsync(c->xa, 0, xb_bytes, c->st) != cudaSuccess || cudaMemsetAsync(c->xb, 0, xb_bytes, c->st) != cudaSuccess) {
+                cudaGetLastError();
+                return CAV_ECUDA;
+            }
+            c->epoch = 0;
+        }
         LAUNCH(cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, c->tables, w_in, c->err_word, &c->epoch, nsweeps, c->st));
         std::swap(c->psi, c->psi2);
     } else {
@@ -457,6 +467,14 @@ CAV_API int cav_trace_sweeps(cav_ctx* c, int nsweeps, long long* stamps_out, int
     try { c10::cuda::CUDACachingAllocator::raw_delete(dev); } catch (...) {}
     if (ntiles_out) *ntiles_out = c->plan.ntiles;
     return rc == CAV_OK ? check_resident_error(c) : rc;
+}
+
+CAV_API int cav_debug_set_epoch(cav_ctx* c, unsigned int epoch) {
+    if (!c) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    CK(cudaStreamSynchronize(c->st));
+    c->epoch = epoch;
+    return CAV_OK;
 }
 
 CAV_API int cav_describe(cav_ctx* c, char* buf, int len) {

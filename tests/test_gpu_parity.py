@@ -392,3 +392,23 @@ def test_trace_sweeps_reports_ordered_phases(cav):
     # the traced call is a real cav_poisson without the a2 pass: psi agrees with the streaming engine bit for bit
     assert np.array_equal(g.get_fields()[0], ref.get_fields()[0])
     g.close(); ref.close()
+
+
+@pytest.mark.parametrize("epoch", [0xEFFFFFF0, 0xF0000001, 0xFFFFFF00])
+def test_tag_epoch_restart_near_wrap(cav, epoch):
+    """Exchange tags are 32-bit: well before the epoch wraps the library clears the exchange buffers and restarts it.  Runs
+    across that point (and with tags above 2^31) must stay bit-exact."""
+    wl = W.config(3)                                   # 513 x 513, multi-tile plan; 9 sweeps per stage: two rounds per launch
+    psi0, w0 = W.initial_fields(wl)
+    g = cav.Cavity(wl.N, wl.Re, wl.dt, wl.sor_omega, 9, engine="resident")
+    s = cav.Cavity(wl.N, wl.Re, wl.dt, wl.sor_omega, 9, engine="stream")
+    for c in (g, s):
+        c.set_fields(psi0, w0)
+        c.step(1)
+    g.debug_set_epoch(epoch)
+    for c in (g, s):
+        c.step(3)
+    (gp, gw), (sp, sw) = g.get_fields(), s.get_fields()
+    assert np.isfinite(gp).all() and np.isfinite(gw).all() and np.abs(gp).max() > 0
+    assert np.array_equal(gp, sp) and np.array_equal(gw, sw)
+    g.close(); s.close()
