@@ -223,13 +223,20 @@ def check_against_golden(cav, k, engine, max_step=None):
         ewi = np.max(np.abs(ws[inner, inner] - np.array(cp["omega"])[inner, inner])) / cp["omega_absmax_interior"]
         assert ep <= TOL and ew <= TOL and ewi <= TOL, (k, engine, cp["label"], ep, ew, ewi)
         d = g.diag()
-        # The residual r = lap_h(psi) + omega carries a rounding error of a few eps * 4 max|psi| / h^2 per point however it
-        # is evaluated; after config 5's 10 000 Poisson-only sweeps the residual IS that floor (1.7e-10), so there the FMA
-        # kernels and the plain oracle agree only to that absolute level (tolerance).
-        floor = 64.0 * np.finfo(np.float64).eps * 4.0 * cp["psi_absmax"] * wl.N * wl.N
-        for key in ("kinetic_energy", "enstrophy", "res_l2", "res_inf"):
-            atol = floor if key.startswith("res_") else 0.0
-            assert abs(d[key] - cp[key]) <= 1e-8 * abs(cp[key]) + atol, (k, engine, cp["label"], key, d[key], cp[key])
+        for key in ("kinetic_energy", "enstrophy"):
+            assert abs(d[key] - cp[key]) <= 1e-8 * abs(cp[key]), (k, engine, cp["label"], key, d[key], cp[key])
+        if cp["label"] == "poisson":
+            # After config 5's 10 000 Poisson-only sweeps the residual r = lap_h(psi) + omega IS the rounding error of its own
+            # evaluation (golden: res_inf 1.25e-9, res_l2 1.68e-10 = 21 and 2.9 units of eps * 4 max|psi| N^2 = 5.9e-11), so
+            # the FMA kernels and the plain oracle cannot agree digit for digit there.  What is checked at THIS checkpoint
+            # only: both sit below 64 such units (3.8e-9) and within a factor 4 of each other.
+            floor = 64.0 * np.finfo(np.float64).eps * 4.0 * cp["psi_absmax"] * wl.N * wl.N
+            for key in ("res_l2", "res_inf"):
+                assert d[key] <= floor and cp[key] <= floor, (k, engine, key, d[key], cp[key], floor)
+                assert 0.25 * cp[key] <= d[key] <= 4.0 * cp[key], (k, engine, key, d[key], cp[key])
+        else:
+            for key in ("res_l2", "res_inf"):
+                assert abs(d[key] - cp[key]) <= 1e-8 * abs(cp[key]), (k, engine, cp["label"], key, d[key], cp[key])
         assert abs(np.max(np.abs(psi)) - cp["psi_absmax"]) <= TOL * cp["psi_absmax"]
         assert abs(np.min(psi) - cp["psi_min"]) <= TOL * cp["psi_absmax"]
         # invariants that hold at any size: psi is exactly 0 on the walls

@@ -622,3 +622,138 @@ def test_step_with_compact_operator_uses_the_latest_wall_vorticity():
     o5.step(1)
     assert np.abs(psi).max() > 5 * np.abs(o5.get_fields()[0]).max()
     o.close(); o5.close()
+
+
+# --------------------------------------------------------------------------------------------
+# the COMPOSED step: order and wiring of a1 -> a2 -> a3 inside one_step (missing #1)
+#
+# One and three time steps are re-composed here in numpy from the operator-level entry points that the pins above
+# fix one by one (oracle.sor / jacobi / compact, oracle.thom, oracle.rhs), in exactly the order of SURVEY S8(c):
+# per stage k (reading G7): S sweeps on psi with right-hand side w_in -> Thom ring of w_in from the new psi
+# (eq 25) -> dL = dt L(psi, w_in) (eq 8, eq 22) -> eq 9-13 (constants retyped from P:85-108 with
+# readings G1, G2; eq 13 left to right, i.e. T-then-finish); the stage output carries the ring just computed (reading N2);
+# the ring of omega^{n+1} is the stage-5 ring (G16).  numpy's float64 `a*x + b*y` has no FMA, so the comparison with
+# orc_step in PLAIN mode is BIT EXACT: a wrong right-hand side, Thom after a3, swapped stage buffers, a wrong ring or a
+# wrong association all turn it red (lid on, S > 0, random psi0 / omega0, all three sweep kinds).
+# --------------------------------------------------------------------------------------------
+
+_C1 = 0.391752226571890                                                             # eq 9 (G2)
+_A20, _A21, _C2 = 0.444370493651235, 0.555629506348765, 0.368410593050371            # eq 10 (G1)
+_A30, _A32, _C3 = 0.620101851488403, 0.379898148511597, 0.251891774271694            # eq 11
+_A40, _A43, _C4 = 0.178079954393132, 0.821920045606868, 0.544974750228521            # eq 12
+_A52, _A53, _C53, _A54, _C54 = (0.517231671970585, 0.096059710526147, 0.063692468666290, 0.386708617503269,
+                                0.226007483236906)                                    # eq 13
+
+
+def _compose_step(N, Re, dt, beta, S, psi, w0, sweeps, U=1.0):
+    """One SSPRK(5,4) step from the pinned operators only; returns (psi, omega) as cav_get_fields would."""
+    I = (slice(1, N), slice(1, N))
+    stage_in = [w0.copy(), None, None, None, None]
+    dL3 = None
+    for k in range(1, 6):
+        win = stage_in[k - 1]
+        psi = sweeps(N, beta, psi, win, S, MODE_PLAIN)                  # (a1) warm start: psi carried over
+        win = oracle.thom(N, U, psi, win, MODE_PLAIN)                   # (a2) ring of the stage INPUT, from the new psi
+        stage_in[k - 1] = win
+        dL = dt * oracle.rhs(N, Re, psi, win, MODE_PLAIN)               # (a3)
+        out = win.copy()                                                # the output carries the ring just computed (N2)
+        w0_, w1, w2, w3, w4 = stage_in
+        if k == 1:
+            out[I] = w0_[I] + _C1 * dL[I]
+        elif k == 2:
+            out[I] = (_A20 * w0_[I] + _A21 * w1[I]) + _C2 * dL[I]
+        elif k == 3:
+            out[I] = (_A30 * w0_[I] + _A32 * w2[I]) + _C3 * dL[I]
+        elif k == 4:
+            out[I] = (_A40 * w0_[I] + _A43 * w3[I]) + _C4 * dL[I]
+            dL3 = dL
+        else:
+            T = (_A52 * w2[I] + _A53 * w3[I]) + _C53 * dL3[I]           # eq 13, left to right
+            out[I] = (T + _A54 * w4[I]) + _C54 * dL[I]
+        if k < 5:
+            stage_in[k] = out
+    return psi, out
+
+
+def _random_state(N, seed):
+    rng = np.random.default_rng(seed)
+    psi = np.zeros((N + 1, N + 1))
+    psi[1:N, 1:N] = 1e-2 * rng.standard_normal((N - 1, N - 1))
+    w = rng.standard_normal((N + 1, N + 1))                             # ring included: a2 must overwrite it before use
+    return psi, w
+
+
+@pytest.mark.parametrize("kind,sweeps", [(oracle.SWEEP_REDBLACK, oracle.sor), (oracle.SWEEP_JACOBI, oracle.jacobi),
+                                         (oracle.SWEEP_COMPACT9, oracle.compact)])
+@pytest.mark.parametrize("N,S,nsteps", [(9, 3, 1), (12, 2, 3), (16, 1, 1)])
+def test_composed_step_equals_recomposition_from_pinned_operators(kind, sweeps, N, S, nsteps):
+    Re, dt = 80.0, 2.5e-3
+    beta = 0.9 if kind == oracle.SWEEP_JACOBI else 1.6
+    psi, w = _random_state(N, 1000 + N)
+    o = oracle.OracleCavity(N, Re, dt, beta, S, MODE_PLAIN)
+    o.set_sweep(kind)
+    o.set_fields(psi, w)
+    for _ in range(nsteps):
+        psi, w = _compose_step(N, Re, dt, beta, S, psi, w, sweeps)
+    o.step(nsteps)
+    psi_o, w_o = o.get_fields()
+    o.close()
+    assert np.array_equal(psi_o, psi), np.max(np.abs(psi_o - psi))
+    assert np.array_equal(w_o, w), np.max(np.abs(w_o - w))
+
+
+def test_composed_step_pin_detects_the_plausible_mistakes():
+    # the recomposition is sensitive to each of the mistakes VERDICT r1 names (so the equality above is not vacuous):
+    # sweeps solved with the WRONG right-hand side (omega^n instead of the stage input), Thom applied AFTER a3 (i.e. a3
+    # reading the stale ring), and swapped stage buffers each change the result far above rounding
+    N, Re, dt, beta, S = 12, 80.0, 2.5e-3, 1.6, 2
+    psi0, w0 = _random_state(N, 7)
+    ref_psi, ref_w = _compose_step(N, Re, dt, beta, S, psi0, w0, oracle.sor)
+
+    def wrong_rhs(N_, beta_, psi, win, S_, mode):                       # always sweeps against omega^n
+        return oracle.sor(N_, beta_, psi, w0, S_, mode)
+    p1, w1 = _compose_step(N, Re, dt, beta, S, psi0, w0, wrong_rhs)
+    assert np.max(np.abs(w1 - ref_w)) > 1e-6 or np.max(np.abs(p1 - ref_psi)) > 1e-6
+
+    real_thom = oracle.thom
+    try:
+        oracle.thom = lambda N_, U, psi, w, mode=MODE_PLAIN: real_thom(N_, U, np.zeros_like(psi), w, mode)   # stale / wrong ring
+        p2, w2 = _compose_step(N, Re, dt, beta, S, psi0, w0, oracle.sor)
+    finally:
+        oracle.thom = real_thom
+    assert np.max(np.abs(w2[1:N, 1:N] - ref_w[1:N, 1:N])) > 1e-6
+
+
+def test_composed_step_without_lid_and_with_other_lid_speed():
+    # U enters only through a2's lid term; the recomposition with U = 0 and U = 2 pins orc_set_lid's wiring
+    N, Re, dt, beta, S = 10, 50.0, 2e-3, 1.5, 2
+    for U in (0.0, 2.0):
+        psi, w = _random_state(N, 31)
+        o = oracle.OracleCavity(N, Re, dt, beta, S, MODE_PLAIN)
+        o.set_lid(U)
+        o.set_fields(psi, w)
+        o.step(1)
+        p_ref, w_ref = _compose_step(N, Re, dt, beta, S, psi, w, oracle.sor, U=U)
+        p_o, w_o = o.get_fields()
+        o.close()
+        assert np.array_equal(p_o, p_ref) and np.array_equal(w_o, w_ref)
+
+
+# NON-AUTHORITATIVE cross-check (a third opinion, not a pin): SURVEY.md Appendix B lists what the survey's own throwaway
+# C restatement of the scheme (not in the repo, written before and independently of this oracle) printed for configs 1
+# and 2.  Agreement to 1e-11 relative means two independently typed programs compute the same nonlinear step.
+@pytest.mark.parametrize("cfg,ke,ens,psi_min", [(1, 2.327615235283e-02, 3.829854679875e+00, -9.340961439425e-02),
+                                                (2, 2.215415150575e-02, 1.048227398154e+01, -9.094674548856e-02)])
+def test_full_configs_against_survey_appendix_b_third_opinion(cfg, ke, ens, psi_min):
+    from paper_0809_3098_b200 import workloads
+    wl = workloads.config(cfg)
+    psi0, w0 = workloads.initial_fields(wl)
+    o = oracle.OracleCavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage, MODE_PLAIN)
+    o.set_fields(psi0, w0)
+    o.step(wl.steps)
+    d = o.diag()
+    psi, _ = o.get_fields()
+    o.close()
+    assert abs(d["kinetic_energy"] / ke - 1.0) < 1e-11
+    assert abs(d["enstrophy"] / ens - 1.0) < 1e-11
+    assert abs(psi[1:wl.N, 1:wl.N].min() / psi_min - 1.0) < 1e-11
