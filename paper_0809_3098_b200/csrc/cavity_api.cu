@@ -11,6 +11,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -27,22 +28,25 @@ struct cav_ctx {
     double Re = 0, dt = 0, beta = 0;
     cavk::Params P{};
     cudaStream_t st = nullptr;
-    void* slab = nullptr;            // one allocation from PyTorch's caching allocator
+    void* slab = nullptr;            // one allocation from PyTorch's caching allocator: the fields every engine needs
     double* psi = nullptr;           // stream function (current)
-    double* psi2 = nullptr;          // resident engine: the field the next sweep launch writes (then swapped with psi)
-    double* xa = nullptr;            // resident engine: exchange buffer of even rounds (16-byte units, 2 fields long)
-    double* xb = nullptr;            // resident engine: exchange buffer of odd rounds
-    double* q = nullptr;             // (beta/4) h^2 w_in, the scaled right-hand side of the current stage
-    double* w[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // omega^n (state), omega^(1..4)
+    double* psi2 = nullptr;          // the field the next resident launch / Jacobi sweep writes (then swapped with psi)
+    void* xbuf = nullptr;            // resident engine, multi-tile plans: the two exchange buffers (allocated with the plan)
+    void* xa = nullptr;              //   ... of even rounds (32-byte units)
+    void* xb = nullptr;              //   ... of odd rounds
+    double* q = nullptr;             // stream / Jacobi / compact sweeps: scaled right-hand side of the stage (allocated on first use)
+    double* w[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // omega^n (state), omega^(1..4): consecutive fields, then T
     double* T = nullptr;             // first three terms of eq 13
-    double* psi_prev = nullptr;      // NEXT-2 monitors: psi and omega before the monitored step
+    double* prev = nullptr;          // NEXT-2 monitors: psi and omega before the monitored step (allocated on first use)
+    double* psi_prev = nullptr;
     double* w_prev = nullptr;
     int sweep = CAV_SWEEP_REDBLACK;  // a1 variant
     double* scratch = nullptr;       // diagnostics partials
     double* out4 = nullptr;          // diagnostics result (device)
     void* tables = nullptr;          // resident engine: per-plan exchange tables (own allocation, rebuilt on re-plan)
     unsigned int* err_word = nullptr;// resident engine: device error word (a tile gave up waiting for a neighbour)
-    unsigned int epoch = 0;          // resident engine: tag epoch (host side)
+    unsigned int epoch = 0;          // resident engine: exchange rounds done so far (host side; the tag of a round derives from it)
+    bool resident_ran = false;       // a resident launch has been enqueued since the error word was last cleared
     size_t field_doubles = 0;
     long long step = 0;
     long long launches = 0;
@@ -89,8 +93,29 @@ cavk::Params make_params(int N, double Re, double dt, double beta) {
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-#define CK(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { cudaGetLastError(); return CAV_ECUDA; } } while (0)
-#define LAUNCH(expr) do { int n_ = (expr); if (n_ < 0) { cudaGetLastError(); return CAV_ECUDA; } nl += n_; } while (0)
+// CAV_DEBUG=1 in the environment: the CUDA error behind a CAV_ECUDA goes to stderr
+inline void debug_cuda(const char* what, int code, int line) {
+    static const bool on = std::getenv("CAV_DEBUG") != nullptr;
+    if (on) std::fprintf(stderr, "[cavity] line %d: %s -> %s\n", line, what, cudaGetErrorString((cudaError_t)code));
+}
+#define CK(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { debug_cuda(#expr, (int)e_, __LINE__); cudaGetLastError(); return CAV_ECUDA; } } while (0)
+#define LAUNCH(expr) do { int n_ = (expr); if (n_ < 0) { debug_cuda(#expr, -n_, __LINE__); cudaGetLastError(); return CAV_ECUDA; } nl += n_; } while (0)
+
+void* dev_alloc(cav_ctx* c, size_t bytes) {
+    try { return c10::cuda::CUDACachingAllocator::raw_alloc_with_stream(bytes, c->st); } catch (...) { cudaGetLastError(); return nullptr; }
+}
+void dev_free(void*& p) {
+    if (p) { try { c10::cuda::CUDACachingAllocator::raw_delete(p); } catch (...) {} p = nullptr; }
+}
+
+// q: only the stream engine and the Jacobi / compact sweeps need the scaled right-hand side as a field
+int need_q(cav_ctx* c) {
+    if (c->q) return CAV_OK;
+    c->q = (double*)dev_alloc(c, c->field_doubles * sizeof(double));
+    if (!c->q) return CAV_ENOMEM;
+    if (cudaMemsetAsync(c->q, 0, c->field_doubles * sizeof(double), c->st) != cudaSuccess) { cudaGetLastError(); return CAV_ECUDA; }
+    return CAV_OK;
+}
 
 void drop_graph(cav_ctx* c) {
     if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }
@@ -98,16 +123,31 @@ void drop_graph(cav_ctx* c) {
     c->graph_launches = 0;
 }
 
-// (re)builds the exchange tables of c->plan; on failure the plan is marked unusable
+// (re)builds the exchange tables and (re)allocates / clears the exchange buffers of c->plan; on failure the plan is marked
+// unusable.  Cleared buffers carry tag 0 = never valid, so units of another plan can never be taken for this one's.
 void build_plan_tables(cav_ctx* c) {
-    if (c->tables) { try { c10::cuda::CUDACachingAllocator::raw_delete(c->tables); } catch (...) {} c->tables = nullptr; }
+    dev_free(c->tables);
     const size_t nb = cavk::resident_table_bytes(c->plan);
-    if (!c->plan.ok || nb == 0) return;
-    try { c->tables = c10::cuda::CUDACachingAllocator::raw_alloc_with_stream(nb, c->st); } catch (...) { c->tables = nullptr; }
-    if (!c->tables) { c->plan.ok = false; return; }
+    if (!c->plan.ok || nb == 0) { dev_free(c->xbuf); c->xa = c->xb = nullptr; return; }
+    const size_t xbytes = (cavk::resident_exchange_bytes(c->N) + 255) / 256 * 256;
+    if (!c->xbuf) c->xbuf = dev_alloc(c, 2 * xbytes);
+    c->tables = dev_alloc(c, nb);
+    if (!c->tables || !c->xbuf) { c->plan.ok = false; return; }
+    c->xa = c->xbuf;
+    c->xb = (char*)c->xbuf + xbytes;
+    if (cudaMemsetAsync(c->xbuf, 0, 2 * xbytes, c->st) != cudaSuccess) { cudaGetLastError(); c->plan.ok = false; return; }
     const int nl = cavk::resident_build_tables(c->P, c->plan, c->tables, c->st);
     if (nl < 0 || cudaStreamSynchronize(c->st) != cudaSuccess) { cudaGetLastError(); c->plan.ok = false; return; }
     c->launches += nl;
+}
+
+// The resident engine's tiles give up (and say so) instead of spinning forever on a neighbour that never arrives.  The word
+// is cleared whenever the state or the engine is set anew (cav_set_fields, cav_set_engine, cav_set_resident_plan).
+int clear_resident_error(cav_ctx* c) {
+    c->resident_ran = false;
+    if (!c->err_word) return CAV_OK;
+    if (cudaMemsetAsync(c->err_word, 0, sizeof(unsigned int), c->st) != cudaSuccess) { cudaGetLastError(); return CAV_ECUDA; }
+    return CAV_OK;
 }
 
 void resolve_engine(cav_ctx* c) {
@@ -116,28 +156,31 @@ void resolve_engine(cav_ctx* c) {
     if (e != c->engine) { c->engine = e; drop_graph(c); }
 }
 
-// a1: nsweeps red-black sweeps on psi with right-hand side w_in
+inline bool resident_path(const cav_ctx* c) { return c->engine == CAV_ENGINE_RESIDENT && c->sweep == CAV_SWEEP_REDBLACK; }
+
+// one launch of the resident kernel: nsteps whole time steps, or (nsteps = 0) S sweeps of a1 with right-hand side omega^n
+int enqueue_resident(cav_ctx* c, int nsteps, int S, long long& nl, long long* trace_dev = nullptr, int trace_cap = 0) {
+    if (nsteps == 0 && S <= 0) return CAV_OK;
+    LAUNCH(cavk::resident_launch(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, c->tables, c->w[0], c->field_doubles, c->err_word,
+                                 &c->epoch, nsteps, S, c->st, trace_dev, trace_cap));
+    std::swap(c->psi, c->psi2);
+    c->resident_ran = true;
+    drop_graph(c);                 // a captured step of another path holds the old psi / psi2
+    return CAV_OK;
+}
+
+// a1: nsweeps sweeps on psi with right-hand side w_in (every path but the resident kernel's whole steps)
 int enqueue_sweeps(cav_ctx* c, const double* w_in, int nsweeps, long long& nl) {
     if (nsweeps <= 0) return CAV_OK;
+    if (resident_path(c) && w_in == c->w[0]) return enqueue_resident(c, 0, nsweeps, nl);
+    int rc = need_q(c);
+    if (rc != CAV_OK) return rc;
     if (c->sweep == CAV_SWEEP_COMPACT9) {
         LAUNCH(cavk::compact_rhs(c->P, w_in, c->q, c->st));
         LAUNCH(cavk::compact_sweeps(c->P, c->psi, c->q, nsweeps, c->st));
     } else if (c->sweep == CAV_SWEEP_JACOBI) {
         LAUNCH(cavk::scale_rhs(c->P, w_in, c->q, c->st));
         LAUNCH(cavk::jacobi_sweeps(c->P, c->psi, c->psi2, c->q, nsweeps, c->st));
-    } else if (c->engine == CAV_ENGINE_RESIDENT) {
-        if (c->epoch > 0xF0000000u) {
-            // Tags are 32-bit and must never repeat while an older unit with the same tag can still sit in an exchange
-            // buffer: long before the epoch wraps, clear the buffers (tag 0 = never valid) and start over.
-            const size_t xb_bytes = cavk::resident_exchange_doubles(c->field_doubles) * sizeof(double);
-            if (cudaMemsetAsync(c->xa, 0, xb_bytes, c->st) != cudaSuccess || cudaMemsetAsync(c->xb, 0, xb_bytes, c->st) != cudaSuccess) {
-                cudaGetLastError();
-                return CAV_ECUDA;
-            }
-            c->epoch = 0;
-        }
-        LAUNCH(cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, c->tables, w_in, c->err_word, &c->epoch, nsweeps, c->st));
-        std::swap(c->psi, c->psi2);
     } else {
         LAUNCH(cavk::scale_rhs(c->P, w_in, c->q, c->st));
         LAUNCH(cavk::stream_sweeps(c->P, c->psi, c->q, nsweeps, c->st));
@@ -145,16 +188,20 @@ int enqueue_sweeps(cav_ctx* c, const double* w_in, int nsweeps, long long& nl) {
     return CAV_OK;
 }
 
-// the resident engine's tiles give up (and say so) instead of spinning forever on a neighbour that never arrives
 int check_resident_error(cav_ctx* c) {
-    if (!c->plan.ok || !c->err_word) return CAV_OK;
-    unsigned int e = 0;
-    if (cudaMemcpyAsync(&e, c->err_word, sizeof e, cudaMemcpyDeviceToHost, c->st) != cudaSuccess ||
-        cudaStreamSynchronize(c->st) != cudaSuccess) { cudaGetLastError(); return CAV_ECUDA; }
-    return e ? CAV_ECUDA : CAV_OK;
+    if (!c->resident_ran || !c->err_word) return CAV_OK;
+    unsigned int e[10] = {0};
+    cudaError_t ce = cudaMemcpyAsync(e, c->err_word, sizeof e, cudaMemcpyDeviceToHost, c->st);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(c->st);
+    if (ce != cudaSuccess) { debug_cuda("resident launch", (int)ce, __LINE__); cudaGetLastError(); return CAV_ECUDA; }
+    if (e[0] && std::getenv("CAV_DEBUG"))
+        std::fprintf(stderr, "[cavity] tile %u thread %u gave up on unit %u (row %u, group %u) in round %u: tag wanted %u, found %u %u %u %u\n",
+                     e[1], e[9], e[2], e[2] / (unsigned)cavk::resident_unit_pitch(c->N), e[2] % (unsigned)cavk::resident_unit_pitch(c->N),
+                     e[3], e[4], e[5], e[6], e[7], e[8]);
+    return e[0] ? CAV_ECUDA : CAV_OK;
 }
 
-// one SSPRK(5,4) step: 5 x [a1 x S, a2 + a3]
+// one SSPRK(5,4) step, stage by stage: 5 x [a1 x S, a2 + a3] (stream engine, Jacobi and compact sweeps)
 int enqueue_step(cav_ctx* c, long long& nl) {
     double* const* w = c->w;
     const double* win[5] = {w[0], w[1], w[2], w[3], w[4]};
@@ -173,7 +220,7 @@ int enqueue_step(cav_ctx* c, long long& nl) {
 void try_build_graph(cav_ctx* c) {
     if (c->graph_tried) return;
     c->graph_tried = true;
-    if (c->engine == CAV_ENGINE_RESIDENT && c->sweep == CAV_SWEEP_REDBLACK) return;     // 10 launches per step: a graph buys nothing
+    if (resident_path(c)) return;     // whole time steps in one launch
     cudaGraph_t g = nullptr;
     if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return; }
     long long nl = 0;
@@ -191,8 +238,18 @@ int step_impl(cav_ctx* c, int nsteps, bool sync) {
     DeviceGuard dg(c->device);
     if (nsteps == 0) return CAV_OK;
     resolve_engine(c);
+    if (!resident_path(c)) {           // allocated here, never inside a stream capture
+        const int rc = need_q(c);
+        if (rc != CAV_OK) return rc;
+    }
     try_build_graph(c);
     CK(cudaEventRecord(c->ev0, c->st));
+    if (resident_path(c)) {
+        long long nl = 0;
+        int rc = enqueue_resident(c, nsteps, c->S, nl);
+        c->launches += nl;
+        if (rc != CAV_OK) return rc;
+    } else
     for (int n = 0; n < nsteps; ++n) {
         if (c->graph) {
             CK(cudaGraphLaunch(c->graph, c->st));
@@ -209,7 +266,7 @@ int step_impl(cav_ctx* c, int nsteps, bool sync) {
     c->step += nsteps;
     if (sync) {
         CK(cudaStreamSynchronize(c->st));
-        if (c->engine == CAV_ENGINE_RESIDENT) return check_resident_error(c);
+        return check_resident_error(c);
     }
     return CAV_OK;
 }
@@ -236,24 +293,18 @@ CAV_API int cav_create(cav_ctx** out, int N, double Re, double dt, double sor_om
 
         const size_t fd = align_up((size_t)c->P.pitch * (size_t)(N + 1), 32);   // doubles per field, 256 B multiple
         c->field_doubles = fd;
-        const size_t xd = cavk::resident_exchange_doubles(fd);
-        const size_t nfields = 11;   // psi, psi2, q, w0..w4, T, psi_prev, w_prev  (+ the two exchange buffers)
+        const size_t nfields = 8;    // psi, psi2, w0..w4, T; q, the monitors' snapshots and the exchange buffers come when needed
         const size_t scratch_d = align_up(4 * (size_t)cavk::diag_scratch_doubles(), 32);
         const size_t flags_b = 256;
-        const size_t bytes = (nfields * fd + 2 * xd + scratch_d + 32) * sizeof(double) + flags_b;
+        const size_t bytes = (nfields * fd + scratch_d + 32) * sizeof(double) + flags_b;
         c->slab = c10::cuda::CUDACachingAllocator::raw_alloc_with_stream(bytes, c->st);
         if (!c->slab) throw (int)CAV_ENOMEM;
         if (cudaMemsetAsync(c->slab, 0, bytes, c->st) != cudaSuccess) throw (int)CAV_ECUDA;
         double* p = (double*)c->slab;
         c->psi = p; p += fd;
         c->psi2 = p; p += fd;
-        c->xa = p; p += xd;
-        c->xb = p; p += xd;
-        c->q = p; p += fd;
-        for (int k = 0; k < 5; ++k) { c->w[k] = p; p += fd; }
+        for (int k = 0; k < 5; ++k) { c->w[k] = p; p += fd; }      // the resident kernel addresses them as w[0] + k fd
         c->T = p; p += fd;
-        c->psi_prev = p; p += fd;
-        c->w_prev = p; p += fd;
         c->scratch = p; p += scratch_d;
         c->out4 = p; p += 32;
         c->err_word = (unsigned int*)p;
@@ -287,9 +338,10 @@ CAV_API void cav_destroy(cav_ctx* c) {
         if (c->slab) {
             try { c10::cuda::CUDACachingAllocator::raw_delete(c->slab); } catch (...) {}
         }
-        if (c->tables) {
-            try { c10::cuda::CUDACachingAllocator::raw_delete(c->tables); } catch (...) {}
-        }
+        dev_free(c->tables);
+        dev_free(c->xbuf);
+        void* qv = c->q; dev_free(qv); c->q = nullptr;
+        void* pv = c->prev; dev_free(pv); c->prev = nullptr;
         cudaGetLastError();
     }
     delete c;
@@ -307,6 +359,8 @@ CAV_API int cav_set_fields(cav_ctx* c, const double* psi, const double* omega) {
     CK(cudaMemcpy2DAsync(c->w[0], dp, omega, row, row, N + 1, cudaMemcpyHostToDevice, c->st));
     c->launches += nl;
     c->step = 0;
+    int rc = clear_resident_error(c);
+    if (rc != CAV_OK) return rc;
     CK(cudaStreamSynchronize(c->st));
     return CAV_OK;
 }
@@ -351,8 +405,7 @@ CAV_API int cav_poisson(cav_ctx* c, int nsweeps, double* res_inf_out) {
     c->launches += nl;
     CK(cudaStreamSynchronize(c->st));
     if (res_inf_out) *res_inf_out = r;
-    if (c->engine == CAV_ENGINE_RESIDENT) return check_resident_error(c);
-    return CAV_OK;
+    return check_resident_error(c);
 }
 
 CAV_API int cav_get_diag(cav_ctx* c, cav_diag* out) {
@@ -382,6 +435,12 @@ CAV_API int cav_step_res(cav_ctx* c, double* res_psi_out, double* res_omega_out)
     if (!c) return CAV_EINVAL;
     DeviceGuard dg(c->device);
     const size_t nb = c->field_doubles * sizeof(double);
+    if (!c->prev) {
+        c->prev = (double*)dev_alloc(c, 2 * nb);
+        if (!c->prev) return CAV_ENOMEM;
+        c->psi_prev = c->prev;
+        c->w_prev = c->prev + c->field_doubles;
+    }
     CK(cudaMemcpyAsync(c->psi_prev, c->psi, nb, cudaMemcpyDeviceToDevice, c->st));
     CK(cudaMemcpyAsync(c->w_prev, c->w[0], nb, cudaMemcpyDeviceToDevice, c->st));
     int rc = step_impl(c, 1, false);
@@ -394,8 +453,7 @@ CAV_API int cav_step_res(cav_ctx* c, double* res_psi_out, double* res_omega_out)
     CK(cudaStreamSynchronize(c->st));
     if (res_psi_out) *res_psi_out = r[0];
     if (res_omega_out) *res_omega_out = r[1];
-    if (c->engine == CAV_ENGINE_RESIDENT) return check_resident_error(c);
-    return CAV_OK;
+    return check_resident_error(c);
 }
 
 CAV_API int cav_run_to_steady(cav_ctx* c, int max_steps, int check_every, double tol_psi, double tol_omega, cav_monitor* out) {
@@ -418,8 +476,7 @@ CAV_API int cav_run_to_steady(cav_ctx* c, int max_steps, int check_every, double
     out->steps = n;
     DeviceGuard dg(c->device);
     CK(cudaStreamSynchronize(c->st));
-    if (c->engine == CAV_ENGINE_RESIDENT) return check_resident_error(c);
-    return CAV_OK;
+    return check_resident_error(c);
 }
 
 CAV_API int cav_set_engine(cav_ctx* c, int engine) {
@@ -429,7 +486,7 @@ CAV_API int cav_set_engine(cav_ctx* c, int engine) {
     CK(cudaStreamSynchronize(c->st));
     c->engine_req = engine;
     resolve_engine(c);
-    return CAV_OK;
+    return clear_resident_error(c);
 }
 
 CAV_API int cav_set_resident_plan(cav_ctx* c, int sweeps_per_exchange, int variant) {
@@ -442,29 +499,28 @@ CAV_API int cav_set_resident_plan(cav_ctx* c, int sweeps_per_exchange, int varia
     c->plan = pl;
     build_plan_tables(c);
     if (!c->plan.ok) { c->plan = old; build_plan_tables(c); resolve_engine(c); return CAV_ENOMEM; }
-    return CAV_OK;
+    return clear_resident_error(c);
 }
 
 CAV_API int cav_trace_sweeps(cav_ctx* c, int nsweeps, long long* stamps_out, int slots_per_tile, int* ntiles_out) {
     if (!c || nsweeps < 1 || !stamps_out || slots_per_tile < 2) return CAV_EINVAL;
     DeviceGuard dg(c->device);
     resolve_engine(c);
-    if (c->engine != CAV_ENGINE_RESIDENT) return CAV_ENOTSUP;
+    if (!resident_path(c)) return CAV_ENOTSUP;          // the red-black sweeps of the resident engine only
     const size_t n = (size_t)c->plan.ntiles * (size_t)slots_per_tile;
-    long long* dev = nullptr;
-    try { dev = (long long*)c10::cuda::CUDACachingAllocator::raw_alloc_with_stream(n * sizeof(long long), c->st); }
-    catch (...) { return CAV_ENOMEM; }
+    long long* dev = (long long*)dev_alloc(c, n * sizeof(long long));
+    if (!dev) return CAV_ENOMEM;
     int rc = CAV_OK;
     if (cudaMemsetAsync(dev, 0, n * sizeof(long long), c->st) != cudaSuccess) rc = CAV_ECUDA;
     if (rc == CAV_OK) {
-        int nl = cavk::resident_sweeps(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, c->tables, c->w[0], c->err_word, &c->epoch, nsweeps,
-                                       c->st, dev, slots_per_tile);
-        if (nl < 0) rc = CAV_ECUDA; else { c->launches += nl; std::swap(c->psi, c->psi2); }
+        long long nl = 0;
+        rc = enqueue_resident(c, 0, nsweeps, nl, dev, slots_per_tile);
+        c->launches += nl;
     }
     if (rc == CAV_OK && (cudaMemcpyAsync(stamps_out, dev, n * sizeof(long long), cudaMemcpyDeviceToHost, c->st) != cudaSuccess ||
                          cudaStreamSynchronize(c->st) != cudaSuccess)) rc = CAV_ECUDA;
     if (rc != CAV_OK) cudaGetLastError();
-    try { c10::cuda::CUDACachingAllocator::raw_delete(dev); } catch (...) {}
+    void* dv = dev; dev_free(dv);
     if (ntiles_out) *ntiles_out = c->plan.ntiles;
     return rc == CAV_OK ? check_resident_error(c) : rc;
 }
@@ -473,6 +529,8 @@ CAV_API int cav_debug_set_epoch(cav_ctx* c, unsigned int epoch) {
     if (!c) return CAV_EINVAL;
     DeviceGuard dg(c->device);
     CK(cudaStreamSynchronize(c->st));
+    // a jump of the round counter breaks the "this round or the one two before" invariant of the tags: start from cleared buffers
+    if (c->xbuf) CK(cudaMemsetAsync(c->xbuf, 0, 2 * ((cavk::resident_exchange_bytes(c->N) + 255) / 256 * 256), c->st));
     c->epoch = epoch;
     return CAV_OK;
 }

@@ -1,39 +1,53 @@
-// cavity_resident.cu — the resident sweep engine (a1) for sm_100a.  DESIGN.md section 6.
+// cavity_resident.cu — the resident engine for sm_100a: ONE persistent cooperative kernel runs whole SSPRK(5,4) time
+// steps (a1 + a2 + a3 of every stage, any number of steps per launch), or a1 sweeps alone (cav_poisson).  DESIGN.md section 6.
 //
-// What it computes is exactly S red-black SOR sweeps of the 5-point Poisson problem (eq 15-21 P:114-138 reduced,
+// What it computes.  a1: S red-black SOR sweeps of the 5-point Poisson problem per stage (eq 15-21 P:114-138 reduced,
 // DESIGN.md D1-D3), red = (i + j) even first (G9), with the arithmetic of DESIGN.md "Canonical arithmetic":
 //     nb = (psi_W + psi_E) + (psi_S + psi_N);   psi <- fma(1 - beta, psi, fma(beta / 4, nb, q)),   q = ((beta / 4) h^2) w
-// Inside one colour every update reads only the other colour, so the schedule below cannot change a bit of
-// the result; the tests compare with the FMA-mode oracle bit for bit.
+// a2 + a3 (eq 25, eq 8, eq 22, eq 9-13): exactly the expressions of k_rk_stage in
+// cavity_kernels.cu.  Inside one colour every update reads only the other colour and a3 is pointwise in its output, so the
+// schedule below cannot change a bit of the result; the tests compare with the FMA-mode oracle bit for bit.
 //
 // Schedule.  The (N+1)^2 grid is cut into ntx x nty tiles; tile (bi, bj) OWNS the core [bi CW, (bi+1) CW) x
-// [bj CH, (bj+1) CH) and additionally carries a halo of `halo` = 2T points on every side.  One CTA per tile,
-// all CTAs co-resident (cooperative launch).  A thread owns a C x R micro-tile (C consecutive x, R rows) of
-// psi AND q in registers for the whole call; a warp spans 32 C points of R rows.  Threads exchange only the
-// perimeter of their micro-tile: left / right columns by warp shuffle, bottom / top rows through shared memory
-// (edge arrays laid out so that every access is unit-stride over the lanes), one __syncthreads per colour half-sweep.
+// [bj CH, (bj+1) CH) and additionally carries a halo of `halo` = 2T points on every side.  One CTA per tile, all CTAs
+// co-resident (cooperative launch).  A thread owns a C x R micro-tile (C consecutive x, R rows) of psi AND q in
+// registers for the whole launch; a warp spans 32 C points of R rows.  Threads exchange only the perimeter of their
+// micro-tile: left / right columns by warp shuffle, bottom / top rows through shared memory (edge arrays laid out so
+// that every access is unit-stride over the lanes), one __syncthreads per colour half-sweep.
 //
 // Walls cost nothing inside the sweeps.  The origin of an edge tile is shifted so that the wall column x = 0 is the LAST
 // column of a lane (x = N: the FIRST column of a lane) and the wall row y = 0 the LAST row of a warp (y = N: the FIRST row
 // of a warp).  Such a lane / warp owns no interior point; what it computes is never used: the adjacent lane substitutes
 // 0 for what the shuffle brings (the select that the tile edge needs anyway), and the warp never publishes that edge row,
 // so the shared-memory slot keeps the +0.0 it was initialised with (eq 23-24: psi = 0 on the walls).  A tile
-// whose origin parity is odd sweeps its local colour 1 first.  Walls that cannot be aligned (both walls of one direction in
-// the same tile: small grids) fall back to a bit mask of points that are put back to +0.0 after every half-sweep.
+// whose origin parity is odd sweeps its local colour 1 first.  Walls that cannot be aligned (both walls of one direction in the same
+// tile: small grids) fall back to a bit mask of points that are put back to +0.0 after every half-sweep (FIX variant).
 //
-// Every T sweeps (2T half-sweeps, each of which invalidates one more ring of the halo) the CTAs refresh their
-// halos through L2 WITHOUT any fence, flag or barrier between CTAs: the validity tag travels inside the data.
-// A point is exchanged as one 16-byte unit {lo32(psi), tag, hi32(psi), tag} written by one st.v4.b32; each 8-byte half is
-// a single-copy-atomic access carrying its own tag, so a reader that finds both tags equal to the tag of the round it waits
-// for holds the two halves of that round's value, however the stores of the sender were ordered or torn.  Tags are unique
-// per round and per launch (a host-side epoch).  Two exchange buffers alternate by round parity: a tile can write round
-// r + 1 only after it has received round r from every neighbour, and a neighbour posts round r only after it has consumed
-// round r - 1, so the buffer a tile overwrites is never still being read.
-// The exchange is cooperative and coalesced: owners put the border-strip values into a shared-memory staging array, then
-// ALL threads of the CTA store the strip units (consecutive threads = consecutive x) and fetch the ring units the same
-// way (a few units per thread, all in flight together; a unit that does not carry the tag yet is polled), and the owners
-// pick the ring values up from the staging array.  Which unit a thread moves is precomputed once per launch into
-// shared-memory tables.
+// Halo exchange: every T sweeps (2T half-sweeps, each of which invalidates one more ring of the halo), after the last
+// sweep of a stage, and once per stage for the new vorticity, the CTAs refresh their halos through L2 WITHOUT any fence,
+// flag or barrier between CTAs: the validity tag travels inside the data.  Three consecutive points of a row (x = 3g,
+// 3g + 1, 3g + 2: core widths are multiples of 3, so a group has one owner) travel as one 32-byte unit of four 64-bit
+// words, each word = 48 payload bits | 16-bit tag, written by two st.relaxed.gpu.v2.b64 and read by two
+// ld.relaxed.gpu.v2.b64.  The PTX memory model treats a vector access as a set of scalar accesses of the element
+// type in unspecified order; every 64-bit element is single-copy atomic and carries its own tag, so a reader that finds the
+// tag of the round it waits for in all four words holds that round's three values, however the four were ordered or
+// torn.  At a given location a reader can only ever find the round it waits for or the one two rounds earlier (two buffers
+// alternate by round parity: a tile writes round r + 1 only after it has received round r from every neighbour, and a
+// neighbour posts round r only after it has consumed round r - 1), so 16-bit tags 1 + r mod 65535 never alias; 0 = never
+// valid (freshly cleared buffers).  The exchange is cooperative and coalesced: every thread copies its micro-tile into a
+// shared-memory image of the tile (row-major), then ALL threads of the CTA store the strip units (consecutive threads =
+// consecutive units) and fetch the ring units the same way (a unit that does not carry the tag yet is polled by one lane
+// of the warp), unpack them into the image, and every thread reads its micro-tile back.  Which unit a thread moves is
+// precomputed once per plan (k_build_tables) and copied to shared memory at launch.
+//
+// a2 + a3 in the tile.  After the last sweep of a stage and one more psi exchange the tile holds psi on core + halo; the
+// stage input vorticity of the core is re-read from the tile's own global buffer into the shared-memory image, its first
+// ring comes from a small shared-memory copy kept since the vorticity exchange of the previous stage, the wall values next
+// to the core are Thom's formula applied to the adjacent psi (which also goes to the ring of the stage output in global
+// memory, G16).  Each thread evaluates eq 8 / 22 and the stage combination for its core points, stores them to the global
+// stage buffer (pointwise operands of later stages are read back from there by the same tile), the new vorticity is then
+// exchanged like psi and scaled into q for the next stage's sweeps.
+//
 // The kernel reads psi_in and writes psi_out (the API ping-pongs two fields), so no tile ever overwrites input a
 // neighbour has not loaded yet.
 #include "cavity_resident.cuh"
@@ -45,28 +59,47 @@ namespace cavk {
 
 namespace {
 
-constexpr long long SPIN_TIMEOUT_CYCLES = 4000000000LL;   // ~2 s: a neighbour whose data never arrives is a bug, not a wait
+#ifndef CAV_SPIN_TIMEOUT
+#define CAV_SPIN_TIMEOUT 20000000000LL      // ~10 s at 2 GHz: a neighbour whose data never arrives is a bug, not a wait
+#endif
+constexpr long long SPIN_TIMEOUT_CYCLES = CAV_SPIN_TIMEOUT;
 constexpr unsigned int NO_UNIT = 0xffffffffu;
 #ifndef CAV_QROWS
 #define CAV_QROWS 2             // rows of the micro-tile whose q lives in shared memory instead of registers
 #endif
 #ifndef CAV_RECV_BATCH
-#define CAV_RECV_BATCH 2        // ring units a thread keeps in flight at a time (4 registers each; more than 2 makes ptxas spill around the exchange, which costs more than the extra L2 round trips: profiles/)
+#define CAV_RECV_BATCH 1        // ring units (32 bytes, 8 registers each) a thread keeps in flight at a time.  One is enough: 512 threads x 32 B
+                                // in flight per SM already exceed the SM's share of L2 bandwidth x latency; with more, the caller of
+                                // exchange_units keeps q in local memory across the sweeps (ptxas: registers saved around the call)
 #endif
+
+// SSPRK(5,4) in Shu-Osher form, eq 9-13, readings G1 / G2 (the same table as cavity_kernels.cu, typed here again
+// because that one is file-local).
+__device__ constexpr double RK1_C  = 0.391752226571890;
+__device__ constexpr double RK2_A0 = 0.444370493651235, RK2_A1 = 0.555629506348765, RK2_C = 0.368410593050371;
+__device__ constexpr double RK3_A0 = 0.620101851488403, RK3_A2 = 0.379898148511597, RK3_C = 0.251891774271694;
+__device__ constexpr double RK4_A0 = 0.178079954393132, RK4_A3 = 0.821920045606868, RK4_C = 0.544974750228521;
+__device__ constexpr double RK5_A2 = 0.517231671970585, RK5_A3 = 0.096059710526147, RK5_C3 = 0.063692468666290;
+__device__ constexpr double RK5_A4 = 0.386708617503269, RK5_C4 = 0.226007483236906;
 
 struct ResArgs {
     int N, pitch;
-    double cb, omb, cq;
-    const double* w;        // stage input vorticity; q = cq * w on interior points
-    const double* psi_in;   // stream function before the sweeps
+    double cb, omb, cq;                 // a1
+    double i2h, ih2, nu, c2h2, lid, dt; // a2, a3
+    const double* psi_in;   // stream function before the launch
     double* psi_out;        // ... and after (a different field)
-    uint4* x0;              // exchange buffer of even rounds: one 16-byte unit per grid point, same (pitch) indexing as a field
-    uint4* x1;              // exchange buffer of odd rounds
+    double* wbase;          // omega^n, omega^(1..4), T: six fields, `fstride` doubles apart; sweeps-only launches read field 0
+    size_t fstride;
+    ulonglong4* x0;         // exchange buffer of even rounds: one 32-byte unit per group of 3 points, upitch units per grid row
+    ulonglong4* x1;         // exchange buffer of odd rounds
+    int upitch;
     unsigned int* err;      // error word: set if a tile gave up waiting for a neighbour
-    unsigned int base;      // tag epoch of this launch: round r is tagged base + 1 + r
-    int nsweeps, T, halo, CW, CH, ntx, nty;
+    unsigned int base;      // exchange rounds done by earlier launches (tag of round r: 1 + r mod 65535; buffer: r & 1)
+    int nsteps;             // > 0: that many whole time steps (a1 + a2 + a3, five stages each); 0: S sweeps of a1 only
+    int S;                  // sweeps per stage (nsteps > 0) or in total (nsteps == 0)
+    int T, halo, CW, CH, ntx, nty;
     int ns_per, nr_per;     // table entries per thread: strip units to store / ring units to fetch
-    const uint4* tables;    // per-plan exchange tables, one block per tile (k_build_tables)
+    const uint2* tables;    // per-plan exchange tables, one block per tile (k_build_tables)
     long long* trace;       // profiling only (cav_trace_sweeps): per tile, %globaltimer at the phase boundaries; else null
     int trace_cap;          // slots per tile
 };
@@ -102,18 +135,37 @@ __host__ __device__ inline TileGeom tile_geom(int N, int CW, int CH, int halo, i
     return g;
 }
 
-// One exchanged point: {lo32, tag, hi32, tag}.  Each aligned 8-byte half is single-copy atomic and self-validating.
-__device__ __forceinline__ void st_unit(uint4* p, double v, unsigned int tag) {
-    const unsigned int lo = (unsigned int)__double2loint(v), hi = (unsigned int)__double2hiint(v);
-    asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(lo), "r"(tag), "r"(hi), "r"(tag) : "memory");
+// ---- one exchanged unit: three doubles in four 64-bit words, each word = 48 payload bits | tag << 48 ----------------
+__device__ __forceinline__ void st_unit(ulonglong4* p, double d0, double d1, double d2, unsigned int tag) {
+    const unsigned long long a = (unsigned long long)__double_as_longlong(d0), b = (unsigned long long)__double_as_longlong(d1),
+                             c = (unsigned long long)__double_as_longlong(d2), t = (unsigned long long)tag << 48;
+    const unsigned long long M48 = 0x0000ffffffffffffull;
+    const unsigned long long w0 = (a & M48) | t;
+    const unsigned long long w1 = (a >> 48) | ((b << 16) & M48) | t;
+    const unsigned long long w2 = (b >> 32) | ((c << 32) & M48) | t;
+    const unsigned long long w3 = (c >> 16) | t;
+    // two 16-byte accesses: on this silicon (B200, driver 580) the 32-byte form st / ld.relaxed.gpu.v4.b64 was observed to
+    // deliver only the first word of a unit (profiles/r2_notes.md); the tags make the split harmless
+    asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"(w0), "l"(w1) : "memory");
+    asm volatile("st.relaxed.gpu.global.v2.b64 [%0+16], {%1, %2};" ::"l"(p), "l"(w2), "l"(w3) : "memory");
 }
-__device__ __forceinline__ uint4 ld_unit(const uint4* p) {
-    uint4 v;
-    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+__device__ __forceinline__ ulonglong4 ld_unit(const ulonglong4* p) {
+    ulonglong4 v;
+    asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "l"(p) : "memory");
+    asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2+16];" : "=l"(v.z), "=l"(v.w) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ bool unit_ok(const uint4& v, unsigned int tag) { return v.y == tag && v.w == tag; }
-__device__ __forceinline__ double unit_value(const uint4& v) { return __hiloint2double((int)v.z, (int)v.x); }
+__device__ __forceinline__ bool unit_ok(const ulonglong4& v, unsigned int tag) {
+    return (unsigned int)(v.x >> 48) == tag && (unsigned int)(v.y >> 48) == tag && (unsigned int)(v.z >> 48) == tag &&
+           (unsigned int)(v.w >> 48) == tag;
+}
+__device__ __forceinline__ void unit_values(const ulonglong4& v, double& d0, double& d1, double& d2) {
+    const unsigned long long M48 = 0x0000ffffffffffffull;
+    d0 = __longlong_as_double((long long)((v.x & M48) | (v.y << 48)));
+    d1 = __longlong_as_double((long long)(((v.y >> 16) & 0xffffffffull) | (v.z << 32)));
+    d2 = __longlong_as_double((long long)(((v.z >> 32) & 0xffffull) | (v.w << 16)));
+}
+__host__ __device__ inline unsigned int round_tag(unsigned int round) { return 1u + round % 65535u; }
 
 __device__ __forceinline__ long long globaltimer_ns() {
     unsigned long long t;
@@ -132,11 +184,12 @@ __device__ __forceinline__ int opaque_zero() {
     return z;
 }
 
-// Per-thread flags of the sweep (one register): what the lane / warp must NOT take from / give to its neighbours.
+// Per-thread flags of the sweep (one register).
 constexpr unsigned int FL_ZERO_LEFT = 1u;     // the left neighbour column is a wall or the tile edge: use 0
 constexpr unsigned int FL_ZERO_RIGHT = 2u;    // same on the right
 constexpr unsigned int FL_PUB_BOTTOM = 4u;    // publish the bottom row of the micro-tile to the warp below
 constexpr unsigned int FL_PUB_TOP = 8u;       // publish the top row to the warp above
+constexpr unsigned int FL_ODD = 16u;          // the tile origin has odd parity: local colour = global colour ^ 1
 
 // One colour half-sweep on the register micro-tile.  K = LOCAL colour being updated: local point (ci, rj) has local colour
 // (ci + rj) & 1 (C, R even); the kernel maps the global colour to the local one through the parity of the tile origin.
@@ -146,7 +199,9 @@ constexpr unsigned int FL_PUB_TOP = 8u;       // publish the top row to the warp
 // +0.0 after the update (eq 23-24).
 template <int C, int R, int K, bool FIX, int TOPOFF>
 __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[R][C], const double cb, const double omb,
-                                           double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl) {
+                                           double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl_) {
+    unsigned int fl = fl_;
+    asm volatile("" : "+r"(fl));               // opaque: the bit tests below are redone here, not hoisted into registers of their own
     // sB / sT point at [warp][0][lane] of the bottom / top edge arrays (stride 32 per ci, C * 32 per warp);
     // the top array starts TOPOFF doubles after the bottom one (a compile-time distance: one address register)
     // q of the two middle rows of the micro-tile lives in shared memory, in two more arrays of the same shape 2 TOPOFF and
@@ -226,176 +281,401 @@ __device__ __forceinline__ void publish_all(const double (&p)[R][C], double* __r
     __syncthreads();
 }
 
-// ---- the points a tile sends (border strips of its core) and receives (its ring): four disjoint rectangles each ----
-struct Rect { int x0, x1, y0, y1; };                     // [x0, x1) x [y0, y1)
-struct Region { Rect r[4]; };
+// ---- the units a tile sends (border strips of its core) and receives (its ring): four disjoint rectangles each -------
+// A unit is the group g of a grid row y: the points x = 3g, 3g + 1, 3g + 2.  Core widths are multiples of 3 whenever a tile
+// has a neighbour in x, so every group lies in exactly one core.
+struct URect { int g0, g1, y0, y1; };                    // groups [g0, g1) x rows [y0, y1)
+struct URegion { URect r[4]; };
 __host__ __device__ inline int imax(int a, int b) { return a > b ? a : b; }
 __host__ __device__ inline int imin(int a, int b) { return a < b ? a : b; }
-__host__ __device__ inline int rect_count(const Rect& r) {
-    const int w = r.x1 - r.x0, h = r.y1 - r.y0;
+__host__ __device__ inline int urect_count(const URect& r) {
+    const int w = r.g1 - r.g0, h = r.y1 - r.y0;
     return (w > 0 && h > 0) ? w * h : 0;
 }
-__device__ __forceinline__ bool region_has(const Region& g, int x, int y) {
-    bool in = false;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) in = in || (x >= g.r[k].x0 && x < g.r[k].x1 && y >= g.r[k].y0 && y < g.r[k].y1);
-    return in;
+__host__ __device__ inline int uregion_total(const URegion& g) {
+    return urect_count(g.r[0]) + urect_count(g.r[1]) + urect_count(g.r[2]) + urect_count(g.r[3]);
 }
-// u-th point of the region (row-major inside each rectangle, rectangles in order); false if u is past the end
-__device__ __forceinline__ bool region_point(const Region& g, int u, int& x, int& y) {
-#pragma unroll
+// u-th unit of the region (row-major inside each rectangle, rectangles in order); false if u is past the end
+__host__ __device__ inline bool uregion_unit(const URegion& g, int u, int& gi, int& y) {
     for (int k = 0; k < 4; ++k) {
-        const int n = rect_count(g.r[k]);
+        const int n = urect_count(g.r[k]);
         if (u < n) {
-            const int w = g.r[k].x1 - g.r[k].x0;
+            const int w = g.r[k].g1 - g.r[k].g0;
             y = g.r[k].y0 + u / w;
-            x = g.r[k].x0 + u % w;
+            gi = g.r[k].g0 + u % w;
             return true;
         }
         u -= n;
     }
     return false;
 }
-// Interior points of the core within `halo` of a core edge that has a neighbour tile behind it (walls are never sent).
-__host__ __device__ inline Region send_region(const TileGeom& t, int N, int halo, int bi, int bj, int ntx, int nty) {
+__host__ __device__ inline URect urect_of(int x0, int x1, int y0, int y1) {      // the groups that meet the points [x0, x1)
+    URect r;
+    r.y0 = y0; r.y1 = y1;
+    if (x1 > x0) { r.g0 = x0 / 3; r.g1 = (x1 - 1) / 3 + 1; } else { r.g0 = r.g1 = 0; }
+    return r;
+}
+// Interior points of the core within `halo` of a core edge that has a neighbour tile behind it (walls are never needed).
+__host__ __device__ inline URegion send_units(const TileGeom& t, int N, int halo, int bi, int bj, int ntx, int nty) {
     const int X0 = imax(t.cx0, 1), X1 = imin(t.cx1, N), Y0 = imax(t.cy0, 1), Y1 = imin(t.cy1, N);
     const int hb = bj > 0 ? halo : 0, ht = bj < nty - 1 ? halo : 0, wl = bi > 0 ? halo : 0, wr = bi < ntx - 1 ? halo : 0;
     const int yB = imin(Y0 + hb, Y1), yT = imax(Y1 - ht, yB), xL = imin(X0 + wl, X1), xR = imax(X1 - wr, xL);
-    Region g;
-    g.r[0] = Rect{X0, X1, Y0, yB};
-    g.r[1] = Rect{X0, X1, yT, Y1};
-    g.r[2] = Rect{X0, xL, yB, yT};
-    g.r[3] = Rect{xR, X1, yB, yT};
+    URegion g;
+    g.r[0] = urect_of(X0, X1, Y0, yB);
+    g.r[1] = urect_of(X0, X1, yT, Y1);
+    g.r[2] = urect_of(X0, xL, yB, yT);
+    g.r[3] = urect_of(xR, X1, yB, yT);
+    if (urect_count(g.r[2]) > 0 && urect_count(g.r[3]) > 0 && g.r[3].g0 < g.r[2].g1) g.r[3].g0 = imin(g.r[2].g1, g.r[3].g1);   // narrow core: no unit twice
     return g;
 }
 // Interior points within `halo` of the core, outside it (the ring).
-__host__ __device__ inline Region recv_region(const TileGeom& t, int N, int halo) {
+__host__ __device__ inline URegion recv_units(const TileGeom& t, int N, int halo) {
     const int xlo = imax(t.cx0 - halo, 1), xhi = imin(t.cx1 + halo, N), ylo = imax(t.cy0 - halo, 1), yhi = imin(t.cy1 + halo, N);
     const int yc0 = imax(t.cy0, ylo), yc1 = imin(t.cy1, yhi), xc0 = imax(t.cx0, xlo), xc1 = imin(t.cx1, xhi);
-    // Order = the order in which the neighbours STORE these points (send_region: bottom strip, top strip, left, right), so
-    // that what was stored first is fetched first: the ring above comes from the northern tile's bottom strip, etc.
-    Region g;
-    g.r[0] = Rect{xlo, xhi, yc1, yhi};      // ring above   <- bottom strips of the tiles above
-    g.r[1] = Rect{xlo, xhi, ylo, yc0};      // ring below   <- top strips of the tiles below
-    g.r[2] = Rect{xc1, xhi, yc0, yc1};      // ring right   <- left strip of the tile to the right
-    g.r[3] = Rect{xlo, xc0, yc0, yc1};      // ring left    <- right strip of the tile to the left
+    // Order = the order in which the neighbours STORE these units (send_units: bottom strip, top strip, left, right), so
+    // that what was stored first is fetched first: the ring above comes from the northern tiles' bottom strips, etc.
+    URegion g;
+    g.r[0] = urect_of(xlo, xhi, yc1, yhi);      // ring above   <- bottom strips of the tiles above
+    g.r[1] = urect_of(xlo, xhi, ylo, yc0);      // ring below   <- top strips of the tiles below
+    g.r[2] = urect_of(xc1, xhi, yc0, yc1);      // ring right   <- left strip of the tile to the right (xc1 = its cx0: a multiple of 3)
+    g.r[3] = urect_of(xlo, xc0, yc0, yc1);      // ring left    <- right strip of the tile to the left (xc0 = cx0: a multiple of 3)
     return g;
 }
 
-__host__ __device__ inline size_t xtab_bytes(int nth, int ns_per, int nr_per) {
-    return (4 + 2) * (size_t)(ns_per + nr_per) * nth + 4 * 2 * (size_t)nth;      // a multiple of 64
-}
-// Shared-memory layout (doubles unless said otherwise), nthreads = 32 nwarps:
+// Shared-memory layout (doubles unless said otherwise), nthreads = 32 nwarps, H = R nwarps, SW = 32 C:
 //   edges   4 (MAXW + 1) C 32            bottom / top rows of the micro-tiles, q of the two middle rows (sized for MAXW warps)
-//   stage   R C (nthreads + 4)           one slot per thread and micro-tile point, [point][thread] (+4: the 4 points of a chunk fall in different banks)
-//   offS    ns_per nthreads u32          unit offset in the exchange buffer of the strip units this thread stores (NO_UNIT: none)
-//   offR    nr_per nthreads u32          same for the ring units this thread fetches
-//   masks   2 nthreads u32               bit k: point k of this thread's micro-tile is in the send region / in the ring
-//   slotS   ns_per nthreads u16          staging slot of each of those units
-//   slotR   nr_per nthreads u16
+//   image   H SW                         the tile, row-major: staging area of every exchange, and omega of the stage input during a3
+//   wring   2 SW + 2 H                   first ring of the stage input vorticity around the core (rows below / above, columns left / right)
+//   table   (ns_per + nr_per) nthreads uint2   {unit index in the exchange buffer (NO_UNIT: none), position in the image}
 __host__ __device__ inline size_t smem_layout_bytes(int C, int R, int maxw, int warps, int ns_per, int nr_per) {
-    const size_t nth = 32 * (size_t)warps;
-    return 8 * ((2 + CAV_QROWS) * (size_t)(maxw + 1) * C * 32 + (size_t)R * C * (nth + 4)) + xtab_bytes((int)nth, ns_per, nr_per);
+    const size_t nth = 32 * (size_t)warps, H = (size_t)R * warps, SW = 32 * (size_t)C;
+    return 8 * ((2 + CAV_QROWS) * (size_t)(maxw + 1) * C * 32 + H * SW + 2 * SW + 2 * H) + 8 * (size_t)(ns_per + nr_per) * nth;
+}
+__host__ __device__ inline size_t xtab_entries(int nth, int ns_per, int nr_per) { return (size_t)(ns_per + nr_per) * nth; }
+
+// table entry .y: bits 0-7 = local x of the first point + 8, bits 8-15 = local row, bits 16-18 = which of the three points
+// lie inside the image
+__host__ __device__ inline unsigned int loc_pack(int lx0, int row, int W) {
+    unsigned int m = 0;
+    for (int j = 0; j < 3; ++j)
+        if (lx0 + j >= 0 && lx0 + j < W) m |= 1u << j;
+    return (unsigned int)(lx0 + 8) | ((unsigned int)row << 8) | (m << 16);
 }
 
-// Global <-> micro-tile transfers of one warp, coalesced: the warp moves rows of 32 C consecutive doubles (lane = x), and a
-// per-warp shared-memory buffer of R rows x 32 C doubles transposes between that and the C-consecutive-points-per-lane
-// layout of the registers.  Points that are not interior (walls, outside, row padding) read as +0.0.
+// Builds, once per plan, the exchange tables of every tile in global memory (in the layout the kernel copies to shared
+// memory at launch): which unit each thread stores / fetches and where its three points sit in the image.
 template <int C, int R>
-__device__ __forceinline__ void warp_load_tile(double (&v)[R][C], const double* __restrict__ g, const int x0w, const int y0,
-                                               const int N, const int pitch, double* __restrict__ wbuf, const int lane) {
-#pragma unroll
-    for (int rj = 0; rj < R; ++rj) {
-        const int gy = y0 + rj;
-#pragma unroll
-        for (int j = 0; j < C; ++j) {
-            const int gx = x0w + j * 32 + lane;
-            const bool upd = gx >= 1 && gx <= N - 1 && gy >= 1 && gy <= N - 1;
-            wbuf[rj * (32 * C) + j * 32 + lane] = upd ? g[(size_t)gy * pitch + gx] : 0.0;
-        }
-    }
-    __syncwarp();
-#pragma unroll
-    for (int rj = 0; rj < R; ++rj)
-#pragma unroll
-        for (int ci = 0; ci < C; ci += 2) {
-            const double2 d = *reinterpret_cast<const double2*>(wbuf + rj * (32 * C) + lane * C + ci);
-            v[rj][ci] = d.x; v[rj][ci + 1] = d.y;
-        }
-    __syncwarp();
-}
-
-struct XTab {
-    unsigned int *offS, *offR, *masks;
-    unsigned short *slotS, *slotR;
-};
-__device__ __forceinline__ XTab xtab(void* base, int nth, int ns_per, int nr_per) {
-    XTab t;
-    t.offS = reinterpret_cast<unsigned int*>(base);
-    t.offR = t.offS + ns_per * nth;
-    t.masks = t.offR + nr_per * nth;
-    t.slotS = reinterpret_cast<unsigned short*>(t.masks + 2 * nth);
-    t.slotR = t.slotS + ns_per * nth;
-    return t;
-}
-
-// Builds, once per plan, the exchange tables of every tile in global memory (one block of xtab_bytes per tile, in the
-// layout the sweep kernel copies to shared memory at launch): which exchange unit each thread stores / fetches and which
-// staging slot it belongs to, and each thread's masks of micro-tile points that are sent / received.
-template <int C, int R>
-__global__ void k_build_tables(const ResArgs a, unsigned char* __restrict__ out) {
+__global__ void k_build_tables(const ResArgs a, uint2* __restrict__ out) {
     const int lane = threadIdx.x, warp = threadIdx.y, nwarps = blockDim.y;
     const int tid = warp * 32 + lane, nthreads = nwarps * 32;
     const int N = a.N, bi = blockIdx.x, bj = blockIdx.y;
     const TileGeom t = tile_geom(N, a.CW, a.CH, a.halo, a.ntx, a.nty, bi, bj, C, R, 32 * C, nwarps * R);
-    const int gx0 = t.ox + lane * C, gy0 = t.oy + warp * R;
-    const XTab xt = xtab(out + (size_t)(bj * a.ntx + bi) * xtab_bytes(nthreads, a.ns_per, a.nr_per), nthreads, a.ns_per, a.nr_per);
-    const Region gs = send_region(t, N, a.halo, bi, bj, a.ntx, a.nty), gr = recv_region(t, N, a.halo);
+    uint2* const o = out + (size_t)(bj * a.ntx + bi) * xtab_entries(nthreads, a.ns_per, a.nr_per);
+    const URegion gs = send_units(t, N, a.halo, bi, bj, a.ntx, a.nty), gr = recv_units(t, N, a.halo);
     for (int i = 0; i < a.ns_per + a.nr_per; ++i) {
         const bool snd = i < a.ns_per;
         const int u = (snd ? i : i - a.ns_per) * nthreads + tid;
-        int x = 0, y = 0;
+        int g = 0, y = 0;
         uint2 e = make_uint2(NO_UNIT, 0u);
-        if (region_point(snd ? gs : gr, u, x, y)) {
-            const int lx = x - t.ox, ly = y - t.oy;                        // owner: lane lx / C, warp ly / R
-            e.x = (unsigned int)(y * a.pitch + x);                         // < 2^31: N <= 32766
-            e.y = (unsigned int)(((ly % R) * C + lx % C) * (nthreads + 4) + (ly / R) * 32 + lx / C);
+        if (uregion_unit(snd ? gs : gr, u, g, y)) {
+            e.x = (unsigned int)(y * a.upitch + g);
+            e.y = loc_pack(3 * g - t.ox, y - t.oy, 32 * C);
         }
-        (snd ? xt.offS : xt.offR)[(snd ? i : i - a.ns_per) * nthreads + tid] = e.x;
-        (snd ? xt.slotS : xt.slotR)[(snd ? i : i - a.ns_per) * nthreads + tid] = (unsigned short)e.y;
+        o[(size_t)i * nthreads + tid] = e;
     }
-    unsigned int smask = 0, rmask = 0;
-    for (int k = 0; k < R * C; ++k) {
-        if (region_has(gs, gx0 + k % C, gy0 + k / C)) smask |= 1u << k;
-        if (region_has(gr, gx0 + k % C, gy0 + k / C)) rmask |= 1u << k;
-    }
-    xt.masks[tid] = smask;
-    xt.masks[nthreads + tid] = rmask;
 }
 
-// MAXW = most warps per CTA this variant is launched with: 65536 / (32 MAXW) registers per thread are available.
-// PERSM = CTAs per SM the variant is built for (two half-size CTAs per SM hide each other's exchange and barrier latency).
-template <int C, int R, int MAXW, int PERSM, bool FIX>
-__global__ void __launch_bounds__(32 * MAXW, PERSM) k_resident(const ResArgs a) {
+// ---- the tile image in shared memory ----------------------------------------------------------------------------
+template <int C, int R>
+__device__ __forceinline__ void stage_tile(const double (&v)[R][C], double* __restrict__ img, const int lane, const int warp) {
+    double* const d = img + (warp * R) * (32 * C) + lane * C;
+#pragma unroll
+    for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+        for (int ci = 0; ci < C; ci += 2) *reinterpret_cast<double2*>(d + rj * (32 * C) + ci) = make_double2(v[rj][ci], v[rj][ci + 1]);
+}
+template <int C, int R>
+__device__ __forceinline__ void read_tile(double (&v)[R][C], const double* __restrict__ img, const int lane, const int warp) {
+    const double* const s = img + (warp * R) * (32 * C) + lane * C;
+#pragma unroll
+    for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+        for (int ci = 0; ci < C; ci += 2) {
+            const double2 d = *reinterpret_cast<const double2*>(s + rj * (32 * C) + ci);
+            v[rj][ci] = d.x; v[rj][ci + 1] = d.y;
+        }
+}
+// image <- field g on the interior points of [x0, x1) x [y0, y1) (grid coordinates), +0.0 everywhere else.  Coalesced:
+// consecutive threads = consecutive x.  cg: the field may have been written by this CTA during this launch.
+template <int C>
+__device__ __forceinline__ void fill_image(double* __restrict__ img, const double* __restrict__ g, const int x0, const int x1,
+                                           const int y0, const int y1, const int ox, const int oy, const int H, const int N,
+                                           const int pitch, const int tid, const int nth) {
+    constexpr int SW = 32 * C;
+    const int xa = imax(x0, 1), xb = imin(x1, N), ya = imax(y0, 1), yb = imin(y1, N);
+    for (int k = tid; k < H * SW; k += nth) {
+        const int row = k / SW, lx = k % SW;
+        const int gx = ox + lx, gy = oy + row;
+        double v = 0.0;
+        if (gx >= xa && gx < xb && gy >= ya && gy < yb) v = __ldcg(g + (size_t)gy * pitch + gx);
+        img[k] = v;
+    }
+}
+
+// Stores this tile's strip units from the image, fetches its ring units into the image.  All threads; no barrier inside.
+// Not inlined (like rhs_phase below): its registers are allocated apart from the sweep loops, which hold psi and q in
+// registers and have none to spare.
+__device__ __noinline__ void exchange_units(const ResArgs& a, double* __restrict__ img, const uint2* __restrict__ tab,
+                                               const int tid_o, const int nth_o, const unsigned int round, const int SW,
+                                               const int mark_slot) {
+    ulonglong4* const xb = (round & 1u) ? a.x1 : a.x0;
+    const unsigned int tag = round_tag(round);
+    for (int i = 0; i < a.ns_per; ++i) {
+        const uint2 e = tab[i * nth_o + tid_o];
+        if (e.x != NO_UNIT) {
+            const double* const s = img + (int)((e.y >> 8) & 0xffu) * SW + ((int)(e.y & 0xffu) - 8);
+            const double d0 = (e.y & 0x10000u) ? s[0] : 0.0, d1 = (e.y & 0x20000u) ? s[1] : 0.0, d2 = (e.y & 0x40000u) ? s[2] : 0.0;
+            st_unit(xb + e.x, d0, d1, d2, tag);
+        }
+    }
+    mark(a, mark_slot);
+    // All threads fetch ring units (NB in flight per thread), validate, and unpack them into the image.  While some unit of
+    // the warp does not carry the tag yet, ONE lane polls one such unit (waiting tiles do not load L2), then every lane
+    // fetches its missing units again.
+    constexpr int NB = CAV_RECV_BATCH;
+    const uint2* const tabr = tab + a.ns_per * nth_o;
+    for (int i0 = 0; i0 < a.nr_per; i0 += NB) {
+        uint2 e[NB];
+        ulonglong4 v[NB];
+        unsigned int bad = 0;
+#pragma unroll
+        for (int j = 0; j < NB; ++j) e[j] = i0 + j < a.nr_per ? tabr[(i0 + j) * nth_o + tid_o] : make_uint2(NO_UNIT, 0u);
+#pragma unroll
+        for (int j = 0; j < NB; ++j)
+            if (e[j].x != NO_UNIT) v[j] = ld_unit(xb + e[j].x);
+#pragma unroll
+        for (int j = 0; j < NB; ++j)
+            if (e[j].x != NO_UNIT && !unit_ok(v[j], tag)) bad |= 1u << j;
+        unsigned int waiting = __ballot_sync(0xffffffffu, bad != 0u);
+        if (waiting) {
+            const long long t0 = clock64();
+            while (waiting) {
+                int giveup = 0;
+                if ((int)threadIdx.x == __ffs((int)waiting) - 1) {
+                    unsigned int off = e[NB - 1].x;                // the first missing unit of this lane
+#pragma unroll
+                    for (int j = NB - 2; j >= 0; --j)
+                        if ((bad >> j) & 1u) off = e[j].x;
+                    while (!unit_ok(ld_unit(xb + off), tag)) {
+                        if (*(volatile unsigned int*)a.err != 0u) { giveup = 1; break; }      // some tile gave up: do not wait again
+                        if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) {
+                            if (atomicExch(a.err, 1u) == 0u) {      // the first tile to give up says what it was waiting for (CAV_DEBUG)
+                                const ulonglong4 w = ld_unit(xb + off);
+                                a.err[1] = blockIdx.y * a.ntx + blockIdx.x; a.err[2] = off; a.err[3] = round; a.err[4] = tag;
+                                a.err[5] = (unsigned int)(w.x >> 48); a.err[6] = (unsigned int)(w.y >> 48);
+                                a.err[7] = (unsigned int)(w.z >> 48); a.err[8] = (unsigned int)(w.w >> 48);
+                                a.err[9] = (unsigned int)tid_o;
+                            }
+                            giveup = 1; break;
+                        }
+                    }
+                }
+                if (__any_sync(0xffffffffu, giveup)) break;
+#pragma unroll
+                for (int j = 0; j < NB; ++j)
+                    if ((bad >> j) & 1u) {
+                        v[j] = ld_unit(xb + e[j].x);
+                        if (unit_ok(v[j], tag)) bad &= ~(1u << j);
+                    }
+                waiting = __ballot_sync(0xffffffffu, bad != 0u);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < NB; ++j)
+            if (e[j].x != NO_UNIT) {
+                double d0, d1, d2;
+                unit_values(v[j], d0, d1, d2);
+                double* const s = img + (int)((e[j].y >> 8) & 0xffu) * SW + ((int)(e[j].y & 0xffu) - 8);
+                if (e[j].y & 0x10000u) s[0] = d0;
+                if (e[j].y & 0x20000u) s[1] = d1;
+                if (e[j].y & 0x40000u) s[2] = d2;
+            }
+    }
+}
+
+__device__ __forceinline__ double thom_wall(double c2h2, double p_adj) { return -(c2h2 * p_adj); }
+__device__ __forceinline__ double thom_lid(double c2h2, double lid, double p_adj) { return -(c2h2 * p_adj) - lid; }
+
+// a2 + a3 of one stage for this tile (see the file header).  pl: the thread's psi micro-tile, [rj * C + ci].  On return the
+// image holds the NEW vorticity on core + halo (+0.0 elsewhere) and the ring copy is refreshed; the caller turns it into q.
+// Not inlined: see exchange_units.
+template <int C, int R, int MAXW>
+__device__ __noinline__ void rhs_phase(const ResArgs& a, const double* __restrict__ pl, double* __restrict__ sm, const int stage,
+                                       const unsigned int round, const unsigned int fl) {
     constexpr int TOPOFF = (MAXW + 1) * C * 32;
+    constexpr int SW = 32 * C;
+    constexpr int edge_doubles = (2 + CAV_QROWS) * TOPOFF;
+    double* const sB = sm + (int)threadIdx.y * C * 32 + (int)threadIdx.x;
+    {
+    const int z = opaque_zero();
+    const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
+    const int nw = (int)blockDim.y + z, tid_o = wp * 32 + ln, nth_o = nw * 32, H = nw * R;
+    const int Ne = a.N + z, pitch = a.pitch;
+    const TileGeom te = tile_geom(Ne, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, H);
+    const int k = stage % 5 + 1;                                    // RK stage 1..5
+    const double* const win = a.wbase + (size_t)(k - 1) * a.fstride;    // omega^(k-1)
+    double* const wout = a.wbase + (size_t)(k % 5) * a.fstride;         // omega^(k); stage 5 writes omega^{n+1} over omega^n
+    double* const tbuf = a.wbase + (size_t)(5 + z) * a.fstride;         // T: first three terms of eq 13 (+ z: not hoisted)
+    const double* const w0b = a.wbase + (size_t)z * a.fstride;          // omega^n
+    const double* const w2b = a.wbase + (size_t)(2 + z) * a.fstride;
+    double* const img = sm + edge_doubles;
+    const double* const wr = img + H * SW;
+    // interior points of the core, in grid and in local coordinates
+    const int X0 = imax(te.cx0, 1), X1 = imin(te.cx1, Ne), Y0 = imax(te.cy0, 1), Y1 = imin(te.cy1, Ne);
+    const int lx0 = ln * C, row0 = wp * R, gx0 = te.ox + lx0, gy0 = te.oy + row0;
+
+    // (1) the image receives the stage input: core from the tile's own global buffer, first ring from the copy kept
+    //     since the last vorticity exchange, walls next to the core from Thom's formula (written by the owner of the
+    //     adjacent point, who also stores it to the ring of the stage output: k_rk_stage does the same).
+    fill_image<C>(img, win, X0, X1, Y0, Y1, te.ox, te.oy, H, Ne, pitch, tid_o, nth_o);
+    __syncthreads();              // fill_image writes zeros everywhere else: the ring and wall writers come after it
+    {
+        const int rB = Y0 - 1 - te.oy, rT = Y1 - te.oy, cL = X0 - 1 - te.ox, cR = X1 - te.ox;
+        for (int c = tid_o; c < SW; c += nth_o) {
+            const int gx = te.ox + c;
+            if (gx >= X0 && gx < X1) {
+                if (Y0 - 1 >= 1) img[rB * SW + c] = wr[c];
+                if (Y1 <= Ne - 1) img[rT * SW + c] = wr[SW + c];
+            }
+        }
+        for (int r2 = tid_o; r2 < H; r2 += nth_o) {
+            const int gy = te.oy + r2;
+            if (gy >= Y0 && gy < Y1) {
+                if (X0 - 1 >= 1) img[r2 * SW + cL] = wr[2 * SW + r2];
+                if (X1 <= Ne - 1) img[r2 * SW + cR] = wr[2 * SW + H + r2];
+            }
+        }
+    }
+    if ((gx0 <= 1 || gx0 + C - 1 >= Ne - 1 || gy0 <= 1 || gy0 + R - 1 >= Ne - 1)) {
+#pragma unroll
+        for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+            for (int ci = 0; ci < C; ++ci) {
+                const int gx = gx0 + ci, gy = gy0 + rj;
+                if (gx < X0 || gx >= X1 || gy < Y0 || gy >= Y1) continue;
+                double* const ic = img + (row0 + rj) * SW + lx0 + ci;
+                const double pv = pl[rj * C + ci];
+                if (gx == 1) { const double v = thom_wall(a.c2h2, pv); ic[-1] = v; wout[(size_t)gy * pitch] = v; }
+                if (gx == Ne - 1) { const double v = thom_wall(a.c2h2, pv); ic[1] = v; wout[(size_t)gy * pitch + Ne] = v; }
+                if (gy == 1) {
+                    const double v = thom_wall(a.c2h2, pv); ic[-SW] = v; wout[gx] = v;
+                    if (gx == 1) wout[0] = thom_wall(a.c2h2, 0.0);                      // the bottom and top rows own the corners (G10)
+                    if (gx == Ne - 1) wout[Ne] = thom_wall(a.c2h2, 0.0);
+                }
+                if (gy == Ne - 1) {
+                    const double v = thom_lid(a.c2h2, a.lid, pv); ic[SW] = v; wout[(size_t)Ne * pitch + gx] = v;
+                    if (gx == 1) wout[(size_t)Ne * pitch] = thom_lid(a.c2h2, a.lid, 0.0);
+                    if (gx == Ne - 1) wout[(size_t)Ne * pitch + Ne] = thom_lid(a.c2h2, a.lid, 0.0);
+                }
+            }
+    }
+    __syncthreads();
+
+    // (2) eq 8 + eq 22 and the combination of eq 9-13 for the core points of this thread, row by row
+#pragma unroll
+    for (int rj = 0; rj < R; ++rj) {
+        const int gy = gy0 + rj;
+        if (gy < Y0 || gy >= Y1) continue;                              // the same for the whole warp
+        const double* const ir = img + (row0 + rj) * SW + lx0;
+        double lnb = __shfl_up_sync(0xffffffffu, pl[rj * C + C - 1], 1);
+        double rnb = __shfl_down_sync(0xffffffffu, pl[rj * C], 1);
+        if (fl & FL_ZERO_LEFT) lnb = 0.0;                               // the wall (or the end of the thread grid), as in the sweeps
+        if (fl & FL_ZERO_RIGHT) rnb = 0.0;
+        if (gx0 + C - 1 < X0 || gx0 >= X1) continue;
+        double wc[C + 2], ws[C], wn[C];
+        wc[0] = ir[-1]; wc[C + 1] = ir[C];
+#pragma unroll
+        for (int ci = 0; ci < C; ci += 2) {
+            const double2 c2 = *reinterpret_cast<const double2*>(ir + ci);
+            const double2 s2 = *reinterpret_cast<const double2*>(ir - SW + ci);
+            const double2 n2 = *reinterpret_cast<const double2*>(ir + SW + ci);
+            wc[1 + ci] = c2.x; wc[2 + ci] = c2.y; ws[ci] = s2.x; ws[ci + 1] = s2.y; wn[ci] = n2.x; wn[ci + 1] = n2.y;
+        }
+#pragma unroll
+        for (int ci = 0; ci < C; ++ci) {
+            const int gx = gx0 + ci;
+            if (gx < X0 || gx >= X1) continue;
+            const double pW = ci > 0 ? pl[rj * C + ci - 1] : lnb;
+            const double pE = ci < C - 1 ? pl[rj * C + ci + 1] : rnb;
+            const double pS = rj > 0 ? pl[(rj - 1) * C + ci] : sB[TOPOFF + ci * 32];            // top row of the warp below
+            const double pN = rj < R - 1 ? pl[(rj + 1) * C + ci] : sB[C * 32 + ci * 32];        // bottom row of the warp above
+            const double w0 = wc[1 + ci], wW = wc[ci], wE = wc[2 + ci], wS = ws[ci], wN = wn[ci];
+            // eq 22: u = dpsi/dy, v = -dpsi/dx;  eq 8
+            const double u = (pN - pS) * a.i2h;
+            const double v = (pW - pE) * a.i2h;
+            const double wx = (wE - wW) * a.i2h;
+            const double wy = (wN - wS) * a.i2h;
+            const double lap = (((wW + wE) + (wS + wN)) - 4.0 * w0) * a.ih2;
+            const double L = fma(a.nu, lap, -fma(u, wx, v * wy));
+            const double dL = a.dt * L;
+            const size_t gk = (size_t)gy * pitch + gx;
+            double out;
+            if (k == 1) {
+                out = fma(RK1_C, dL, w0);                                               // eq 9
+            } else if (k == 2) {
+                out = fma(RK2_C, dL, fma(RK2_A1, w0, RK2_A0 * w0b[gk]));                // eq 10 (w0 here is omega^(1))
+            } else if (k == 3) {
+                out = fma(RK3_C, dL, fma(RK3_A2, w0, RK3_A0 * w0b[gk]));                // eq 11
+            } else if (k == 4) {
+                out = fma(RK4_C, dL, fma(RK4_A3, w0, RK4_A0 * w0b[gk]));                // eq 12
+                tbuf[gk] = fma(RK5_C3, dL, fma(RK5_A3, w0, RK5_A2 * w2b[gk]));          // eq 13, first three terms
+            } else {
+                out = fma(RK5_C4, dL, fma(RK5_A4, w0, tbuf[gk]));                       // eq 13, the rest
+            }
+            wout[gk] = out;
+        }
+    }
+    __syncthreads();              // every read of the image and every store of the stage output is done
+
+    // (3) the new vorticity: core from the global buffer just written, ring from the neighbours, q = cq w
+    fill_image<C>(img, wout, X0, X1, Y0, Y1, te.ox, te.oy, H, Ne, pitch, tid_o, nth_o);
+    __syncthreads();
+    if (a.ntx * a.nty > 1) {
+        const uint2* const tab = reinterpret_cast<const uint2*>(img + H * SW + 2 * SW + 2 * H);
+        exchange_units(a, img, tab, tid_o, nth_o, round, SW, a.trace_cap);
+        __syncthreads();
+    }
+    {   // first ring of the new vorticity around the core, kept for a3 of the next stage
+        double* const wrw = img + H * SW;
+        const int rB = Y0 - 1 - te.oy, rT = Y1 - te.oy, cL = X0 - 1 - te.ox, cR = X1 - te.ox;
+        for (int c = tid_o; c < SW; c += nth_o) { wrw[c] = img[rB * SW + c]; wrw[SW + c] = img[rT * SW + c]; }
+        for (int r2 = tid_o; r2 < H; r2 += nth_o) { wrw[2 * SW + r2] = img[r2 * SW + cL]; wrw[2 * SW + H + r2] = img[r2 * SW + cR]; }
+    }
+    }
+}
+
+// MAXW = most warps per CTA the kernel is launched with: 65536 / (32 MAXW) registers per thread are available.
+template <int C, int R, int MAXW, bool FIX>
+__global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant__ ResArgs a) {
+    constexpr int TOPOFF = (MAXW + 1) * C * 32;
+    constexpr int SW = 32 * C;
     static_assert(C % 2 == 0 && R % 2 == 0 && R * C <= 32, "even micro-tile that fits the 32-bit point masks");
     extern __shared__ __align__(16) double sm[];
     const int lane = threadIdx.x, warp = threadIdx.y, nwarps = blockDim.y;
     const int tid = warp * 32 + lane, nthreads = nwarps * 32;
-    const int N = a.N, pitch = a.pitch;
+    const int N = a.N;
     const int bi = blockIdx.x, bj = blockIdx.y;
     mark(a, 0);
 
-    // edge arrays; the slots no thread ever writes (warp -1, warp nwarps, unpublished wall rows) stay +0.0
+    // edge arrays; the slots no thread ever writes (warp -1, warp nwarps) stay +0.0
     constexpr int edge_doubles = (2 + CAV_QROWS) * TOPOFF;       // bottom edges, top edges, q of the CAV_QROWS middle rows
     for (int k = tid; k < edge_doubles; k += nthreads) sm[k] = 0.0;
     double* const sB = sm + warp * C * 32 + lane;      // [MAXW + 1][C][32] bottom row of warp at [warp]; top rows TOPOFF further, at [warp + 1]
 
-    const TileGeom t = tile_geom(N, a.CW, a.CH, a.halo, a.ntx, a.nty, bi, bj, C, R, 32 * C, nwarps * R);
+    const TileGeom t = tile_geom(N, a.CW, a.CH, a.halo, a.ntx, a.nty, bi, bj, C, R, SW, nwarps * R);
     const int gx0_ = t.ox + lane * C, gy0_ = t.oy + warp * R;
-    const bool odd_origin = ((t.ox + t.oy) & 1) != 0;          // local colour = global colour ^ odd_origin
-
     unsigned int fl = FL_PUB_BOTTOM | FL_PUB_TOP;
+    if ((t.ox + t.oy) & 1) fl |= FL_ODD;                                       // local colour = global colour ^ 1
     {
         const int lzl = t.left_al ? 1 : 0;                                     // lane 0 holds x = -(C-1) .. 0
         const int lzr = t.right_al ? (N - t.ox) / C - 1 : 31;                  // lane (N - ox) / C holds x = N .. N + C - 1
@@ -405,21 +685,36 @@ __global__ void __launch_bounds__(32 * MAXW, PERSM) k_resident(const ResArgs a) 
         if (t.top_al && warp == (N - t.oy) / R) fl &= ~FL_PUB_BOTTOM;          // that warp holds y = N .. N + R - 1
     }
 
-    // ---- exchange tables and masks (multi-tile plans only): copied from the per-plan tables in global memory ----
-    if (a.ntx * a.nty > 1) {
-        const int n16 = (int)(xtab_bytes(nthreads, a.ns_per, a.nr_per) / 16);
-        const uint4* const src = a.tables + (size_t)(bj * a.ntx + bi) * n16;
-        uint4* const dst = reinterpret_cast<uint4*>(sm + edge_doubles + R * C * (nthreads + 4));
-        for (int k = tid; k < n16; k += nthreads) dst[k] = src[k];
+    // ---- exchange tables (multi-tile plans only): copied from the per-plan tables in global memory ----
+    {
+        const int H = nwarps * R;
+        uint2* const tabs = reinterpret_cast<uint2*>(sm + edge_doubles + H * SW + 2 * SW + 2 * H);
+        if (a.ntx * a.nty > 1) {
+            const int n = (int)xtab_entries(nthreads, a.ns_per, a.nr_per);
+            const uint2* const src = a.tables + (size_t)(bj * a.ntx + bi) * n;
+            for (int k = tid; k < n; k += nthreads) tabs[k] = src[k];
+        }
     }
 
-    // ---- load the micro-tile ----
+    // ---- load the micro-tile: psi, and the right-hand side q = cq w of the first stage ----
     double p[R][C], q[R][C];
     unsigned int wallmask = 0;            // wall points that alignment could not isolate (psi = 0 there, eq 23-24)
     {
-        double* const wbuf = sm + edge_doubles + warp * (R * 32 * C);         // inside the staging array, which is idle now
-        warp_load_tile<C, R>(p, a.psi_in, t.ox, gy0_, N, pitch, wbuf, lane);
-        warp_load_tile<C, R>(q, a.w, t.ox, gy0_, N, pitch, wbuf, lane);
+        const int H = nwarps * R;
+        double* const img = sm + edge_doubles;
+        fill_image<C>(img, a.psi_in, 0, N + 1, 0, N + 1, t.ox, t.oy, H, N, a.pitch, tid, nthreads);
+        __syncthreads();
+        read_tile<C, R>(p, img, lane, warp);
+        __syncthreads();
+        fill_image<C>(img, a.wbase, 0, N + 1, 0, N + 1, t.ox, t.oy, H, N, a.pitch, tid, nthreads);
+        __syncthreads();
+        read_tile<C, R>(q, img, lane, warp);
+        if (a.nsteps > 0) {               // first ring of the stage input around the core, kept for a3
+            double* const wr = img + H * SW;
+            const int rB = imax(t.cy0, 1) - 1 - t.oy, rT = imin(t.cy1, N) - t.oy, cL = imax(t.cx0, 1) - 1 - t.ox, cR = imin(t.cx1, N) - t.ox;
+            for (int k = tid; k < SW; k += nthreads) { wr[k] = img[rB * SW + k]; wr[SW + k] = img[rT * SW + k]; }
+            for (int k = tid; k < H; k += nthreads) { wr[2 * SW + k] = img[k * SW + cL]; wr[2 * SW + H + k] = img[k * SW + cR]; }
+        }
     }
 #pragma unroll
     for (int rj = 0; rj < R; ++rj)
@@ -435,7 +730,7 @@ __global__ void __launch_bounds__(32 * MAXW, PERSM) k_resident(const ResArgs a) 
             if (wall && !isolated) wallmask |= 1u << k;
         }
     }
-    __syncthreads();                      // the zero fill of the edge arrays and the tables are complete
+    __syncthreads();                      // the zero fill of the edge arrays, the tables and the ring copy are complete
 #pragma unroll
     for (int ci = 0; ci < C; ++ci) {      // q of the two middle rows moves to shared memory (read back by this thread only)
 #pragma unroll
@@ -444,157 +739,105 @@ __global__ void __launch_bounds__(32 * MAXW, PERSM) k_resident(const ResArgs a) 
     publish_all<C, R, TOPOFF>(p, sB, fl);
     mark(a, 1);
 
-    const int T = a.T;
-    const int nrounds = (a.nsweeps + T - 1) / T;
-    for (int r = 0; r < nrounds; ++r) {
-        const int ns = min(T, a.nsweeps - r * T);
-        if (odd_origin) {
-            for (int s = 0; s < ns; ++s) {                                    // red = (i + j) even first (G9): local colour 1 here
-                half_sweep<C, R, 1, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
-                half_sweep<C, R, 0, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
-            }
-        } else {
-            for (int s = 0; s < ns; ++s) {
-                half_sweep<C, R, 0, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
-                half_sweep<C, R, 1, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
-            }
-        }
-        mark(a, 2 + 4 * r);
-        if (r == nrounds - 1) break;
-
-        // ---- halo exchange through L2: tagged data, no fence, no flag ----
-        // Opaque copies: everything derived from them is recomputed here every round instead of being hoisted out of
-        // the round loop, where it would stay live across the sweeps and push q into local memory.
-        const int z = opaque_zero();
-        const int tid_o = ((int)threadIdx.y + z) * 32 + (int)threadIdx.x, nth_o = ((int)blockDim.y + z) * 32;
-        double* const stage = sm + edge_doubles;
-        const XTab xt = xtab(stage + R * C * (nth_o + 4), nth_o, a.ns_per, a.nr_per);
-        const unsigned int* const masks = xt.masks;
-        uint4* const xb = (r & 1) ? a.x1 : a.x0;
-        const unsigned int tag = a.base + 1u + (unsigned int)r;
-
-        {   // owners stage the strip values, then all threads store strip units, consecutive threads = consecutive x
-            const unsigned int smask = masks[tid_o];
-#pragma unroll
-            for (int k = 0; k < R * C; ++k)
-                if ((smask >> k) & 1u) stage[k * (nth_o + 4) + tid_o] = p[k / C][k % C];
-            __syncthreads();
-            for (int i = 0; i < a.ns_per; ++i) {
-                const unsigned int off = xt.offS[i * nth_o + tid_o];
-                if (off != NO_UNIT) st_unit(xb + off, stage[xt.slotS[i * nth_o + tid_o]], tag);
-            }
-        }
-        mark(a, 3 + 4 * r);
-        // All threads fetch ring units (4 in flight per thread), validate, and stage the values for their owners.
-        // While some unit of the warp does not carry the tag yet, ONE lane polls one such unit (2 100 pollers on the whole
-        // chip: waiting tiles do not load L2), then every lane fetches its missing units again.
-        constexpr int NB = CAV_RECV_BATCH;
-        for (int i0 = 0; i0 < a.nr_per; i0 += NB) {
-            uint2 e[NB];
-            uint4 v[NB];
-            unsigned int bad = 0;
-#pragma unroll
-            for (int j = 0; j < NB; ++j)
-                e[j] = i0 + j < a.nr_per ? make_uint2(xt.offR[(i0 + j) * nth_o + tid_o], xt.slotR[(i0 + j) * nth_o + tid_o])
-                                         : make_uint2(NO_UNIT, 0u);
-#pragma unroll
-            for (int j = 0; j < NB; ++j)
-                if (e[j].x != NO_UNIT) v[j] = ld_unit(xb + e[j].x);
-#pragma unroll
-            for (int j = 0; j < NB; ++j)
-                if (e[j].x != NO_UNIT && !unit_ok(v[j], tag)) bad |= 1u << j;
-            unsigned int waiting = __ballot_sync(0xffffffffu, bad != 0u);
-            if (waiting) {
-                const long long t0 = clock64();
-                while (waiting) {
-                    int giveup = 0;
-                    if ((int)threadIdx.x == __ffs((int)waiting) - 1) {
-                        unsigned int off = e[NB - 1].x;                // the first missing unit of this lane
-#pragma unroll
-                        for (int j = NB - 2; j >= 0; --j)
-                            if ((bad >> j) & 1u) off = e[j].x;
-                        while (!unit_ok(ld_unit(xb + off), tag)) {
-                            if (*(volatile unsigned int*)a.err != 0u) { giveup = 1; break; }      // some tile gave up: do not wait again
-                            if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) { atomicExch(a.err, 1u); giveup = 1; break; }
-                        }
-                    }
-                    if (__any_sync(0xffffffffu, giveup)) break;
-#pragma unroll
-                    for (int j = 0; j < NB; ++j)
-                        if ((bad >> j) & 1u) {
-                            v[j] = ld_unit(xb + e[j].x);
-                            if (unit_ok(v[j], tag)) bad &= ~(1u << j);
-                        }
-                    waiting = __ballot_sync(0xffffffffu, bad != 0u);
+    // Few scalars stay live across the sweeps (they would push q into local memory): the stage counter, the sweeps left in
+    // the stage and the exchange round; everything else is recomputed from the kernel parameters where it is used.
+    unsigned int round = a.base;          // exchange rounds done so far (all tiles count alike)
+    for (int stage = 0; stage < (a.nsteps > 0 ? 5 * a.nsteps : 1); ++stage) {
+        // ================= a1: S sweeps, a halo exchange after every T of them =================
+        for (int rem = a.S; rem > 0; rem -= a.T) {
+            if (fl & FL_ODD) {
+                for (int s = min(a.T, rem); s > 0; --s) {                         // red = (i + j) even first (G9): local colour 1 here
+                    half_sweep<C, R, 1, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
+                    half_sweep<C, R, 0, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
+                }
+            } else {
+                for (int s = min(a.T, rem); s > 0; --s) {
+                    half_sweep<C, R, 0, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
+                    half_sweep<C, R, 1, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
                 }
             }
-#pragma unroll
-            for (int j = 0; j < NB; ++j)
-                if (e[j].x != NO_UNIT) stage[e[j].y] = unit_value(v[j]);
+            const int tslot = 2 + 4 * (int)(round - a.base);                    // trace slot (meaningful in sweeps-only launches)
+            mark(a, tslot);
+            if (a.ntx * a.nty == 1 || (a.nsteps == 0 && rem <= a.T)) continue;  // sweeps only: the last round needs no exchange
+
+            // ---- halo exchange of psi through L2: tagged data, no fence, no flag ----
+            // Opaque copies: everything derived from them is recomputed here every round instead of being hoisted out of
+            // the round loop, where it would stay live across the sweeps and push q into local memory.
+            const int z = opaque_zero();
+            const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
+            const int nw = (int)blockDim.y + z, tid_o = wp * 32 + ln, nth_o = nw * 32, H = nw * R;
+            double* const img = sm + edge_doubles;
+            const uint2* const tab = reinterpret_cast<const uint2*>(img + H * SW + 2 * SW + 2 * H);
+            stage_tile<C, R>(p, img, ln, wp);
+            __syncthreads();
+            exchange_units(a, img, tab, tid_o, nth_o, round, SW, tslot + 1);
+            ++round;
+            __syncthreads();
+            mark(a, tslot + 2);
+            read_tile<C, R>(p, img, ln, wp);
+            publish_all<C, R, TOPOFF>(p, sB, fl);
+            mark(a, tslot + 3);
         }
-        __syncthreads();
+        if (a.nsteps == 0) break;
+
+        // ================= a2 + a3: wall vorticity, transport right-hand side, stage combination =================
         {
-            const unsigned int rmask = masks[nth_o + tid_o];
+            double pl[R * C];             // a copy in local memory: the callee's registers are its own
 #pragma unroll
-            for (int k = 0; k < R * C; ++k)
-                if ((rmask >> k) & 1u) p[k / C][k % C] = stage[k * (nth_o + 4) + tid_o];
+            for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+                for (int ci = 0; ci < C; ++ci) pl[rj * C + ci] = p[rj][ci];
+            rhs_phase<C, R, MAXW>(a, pl, sm, stage, round, fl);
+            if (a.ntx * a.nty > 1) ++round;                                     // the vorticity exchange
+            const int z = opaque_zero();
+            const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
+            double* const img = sm + edge_doubles;
+            read_tile<C, R>(q, img, ln, wp);
+#pragma unroll
+            for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+                for (int ci = 0; ci < C; ++ci) q[rj][ci] = a.cq * q[rj][ci];
+#pragma unroll
+            for (int ci = 0; ci < C; ++ci) {
+#pragma unroll
+                for (int kq = 0; kq < CAV_QROWS; ++kq) sB[(2 + kq) * TOPOFF + ci * 32] = q[(R - CAV_QROWS) / 2 + kq][ci];
+            }
+            __syncthreads();              // the ring copy is complete before the image is staged again
         }
-        mark(a, 4 + 4 * r);
-        publish_all<C, R, TOPOFF>(p, sB, fl);
-        mark(a, 5 + 4 * r);
     }
 
-    // ---- store the core (walls are exactly +0.0); the geometry is recomputed, not kept live across the sweeps ----
+    // ---- store the core of psi (walls are exactly +0.0); the geometry is recomputed, not kept live across the sweeps ----
     {
         const int z = opaque_zero();
-        const int nw = (int)blockDim.y + z;
-        const TileGeom te = tile_geom(a.N + z, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R,
-                                      32 * C, nw * R);
         const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
-        const int ex0 = te.ox + ln * C, ey0 = te.oy + wp * R, Ne = a.N + z;
-        double* const wbuf = sm + (2 + CAV_QROWS) * TOPOFF + wp * (R * 32 * C);     // the staging array is idle again
-#pragma unroll
-        for (int rj = 0; rj < R; ++rj)
-#pragma unroll
-            for (int ci = 0; ci < C; ci += 2) {
-                const int gy = ey0 + rj;
-                const bool rowi = gy >= 1 && gy <= Ne - 1;
-                double2 d;
-                d.x = (rowi && ex0 + ci >= 1 && ex0 + ci <= Ne - 1) ? p[rj][ci] : 0.0;
-                d.y = (rowi && ex0 + ci + 1 >= 1 && ex0 + ci + 1 <= Ne - 1) ? p[rj][ci + 1] : 0.0;
-                *reinterpret_cast<double2*>(wbuf + rj * (32 * C) + ln * C + ci) = d;
-            }
-        __syncwarp();
-#pragma unroll
-        for (int rj = 0; rj < R; ++rj) {
-            const int gy = ey0 + rj;
-#pragma unroll
-            for (int j = 0; j < C; ++j) {
-                const int gx = te.ox + j * 32 + ln;
-                if (gx >= te.cx0 && gx < te.cx1 && gy >= te.cy0 && gy < te.cy1)
-                    a.psi_out[(size_t)gy * a.pitch + gx] = wbuf[rj * (32 * C) + j * 32 + ln];
-            }
+        const int nw = (int)blockDim.y + z, tid_o = wp * 32 + ln, nth_o = nw * 32, H = nw * R;
+        const int Ne = a.N + z;
+        const TileGeom te = tile_geom(Ne, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, H);
+        double* const img = sm + edge_doubles;
+        stage_tile<C, R>(p, img, ln, wp);
+        __syncthreads();
+        const int cw = te.cx1 - te.cx0, ch = te.cy1 - te.cy0;
+        for (int k = tid_o; k < cw * ch; k += nth_o) {
+            const int gy = te.cy0 + k / cw, gx = te.cx0 + k % cw;
+            const bool inter = gx >= 1 && gx <= Ne - 1 && gy >= 1 && gy <= Ne - 1;
+            a.psi_out[(size_t)gy * a.pitch + gx] = inter ? img[(gy - te.oy) * SW + (gx - te.ox)] : 0.0;
         }
     }
 }
 
 // ---- compiled variants ------------------------------------------------------------------------------
 struct Variant {
-    int C, R, maxw, persm;
+    int C, R, maxw;
     const void* fn;        // every wall isolated by alignment (the plans of large grids)
     const void* fn_fix;    // with the wall-mask fix-up (a tile that holds both walls of one direction)
 };
 const Variant VARIANTS[] = {
     // one CTA of up to 16 warps per SM (also the single-tile plans of small grids)
-    {4, 6, 16, 1, (const void*)k_resident<4, 6, 16, 1, false>, (const void*)k_resident<4, 6, 16, 1, true>},
-    // two CTAs of up to 8 warps per SM: while one exchanges its halo or sits in a barrier, the other computes
-    {4, 6, 8, 2, (const void*)k_resident<4, 6, 8, 2, false>, (const void*)k_resident<4, 6, 8, 2, true>},
+    {4, 6, 16, (const void*)k_resident<4, 6, 16, false>, (const void*)k_resident<4, 6, 16, true>},
 };
 constexpr int NVARIANTS = sizeof(VARIANTS) / sizeof(VARIANTS[0]);
 
 inline int cdiv(int a, int b) { return (a + b - 1) / b; }
-
-int region_total(const Region& g) { return rect_count(g.r[0]) + rect_count(g.r[1]) + rect_count(g.r[2]) + rect_count(g.r[3]); }
 
 // Checks that every tile of the candidate fits its thread grid and counts the exchange units per thread.
 bool finish_plan(ResidentPlan& pl, int N, int max_smem) {
@@ -605,32 +848,35 @@ bool finish_plan(ResidentPlan& pl, int N, int max_smem) {
             const TileGeom t = tile_geom(N, pl.CW, pl.CH, pl.halo, pl.ntx, pl.nty, bi, bj, pl.C, pl.R, W, H);
             if (!t.fits) return false;
             if (pl.ntiles > 1) {
-                smax = std::max(smax, region_total(send_region(t, N, pl.halo, bi, bj, pl.ntx, pl.nty)));
-                rmax = std::max(rmax, region_total(recv_region(t, N, pl.halo)));
+                smax = std::max(smax, uregion_total(send_units(t, N, pl.halo, bi, bj, pl.ntx, pl.nty)));
+                rmax = std::max(rmax, uregion_total(recv_units(t, N, pl.halo)));
             }
         }
     pl.ns_per = cdiv(smax, nth);
     pl.nr_per = cdiv(rmax, nth);
     const int maxw = VARIANTS[pl.variant].maxw;
-    const size_t smem = pl.ntiles > 1 ? smem_layout_bytes(pl.C, pl.R, maxw, pl.warps, pl.ns_per, pl.nr_per)
-                                      : 8 * (size_t)((2 + CAV_QROWS) * (maxw + 1) * pl.C * 32 + pl.R * pl.C * (nth + 4));
+    const size_t smem = smem_layout_bytes(pl.C, pl.R, maxw, pl.warps, pl.ns_per, pl.nr_per);
     pl.fixup = pl.ntx == 1 || pl.nty == 1;
     if (smem > (size_t)max_smem) return false;
     pl.smem_bytes = (int)smem;
     return true;
 }
 
-// One direction of the tiling: G points, thread grid of L points, halo h.  false if no uniform core size works.
-bool split(int G, int L, int lead, int h, int& core, int& n) {
+// One direction of the tiling: G points, thread grid of L points, halo h; core sizes are multiples of `align` when there
+// is more than one tile.  false if no uniform core size works.
+bool split(int G, int L, int lead, int h, int align, int& core, int& n) {
     if (G + lead <= L) { core = G; n = 1; return true; }       // one tile holds both walls (lead = alignment slack of the first wall)
-    const int cmax = L - 2 * h;
+    const int cmax = (L - 2 * h) / align * align;
     if (cmax <= h) return false;
-    n = cdiv(G, cmax);
-    core = cdiv(G, n);
-    n = cdiv(G, core);
-    // the halo must come from adjacent tiles only, and must not reach a wall through an edge tile (only an
-    // edge tile isolates the wall; elsewhere nothing keeps a wall point inside the thread grid at 0)
-    return core > h && G - (n - 1) * core > h;
+    for (n = cdiv(G, cmax); n <= G; ++n) {
+        core = cdiv(cdiv(G, n), align) * align;
+        if (core > cmax) continue;
+        n = cdiv(G, core);
+        // the halo must come from adjacent tiles only, and must not reach a wall through an edge tile (only an
+        // edge tile isolates the wall; elsewhere nothing keeps a wall point inside the thread grid at 0)
+        return n >= 2 && core > h && G - (n - 1) * core > h;
+    }
+    return false;
 }
 
 }  // namespace
@@ -656,14 +902,13 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
         const int max_warps = std::min(v.maxw, std::min(max_threads / 32, (int)(prop.regsPerBlock / (32 * std::max(regs, 1)))));
         const int W = 32 * v.C;                  // tile width in points
         const int smem_cap = std::min((int)prop.sharedMemPerBlockOptin,
-                                      (int)(prop.sharedMemPerMultiprocessor / v.persm) - (int)prop.reservedSharedMemPerBlock);
+                                      (int)prop.sharedMemPerMultiprocessor - (int)prop.reservedSharedMemPerBlock);
         for (int warps = 1; warps <= max_warps; ++warps) {
             const int H = warps * v.R;           // tile height in points
             ResidentPlan c;
-            c.ok = true; c.variant = vi; c.C = v.C; c.R = v.R; c.warps = warps; c.regs = regs; c.sm_count = sms; c.per_sm = v.persm;
+            c.ok = true; c.variant = vi; c.C = v.C; c.R = v.R; c.warps = warps; c.regs = regs; c.sm_count = sms; c.per_sm = 1;
             // single tile: the whole grid in one CTA, no exchange at all
             if (G + v.C - 1 <= W && G + v.R - 1 <= H) {
-                if (v.persm != 1) continue;
                 const double cost = (double)H * W * 0.135 + 150.0;
                 c.T = 1 << 30; c.halo = 0; c.CW = G; c.CH = G; c.ntx = c.nty = c.ntiles = 1;
                 if (cost < best_cost && finish_plan(c, P.N, smem_cap)) { best_cost = cost; best = c; }
@@ -673,15 +918,13 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
                 if (T_override > 0 && T != T_override) continue;
                 const int halo = 2 * T;
                 int CW, ntx, CH, nty;
-                if (!split(G, W, v.C - 1, halo, CW, ntx) || !split(G, H, v.R - 1, halo, CH, nty)) continue;
+                if (!split(G, W, v.C - 1, halo, 3, CW, ntx) || !split(G, H, v.R - 1, halo, 1, CH, nty)) continue;
                 const int ntiles = ntx * nty;
-                if (ntiles < 2 || ntiles > v.persm * sms) continue;
-                // Cost per sweep in SM cycles, calibrated on B200 at 1025^2 (profiles/): 0.135 cycles per point of the thread
-                // grid(s) an SM holds (the CTAs of an SM share its fp64 pipe), plus one exchange per T sweeps whose cost is
-                // mostly latency (staging, store burst, L2 round trips) and grows with the halo depth.  Two CTAs per SM were
-                // measured NOT to hide each other's exchange (1.95 vs 1.67 us per sweep), so they get no discount.
-                const int ctas = cdiv(ntiles, sms);
-                const double cost = ctas * (double)H * W * 0.135 + (5000.0 + 600.0 * T) / T;
+                if (ntiles < 2 || ntiles > sms) continue;
+                // Cost per sweep in SM cycles, calibrated on B200 (profiles/): 0.135 cycles per point of the thread grid
+                // plus one exchange per T sweeps whose cost is mostly latency (staging, store burst, L2 round trips) and grows
+                // with the halo depth.
+                const double cost = (double)H * W * 0.135 + (5000.0 + 600.0 * T) / T;
                 c.T = T; c.halo = halo; c.CW = CW; c.CH = CH; c.ntx = ntx; c.nty = nty; c.ntiles = ntiles;
                 if (cost < best_cost && finish_plan(c, P.N, smem_cap)) { best_cost = cost; best = c; }
             }
@@ -707,53 +950,61 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
 void resident_describe(const ResidentPlan& pl, char* buf, int len) {
     if (!pl.ok) { std::snprintf(buf, (size_t)len, "none"); return; }
     if (pl.ntiles == 1)
-        std::snprintf(buf, (size_t)len, "1 tile, %d warps x (%dx%d micro-tiles), all sweeps on chip, %d regs, %d B smem",
+        std::snprintf(buf, (size_t)len, "1 tile, %d warps x (%dx%d micro-tiles), whole time steps on chip, %d regs, %d B smem",
                       pl.warps, pl.C, pl.R, pl.regs, pl.smem_bytes);
     else
         std::snprintf(buf, (size_t)len,
                       "%dx%d tiles of %dx%d core + halo %d, T=%d sweeps per exchange, %d warps x (%dx%d micro-tiles), "
-                      "%d+%d exchange units per thread, %d regs, %d B smem, up to %d CTAs per SM on %d SMs",
+                      "%d+%d exchange units (32 B) per thread, %d regs, %d B smem, one CTA per SM on %d SMs",
                       pl.ntx, pl.nty, pl.CW, pl.CH, pl.halo, pl.T, pl.warps, pl.C, pl.R, pl.ns_per, pl.nr_per, pl.regs,
-                      pl.smem_bytes, pl.per_sm, pl.sm_count);
+                      pl.smem_bytes, pl.sm_count);
 }
 
 int resident_variants() { return NVARIANTS; }
 
 size_t resident_table_bytes(const ResidentPlan& pl) {
-    return (pl.ok && pl.ntiles > 1) ? (size_t)pl.ntiles * xtab_bytes(32 * pl.warps, pl.ns_per, pl.nr_per) : 0;
+    return (pl.ok && pl.ntiles > 1) ? (size_t)pl.ntiles * xtab_entries(32 * pl.warps, pl.ns_per, pl.nr_per) * sizeof(uint2) : 0;
 }
 
 int resident_build_tables(const Params& P, const ResidentPlan& pl, void* tables_dev, cudaStream_t st) {
     if (!pl.ok || pl.ntiles <= 1) return 0;
     ResArgs a{};
-    a.N = P.N; a.pitch = P.pitch;
+    a.N = P.N; a.pitch = P.pitch; a.upitch = resident_unit_pitch(P.N);
     a.halo = pl.halo; a.CW = pl.CW; a.CH = pl.CH; a.ntx = pl.ntx; a.nty = pl.nty;
     a.ns_per = pl.ns_per; a.nr_per = pl.nr_per;
     const dim3 grid(pl.ntx, pl.nty), block(32, pl.warps);
-    if (pl.C == 4 && pl.R == 6) k_build_tables<4, 6><<<grid, block, 0, st>>>(a, (unsigned char*)tables_dev);
+    if (pl.C == 4 && pl.R == 6) k_build_tables<4, 6><<<grid, block, 0, st>>>(a, (uint2*)tables_dev);
     else return -(int)cudaErrorNotSupported;
     const cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? 1 : -(int)e;
 }
 
-int resident_sweeps(const Params& P, const ResidentPlan& pl, const double* psi_in, double* psi_out, void* xa, void* xb,
-                    const void* tables, const double* w, unsigned int* err_word, unsigned int* epoch, int nsweeps,
-                    cudaStream_t st, long long* trace_dev, int trace_cap) {
+long long resident_rounds(const ResidentPlan& pl, int nsteps, int S) {
+    if (!pl.ok || pl.ntiles <= 1) return 0;
+    const long long nrounds = (S + pl.T - 1) / pl.T;
+    return nsteps > 0 ? (long long)nsteps * 5 * (nrounds + 1) : std::max(nrounds - 1, 0LL);
+}
+
+int resident_launch(const Params& P, const ResidentPlan& pl, const double* psi_in, double* psi_out, void* xa, void* xb,
+                    const void* tables, double* wbase, size_t fstride, unsigned int* err_word, unsigned int* epoch,
+                    int nsteps, int S, cudaStream_t st, long long* trace_dev, int trace_cap) {
     if (!pl.ok) return -(int)cudaErrorNotSupported;
-    if (nsweeps <= 0 || psi_in == psi_out || (pl.ntiles > 1 && !tables)) return -(int)cudaErrorInvalidValue;
-    ResArgs a;
-    a.tables = (const uint4*)tables;
+    if (nsteps < 0 || S < 0 || (nsteps == 0 && S == 0) || psi_in == psi_out || (pl.ntiles > 1 && (!tables || !xa || !xb)))
+        return -(int)cudaErrorInvalidValue;
+    ResArgs a{};
+    a.tables = (const uint2*)tables;
     a.N = P.N; a.pitch = P.pitch; a.cb = P.cb; a.omb = P.omb; a.cq = P.cq;
-    a.w = w; a.psi_in = psi_in; a.psi_out = psi_out; a.x0 = (uint4*)xa; a.x1 = (uint4*)xb;
+    a.i2h = P.i2h; a.ih2 = P.ih2; a.nu = P.nu; a.c2h2 = P.c2h2; a.lid = P.lid; a.dt = P.dt;
+    a.psi_in = psi_in; a.psi_out = psi_out; a.wbase = wbase; a.fstride = fstride;
+    a.x0 = (ulonglong4*)xa; a.x1 = (ulonglong4*)xb; a.upitch = resident_unit_pitch(P.N);
     a.err = err_word;
     a.base = *epoch;
-    a.nsweeps = nsweeps;
-    a.T = pl.ntiles == 1 ? nsweeps : pl.T;
+    a.nsteps = nsteps; a.S = S;
+    a.T = pl.ntiles == 1 ? std::max(S, 1) : pl.T;
     a.halo = pl.halo; a.CW = pl.CW; a.CH = pl.CH; a.ntx = pl.ntx; a.nty = pl.nty;
     a.ns_per = pl.ns_per; a.nr_per = pl.nr_per;
     a.trace = trace_dev; a.trace_cap = trace_cap;
-    const int nrounds = (nsweeps + a.T - 1) / a.T;
-    *epoch += (unsigned int)nrounds;                // tags base + 1 .. base + nrounds - 1 are used by this launch
+    *epoch += (unsigned int)resident_rounds(pl, nsteps, S);      // wraps harmlessly: tags only tell round r from round r - 2
     void* args[] = {&a};
     const dim3 grid(pl.ntx, pl.nty), block(32, pl.warps);
     const void* fn = pl.fixup ? VARIANTS[pl.variant].fn_fix : VARIANTS[pl.variant].fn;

@@ -1,6 +1,6 @@
-// cavity_resident.cuh — the resident sweep engine (a1): one persistent CTA per tile, psi and the scaled
-// right-hand side held in registers for all S sweeps of a stage, temporal blocking with a 2T-deep halo that
-// is refreshed through L2 every T sweeps as self-validating tagged data (no fence, flag or grid barrier).
+// cavity_resident.cuh — the resident engine: one persistent CTA per tile, psi and the scaled right-hand side held in
+// registers, temporal blocking with a 2T-deep halo that is refreshed through L2 every T sweeps as self-validating tagged
+// data (no fence, flag or grid barrier), a2 + a3 of every stage evaluated in the tile: whole time steps in one launch.
 // See DESIGN.md "Resident engine".  Plain CUDA: no torch types.
 #pragma once
 #include <cuda_runtime.h>
@@ -20,12 +20,12 @@ struct ResidentPlan {
     int CW = 0, CH = 0;   // core (owned) points per tile in x and y; tile (bi, bj) owns [bi CW, (bi+1) CW) x [bj CH, (bj+1) CH)
     int ntx = 0, nty = 0; // tiles in x and y
     int ntiles = 0;
-    int ns_per = 0, nr_per = 0;   // exchange units each thread stores / fetches per round (0 for a single tile)
+    int ns_per = 0, nr_per = 0;   // 32-byte exchange units each thread stores / fetches per round (0 for a single tile)
     bool fixup = false;           // some tile holds both walls of one direction: the kernel variant with the wall-mask fix-up
     int smem_bytes = 0;
     int regs = 0;         // registers per thread of the chosen variant (as compiled)
     int sm_count = 0;
-    int per_sm = 1;       // CTAs per SM the chosen kernel variant is built for
+    int per_sm = 1;       // CTAs per SM
 };
 
 // T_override > 0 forces the sweeps per round (1..8; tests use it to exercise short and ragged rounds);
@@ -34,23 +34,30 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override = 0, int 
 int resident_variants();
 void resident_describe(const ResidentPlan& plan, char* buf, int len);
 
-// Doubles behind ONE exchange buffer (the engine needs two): a 16-byte unit per point of a pitch x (N+1) field.
-inline size_t resident_exchange_doubles(size_t field_doubles) { return 2 * field_doubles; }
+// ONE exchange buffer (the engine needs two, zero-filled before first use and whenever the plan changes): a 32-byte unit
+// per group of three consecutive points of a grid row.
+inline int resident_unit_pitch(int N) { return (N + 1 + 2) / 3; }
+inline size_t resident_exchange_bytes(int N) { return (size_t)resident_unit_pitch(N) * (size_t)(N + 1) * 32; }
 
 // Per-plan exchange tables (device memory, built once per plan): their size, and the kernel that fills them.
 size_t resident_table_bytes(const ResidentPlan& plan);
 int resident_build_tables(const Params& P, const ResidentPlan& plan, void* tables_dev, cudaStream_t st);
 
-// nsweeps red-black sweeps of a1: reads psi_in, writes psi_out (two different fields), right-hand side cq * w (w = the
-// stage's input vorticity, scaled on the fly exactly as scale_rhs does).  xa, xb: the two exchange buffers (zero-filled once
-// by the caller).  tables: what resident_build_tables wrote for this plan (may be null for a single-tile plan).
-// err_word: one device word, zero-filled once; non-zero afterwards = a tile gave up waiting for a neighbour.
-// *epoch is the host-side tag epoch, advanced by this call (tags are unique per round and per launch).
-// trace_dev (profiling only): device array of ntiles x trace_cap %globaltimer stamps (ns), slot 0 = start, 1 = inputs loaded,
-// then per round r: 2 + 4r sweeps done, 3 + 4r border strips stored, 4 + 4r ring received, 5 + 4r edges republished.
+// Halo-exchange rounds one launch performs (the host-side round counter advances by this).
+long long resident_rounds(const ResidentPlan& plan, int nsteps, int S);
+
+// One launch of the resident kernel.
+//   nsteps > 0: nsteps whole SSPRK(5,4) time steps, each 5 x [S sweeps of a1, a2, a3].  wbase points at six fields fstride
+//               doubles apart: omega^n (in: the state; out: the new state, ring = stage-5 Thom ring), omega^(1..4), T.
+//   nsteps = 0: S sweeps of a1 with right-hand side cq * (field 0 of wbase); nothing but psi is written.
+// Reads psi_in, writes psi_out (two different fields).  xa, xb: the two exchange buffers; tables: what resident_build_tables
+// wrote for this plan (all three may be null for a single-tile plan).  err_word: one device word, zero-filled; non-zero
+// afterwards = a tile gave up waiting for a neighbour.  *epoch is the host-side count of exchange rounds, advanced by this call.
+// trace_dev (profiling only, sweeps-only launches): device array of ntiles x trace_cap %globaltimer stamps (ns), slot 0 = start,
+// 1 = inputs loaded, then per round r: 2 + 4r sweeps done, 3 + 4r border strips stored, 4 + 4r ring received, 5 + 4r edges republished.
 // Returns the number of kernel launches (1), or a negative cudaError_t.
-int resident_sweeps(const Params& P, const ResidentPlan& plan, const double* psi_in, double* psi_out, void* xa, void* xb,
-                    const void* tables, const double* w, unsigned int* err_word, unsigned int* epoch, int nsweeps,
-                    cudaStream_t st, long long* trace_dev = nullptr, int trace_cap = 0);
+int resident_launch(const Params& P, const ResidentPlan& plan, const double* psi_in, double* psi_out, void* xa, void* xb,
+                    const void* tables, double* wbase, size_t fstride, unsigned int* err_word, unsigned int* epoch,
+                    int nsteps, int S, cudaStream_t st, long long* trace_dev = nullptr, int trace_cap = 0);
 
 }  // namespace cavk

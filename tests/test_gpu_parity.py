@@ -359,13 +359,13 @@ def test_two_contexts_are_independent(cav):
 
 
 # ------------------------------------------------------------------------------------------------------
-# both compiled variants of the resident kernel (one 16-warp CTA or two 8-warp CTAs per SM), odd and even
-# exchange periods, against the streaming engine bit for bit; and the phase trace
+# the resident kernel with odd and even exchange periods against the streaming engine bit for bit (sweeps-only launches
+# and whole time steps); and the phase trace
 # ------------------------------------------------------------------------------------------------------
 
 @pytest.mark.parametrize("N,S", [(257, 11), (513, 9), (1024, 13)])
-@pytest.mark.parametrize("variant", [0, 1])
-@pytest.mark.parametrize("T", [1, 3, 5, 8])
+@pytest.mark.parametrize("variant", [0])
+@pytest.mark.parametrize("T", [1, 2, 3, 5, 8])
 def test_resident_variants_agree_with_stream_engine(cav, N, S, variant, T):
     psi0, w0 = random_fields(N, 9000 + N + T)
     g = cav.Cavity(N, 2000.0, 0.5 / N, 1.97, S, engine="resident")
@@ -374,7 +374,7 @@ def test_resident_variants_agree_with_stream_engine(cav, N, S, variant, T):
     except cav.CavityError:
         g.close()
         pytest.skip("no plan with T=%d, variant %d for N=%d" % (T, variant, N))
-    assert "T=%d " % T in g.describe() and ("up to %d CTAs per SM" % (variant + 1)) in g.describe()
+    assert "T=%d " % T in g.describe() and "one CTA per SM" in g.describe()
     s = cav.Cavity(N, 2000.0, 0.5 / N, 1.97, S, engine="stream")
     for c in (g, s):
         c.set_fields(psi0, w0)
@@ -401,10 +401,10 @@ def test_trace_sweeps_reports_ordered_phases(cav):
     g.close(); ref.close()
 
 
-@pytest.mark.parametrize("epoch", [0xEFFFFFF0, 0xF0000001, 0xFFFFFF00])
+@pytest.mark.parametrize("epoch", [65535 - 20, 2 * 65535 - 7, 0xFFFFFFF0 - 10, 0x80000000 - 3])
 def test_tag_epoch_restart_near_wrap(cav, epoch):
-    """Exchange tags are 32-bit: well before the epoch wraps the library clears the exchange buffers and restarts it.  Runs
-    across that point (and with tags above 2^31) must stay bit-exact."""
+    """Exchange tags are 16-bit (1 + round mod 65535) and the round counter is 32-bit: runs across the wrap of either (45
+    exchange rounds follow the point the counter is set to) must stay bit-exact."""
     wl = W.config(3)                                   # 513 x 513, multi-tile plan; 9 sweeps per stage: two rounds per launch
     psi0, w0 = W.initial_fields(wl)
     g = cav.Cavity(wl.N, wl.Re, wl.dt, wl.sor_omega, 9, engine="resident")
