@@ -68,9 +68,7 @@ constexpr unsigned int NO_UNIT = 0xffffffffu;
 #define CAV_QROWS 2             // rows of the micro-tile whose q lives in shared memory instead of registers
 #endif
 #ifndef CAV_RECV_BATCH
-#define CAV_RECV_BATCH 1        // ring units (32 bytes, 8 registers each) a thread keeps in flight at a time.  One is enough: 512 threads x 32 B
-                                // in flight per SM already exceed the SM's share of L2 bandwidth x latency; with more, the caller of
-                                // exchange_units keeps q in local memory across the sweeps (ptxas: registers saved around the call)
+#define CAV_RECV_BATCH 3        // ring half-units (16 bytes) a thread keeps in flight at a time, as asynchronous copies into shared memory
 #endif
 
 // SSPRK(5,4) in Shu-Osher form, eq 9-13, readings G1 / G2 (the same table as cavity_kernels.cu, typed here again
@@ -135,36 +133,38 @@ __host__ __device__ inline TileGeom tile_geom(int N, int CW, int CH, int halo, i
     return g;
 }
 
-// ---- one exchanged unit: three doubles in four 64-bit words, each word = 48 payload bits | tag << 48 ----------------
-__device__ __forceinline__ void st_unit(ulonglong4* p, double d0, double d1, double d2, unsigned int tag) {
-    const unsigned long long a = (unsigned long long)__double_as_longlong(d0), b = (unsigned long long)__double_as_longlong(d1),
-                             c = (unsigned long long)__double_as_longlong(d2), t = (unsigned long long)tag << 48;
-    const unsigned long long M48 = 0x0000ffffffffffffull;
-    const unsigned long long w0 = (a & M48) | t;
-    const unsigned long long w1 = (a >> 48) | ((b << 16) & M48) | t;
-    const unsigned long long w2 = (b >> 32) | ((c << 32) & M48) | t;
-    const unsigned long long w3 = (c >> 16) | t;
-    // two 16-byte accesses: on this silicon (B200, driver 580) the 32-byte form st / ld.relaxed.gpu.v4.b64 was observed to
-    // deliver only the first word of a unit (profiles/r2_notes.md); the tags make the split harmless
-    asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"(w0), "l"(w1) : "memory");
-    asm volatile("st.relaxed.gpu.global.v2.b64 [%0+16], {%1, %2};" ::"l"(p), "l"(w2), "l"(w3) : "memory");
+// ---- one exchanged unit: three consecutive doubles of an image row = six 32-bit words c0 .. c5, moved by a PAIR of adjacent
+// lanes, 16 bytes each (one warp instruction covers 512 contiguous bytes: whole 32-byte sectors).  Lane h = 0 takes
+// (A, B, C) = (c0, c1, c2), lane h = 1 takes (c3, c4, c5), and each packs its three words with two copies of the 16-bit tag into
+// two 64-bit elements, tag in the top 16 bits of each:
+//     element 0 = A | (B[15:0] | tag << 16) << 32        element 1 = (B[31:16] | C[15:0] << 16) | (C[31:16] | tag << 16) << 32
+// No word straddles the two lanes, so packing and unpacking are three byte permutes each and need no shuffle.
+struct HalfUnit { unsigned int w0, w1, w2, w3; };      // elements {w0, w1} and {w2, w3}, little endian
+__device__ __forceinline__ HalfUnit half_pack(unsigned int A, unsigned int B, unsigned int C, unsigned int tag) {
+    HalfUnit u;
+    u.w0 = A;
+    u.w1 = __byte_perm(B, tag, 0x5410);        // B[15:0] | tag << 16
+    u.w2 = __byte_perm(B, C, 0x5432);          // B[31:16] | C[15:0] << 16
+    u.w3 = __byte_perm(C, tag, 0x5432);        // C[31:16] | tag << 16
+    return u;
 }
-__device__ __forceinline__ ulonglong4 ld_unit(const ulonglong4* p) {
-    ulonglong4 v;
-    asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "l"(p) : "memory");
-    asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2+16];" : "=l"(v.z), "=l"(v.w) : "l"(p) : "memory");
-    return v;
+__device__ __forceinline__ void half_unpack(const HalfUnit& u, unsigned int& A, unsigned int& B, unsigned int& C) {
+    A = u.w0;
+    B = __byte_perm(u.w1, u.w2, 0x5410);       // w1[15:0] | w2[15:0] << 16
+    C = __byte_perm(u.w2, u.w3, 0x5432);       // w2[31:16] | w3[15:0] << 16
 }
-__device__ __forceinline__ bool unit_ok(const ulonglong4& v, unsigned int tag) {
-    return (unsigned int)(v.x >> 48) == tag && (unsigned int)(v.y >> 48) == tag && (unsigned int)(v.z >> 48) == tag &&
-           (unsigned int)(v.w >> 48) == tag;
+__device__ __forceinline__ void st_half(void* p, const HalfUnit& u) {
+    asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"((unsigned long long)u.w0 | ((unsigned long long)u.w1 << 32)),
+                 "l"((unsigned long long)u.w2 | ((unsigned long long)u.w3 << 32)) : "memory");
 }
-__device__ __forceinline__ void unit_values(const ulonglong4& v, double& d0, double& d1, double& d2) {
-    const unsigned long long M48 = 0x0000ffffffffffffull;
-    d0 = __longlong_as_double((long long)((v.x & M48) | (v.y << 48)));
-    d1 = __longlong_as_double((long long)(((v.y >> 16) & 0xffffffffull) | (v.z << 32)));
-    d2 = __longlong_as_double((long long)(((v.z >> 32) & 0xffffull) | (v.w << 16)));
+__device__ __forceinline__ HalfUnit ld_half(const void* p) {
+    unsigned long long a, b;
+    asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+    HalfUnit u;
+    u.w0 = (unsigned int)a; u.w1 = (unsigned int)(a >> 32); u.w2 = (unsigned int)b; u.w3 = (unsigned int)(b >> 32);
+    return u;
 }
+__device__ __forceinline__ bool half_ok(const HalfUnit& u, unsigned int tag) { return (u.w1 >> 16) == tag && (u.w3 >> 16) == tag; }
 __host__ __device__ inline unsigned int round_tag(unsigned int round) { return 1u + round % 65535u; }
 
 __device__ __forceinline__ long long globaltimer_ns() {
@@ -189,7 +189,6 @@ constexpr unsigned int FL_ZERO_LEFT = 1u;     // the left neighbour column is a 
 constexpr unsigned int FL_ZERO_RIGHT = 2u;    // same on the right
 constexpr unsigned int FL_PUB_BOTTOM = 4u;    // publish the bottom row of the micro-tile to the warp below
 constexpr unsigned int FL_PUB_TOP = 8u;       // publish the top row to the warp above
-constexpr unsigned int FL_ODD = 16u;          // the tile origin has odd parity: local colour = global colour ^ 1
 
 // One colour half-sweep on the register micro-tile.  K = LOCAL colour being updated: local point (ci, rj) has local colour
 // (ci + rj) & 1 (C, R even); the kernel maps the global colour to the local one through the parity of the tile origin.
@@ -346,20 +345,25 @@ __host__ __device__ inline URegion recv_units(const TileGeom& t, int N, int halo
 //   edges   4 (MAXW + 1) C 32            bottom / top rows of the micro-tiles, q of the two middle rows (sized for MAXW warps)
 //   image   H SW                         the tile, row-major: staging area of every exchange, and omega of the stage input during a3
 //   wring   2 SW + 2 H                   first ring of the stage input vorticity around the core (rows below / above, columns left / right)
-//   table   (ns_per + nr_per) nthreads uint2   {unit index in the exchange buffer (NO_UNIT: none), position in the image}
+//   land    2 CAV_RECV_BATCH nthreads    landing zone of the asynchronous ring fetches: 16 bytes per thread and slot
+//   table   (ns_per + nr_per) nthreads / 2 uint2   per pair of lanes: {unit index in the exchange buffer (NO_UNIT: none), position in the image},
+//           then nthreads u32: the rows of the micro-tile that are staged / read back around an exchange
+// uint2 words per tile: the entries, then one 32-bit word per thread: bits 0-5 = micro-tile rows that hold points of units this
+// tile sends (staged before an exchange), bits 8-13 = rows that hold points of units it receives (read back after it)
+__host__ __device__ inline size_t xtab_entries(int nth, int ns_per, int nr_per) { return (size_t)(ns_per + nr_per) * (nth / 2) + (size_t)nth / 2; }
 __host__ __device__ inline size_t smem_layout_bytes(int C, int R, int maxw, int warps, int ns_per, int nr_per) {
     const size_t nth = 32 * (size_t)warps, H = (size_t)R * warps, SW = 32 * (size_t)C;
-    return 8 * ((2 + CAV_QROWS) * (size_t)(maxw + 1) * C * 32 + H * SW + 2 * SW + 2 * H) + 8 * (size_t)(ns_per + nr_per) * nth;
+    return 8 * ((2 + CAV_QROWS) * (size_t)(maxw + 1) * C * 32 + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nth) +
+           8 * xtab_entries((int)nth, ns_per, nr_per);
 }
-__host__ __device__ inline size_t xtab_entries(int nth, int ns_per, int nr_per) { return (size_t)(ns_per + nr_per) * nth; }
 
-// table entry .y: bits 0-7 = local x of the first point + 8, bits 8-15 = local row, bits 16-18 = which of the three points
-// lie inside the image
+// table entry .y: bits 0-15 = index of the unit's first point in the image (row SW + lx) + 8 (lx may be -2: groups are aligned
+// to the grid, not to the tile), bits 16-18 = which of the three points lie inside the image row
 __host__ __device__ inline unsigned int loc_pack(int lx0, int row, int W) {
     unsigned int m = 0;
     for (int j = 0; j < 3; ++j)
         if (lx0 + j >= 0 && lx0 + j < W) m |= 1u << j;
-    return (unsigned int)(lx0 + 8) | ((unsigned int)row << 8) | (m << 16);
+    return (unsigned int)(row * W + lx0 + 8) | (m << 16);
 }
 
 // Builds, once per plan, the exchange tables of every tile in global memory (in the layout the kernel copies to shared
@@ -372,109 +376,150 @@ __global__ void k_build_tables(const ResArgs a, uint2* __restrict__ out) {
     const TileGeom t = tile_geom(N, a.CW, a.CH, a.halo, a.ntx, a.nty, bi, bj, C, R, 32 * C, nwarps * R);
     uint2* const o = out + (size_t)(bj * a.ntx + bi) * xtab_entries(nthreads, a.ns_per, a.nr_per);
     const URegion gs = send_units(t, N, a.halo, bi, bj, a.ntx, a.nty), gr = recv_units(t, N, a.halo);
+    const int npr = nthreads / 2;                                              // one entry per pair of adjacent lanes
     for (int i = 0; i < a.ns_per + a.nr_per; ++i) {
+        if (tid >= npr) break;
         const bool snd = i < a.ns_per;
-        const int u = (snd ? i : i - a.ns_per) * nthreads + tid;
+        const int u = (snd ? i : i - a.ns_per) * npr + tid;
         int g = 0, y = 0;
         uint2 e = make_uint2(NO_UNIT, 0u);
         if (uregion_unit(snd ? gs : gr, u, g, y)) {
             e.x = (unsigned int)(y * a.upitch + g);
             e.y = loc_pack(3 * g - t.ox, y - t.oy, 32 * C);
         }
-        o[(size_t)i * nthreads + tid] = e;
+        o[(size_t)i * npr + tid] = e;
     }
+    unsigned int rows = 0;
+    for (int rj = 0; rj < R; ++rj)
+        for (int ci = 0; ci < C; ++ci) {
+            const int gx = t.ox + lane * C + ci, gy = t.oy + warp * R + rj;
+            if (gx < 0) continue;
+            for (int k = 0; k < 4; ++k) {
+                if (gx / 3 >= gs.r[k].g0 && gx / 3 < gs.r[k].g1 && gy >= gs.r[k].y0 && gy < gs.r[k].y1) rows |= 1u << rj;
+                if (gx / 3 >= gr.r[k].g0 && gx / 3 < gr.r[k].g1 && gy >= gr.r[k].y0 && gy < gr.r[k].y1) rows |= 1u << (8 + rj);
+            }
+        }
+    reinterpret_cast<unsigned int*>(o + (size_t)(a.ns_per + a.nr_per) * npr)[tid] = rows;
 }
 
 // ---- the tile image in shared memory ----------------------------------------------------------------------------
+// Row-major, SW = 32 C doubles per row.
+__host__ __device__ __forceinline__ int img_ix(int row, int lx, int SW) { return row * SW + lx; }
+// rows: bit rj set = row rj of the micro-tile is copied (only the rows that meet the strips / the ring need to move)
 template <int C, int R>
-__device__ __forceinline__ void stage_tile(const double (&v)[R][C], double* __restrict__ img, const int lane, const int warp) {
+__device__ __forceinline__ void stage_tile(const double (&v)[R][C], double* __restrict__ img, const int lane, const int warp,
+                                           const unsigned int rows) {
+    static_assert(C == 4, "two 16-byte chunks per micro-tile row");
     double* const d = img + (warp * R) * (32 * C) + lane * C;
 #pragma unroll
     for (int rj = 0; rj < R; ++rj)
-#pragma unroll
-        for (int ci = 0; ci < C; ci += 2) *reinterpret_cast<double2*>(d + rj * (32 * C) + ci) = make_double2(v[rj][ci], v[rj][ci + 1]);
+        if ((rows >> rj) & 1u) {
+            *reinterpret_cast<double2*>(d + rj * (32 * C)) = make_double2(v[rj][0], v[rj][1]);
+            *reinterpret_cast<double2*>(d + rj * (32 * C) + 2) = make_double2(v[rj][2], v[rj][3]);
+        }
 }
 template <int C, int R>
-__device__ __forceinline__ void read_tile(double (&v)[R][C], const double* __restrict__ img, const int lane, const int warp) {
+__device__ __forceinline__ void read_tile(double (&v)[R][C], const double* __restrict__ img, const int lane, const int warp,
+                                          const unsigned int rows) {
+    static_assert(C == 4, "two 16-byte chunks per micro-tile row");
     const double* const s = img + (warp * R) * (32 * C) + lane * C;
 #pragma unroll
     for (int rj = 0; rj < R; ++rj)
-#pragma unroll
-        for (int ci = 0; ci < C; ci += 2) {
-            const double2 d = *reinterpret_cast<const double2*>(s + rj * (32 * C) + ci);
-            v[rj][ci] = d.x; v[rj][ci + 1] = d.y;
+        if ((rows >> rj) & 1u) {
+            const double2 lo = *reinterpret_cast<const double2*>(s + rj * (32 * C));
+            const double2 hi = *reinterpret_cast<const double2*>(s + rj * (32 * C) + 2);
+            v[rj][0] = lo.x; v[rj][1] = lo.y; v[rj][2] = hi.x; v[rj][3] = hi.y;
         }
 }
 // image <- field g on the interior points of [x0, x1) x [y0, y1) (grid coordinates), +0.0 everywhere else.  Coalesced:
 // consecutive threads = consecutive x.  cg: the field may have been written by this CTA during this launch.
-template <int C>
+template <int C, int R>
 __device__ __forceinline__ void fill_image(double* __restrict__ img, const double* __restrict__ g, const int x0, const int x1,
                                            const int y0, const int y1, const int ox, const int oy, const int H, const int N,
                                            const int pitch, const int tid, const int nth) {
     constexpr int SW = 32 * C;
     const int xa = imax(x0, 1), xb = imin(x1, N), ya = imax(y0, 1), yb = imin(y1, N);
-    for (int k = tid; k < H * SW; k += nth) {
-        const int row = k / SW, lx = k % SW;
-        const int gx = ox + lx, gy = oy + row;
-        double v = 0.0;
-        if (gx >= xa && gx < xb && gy >= ya && gy < yb) v = __ldcg(g + (size_t)gy * pitch + gx);
-        img[k] = v;
+    // H SW = R C nth elements: a fixed trip count, unrolled in batches so that the loads of a batch are in flight together
+    // (an L2 round trip per element, one after the other, would cost more than the whole stage combination)
+    constexpr int BATCH = 8;
+    static_assert((R * C) % BATCH == 0, "whole batches");
+#pragma unroll 1
+    for (int it0 = 0; it0 < R * C; it0 += BATCH) {
+        double v[BATCH];
+#pragma unroll
+        for (int j = 0; j < BATCH; ++j) {
+            const int k = (it0 + j) * nth + tid;
+            const int gx = ox + k % SW, gy = oy + k / SW;
+            v[j] = 0.0;
+            if (gx >= xa && gx < xb && gy >= ya && gy < yb) v[j] = __ldcg(g + (size_t)gy * pitch + gx);
+        }
+#pragma unroll
+        for (int j = 0; j < BATCH; ++j) img[(it0 + j) * nth + tid] = v[j];
     }
 }
 
 // Stores this tile's strip units from the image, fetches its ring units into the image.  All threads; no barrier inside.
 // Not inlined (like rhs_phase below): its registers are allocated apart from the sweep loops, which hold psi and q in
 // registers and have none to spare.
-__device__ __noinline__ void exchange_units(const ResArgs& a, double* __restrict__ img, const uint2* __restrict__ tab,
-                                               const int tid_o, const int nth_o, const unsigned int round, const int SW,
-                                               const int mark_slot) {
-    ulonglong4* const xb = (round & 1u) ? a.x1 : a.x0;
+// Scalar arguments only: a reference to the kernel parameters would be re-read through generic loads after every store.
+// xb: the exchange buffer of this round; stamp: where thread 0 records the time between storing and fetching (or null).
+__device__ __noinline__ void exchange_units(ulonglong4* __restrict__ xb, const unsigned int round, const int ns_per, const int nr_per,
+                                               unsigned int* __restrict__ err, long long* __restrict__ stamp, double* __restrict__ img,
+                                               const uint2* __restrict__ tab, double* __restrict__ land, const int tid_o, const int nth_o,
+                                               const unsigned int tile) {
     const unsigned int tag = round_tag(round);
-    for (int i = 0; i < a.ns_per; ++i) {
-        const uint2 e = tab[i * nth_o + tid_o];
-        if (e.x != NO_UNIT) {
-            const double* const s = img + (int)((e.y >> 8) & 0xffu) * SW + ((int)(e.y & 0xffu) - 8);
-            const double d0 = (e.y & 0x10000u) ? s[0] : 0.0, d1 = (e.y & 0x20000u) ? s[1] : 0.0, d2 = (e.y & 0x40000u) ? s[2] : 0.0;
-            st_unit(xb + e.x, d0, d1, d2, tag);
+    const int h = tid_o & 1, pr = tid_o >> 1, npr = nth_o >> 1;       // half, pair index, pairs in the CTA
+    unsigned int* const img32 = reinterpret_cast<unsigned int*>(img) + 3 * h - 16;      // this lane's three words of a unit start here + 2 loc
+    char* const xbh = reinterpret_cast<char*>(xb) + 16 * h;                            // ... and its 16 bytes of a unit here + 32 unit
+    for (int i = 0; i < ns_per; ++i) {
+        const uint2 e = tab[i * npr + pr];
+        if (e.x != NO_UNIT) {                                          // strip points always lie inside the image: no masks
+            const unsigned int* const s = img32 + 2 * (e.y & 0xffffu);
+            st_half(xbh + 32 * (size_t)e.x, half_pack(s[0], s[1], s[2], tag));
         }
     }
-    mark(a, mark_slot);
-    // All threads fetch ring units (NB in flight per thread), validate, and unpack them into the image.  While some unit of
-    // the warp does not carry the tag yet, ONE lane polls one such unit (waiting tiles do not load L2), then every lane
-    // fetches its missing units again.
+    if (stamp != nullptr && tid_o == 0) *stamp = globaltimer_ns();
+    // All threads fetch ring half-units: NB per thread in flight at a time as 16-byte asynchronous copies into a landing
+    // zone in shared memory (no registers are held while they fly: an L2 round trip for data another SM has just written
+    // costs ~0.5 us here).  A copy is a weak load: it may bring the previous round's bytes, which the tags expose; such
+    // halves are then polled with strong loads: ONE lane of the warp polls one of them (waiting tiles do not load L2),
+    // then every lane fetches its missing halves again.
     constexpr int NB = CAV_RECV_BATCH;
-    const uint2* const tabr = tab + a.ns_per * nth_o;
-    for (int i0 = 0; i0 < a.nr_per; i0 += NB) {
-        uint2 e[NB];
-        ulonglong4 v[NB];
+    const uint2* const tabr = tab + ns_per * npr + pr;
+    HalfUnit* const mine_land = reinterpret_cast<HalfUnit*>(land) + tid_o;                 // slot j of this thread: mine_land[j * nth_o]
+    for (int i0 = 0; i0 < nr_per; i0 += NB) {
         unsigned int bad = 0;
 #pragma unroll
-        for (int j = 0; j < NB; ++j) e[j] = i0 + j < a.nr_per ? tabr[(i0 + j) * nth_o + tid_o] : make_uint2(NO_UNIT, 0u);
+        for (int j = 0; j < NB; ++j) {
+            const unsigned int u = i0 + j < nr_per ? tabr[(i0 + j) * npr].x : NO_UNIT;
+            if (u != NO_UNIT) {
+                const unsigned int dst = (unsigned int)__cvta_generic_to_shared(mine_land + j * nth_o);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(xbh + 32 * (size_t)u) : "memory");
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
 #pragma unroll
-        for (int j = 0; j < NB; ++j)
-            if (e[j].x != NO_UNIT) v[j] = ld_unit(xb + e[j].x);
-#pragma unroll
-        for (int j = 0; j < NB; ++j)
-            if (e[j].x != NO_UNIT && !unit_ok(v[j], tag)) bad |= 1u << j;
+        for (int j = 0; j < NB; ++j) {
+            const unsigned int u = i0 + j < nr_per ? tabr[(i0 + j) * npr].x : NO_UNIT;
+            if (u != NO_UNIT && !half_ok(mine_land[j * nth_o], tag)) bad |= 1u << j;
+        }
         unsigned int waiting = __ballot_sync(0xffffffffu, bad != 0u);
         if (waiting) {
             const long long t0 = clock64();
             while (waiting) {
                 int giveup = 0;
                 if ((int)threadIdx.x == __ffs((int)waiting) - 1) {
-                    unsigned int off = e[NB - 1].x;                // the first missing unit of this lane
-#pragma unroll
-                    for (int j = NB - 2; j >= 0; --j)
-                        if ((bad >> j) & 1u) off = e[j].x;
-                    while (!unit_ok(ld_unit(xb + off), tag)) {
-                        if (*(volatile unsigned int*)a.err != 0u) { giveup = 1; break; }      // some tile gave up: do not wait again
+                    const int j0 = __ffs((int)bad) - 1;            // the first missing half of this lane
+                    const unsigned int off = tabr[(i0 + j0) * npr].x;
+                    while (!half_ok(ld_half(xbh + 32 * (size_t)off), tag)) {
+                        if (*(volatile unsigned int*)err != 0u) { giveup = 1; break; }      // some tile gave up: do not wait again
                         if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) {
-                            if (atomicExch(a.err, 1u) == 0u) {      // the first tile to give up says what it was waiting for (CAV_DEBUG)
-                                const ulonglong4 w = ld_unit(xb + off);
-                                a.err[1] = blockIdx.y * a.ntx + blockIdx.x; a.err[2] = off; a.err[3] = round; a.err[4] = tag;
-                                a.err[5] = (unsigned int)(w.x >> 48); a.err[6] = (unsigned int)(w.y >> 48);
-                                a.err[7] = (unsigned int)(w.z >> 48); a.err[8] = (unsigned int)(w.w >> 48);
-                                a.err[9] = (unsigned int)tid_o;
+                            if (atomicExch(err, 1u) == 0u) {      // the first tile to give up says what it was waiting for (CAV_DEBUG)
+                                const HalfUnit w = ld_half(xbh + 32 * (size_t)off);
+                                err[1] = tile; err[2] = off; err[3] = round; err[4] = tag;
+                                err[5] = w.w1 >> 16; err[6] = w.w3 >> 16; err[7] = (unsigned int)h; err[8] = 0u;
+                                err[9] = (unsigned int)tid_o;
                             }
                             giveup = 1; break;
                         }
@@ -484,22 +529,27 @@ __device__ __noinline__ void exchange_units(const ResArgs& a, double* __restrict
 #pragma unroll
                 for (int j = 0; j < NB; ++j)
                     if ((bad >> j) & 1u) {
-                        v[j] = ld_unit(xb + e[j].x);
-                        if (unit_ok(v[j], tag)) bad &= ~(1u << j);
+                        const HalfUnit v = ld_half(xbh + 32 * (size_t)tabr[(i0 + j) * npr].x);
+                        if (half_ok(v, tag)) { mine_land[j * nth_o] = v; bad &= ~(1u << j); }
                     }
                 waiting = __ballot_sync(0xffffffffu, bad != 0u);
             }
         }
 #pragma unroll
-        for (int j = 0; j < NB; ++j)
-            if (e[j].x != NO_UNIT) {
-                double d0, d1, d2;
-                unit_values(v[j], d0, d1, d2);
-                double* const s = img + (int)((e[j].y >> 8) & 0xffu) * SW + ((int)(e[j].y & 0xffu) - 8);
-                if (e[j].y & 0x10000u) s[0] = d0;
-                if (e[j].y & 0x20000u) s[1] = d1;
-                if (e[j].y & 0x40000u) s[2] = d2;
+        for (int j = 0; j < NB; ++j) {
+            const uint2 e = i0 + j < nr_per ? tabr[(i0 + j) * npr] : make_uint2(NO_UNIT, 0u);
+            if (e.x != NO_UNIT) {
+                unsigned int A, B, C;
+                half_unpack(mine_land[j * nth_o], A, B, C);
+                unsigned int* const d = img32 + 2 * (e.y & 0xffffu);
+                // words 0 1 | 2 of lane 0 belong to points 0 | 1 of the unit, words 0 | 1 2 of lane 1 to points 1 | 2; bits 16-18 of
+                // the entry say which points lie inside the image
+                const unsigned int m = e.y >> (16 + h);
+                if (m & 1u) d[0] = A;
+                if (h ? (m & 2u) : (m & 1u)) d[1] = B;
+                if (m & 2u) d[2] = C;
             }
+        }
     }
 }
 
@@ -510,12 +560,13 @@ __device__ __forceinline__ double thom_lid(double c2h2, double lid, double p_adj
 // image holds the NEW vorticity on core + halo (+0.0 elsewhere) and the ring copy is refreshed; the caller turns it into q.
 // Not inlined: see exchange_units.
 template <int C, int R, int MAXW>
-__device__ __noinline__ void rhs_phase(const ResArgs& a, const double* __restrict__ pl, double* __restrict__ sm, const int stage,
+__device__ __noinline__ void rhs_phase(const ResArgs& a_, const double* __restrict__ pl, double* __restrict__ sm, const int stage,
                                        const unsigned int round, const unsigned int fl) {
     constexpr int TOPOFF = (MAXW + 1) * C * 32;
     constexpr int SW = 32 * C;
     constexpr int edge_doubles = (2 + CAV_QROWS) * TOPOFF;
     double* const sB = sm + (int)threadIdx.y * C * 32 + (int)threadIdx.x;
+    const ResArgs a = a_;             // a local copy: the fields are read once, not again after every store or barrier
     {
     const int z = opaque_zero();
     const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
@@ -537,22 +588,22 @@ __device__ __noinline__ void rhs_phase(const ResArgs& a, const double* __restric
     // (1) the image receives the stage input: core from the tile's own global buffer, first ring from the copy kept
     //     since the last vorticity exchange, walls next to the core from Thom's formula (written by the owner of the
     //     adjacent point, who also stores it to the ring of the stage output: k_rk_stage does the same).
-    fill_image<C>(img, win, X0, X1, Y0, Y1, te.ox, te.oy, H, Ne, pitch, tid_o, nth_o);
+    fill_image<C, R>(img, win, X0, X1, Y0, Y1, te.ox, te.oy, H, Ne, pitch, tid_o, nth_o);
     __syncthreads();              // fill_image writes zeros everywhere else: the ring and wall writers come after it
     {
         const int rB = Y0 - 1 - te.oy, rT = Y1 - te.oy, cL = X0 - 1 - te.ox, cR = X1 - te.ox;
         for (int c = tid_o; c < SW; c += nth_o) {
             const int gx = te.ox + c;
             if (gx >= X0 && gx < X1) {
-                if (Y0 - 1 >= 1) img[rB * SW + c] = wr[c];
-                if (Y1 <= Ne - 1) img[rT * SW + c] = wr[SW + c];
+                if (Y0 - 1 >= 1) img[img_ix(rB, c, SW)] = wr[c];
+                if (Y1 <= Ne - 1) img[img_ix(rT, c, SW)] = wr[SW + c];
             }
         }
         for (int r2 = tid_o; r2 < H; r2 += nth_o) {
             const int gy = te.oy + r2;
             if (gy >= Y0 && gy < Y1) {
-                if (X0 - 1 >= 1) img[r2 * SW + cL] = wr[2 * SW + r2];
-                if (X1 <= Ne - 1) img[r2 * SW + cR] = wr[2 * SW + H + r2];
+                if (X0 - 1 >= 1) img[img_ix(r2, cL, SW)] = wr[2 * SW + r2];
+                if (X1 <= Ne - 1) img[img_ix(r2, cR, SW)] = wr[2 * SW + H + r2];
             }
         }
     }
@@ -563,17 +614,17 @@ __device__ __noinline__ void rhs_phase(const ResArgs& a, const double* __restric
             for (int ci = 0; ci < C; ++ci) {
                 const int gx = gx0 + ci, gy = gy0 + rj;
                 if (gx < X0 || gx >= X1 || gy < Y0 || gy >= Y1) continue;
-                double* const ic = img + (row0 + rj) * SW + lx0 + ci;
+                const int ir_ = row0 + rj, ix_ = lx0 + ci;
                 const double pv = pl[rj * C + ci];
-                if (gx == 1) { const double v = thom_wall(a.c2h2, pv); ic[-1] = v; wout[(size_t)gy * pitch] = v; }
-                if (gx == Ne - 1) { const double v = thom_wall(a.c2h2, pv); ic[1] = v; wout[(size_t)gy * pitch + Ne] = v; }
+                if (gx == 1) { const double v = thom_wall(a.c2h2, pv); img[img_ix(ir_, ix_ - 1, SW)] = v; wout[(size_t)gy * pitch] = v; }
+                if (gx == Ne - 1) { const double v = thom_wall(a.c2h2, pv); img[img_ix(ir_, ix_ + 1, SW)] = v; wout[(size_t)gy * pitch + Ne] = v; }
                 if (gy == 1) {
-                    const double v = thom_wall(a.c2h2, pv); ic[-SW] = v; wout[gx] = v;
+                    const double v = thom_wall(a.c2h2, pv); img[img_ix(ir_ - 1, ix_, SW)] = v; wout[gx] = v;
                     if (gx == 1) wout[0] = thom_wall(a.c2h2, 0.0);                      // the bottom and top rows own the corners (G10)
                     if (gx == Ne - 1) wout[Ne] = thom_wall(a.c2h2, 0.0);
                 }
                 if (gy == Ne - 1) {
-                    const double v = thom_lid(a.c2h2, a.lid, pv); ic[SW] = v; wout[(size_t)Ne * pitch + gx] = v;
+                    const double v = thom_lid(a.c2h2, a.lid, pv); img[img_ix(ir_ + 1, ix_, SW)] = v; wout[(size_t)Ne * pitch + gx] = v;
                     if (gx == 1) wout[(size_t)Ne * pitch] = thom_lid(a.c2h2, a.lid, 0.0);
                     if (gx == Ne - 1) wout[(size_t)Ne * pitch + Ne] = thom_lid(a.c2h2, a.lid, 0.0);
                 }
@@ -593,12 +644,13 @@ __device__ __noinline__ void rhs_phase(const ResArgs& a, const double* __restric
         if (fl & FL_ZERO_RIGHT) rnb = 0.0;
         if (gx0 + C - 1 < X0 || gx0 >= X1) continue;
         double wc[C + 2], ws[C], wn[C];
-        wc[0] = ir[-1]; wc[C + 1] = ir[C];
+        wc[0] = img[img_ix(row0 + rj, lx0 - 1, SW)]; wc[C + 1] = img[img_ix(row0 + rj, lx0 + C, SW)];
 #pragma unroll
         for (int ci = 0; ci < C; ci += 2) {
-            const double2 c2 = *reinterpret_cast<const double2*>(ir + ci);
-            const double2 s2 = *reinterpret_cast<const double2*>(ir - SW + ci);
-            const double2 n2 = *reinterpret_cast<const double2*>(ir + SW + ci);
+            const int o = ci;
+            const double2 c2 = *reinterpret_cast<const double2*>(ir + o);
+            const double2 s2 = *reinterpret_cast<const double2*>(ir - SW + o);
+            const double2 n2 = *reinterpret_cast<const double2*>(ir + SW + o);
             wc[1 + ci] = c2.x; wc[2 + ci] = c2.y; ws[ci] = s2.x; ws[ci + 1] = s2.y; wn[ci] = n2.x; wn[ci + 1] = n2.y;
         }
 #pragma unroll
@@ -638,18 +690,20 @@ __device__ __noinline__ void rhs_phase(const ResArgs& a, const double* __restric
     __syncthreads();              // every read of the image and every store of the stage output is done
 
     // (3) the new vorticity: core from the global buffer just written, ring from the neighbours, q = cq w
-    fill_image<C>(img, wout, X0, X1, Y0, Y1, te.ox, te.oy, H, Ne, pitch, tid_o, nth_o);
+    fill_image<C, R>(img, wout, X0, X1, Y0, Y1, te.ox, te.oy, H, Ne, pitch, tid_o, nth_o);
     __syncthreads();
     if (a.ntx * a.nty > 1) {
-        const uint2* const tab = reinterpret_cast<const uint2*>(img + H * SW + 2 * SW + 2 * H);
-        exchange_units(a, img, tab, tid_o, nth_o, round, SW, a.trace_cap);
+        double* const land = img + H * SW + 2 * SW + 2 * H;
+        const uint2* const tab = reinterpret_cast<const uint2*>(land + 2 * CAV_RECV_BATCH * nth_o);
+        exchange_units((round & 1u) ? a.x1 : a.x0, round, a.ns_per, a.nr_per, a.err, nullptr, img, tab, land, tid_o, nth_o,
+                       blockIdx.y * a.ntx + blockIdx.x);
         __syncthreads();
     }
     {   // first ring of the new vorticity around the core, kept for a3 of the next stage
         double* const wrw = img + H * SW;
         const int rB = Y0 - 1 - te.oy, rT = Y1 - te.oy, cL = X0 - 1 - te.ox, cR = X1 - te.ox;
-        for (int c = tid_o; c < SW; c += nth_o) { wrw[c] = img[rB * SW + c]; wrw[SW + c] = img[rT * SW + c]; }
-        for (int r2 = tid_o; r2 < H; r2 += nth_o) { wrw[2 * SW + r2] = img[r2 * SW + cL]; wrw[2 * SW + H + r2] = img[r2 * SW + cR]; }
+        for (int c = tid_o; c < SW; c += nth_o) { wrw[c] = img[img_ix(rB, c, SW)]; wrw[SW + c] = img[img_ix(rT, c, SW)]; }
+        for (int r2 = tid_o; r2 < H; r2 += nth_o) { wrw[2 * SW + r2] = img[img_ix(r2, cL, SW)]; wrw[2 * SW + H + r2] = img[img_ix(r2, cR, SW)]; }
     }
     }
 }
@@ -674,8 +728,10 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
 
     const TileGeom t = tile_geom(N, a.CW, a.CH, a.halo, a.ntx, a.nty, bi, bj, C, R, SW, nwarps * R);
     const int gx0_ = t.ox + lane * C, gy0_ = t.oy + warp * R;
+    // local colour = global colour ^ odd_origin.  Computed from blockIdx only: the branch on it is uniform for the compiler
+    // too, so the sweep loops stay convergent code (uniform registers for the coefficients, no divergence guards on the shuffles)
+    const bool odd_origin = ((t.ox + t.oy) & 1) != 0;
     unsigned int fl = FL_PUB_BOTTOM | FL_PUB_TOP;
-    if ((t.ox + t.oy) & 1) fl |= FL_ODD;                                       // local colour = global colour ^ 1
     {
         const int lzl = t.left_al ? 1 : 0;                                     // lane 0 holds x = -(C-1) .. 0
         const int lzr = t.right_al ? (N - t.ox) / C - 1 : 31;                  // lane (N - ox) / C holds x = N .. N + C - 1
@@ -688,7 +744,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
     // ---- exchange tables (multi-tile plans only): copied from the per-plan tables in global memory ----
     {
         const int H = nwarps * R;
-        uint2* const tabs = reinterpret_cast<uint2*>(sm + edge_doubles + H * SW + 2 * SW + 2 * H);
+        uint2* const tabs = reinterpret_cast<uint2*>(sm + edge_doubles + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nthreads);
         if (a.ntx * a.nty > 1) {
             const int n = (int)xtab_entries(nthreads, a.ns_per, a.nr_per);
             const uint2* const src = a.tables + (size_t)(bj * a.ntx + bi) * n;
@@ -702,18 +758,18 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
     {
         const int H = nwarps * R;
         double* const img = sm + edge_doubles;
-        fill_image<C>(img, a.psi_in, 0, N + 1, 0, N + 1, t.ox, t.oy, H, N, a.pitch, tid, nthreads);
+        fill_image<C, R>(img, a.psi_in, 0, N + 1, 0, N + 1, t.ox, t.oy, H, N, a.pitch, tid, nthreads);
         __syncthreads();
-        read_tile<C, R>(p, img, lane, warp);
+        read_tile<C, R>(p, img, lane, warp, 0x3fu);
         __syncthreads();
-        fill_image<C>(img, a.wbase, 0, N + 1, 0, N + 1, t.ox, t.oy, H, N, a.pitch, tid, nthreads);
+        fill_image<C, R>(img, a.wbase, 0, N + 1, 0, N + 1, t.ox, t.oy, H, N, a.pitch, tid, nthreads);
         __syncthreads();
-        read_tile<C, R>(q, img, lane, warp);
+        read_tile<C, R>(q, img, lane, warp, 0x3fu);
         if (a.nsteps > 0) {               // first ring of the stage input around the core, kept for a3
             double* const wr = img + H * SW;
             const int rB = imax(t.cy0, 1) - 1 - t.oy, rT = imin(t.cy1, N) - t.oy, cL = imax(t.cx0, 1) - 1 - t.ox, cR = imin(t.cx1, N) - t.ox;
-            for (int k = tid; k < SW; k += nthreads) { wr[k] = img[rB * SW + k]; wr[SW + k] = img[rT * SW + k]; }
-            for (int k = tid; k < H; k += nthreads) { wr[2 * SW + k] = img[k * SW + cL]; wr[2 * SW + H + k] = img[k * SW + cR]; }
+            for (int k = tid; k < SW; k += nthreads) { wr[k] = img[img_ix(rB, k, SW)]; wr[SW + k] = img[img_ix(rT, k, SW)]; }
+            for (int k = tid; k < H; k += nthreads) { wr[2 * SW + k] = img[img_ix(k, cL, SW)]; wr[2 * SW + H + k] = img[img_ix(k, cR, SW)]; }
         }
     }
 #pragma unroll
@@ -745,7 +801,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
     for (int stage = 0; stage < (a.nsteps > 0 ? 5 * a.nsteps : 1); ++stage) {
         // ================= a1: S sweeps, a halo exchange after every T of them =================
         for (int rem = a.S; rem > 0; rem -= a.T) {
-            if (fl & FL_ODD) {
+            if (odd_origin) {
                 for (int s = min(a.T, rem); s > 0; --s) {                         // red = (i + j) even first (G9): local colour 1 here
                     half_sweep<C, R, 1, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
                     half_sweep<C, R, 0, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
@@ -767,14 +823,18 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
             const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
             const int nw = (int)blockDim.y + z, tid_o = wp * 32 + ln, nth_o = nw * 32, H = nw * R;
             double* const img = sm + edge_doubles;
-            const uint2* const tab = reinterpret_cast<const uint2*>(img + H * SW + 2 * SW + 2 * H);
-            stage_tile<C, R>(p, img, ln, wp);
+            double* const land = img + H * SW + 2 * SW + 2 * H;
+            const uint2* const tab = reinterpret_cast<const uint2*>(land + 2 * CAV_RECV_BATCH * nth_o);
+            const unsigned int rows = reinterpret_cast<const unsigned int*>(tab + (a.ns_per + a.nr_per) * (nth_o >> 1))[tid_o];
+            stage_tile<C, R>(p, img, ln, wp, rows);
             __syncthreads();
-            exchange_units(a, img, tab, tid_o, nth_o, round, SW, tslot + 1);
+            exchange_units((round & 1u) ? a.x1 : a.x0, round, a.ns_per, a.nr_per, a.err,
+                           (a.trace != nullptr && tslot + 1 < a.trace_cap) ? a.trace + (size_t)(blockIdx.y * a.ntx + blockIdx.x) * a.trace_cap + tslot + 1 : nullptr,
+                           img, tab, land, tid_o, nth_o, blockIdx.y * a.ntx + blockIdx.x);
             ++round;
             __syncthreads();
             mark(a, tslot + 2);
-            read_tile<C, R>(p, img, ln, wp);
+            read_tile<C, R>(p, img, ln, wp, rows >> 8);
             publish_all<C, R, TOPOFF>(p, sB, fl);
             mark(a, tslot + 3);
         }
@@ -792,7 +852,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
             const int z = opaque_zero();
             const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
             double* const img = sm + edge_doubles;
-            read_tile<C, R>(q, img, ln, wp);
+            read_tile<C, R>(q, img, ln, wp, 0x3fu);
 #pragma unroll
             for (int rj = 0; rj < R; ++rj)
 #pragma unroll
@@ -814,13 +874,13 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
         const int Ne = a.N + z;
         const TileGeom te = tile_geom(Ne, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, H);
         double* const img = sm + edge_doubles;
-        stage_tile<C, R>(p, img, ln, wp);
+        stage_tile<C, R>(p, img, ln, wp, 0x3fu);
         __syncthreads();
         const int cw = te.cx1 - te.cx0, ch = te.cy1 - te.cy0;
         for (int k = tid_o; k < cw * ch; k += nth_o) {
             const int gy = te.cy0 + k / cw, gx = te.cx0 + k % cw;
             const bool inter = gx >= 1 && gx <= Ne - 1 && gy >= 1 && gy <= Ne - 1;
-            a.psi_out[(size_t)gy * a.pitch + gx] = inter ? img[(gy - te.oy) * SW + (gx - te.ox)] : 0.0;
+            a.psi_out[(size_t)gy * a.pitch + gx] = inter ? img[img_ix(gy - te.oy, gx - te.ox, SW)] : 0.0;
         }
     }
 }
@@ -852,8 +912,8 @@ bool finish_plan(ResidentPlan& pl, int N, int max_smem) {
                 rmax = std::max(rmax, uregion_total(recv_units(t, N, pl.halo)));
             }
         }
-    pl.ns_per = cdiv(smax, nth);
-    pl.nr_per = cdiv(rmax, nth);
+    pl.ns_per = cdiv(smax, nth / 2);         // units per PAIR of lanes (a lane moves one 16-byte half of each)
+    pl.nr_per = cdiv(rmax, nth / 2);
     const int maxw = VARIANTS[pl.variant].maxw;
     const size_t smem = smem_layout_bytes(pl.C, pl.R, maxw, pl.warps, pl.ns_per, pl.nr_per);
     pl.fixup = pl.ntx == 1 || pl.nty == 1;
@@ -955,7 +1015,7 @@ void resident_describe(const ResidentPlan& pl, char* buf, int len) {
     else
         std::snprintf(buf, (size_t)len,
                       "%dx%d tiles of %dx%d core + halo %d, T=%d sweeps per exchange, %d warps x (%dx%d micro-tiles), "
-                      "%d+%d exchange units (32 B) per thread, %d regs, %d B smem, one CTA per SM on %d SMs",
+                      "%d+%d exchange half-units (16 B) per thread, %d regs, %d B smem, one CTA per SM on %d SMs",
                       pl.ntx, pl.nty, pl.CW, pl.CH, pl.halo, pl.T, pl.warps, pl.C, pl.R, pl.ns_per, pl.nr_per, pl.regs,
                       pl.smem_bytes, pl.sm_count);
 }
