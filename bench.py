@@ -10,17 +10,22 @@ target is quoted on.  Metric: fp64 grid-point-stage updates per second, GPSU/s =
 (Poisson sweeps included).
 
 One JSON line on stdout (rank 0).  Keys beyond the base contract:
-  roofline      the dominant kernel (the a1 sweep kernel), measured live with CUDA events around sweep-only
-                launches (cav_poisson): SURVEY.md S8(d) item 2 bytes (24 B per point-sweep, what a
-                one-pass-per-sweep streaming kernel must move) / average launch duration, against the measured
-                HBM copy peak of MEASURED_PEAKS.json.  Temporal blocking moves fewer bytes than that, so the
-                fraction may exceed 1; `alu` then gives the bound that is left (fp64 pipe utilisation).
+  roofline      the dominant kernel (k_resident: one launch = one whole time step), bound "alu": the path is bound by the fp64
+                pipe, not by HBM (with the sweeps fused the working set stays on chip).
+                achieved = algorithmic fp64 instructions per launch (5 per point-sweep + 30 per point-stage)
+                / the launch's CUDA-event duration; peak = the DFMA-chain rate MEASURED in the same run
+                (cav_measure_fp64_peak), the nominal 148 SMs x 64 lanes x clock beside it; traffic = DRAM bytes per launch from
+                the ncu capture in profiles/, with the DRAM GB/s that follows.  `sweeps_only` repeats it for a1 alone
+                (cav_poisson launches), `hbm_streaming_equiv` keeps BASELINE's "% of HBM bandwidth" reading as a secondary,
+                clearly labelled figure (bytes a one-pass-per-sweep kernel would move; this kernel does not move them).
+  other_configs / poisson_only   configs 1, 2, 3, 5 with bounded step counts, and the 10 000-sweep Poisson-only run of config 5.
   cpu_baseline  the oracle (oracle/, single thread, as it stands) timed on this box on a bounded sample.
   e2e           the same metric through the C ABI with HOST buffers every step (cav_set_fields from pinned
                 memory -> cav_step(1) -> cav_get_fields), copies inside the timed region.
 
 --impl reference times the CPU oracle instead (there is no reference implementation of the paper).
-N > 1: replicas only (one independent context per GPU, no data-path collective).
+N > 1: replicas only (one independent context per GPU, no data-path collective).  Launched by
+torchrun (RANK / WORLD_SIZE in the environment) or bare: `python bench.py --gpus N` then spawns the N ranks itself.
 """
 import argparse
 import json
@@ -40,10 +45,11 @@ UNIT = "GPSU/s"
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 SM_COUNT, FP64_LANES_PER_SM = 148, 64   # B200: 148 SMs x 64 fp64 lanes
 FP64_INSTR_PER_POINT_SWEEP = 5     # 3 DADD + 2 DFMA
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_resident launch (200 sweeps at 1025^2) from the ncu --set full capture
-# summarised in profiles/ (cold L2 under ncu: psi and omega are read once, the result stays in L2)
-NCU_DRAM_BYTES_PER_LAUNCH = 26.6e6
-NCU_DRAM_SOURCE = "profiles/r1c_final.md (ncu --set full, one launch of 200 sweeps)"
+FP64_INSTR_PER_POINT_STAGE = 30    # a2 + a3 ("5 S + 30 fp64 instructions per grid-point-stage")
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_resident launch (one time step of config 4) from the ncu --set full
+# capture summarised in profiles/ (cold L2 under ncu); None until that capture exists for the build
+NCU_DRAM_BYTES_PER_STEP_LAUNCH = None
+NCU_DRAM_SOURCE = "profiles/r2_final.md (ncu --set full, one launch = one time step of config 4)"
 
 
 def parse():
@@ -56,6 +62,7 @@ def parse():
     ap.add_argument("--engine", default="auto", choices=["auto", "stream", "resident"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-others", action="store_true", help="skip the other configs and the Poisson-only run")
     return ap.parse_args()
 
 
@@ -269,41 +276,84 @@ def run_ours(args, wl, rank, world, local_rank):
         e2e = {"value": ue / tmax_e, "unit": UNIT, "h2d_bytes_per_step": 2 * G * 8, "d2h_bytes_per_step": 2 * G * 8,
                "ms_per_step": 1e3 * tmax_e / Ke, "api": "cav_set_fields(host) -> cav_step(1) -> cav_get_fields(host)"}
 
-    # ---- roofline of the dominant kernel (the a1 sweep kernel), measured live: sweep-only launches of the SAME shape as
-    # inside a step (S sweeps per launch), CUDA events of the library around the a1 launches alone (cav_last_elapsed_ms) ----
+    # ---- roofline of the dominant kernel, measured live.  k_resident runs a whole time step per launch: the per-step CUDA
+    # events above ARE its launch durations.  Bound: the fp64 pipe; peak: a DFMA-chain kernel timed now.
     hbm_gbs, peak_src, sm_max_mhz = measured_peaks()
     desc = cav.describe()
-    extra = 2 if "engine stream" in desc else 1     # cav_poisson also launches Thom (and, streaming engine, the q scaling)
+    resident = "engine resident" in desc
+    dfma_peak, nominal_mhz = cav.measure_fp64_peak()
+    fp64_nominal = SM_COUNT * FP64_LANES_PER_SM * sm_max_mhz * 1e6
+    launches_per_step = launches / float(K)
+    instr_per_step = 5.0 * P * (FP64_INSTR_PER_POINT_SWEEP * S + FP64_INSTR_PER_POINT_STAGE)
+    step_s = statistics.mean(per_step_ms) * 1e-3
+    achieved = instr_per_step / step_s
+    # a1 alone: sweep-only launches of the step's own shape (S sweeps), timed by the library's events around the a1 launch
+    extra = 2 if not resident else 1                # cav_poisson also launches Thom (and, streaming engine, the q scaling)
     for _ in range(3):
         cav.poisson(S, want_residual=False)
     reps, tsw, lsw = 25, 0.0, 0
     for k in range(reps):
         if k % 5 == 0:
-            flush.fill_(1)                          # as in a time step: 5 launches per L2 flush
+            flush.fill_(1)
         l1 = cav.launch_count()
         cav.poisson(S, want_residual=False)
         tsw += cav.last_elapsed_ms() * 1e-3
         lsw += cav.launch_count() - l1 - extra
-    launches_per_call = lsw / reps                   # 1 (resident engine) or 2 S (streaming engine)
-    bytes_per_launch = 24.0 * P * S / launches_per_call      # 24 B per point-sweep
-    avg_launch_s = tsw / lsw
-    achieved = bytes_per_launch / avg_launch_s / 1e9
-    sweep_share = 5.0 * (tsw / reps) / (statistics.mean(per_step_ms) * 1e-3)
-    fp64_rate = FP64_INSTR_PER_POINT_SWEEP * P * S * reps / tsw
-    fp64_peak_max = SM_COUNT * FP64_LANES_PER_SM * sm_max_mhz * 1e6
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
-                "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (wl.N == 1024 and S == 200 and "resident" in desc) else None,
-                "traffic_source": NCU_DRAM_SOURCE, "peak_source": peak_src, "kernel": "a1 sweep kernel, " + desc,
-                "bytes_model": "24 B per point-sweep x (N-1)^2 x sweeps per launch (streaming-equivalent, SURVEY S8(d) item 2); "
-                               "temporal blocking moves fewer bytes, so frac > 1: the binding roofline is `alu`",
-                "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_us": 1e6 * avg_launch_s,
-                "launches_per_step": 5.0 * launches_per_call, "share_of_step": sweep_share,
-                "alu": {"bound": "alu", "achieved": fp64_rate / 1e12, "peak": fp64_peak_max / 1e12,
-                        "unit": "T fp64 instr/s", "frac": fp64_rate / fp64_peak_max,
-                        "model": "5 fp64 instr per point-sweep; peak = 148 SMs x 64 lanes x sm_max_mhz (DESIGN.md section 6)"}}
+    sweep_rate = FP64_INSTR_PER_POINT_SWEEP * P * S * reps / tsw
+    traffic = NCU_DRAM_BYTES_PER_STEP_LAUNCH if (wl.N == 1024 and S == 200 and resident) else None
+    roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": dfma_peak / 1e12, "unit": "T fp64 instr/s",
+                "frac": achieved / dfma_peak, "traffic": traffic, "traffic_source": NCU_DRAM_SOURCE if traffic else None,
+                "dram_GBps": (traffic / step_s / 1e9) if traffic else None,
+                "peak_source": "measured in this run: DFMA-chain kernel, 16 warps per SM, 8 chains per thread (cav_measure_fp64_peak)",
+                "peak_nominal": fp64_nominal / 1e12, "peak_nominal_model": "148 SMs x 64 fp64 lanes x sm_max_mhz",
+                "frac_of_nominal": achieved / fp64_nominal,
+                "kernel": ("k_resident, one launch per time step; " if resident else "") + desc,
+                "instr_model": "5 fp64 instr per point-sweep (3 DADD + 2 DFMA) + 30 per grid-point-stage (a2 + a3), interior points, "
+                               "useful work only (the redundant halo work of temporal blocking is not counted)",
+                "algorithmic_instr_per_launch": instr_per_step / launches_per_step, "avg_launch_us": 1e6 * step_s / launches_per_step,
+                "launches_per_step": launches_per_step,
+                "sweeps_only": {"achieved": sweep_rate / 1e12, "frac": sweep_rate / dfma_peak, "avg_call_us": 1e6 * tsw / reps,
+                                "launches_per_call": lsw / reps, "us_per_sweep": 1e6 * tsw / reps / S,
+                                "share_of_step": 5.0 * (tsw / reps) / step_s,
+                                "note": "S sweeps of a1 alone per cav_poisson call, timed by the library's CUDA events"}}
     b0 = 24.0 * S + 33.6
     hbm_equiv = value / max(world, 1) * b0 / 1e9
-    cav.close()
+
+    # ---- the other configs (bounded step counts) and the Poisson-only run of config 5 (BASELINE.json configs[4]) ----
+    others, poisson_only = None, None
+    if rank == 0 and world == 1 and not args.no_others:
+        cav.close()
+        others = {}
+        for kcfg in (1, 2, 3, 5):
+            if kcfg == args.config:
+                continue
+            w2 = W.config(kcfg)
+            c2 = binding.Cavity(w2.N, w2.Re, w2.dt, w2.sor_omega, w2.sweeps_per_stage, engine=args.engine)
+            c2.set_fields(*W.initial_fields(w2))
+            if w2.poisson_sweeps:
+                # the Poisson-only sweep-throughput run: 10 000 sweeps on the restart field, timed by the library's events
+                c2.poisson(200, want_residual=False)
+                c2.set_fields(*W.initial_fields(w2))
+                c2.poisson(w2.poisson_sweeps, want_residual=False)
+                tp = c2.last_elapsed_ms() * 1e-3
+                poisson_only = {"workload": w2.name, "sweeps": w2.poisson_sweeps, "seconds": tp,
+                                "point_sweeps_per_s": (w2.N - 1) ** 2 * w2.poisson_sweeps / tp,
+                                "us_per_sweep": 1e6 * tp / w2.poisson_sweeps,
+                                "residual_inf_after": c2.diag()["res_inf"]}
+            nst = {1: 400, 2: 200, 3: 100, 5: 50}[kcfg]
+            c2.step(5)
+            ts = []
+            for _ in range(3):
+                c2.step(nst)
+                ts.append(c2.last_elapsed_ms() * 1e-3 / nst)
+            t1 = min(ts)
+            others["cfg%d" % kcfg] = {"workload": w2.name, "ms_per_step": 1e3 * t1, "GPSU_per_s": 5.0 * (w2.N + 1) ** 2 / t1,
+                                      "steps_timed": nst, "timing": "best of 3 cav_step(%d) calls, CUDA events of the library, "
+                                      "device-resident, L2 not flushed (the working set is on chip)" % nst,
+                                      "plan": c2.describe()}
+            c2.close()
+    else:
+        cav.close()
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": 1e3 * t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -316,8 +366,12 @@ def run_ours(args, wl, rank, world, local_rank):
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "hbm_streaming_equiv": {"bytes_per_gpsu": b0, "GBps_per_gpu": hbm_equiv, "frac_of_measured_peak": hbm_equiv / hbm_gbs,
                                     "frac_of_8TBps_nominal": hbm_equiv / 8000.0,
-                                    "note": "BASELINE target: >= 0.70 of nominal for the full step at 1025^2"},
-            "ms_per_step_min": min(per_step_ms), "ms_per_step_median": statistics.median(per_step_ms)}
+                                    "note": "SECONDARY figure: bytes a one-pass-per-sweep streaming kernel would move (24 S + 33.6 per "
+                                            "grid-point-stage, SURVEY S8(d) item 2) x the measured rate.  The resident kernel does "
+                                            "NOT move them (see roofline.traffic): BASELINE's >= 0.70 HBM target does not apply to a "
+                                            "temporally blocked kernel; the binding roofline is roofline (alu)"},
+            "ms_per_step_min": min(per_step_ms), "ms_per_step_median": statistics.median(per_step_ms),
+            "other_configs": others, "poisson_only": poisson_only}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, sample = oracle_sample_rate(W.config(args.config), 15.0)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
@@ -328,8 +382,50 @@ def run_ours(args, wl, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_stub(args, wl, rank, world):
+    """CAV_BENCH_STUB=1 (tests only, CPU): the launch / rendezvous / combine logic of the N-rank path over gloo with a stubbed
+    step (a sleep of 10 ms x (rank + 1)); prints the same line shape with `"stub": true`.  No kernel runs: never a bench value."""
+    import torch
+    import torch.distributed as dist
+    from paper_0809_3098_b200 import replicas
+    if world > 1:
+        dist.init_process_group("gloo", rank=rank, world_size=world)
+    wl = replicas.replica_workload(wl, rank, world)
+    K = args.steps if args.steps is not None else 3
+    t0 = time.perf_counter()
+    for _ in range(K):
+        time.sleep(0.01 * (rank + 1))
+    t_local = time.perf_counter() - t0
+    units, t_max = replicas.combine(5.0 * (wl.N + 1) ** 2 * K, t_local, world, dist if world > 1 else None, torch.device("cpu"))
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": units / t_max, "unit": UNIT, "n_gpus": world, "steps": K, "stub": True,
+                          "ms_per_step": 1e3 * t_max / K, "config": {"workload": wl.name}}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def spawn_ranks(n, argv):
+    """`python bench.py --gpus N` without a launcher: re-executes this file as N ranks (RANK / LOCAL_RANK / WORLD_SIZE /
+    MASTER_* in their environment), one per GPU; rank 0's JSON line is this process's output.  Returns the exit code."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    procs = []
+    for r in range(n):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(n), MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port), BENCH_SPAWNED="1")
+        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__)] + argv, env=env))
+    rc = 0
+    for pr in procs:
+        rc = pr.wait() or rc
+    return rc
+
+
 def main():
     args = parse()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        raise SystemExit(spawn_ranks(args.gpus, sys.argv[1:]))
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -338,6 +434,9 @@ def main():
     if args.impl == "reference":
         if rank == 0:
             run_reference(args, wl)
+        return
+    if os.environ.get("CAV_BENCH_STUB") == "1":
+        run_stub(args, wl, rank, world)
         return
     run_ours(args, wl, rank, world, local_rank)
 

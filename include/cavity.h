@@ -89,7 +89,13 @@ int cav_set_fields(cav_ctx* ctx, const double* psi, const double* omega);
  * After a step: omega interior = omega^{n+1}; psi and the omega ring are those of stage 5 (G16). */
 int cav_get_fields(cav_ctx* ctx, double* psi_out, double* omega_out);
 
-/* Advances nsteps SSPRK(5,4) steps, each 5 x [a1 x S, a2, a3].  nsteps < 0: CAV_EINVAL; 0: no-op. */
+/* Advances nsteps SSPRK(5,4) steps, each 5 x [a1 x S, a2, a3].  nsteps < 0: CAV_EINVAL; 0: no-op.  With the resident engine
+ * and the red-black sweeps the whole call is ONE kernel launch.
+ * CAV_ECUDA from this or any later call of a resident-engine context can also mean that a tile of the persistent kernel waited
+ * ~10 s for a neighbour's halo and gave up (it cannot happen on a healthy device: all tiles are co-resident; a debugger,
+ * time-slicing or a sanitizer can stretch the wait).  The fields are then undefined; the condition is sticky until
+ * cav_set_fields, cav_set_engine or cav_set_resident_plan, which clear it.  CAV_DEBUG=1 in the environment prints which
+ * tile waited for which unit (and the CUDA error string behind any other CAV_ECUDA) to stderr. */
 int cav_step(cav_ctx* ctx, int nsteps);
 
 /* As cav_step but returns after enqueueing on the context's stream (no host synchronisation). */
@@ -108,7 +114,7 @@ int cav_poisson(cav_ctx* ctx, int nsweeps, double* res_inf_out);
  *   psi <- (3/5)(beta/a)(A + B + C) + (1 - beta) psi,  A, B, C of eq 16-18, a = 2/h^2,
  * whose B reads omega on the walls: the stage input carries the wall vorticity a2 computed in the previous stage (for the
  * first stage after cav_set_fields: the ring as given; reading N2).  Both variants run as kernels over global
- * memory whatever the engine (one per Jacobi sweep, four per compact sweep). */
+ * memory whatever the engine (one per Jacobi sweep, four per compact sweep), inside a CUDA graph of the whole time step. */
 int cav_set_sweep(cav_ctx* ctx, int kind);
 
 /* One time step, and the paper's steady-state monitors of that step (eq 26-27):
@@ -130,22 +136,31 @@ int cav_get_diag(cav_ctx* ctx, cav_diag* out);
 int cav_set_engine(cav_ctx* ctx, int engine);
 
 /* Resident engine only: forces T, the number of sweeps between two halo exchanges (1..8; the halo is 2T
- * points deep; 0 = the planner's own choice) and / or the kernel variant (0 = one CTA of up to 16 warps per SM, 1 = two
- * CTAs of up to 8 warps per SM; -1 = the planner's choice), and re-plans the tiling.  The result of every other call is
- * unchanged bit for bit; this is a tuning / testing knob.  CAV_ENOTSUP if no such plan exists (the previous plan is kept). */
+ * points deep; 0 = the planner's own choice) and / or the kernel variant (0 = the only one built: one CTA of up to 16 warps per
+ * SM; -1 = the planner's choice), and re-plans the tiling.  The result of every other call is unchanged bit for bit; this is a
+ * tuning / testing knob.  CAV_ENOTSUP if no such plan exists (the previous plan is kept). */
 int cav_set_resident_plan(cav_ctx* ctx, int sweeps_per_exchange, int variant);
 
-/* Profiling aid, resident engine only: runs nsweeps of a1 on the current (psi, omega) like cav_poisson (without the
- * a2 pass) and returns, for every tile, %globaltimer stamps (ns, one clock for all tiles) at the phase boundaries: stamps_out is a HOST array of
- * ntiles x slots_per_tile; slot 0 = kernel start, 1 = inputs loaded, then for exchange round r: 2 + 4r = sweeps done,
- * 3 + 4r = border strips stored, 4 + 4r = ring received from the neighbours, 5 + 4r = edges republished.  Unused slots are 0;
- * *ntiles_out (if non-NULL) receives the tile count; call once with
- * the capacity of a plan's tile count (at most 1023).  CAV_ENOTSUP if the engine in use is not the resident one. */
+/* Profiling aid, resident engine with the red-black sweeps only (CAV_ENOTSUP otherwise): runs nsweeps of a1 on the current
+ * (psi, omega) like cav_poisson (without the a2 pass) and returns, for every tile, %globaltimer stamps (ns, one clock for all
+ * tiles) at the phase boundaries: stamps_out is a HOST array of ntiles x slots_per_tile; slot 0 = kernel start, 1 = inputs
+ * loaded, then for exchange round r: 2 + 4r = sweeps done, 3 + 4r = border strips stored, 4 + 4r = ring received from the
+ * neighbours, 5 + 4r = edges republished.  Unused slots are 0; *ntiles_out (if non-NULL) receives the tile count; call once
+ * with the capacity of a plan's tile count (at most 1023). */
 int cav_trace_sweeps(cav_ctx* ctx, int nsweeps, long long* stamps_out, int slots_per_tile, int* ntiles_out);
 
-/* Testing aid, resident engine: sets the host-side tag epoch of the halo exchange (tags are epoch + round, unique per round
- * and launch; near 2^32 the library clears the exchange buffers and restarts the epoch at 0: this call lets a test get there). */
+/* Testing aid, resident engine: sets the host-side count of halo-exchange rounds (the 16-bit tag of a round is 1 + round mod
+ * 65535, the buffer round mod 2) and clears the exchange buffers, so that a test can run across the wrap of the tags and of the
+ * 32-bit counter.  Neither wrap needs any action in normal use: a reader can only ever meet the round it waits for or the one
+ * two rounds earlier. */
 int cav_debug_set_epoch(cav_ctx* ctx, unsigned int epoch);
+
+/* Measurement aid (the fp64 roofline needs a MEASURED peak): runs a DFMA-chain micro-kernel on every SM
+ * of the context's device (one CTA of 16 warps per SM, 8 independent dependent chains per thread, best of 4 timed launches by
+ * CUDA events on the context's stream) and writes the achieved rate in fp64 FMA instructions per second, counted per thread
+ * (lane), to *dfma_per_s_out; *sm_clock_mhz_out (may be NULL) receives the device's nominal SM clock.  The nominal figure for
+ * B200 is 148 SMs x 64 fp64 lanes x clock.  Does not touch the state. */
+int cav_measure_fp64_peak(cav_ctx* ctx, double* dfma_per_s_out, double* sm_clock_mhz_out);
 
 /* Describes the launch plan of the current engine in `buf` (NUL-terminated, truncated to len). */
 int cav_describe(cav_ctx* ctx, char* buf, int len);

@@ -16,7 +16,8 @@ _ENGINES = {"auto": ENGINE_AUTO, "stream": ENGINE_STREAM, "resident": ENGINE_RES
 # every symbol include/cavity.h declares
 SYMBOLS = ("cav_create", "cav_destroy", "cav_set_fields", "cav_get_fields", "cav_step", "cav_step_async", "cav_sync",
            "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_set_resident_plan", "cav_trace_sweeps", "cav_describe", "cav_launch_count",
-           "cav_last_elapsed_ms", "cav_strerror", "cav_set_sweep", "cav_step_res", "cav_run_to_steady", "cav_debug_set_epoch")
+           "cav_last_elapsed_ms", "cav_strerror", "cav_set_sweep", "cav_step_res", "cav_run_to_steady", "cav_debug_set_epoch",
+           "cav_measure_fp64_peak")
 
 SWEEP_REDBLACK, SWEEP_JACOBI, SWEEP_COMPACT9 = 0, 1, 2
 _SWEEPS = {"redblack": SWEEP_REDBLACK, "jacobi": SWEEP_JACOBI, "compact9": SWEEP_COMPACT9}
@@ -79,6 +80,7 @@ def lib():
     L.cav_step_res.argtypes = [C.c_void_p, dp, dp]
     L.cav_run_to_steady.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(CavMonitor)]
     L.cav_debug_set_epoch.argtypes = [C.c_void_p, C.c_uint]
+    L.cav_measure_fp64_peak.argtypes = [C.c_void_p, dp, dp]
     L.cav_strerror.argtypes = [C.c_int]
     L.cav_strerror.restype = C.c_char_p
     _lib = L
@@ -199,6 +201,12 @@ class Cavity:
         _chk(lib().cav_get_diag(self._h, C.byref(d)), "cav_get_diag")
         return {"t": d.t, "step": d.step, "res_inf": d.res_inf, "res_l2": d.res_l2,
                 "kinetic_energy": d.kinetic_energy, "enstrophy": d.enstrophy}
+
+    def measure_fp64_peak(self):
+        """(fp64 FMA instructions per second per lane summed over the GPU, nominal SM clock in MHz) of a DFMA-chain kernel."""
+        r, mhz = C.c_double(), C.c_double()
+        _chk(lib().cav_measure_fp64_peak(self._h, C.byref(r), C.byref(mhz)), "cav_measure_fp64_peak")
+        return r.value, mhz.value
 
     def describe(self):
         buf = C.create_string_buffer(1024)

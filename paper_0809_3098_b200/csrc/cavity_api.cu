@@ -535,6 +535,38 @@ CAV_API int cav_debug_set_epoch(cav_ctx* c, unsigned int epoch) {
     return CAV_OK;
 }
 
+CAV_API int cav_measure_fp64_peak(cav_ctx* c, double* dfma_per_s_out, double* sm_clock_mhz_out) {
+    if (!c || !dfma_per_s_out) return CAV_EINVAL;
+    DeviceGuard dg(c->device);
+    int sms = 0, khz = 0;
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device));
+    CK(cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, c->device));
+    const int blocks = sms;                                         // one CTA of 16 warps per SM, like the resident engine
+    double* sink = (double*)dev_alloc(c, (size_t)blocks * 512 * sizeof(double));
+    if (!sink) return CAV_ENOMEM;
+    int rc = CAV_OK;
+    double per_thread = 0.0, best_ms = 1e30;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) rc = CAV_ECUDA;
+    for (int rep = 0; rc == CAV_OK && rep < 6; ++rep) {             // the first two warm up; best of the rest
+        cudaEventRecord(e0, c->st);
+        const int nl = cavk::fp64_peak(blocks, 4000, sink, c->st, &per_thread);
+        cudaEventRecord(e1, c->st);
+        if (nl < 0 || cudaEventSynchronize(e1) != cudaSuccess) { rc = CAV_ECUDA; break; }
+        c->launches += nl;
+        float ms = 0.0f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep >= 2 && ms < best_ms) best_ms = ms;
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    void* sv = sink; dev_free(sv);
+    if (rc != CAV_OK) { cudaGetLastError(); return rc; }
+    *dfma_per_s_out = per_thread * 512.0 * blocks / (best_ms * 1e-3);
+    if (sm_clock_mhz_out) *sm_clock_mhz_out = khz / 1000.0;
+    return CAV_OK;
+}
+
 CAV_API int cav_describe(cav_ctx* c, char* buf, int len) {
     if (!c || !buf || len < 1) return CAV_EINVAL;
     resolve_engine(c);

@@ -285,7 +285,35 @@ k_res_final(int N, const double* __restrict__ scratch, double* __restrict__ out2
     }
 }
 
+// ---- measurement aid: the fp64 issue rate of this GPU ("the builder measures one (DFMA chain)") ----
+// Every thread runs CHAINS independent chains of dependent DFMAs (enough to cover the pipe latency), every SM holds 16 warps
+// (as the resident engine does).  The result is written so that nothing is optimised away.
+constexpr int PEAK_CHAINS = 8;
+constexpr int PEAK_UNROLL = 16;
+__global__ void __launch_bounds__(512)
+k_fp64_peak(int iters, double a, double b, double* __restrict__ sink) {
+    double x[PEAK_CHAINS];
+#pragma unroll
+    for (int c = 0; c < PEAK_CHAINS; ++c) x[c] = 1.0 + 1e-9 * (threadIdx.x + c);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < PEAK_UNROLL; ++u)
+#pragma unroll
+            for (int c = 0; c < PEAK_CHAINS; ++c) x[c] = fma(x[c], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < PEAK_CHAINS; ++c) s += x[c];
+    if (s == 12345.678) sink[blockIdx.x * blockDim.x + threadIdx.x] = s;      // never true for the a, b used; keeps the chains alive
+}
+
 }  // namespace
+
+int fp64_peak(int blocks, int iters, double* sink_dev, cudaStream_t st, double* dfma_per_thread_out) {
+    k_fp64_peak<<<blocks, 512, 0, st>>>(iters, 0.999999, 1e-6, sink_dev);
+    if (dfma_per_thread_out) *dfma_per_thread_out = (double)iters * PEAK_UNROLL * PEAK_CHAINS;
+    return launched(1);
+}
 
 int jacobi_sweeps(const Params& P, double* psi, double* psi_tmp, const double* q, int nsweeps, cudaStream_t st) {
     dim3 b(64, 4), g(cdiv(P.N - 1, 64), cdiv(P.N - 1, 4));

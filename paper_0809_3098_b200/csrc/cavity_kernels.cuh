@@ -76,4 +76,8 @@ int compact_sweeps(const Params& P, double* psi, const double* qB, int nsweeps, 
 int res_monitors(const Params& P, const double* psi_new, const double* psi_old, const double* w_new, const double* w_old,
                  double* scratch_dev, double* out2_dev, cudaStream_t st);
 
+// ---- measurement aid: DFMA-chain micro-kernel (one CTA of 512 threads per block, `blocks` of them; sink_dev: blocks x 512
+// doubles that are never written in practice).  *dfma_per_thread_out = dependent-chain DFMAs each thread executes.
+int fp64_peak(int blocks, int iters, double* sink_dev, cudaStream_t st, double* dfma_per_thread_out);
+
 }  // namespace cavk

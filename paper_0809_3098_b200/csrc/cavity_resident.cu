@@ -348,13 +348,15 @@ __host__ __device__ inline URegion recv_units(const TileGeom& t, int N, int halo
 //   land    2 CAV_RECV_BATCH nthreads    landing zone of the asynchronous ring fetches: 16 bytes per thread and slot
 //   table   (ns_per + nr_per) nthreads / 2 uint2   per pair of lanes: {unit index in the exchange buffer (NO_UNIT: none), position in the image},
 //           then nthreads u32: the rows of the micro-tile that are staged / read back around an exchange
+//   args    sizeof(ResArgs)              a copy of the kernel parameters for rhs_phase (not inlined: it would otherwise read them
+//                                        through generic loads and keep them in registers)
 // uint2 words per tile: the entries, then one 32-bit word per thread: bits 0-5 = micro-tile rows that hold points of units this
 // tile sends (staged before an exchange), bits 8-13 = rows that hold points of units it receives (read back after it)
 __host__ __device__ inline size_t xtab_entries(int nth, int ns_per, int nr_per) { return (size_t)(ns_per + nr_per) * (nth / 2) + (size_t)nth / 2; }
 __host__ __device__ inline size_t smem_layout_bytes(int C, int R, int maxw, int warps, int ns_per, int nr_per) {
     const size_t nth = 32 * (size_t)warps, H = (size_t)R * warps, SW = 32 * (size_t)C;
     return 8 * ((2 + CAV_QROWS) * (size_t)(maxw + 1) * C * 32 + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nth) +
-           8 * xtab_entries((int)nth, ns_per, nr_per);
+           8 * xtab_entries((int)nth, ns_per, nr_per) + (sizeof(ResArgs) + 15) / 16 * 16;
 }
 
 // table entry .y: bits 0-15 = index of the unit's first point in the image (row SW + lx) + 8 (lx may be -2: groups are aligned
@@ -441,7 +443,7 @@ __device__ __forceinline__ void fill_image(double* __restrict__ img, const doubl
     const int xa = imax(x0, 1), xb = imin(x1, N), ya = imax(y0, 1), yb = imin(y1, N);
     // H SW = R C nth elements: a fixed trip count, unrolled in batches so that the loads of a batch are in flight together
     // (an L2 round trip per element, one after the other, would cost more than the whole stage combination)
-    constexpr int BATCH = 8;
+    constexpr int BATCH = R * C >= 12 ? 12 : R * C;
     static_assert((R * C) % BATCH == 0, "whole batches");
 #pragma unroll 1
     for (int it0 = 0; it0 < R * C; it0 += BATCH) {
@@ -560,13 +562,13 @@ __device__ __forceinline__ double thom_lid(double c2h2, double lid, double p_adj
 // image holds the NEW vorticity on core + halo (+0.0 elsewhere) and the ring copy is refreshed; the caller turns it into q.
 // Not inlined: see exchange_units.
 template <int C, int R, int MAXW>
-__device__ __noinline__ void rhs_phase(const ResArgs& a_, const double* __restrict__ pl, double* __restrict__ sm, const int stage,
+__device__ __noinline__ void rhs_phase(const ResArgs* __restrict__ ap, const double* pl, double* __restrict__ sm, const int stage,
                                        const unsigned int round, const unsigned int fl) {
     constexpr int TOPOFF = (MAXW + 1) * C * 32;
     constexpr int SW = 32 * C;
     constexpr int edge_doubles = (2 + CAV_QROWS) * TOPOFF;
     double* const sB = sm + (int)threadIdx.y * C * 32 + (int)threadIdx.x;
-    const ResArgs a = a_;             // a local copy: the fields are read once, not again after every store or barrier
+    const ResArgs& a = *ap;           // the copy of the kernel parameters in shared memory: fields are re-read where they are used
     {
     const int z = opaque_zero();
     const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
@@ -584,6 +586,21 @@ __device__ __noinline__ void rhs_phase(const ResArgs& a_, const double* __restri
     // interior points of the core, in grid and in local coordinates
     const int X0 = imax(te.cx0, 1), X1 = imin(te.cx1, Ne), Y0 = imax(te.cy0, 1), Y1 = imin(te.cy1, Ne);
     const int lx0 = ln * C, row0 = wp * R, gx0 = te.ox + lx0, gy0 = te.oy + row0;
+
+    // (0) the pointwise operand of the combination (omega^n for stages 2-4, T for stage 5) is requested now, for all points of
+    //     the micro-tile at once, and used in (2): its L2 round trip hides behind (1).  The same registers then take the result.
+    double ab[R][C];
+    {
+        const double* const src = k == 5 ? tbuf : w0b;
+#pragma unroll
+        for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+            for (int ci = 0; ci < C; ++ci) {
+                const int gx = gx0 + ci, gy = gy0 + rj;
+                ab[rj][ci] = 0.0;
+                if (k != 1 && gx >= X0 && gx < X1 && gy >= Y0 && gy < Y1) ab[rj][ci] = src[(size_t)gy * pitch + gx];
+            }
+    }
 
     // (1) the image receives the stage input: core from the tile's own global buffer, first ring from the copy kept
     //     since the last vorticity exchange, walls next to the core from Thom's formula (written by the owner of the
@@ -671,26 +688,35 @@ __device__ __noinline__ void rhs_phase(const ResArgs& a_, const double* __restri
             const double L = fma(a.nu, lap, -fma(u, wx, v * wy));
             const double dL = a.dt * L;
             const size_t gk = (size_t)gy * pitch + gx;
+            const double av = ab[rj][ci];
             double out;
             if (k == 1) {
                 out = fma(RK1_C, dL, w0);                                               // eq 9
             } else if (k == 2) {
-                out = fma(RK2_C, dL, fma(RK2_A1, w0, RK2_A0 * w0b[gk]));                // eq 10 (w0 here is omega^(1))
+                out = fma(RK2_C, dL, fma(RK2_A1, w0, RK2_A0 * av));                     // eq 10 (w0 here is omega^(1), av = omega^n)
             } else if (k == 3) {
-                out = fma(RK3_C, dL, fma(RK3_A2, w0, RK3_A0 * w0b[gk]));                // eq 11
+                out = fma(RK3_C, dL, fma(RK3_A2, w0, RK3_A0 * av));                     // eq 11
             } else if (k == 4) {
-                out = fma(RK4_C, dL, fma(RK4_A3, w0, RK4_A0 * w0b[gk]));                // eq 12
+                out = fma(RK4_C, dL, fma(RK4_A3, w0, RK4_A0 * av));                     // eq 12
                 tbuf[gk] = fma(RK5_C3, dL, fma(RK5_A3, w0, RK5_A2 * w2b[gk]));          // eq 13, first three terms
             } else {
-                out = fma(RK5_C4, dL, fma(RK5_A4, w0, tbuf[gk]));                       // eq 13, the rest
+                out = fma(RK5_C4, dL, fma(RK5_A4, w0, av));                             // eq 13, the rest (av = T)
             }
             wout[gk] = out;
+            ab[rj][ci] = out;
         }
     }
-    __syncthreads();              // every read of the image and every store of the stage output is done
+    __syncthreads();              // every read of the image is done
 
-    // (3) the new vorticity: core from the global buffer just written, ring from the neighbours, q = cq w
-    fill_image<C, R>(img, wout, X0, X1, Y0, Y1, te.ox, te.oy, H, Ne, pitch, tid_o, nth_o);
+    // (3) the new vorticity: the core from the registers, +0.0 elsewhere, then the ring from the neighbours
+#pragma unroll
+    for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+        for (int ci = 0; ci < C; ++ci) {
+            const int gx = gx0 + ci, gy = gy0 + rj;
+            if (!(gx >= X0 && gx < X1 && gy >= Y0 && gy < Y1)) ab[rj][ci] = 0.0;
+        }
+    stage_tile<C, R>(ab, img, ln, wp, 0x3fu);
     __syncthreads();
     if (a.ntx * a.nty > 1) {
         double* const land = img + H * SW + 2 * SW + 2 * H;
@@ -750,6 +776,14 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
             const uint2* const src = a.tables + (size_t)(bj * a.ntx + bi) * n;
             for (int k = tid; k < n; k += nthreads) tabs[k] = src[k];
         }
+    }
+
+    {   // a copy of the kernel parameters in shared memory (for rhs_phase)
+        const int H = nwarps * R;
+        unsigned int* const dst = reinterpret_cast<unsigned int*>(sm + edge_doubles + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nthreads) +
+                                  2 * (a.ntx * a.nty > 1 ? xtab_entries(nthreads, a.ns_per, a.nr_per) : 0);
+        const unsigned int* const src = reinterpret_cast<const unsigned int*>(&a);
+        for (int k = tid; k < (int)(sizeof(ResArgs) / 4); k += nthreads) dst[k] = src[k];
     }
 
     // ---- load the micro-tile: psi, and the right-hand side q = cq w of the first stage ----
@@ -847,7 +881,17 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
             for (int rj = 0; rj < R; ++rj)
 #pragma unroll
                 for (int ci = 0; ci < C; ++ci) pl[rj * C + ci] = p[rj][ci];
-            rhs_phase<C, R, MAXW>(a, pl, sm, stage, round, fl);
+            {
+                const int nth_ = (int)blockDim.y * 32, H_ = (int)blockDim.y * R;
+                const ResArgs* const ap = reinterpret_cast<const ResArgs*>(
+                    reinterpret_cast<const unsigned int*>(sm + edge_doubles + H_ * SW + 2 * SW + 2 * H_ + 2 * CAV_RECV_BATCH * nth_) +
+                    2 * (a.ntx * a.nty > 1 ? xtab_entries(nth_, a.ns_per, a.nr_per) : 0));
+                rhs_phase<C, R, MAXW>(ap, pl, sm, stage, round, fl);
+            }
+#pragma unroll
+            for (int rj = 0; rj < R; ++rj)      // read back: psi need not occupy registers across the call
+#pragma unroll
+                for (int ci = 0; ci < C; ++ci) p[rj][ci] = pl[rj * C + ci];
             if (a.ntx * a.nty > 1) ++round;                                     // the vorticity exchange
             const int z = opaque_zero();
             const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;

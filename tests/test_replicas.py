@@ -56,3 +56,26 @@ def test_combine_world_size_2_gloo():
         p.join(30)
         assert p.exitcode == 0
     assert got == [(0, 300.0, 2.0), (1, 300.0, 2.0)]
+
+
+@pytest.mark.timeout(180)
+def test_bench_spawns_its_own_ranks_when_no_launcher_set_the_world():
+    """A bare `python bench.py --gpus 2` (no torchrun, no WORLD_SIZE) re-executes itself as 2 ranks and prints ONE line with
+    n_gpus = 2: the spawn / rendezvous / max-of-times / sum-of-units path over gloo with a stubbed step (CAV_BENCH_STUB=1)."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    env["CAV_BENCH_STUB"] = "1"
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "3"], env=env,
+                         capture_output=True, text=True, timeout=150)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, out.stdout
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["stub"] is True
+    # rank 1 sleeps twice as long: the job time is the MAX over ranks, the units are the SUM
+    assert 55.0 <= d["ms_per_step"] * 3 <= 400.0
+    G = 1025 ** 2
+    assert abs(d["value"] * (d["ms_per_step"] * 3e-3) / (2 * 5.0 * G * 3) - 1.0) < 1e-9
