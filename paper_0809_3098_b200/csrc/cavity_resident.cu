@@ -562,7 +562,7 @@ __device__ __forceinline__ double thom_lid(double c2h2, double lid, double p_adj
 // image holds the NEW vorticity on core + halo (+0.0 elsewhere) and the ring copy is refreshed; the caller turns it into q.
 // Not inlined: see exchange_units.
 template <int C, int R, int MAXW>
-__device__ __noinline__ void rhs_phase(const ResArgs* __restrict__ ap, const double* pl, double* __restrict__ sm, const int stage,
+__device__ __forceinline__ void rhs_phase(const ResArgs* __restrict__ ap, const double (&pp)[R][C], double* __restrict__ sm, const int stage,
                                        const unsigned int round, const unsigned int fl) {
     constexpr int TOPOFF = (MAXW + 1) * C * 32;
     constexpr int SW = 32 * C;
@@ -632,7 +632,7 @@ __device__ __noinline__ void rhs_phase(const ResArgs* __restrict__ ap, const dou
                 const int gx = gx0 + ci, gy = gy0 + rj;
                 if (gx < X0 || gx >= X1 || gy < Y0 || gy >= Y1) continue;
                 const int ir_ = row0 + rj, ix_ = lx0 + ci;
-                const double pv = pl[rj * C + ci];
+                const double pv = pp[rj][ci];
                 if (gx == 1) { const double v = thom_wall(a.c2h2, pv); img[img_ix(ir_, ix_ - 1, SW)] = v; wout[(size_t)gy * pitch] = v; }
                 if (gx == Ne - 1) { const double v = thom_wall(a.c2h2, pv); img[img_ix(ir_, ix_ + 1, SW)] = v; wout[(size_t)gy * pitch + Ne] = v; }
                 if (gy == 1) {
@@ -655,8 +655,8 @@ __device__ __noinline__ void rhs_phase(const ResArgs* __restrict__ ap, const dou
         const int gy = gy0 + rj;
         if (gy < Y0 || gy >= Y1) continue;                              // the same for the whole warp
         const double* const ir = img + (row0 + rj) * SW + lx0;
-        double lnb = __shfl_up_sync(0xffffffffu, pl[rj * C + C - 1], 1);
-        double rnb = __shfl_down_sync(0xffffffffu, pl[rj * C], 1);
+        double lnb = __shfl_up_sync(0xffffffffu, pp[rj][C - 1], 1);
+        double rnb = __shfl_down_sync(0xffffffffu, pp[rj][0], 1);
         if (fl & FL_ZERO_LEFT) lnb = 0.0;                               // the wall (or the end of the thread grid), as in the sweeps
         if (fl & FL_ZERO_RIGHT) rnb = 0.0;
         if (gx0 + C - 1 < X0 || gx0 >= X1) continue;
@@ -674,10 +674,10 @@ __device__ __noinline__ void rhs_phase(const ResArgs* __restrict__ ap, const dou
         for (int ci = 0; ci < C; ++ci) {
             const int gx = gx0 + ci;
             if (gx < X0 || gx >= X1) continue;
-            const double pW = ci > 0 ? pl[rj * C + ci - 1] : lnb;
-            const double pE = ci < C - 1 ? pl[rj * C + ci + 1] : rnb;
-            const double pS = rj > 0 ? pl[(rj - 1) * C + ci] : sB[TOPOFF + ci * 32];            // top row of the warp below
-            const double pN = rj < R - 1 ? pl[(rj + 1) * C + ci] : sB[C * 32 + ci * 32];        // bottom row of the warp above
+            const double pW = ci > 0 ? pp[rj][ci - 1] : lnb;
+            const double pE = ci < C - 1 ? pp[rj][ci + 1] : rnb;
+            const double pS = rj > 0 ? pp[rj - 1][ci] : sB[TOPOFF + ci * 32];            // top row of the warp below
+            const double pN = rj < R - 1 ? pp[rj + 1][ci] : sB[C * 32 + ci * 32];        // bottom row of the warp above
             const double w0 = wc[1 + ci], wW = wc[ci], wE = wc[2 + ci], wS = ws[ci], wN = wn[ci];
             // eq 22: u = dpsi/dy, v = -dpsi/dx;  eq 8
             const double u = (pN - pS) * a.i2h;
@@ -876,22 +876,13 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
 
         // ================= a2 + a3: wall vorticity, transport right-hand side, stage combination =================
         {
-            double pl[R * C];             // a copy in local memory: the callee's registers are its own
-#pragma unroll
-            for (int rj = 0; rj < R; ++rj)
-#pragma unroll
-                for (int ci = 0; ci < C; ++ci) pl[rj * C + ci] = p[rj][ci];
             {
                 const int nth_ = (int)blockDim.y * 32, H_ = (int)blockDim.y * R;
                 const ResArgs* const ap = reinterpret_cast<const ResArgs*>(
                     reinterpret_cast<const unsigned int*>(sm + edge_doubles + H_ * SW + 2 * SW + 2 * H_ + 2 * CAV_RECV_BATCH * nth_) +
                     2 * (a.ntx * a.nty > 1 ? xtab_entries(nth_, a.ns_per, a.nr_per) : 0));
-                rhs_phase<C, R, MAXW>(ap, pl, sm, stage, round, fl);
+                rhs_phase<C, R, MAXW>(ap, p, sm, stage, round, fl);
             }
-#pragma unroll
-            for (int rj = 0; rj < R; ++rj)      // read back: psi need not occupy registers across the call
-#pragma unroll
-                for (int ci = 0; ci < C; ++ci) p[rj][ci] = pl[rj * C + ci];
             if (a.ntx * a.nty > 1) ++round;                                     // the vorticity exchange
             const int z = opaque_zero();
             const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
