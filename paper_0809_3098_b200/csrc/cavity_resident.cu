@@ -68,7 +68,7 @@ constexpr unsigned int NO_UNIT = 0xffffffffu;
 #define CAV_QROWS 2             // rows of the micro-tile whose q lives in shared memory instead of registers
 #endif
 #ifndef CAV_RECV_BATCH
-#define CAV_RECV_BATCH 3        // ring half-units (16 bytes) a thread keeps in flight at a time, as asynchronous copies into shared memory
+#define CAV_RECV_BATCH 6        // ring half-units (16 bytes) a thread keeps in flight at a time, as asynchronous copies into shared memory
 #endif
 
 // SSPRK(5,4) in Shu-Osher form, eq 9-13, readings G1 / G2 (the same table as cavity_kernels.cu, typed here again
@@ -97,7 +97,7 @@ struct ResArgs {
     int S;                  // sweeps per stage (nsteps > 0) or in total (nsteps == 0)
     int T, halo, CW, CH, ntx, nty;
     int ns_per, nr_per;     // table entries per thread: strip units to store / ring units to fetch
-    const uint2* tables;    // per-plan exchange tables, one block per tile (k_build_tables)
+    const unsigned int* tables;   // per-plan exchange tables, one block per tile (k_build_tables)
     long long* trace;       // profiling only (cav_trace_sweeps): per tile, %globaltimer at the phase boundaries; else null
     int trace_cap;          // slots per tile
 };
@@ -203,8 +203,8 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
     asm volatile("" : "+r"(fl));               // opaque: the bit tests below are redone here, not hoisted into registers of their own
     // sB / sT point at [warp][0][lane] of the bottom / top edge arrays (stride 32 per ci, C * 32 per warp);
     // the top array starts TOPOFF doubles after the bottom one (a compile-time distance: one address register)
-    // q of the two middle rows of the micro-tile lives in shared memory, in two more arrays of the same shape 2 TOPOFF and
-    // 3 TOPOFF after the bottom edge array (same address register): 16 registers fewer held across the whole kernel.
+    // q of the two middle rows of the micro-tile lives in shared memory, in two more arrays (of MAXW warps) behind the two edge
+    // arrays (same address register): 16 registers fewer held across the whole kernel.
     double* const sT = sB + TOPOFF;
     constexpr int QR = CAV_QROWS, Q0 = (R - QR) / 2;
     double Lnb[R], Rnb[R], Bnb[C], Tnb[C], qs[QR][C];
@@ -212,7 +212,7 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
     for (int ci = 0; ci < C; ++ci) {
 #pragma unroll
         for (int k = 0; k < QR; ++k)
-            if (((ci + Q0 + k) & 1) == K) qs[k][ci] = sB[(2 + k) * TOPOFF + ci * 32];
+            if (((ci + Q0 + k) & 1) == K) qs[k][ci] = sB[2 * TOPOFF + k * (TOPOFF - C * 32) + ci * 32];
     }
 #pragma unroll
     for (int ci = 0; ci < C; ++ci) {
@@ -342,41 +342,46 @@ __host__ __device__ inline URegion recv_units(const TileGeom& t, int N, int halo
 }
 
 // Shared-memory layout (doubles unless said otherwise), nthreads = 32 nwarps, H = R nwarps, SW = 32 C:
-//   edges   4 (MAXW + 1) C 32            bottom / top rows of the micro-tiles, q of the two middle rows (sized for MAXW warps)
+//   edges   (2 (MAXW + 1) + 2 MAXW) C 32   bottom / top rows of the micro-tiles, q of the two middle rows (sized for MAXW warps)
 //   image   H SW                         the tile, row-major: staging area of every exchange, and omega of the stage input during a3
 //   wring   2 SW + 2 H                   first ring of the stage input vorticity around the core (rows below / above, columns left / right)
 //   land    2 CAV_RECV_BATCH nthreads    landing zone of the asynchronous ring fetches: 16 bytes per thread and slot
-//   table   (ns_per + nr_per) nthreads / 2 uint2   per pair of lanes: {unit index in the exchange buffer (NO_UNIT: none), position in the image},
+//   table   (ns_per + nr_per) nthreads / 2 u32   per pair of lanes and slot: where the unit's points sit in the image (loc_pack; NO_UNIT: none),
 //           then nthreads u32: the rows of the micro-tile that are staged / read back around an exchange
-//   args    sizeof(ResArgs)              a copy of the kernel parameters for rhs_phase (not inlined: it would otherwise read them
-//                                        through generic loads and keep them in registers)
-// uint2 words per tile: the entries, then one 32-bit word per thread: bits 0-5 = micro-tile rows that hold points of units this
+// 32-bit words per tile: one entry per pair of lanes and slot, then one word per thread: bits 0-5 = micro-tile rows that hold points of units this
 // tile sends (staged before an exchange), bits 8-13 = rows that hold points of units it receives (read back after it)
-__host__ __device__ inline size_t xtab_entries(int nth, int ns_per, int nr_per) { return (size_t)(ns_per + nr_per) * (nth / 2) + (size_t)nth / 2; }
+__host__ __device__ inline size_t xtab_words(int nth, int ns_per, int nr_per) { return (size_t)(ns_per + nr_per) * (nth / 2) + (size_t)nth; }
 __host__ __device__ inline size_t smem_layout_bytes(int C, int R, int maxw, int warps, int ns_per, int nr_per) {
     const size_t nth = 32 * (size_t)warps, H = (size_t)R * warps, SW = 32 * (size_t)C;
-    return 8 * ((2 + CAV_QROWS) * (size_t)(maxw + 1) * C * 32 + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nth) +
-           8 * xtab_entries((int)nth, ns_per, nr_per) + (sizeof(ResArgs) + 15) / 16 * 16;
+    return 8 * ((2 * (size_t)(maxw + 1) + CAV_QROWS * (size_t)maxw) * C * 32 + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nth) +
+           4 * xtab_words((int)nth, ns_per, nr_per);
 }
 
-// table entry .y: bits 0-15 = index of the unit's first point in the image (row SW + lx) + 8 (lx may be -2: groups are aligned
-// to the grid, not to the tile), bits 16-18 = which of the three points lie inside the image row
+// table entry (32 bits; NO_UNIT = none): bits 0-7 = local x of the unit's first point + 8 (it may be -2: groups are aligned to
+// the grid, not to the tile), bits 8-14 = local row, bits 16-18 = which of the three points lie inside the image row.
+// The unit's place in the exchange buffer follows from the tile origin: row oy + row, group (ox + lx) / 3.
 __host__ __device__ inline unsigned int loc_pack(int lx0, int row, int W) {
     unsigned int m = 0;
     for (int j = 0; j < 3; ++j)
         if (lx0 + j >= 0 && lx0 + j < W) m |= 1u << j;
-    return (unsigned int)(row * W + lx0 + 8) | (m << 16);
+    return (unsigned int)(lx0 + 8) | ((unsigned int)row << 8) | (m << 16);
+}
+// image index of the first point + 8, and unit index, of an entry
+__device__ __forceinline__ unsigned int entry_loc(unsigned int e, int SW) { return ((e >> 8) & 0x7fu) * (unsigned int)SW + (e & 0xffu); }
+__device__ __forceinline__ unsigned int entry_unit(unsigned int e, int ox, int oy, int upitch) {
+    const unsigned int x = (unsigned int)(ox + (int)(e & 0xffu) - 8);           // = 3 g, below 2^15
+    return (unsigned int)(oy + (int)((e >> 8) & 0x7fu)) * (unsigned int)upitch + ((x * 43691u) >> 17);
 }
 
 // Builds, once per plan, the exchange tables of every tile in global memory (in the layout the kernel copies to shared
 // memory at launch): which unit each thread stores / fetches and where its three points sit in the image.
 template <int C, int R>
-__global__ void k_build_tables(const ResArgs a, uint2* __restrict__ out) {
+__global__ void k_build_tables(const ResArgs a, unsigned int* __restrict__ out) {
     const int lane = threadIdx.x, warp = threadIdx.y, nwarps = blockDim.y;
     const int tid = warp * 32 + lane, nthreads = nwarps * 32;
     const int N = a.N, bi = blockIdx.x, bj = blockIdx.y;
     const TileGeom t = tile_geom(N, a.CW, a.CH, a.halo, a.ntx, a.nty, bi, bj, C, R, 32 * C, nwarps * R);
-    uint2* const o = out + (size_t)(bj * a.ntx + bi) * xtab_entries(nthreads, a.ns_per, a.nr_per);
+    unsigned int* const o = out + (size_t)(bj * a.ntx + bi) * xtab_words(nthreads, a.ns_per, a.nr_per);
     const URegion gs = send_units(t, N, a.halo, bi, bj, a.ntx, a.nty), gr = recv_units(t, N, a.halo);
     const int npr = nthreads / 2;                                              // one entry per pair of adjacent lanes
     for (int i = 0; i < a.ns_per + a.nr_per; ++i) {
@@ -384,11 +389,8 @@ __global__ void k_build_tables(const ResArgs a, uint2* __restrict__ out) {
         const bool snd = i < a.ns_per;
         const int u = (snd ? i : i - a.ns_per) * npr + tid;
         int g = 0, y = 0;
-        uint2 e = make_uint2(NO_UNIT, 0u);
-        if (uregion_unit(snd ? gs : gr, u, g, y)) {
-            e.x = (unsigned int)(y * a.upitch + g);
-            e.y = loc_pack(3 * g - t.ox, y - t.oy, 32 * C);
-        }
+        unsigned int e = NO_UNIT;
+        if (uregion_unit(snd ? gs : gr, u, g, y)) e = loc_pack(3 * g - t.ox, y - t.oy, 32 * C);
         o[(size_t)i * npr + tid] = e;
     }
     unsigned int rows = 0;
@@ -401,7 +403,7 @@ __global__ void k_build_tables(const ResArgs a, uint2* __restrict__ out) {
                 if (gx / 3 >= gr.r[k].g0 && gx / 3 < gr.r[k].g1 && gy >= gr.r[k].y0 && gy < gr.r[k].y1) rows |= 1u << (8 + rj);
             }
         }
-    reinterpret_cast<unsigned int*>(o + (size_t)(a.ns_per + a.nr_per) * npr)[tid] = rows;
+    o[(size_t)(a.ns_per + a.nr_per) * npr + tid] = rows;
 }
 
 // ---- the tile image in shared memory ----------------------------------------------------------------------------
@@ -467,86 +469,80 @@ __device__ __forceinline__ void fill_image(double* __restrict__ img, const doubl
 // xb: the exchange buffer of this round; stamp: where thread 0 records the time between storing and fetching (or null).
 __device__ __noinline__ void exchange_units(ulonglong4* __restrict__ xb, const unsigned int round, const int ns_per, const int nr_per,
                                                unsigned int* __restrict__ err, long long* __restrict__ stamp, double* __restrict__ img,
-                                               const uint2* __restrict__ tab, double* __restrict__ land, const int tid_o, const int nth_o,
-                                               const unsigned int tile) {
+                                               const unsigned int* __restrict__ tab, double* __restrict__ land, const int tid_o,
+                                               const int nth_o, const int ox, const int oy, const int upitch, const unsigned int tile) {
+    constexpr int SW = 128;                                             // image row = 32 lanes x 4 points
     const unsigned int tag = round_tag(round);
     const int h = tid_o & 1, pr = tid_o >> 1, npr = nth_o >> 1;       // half, pair index, pairs in the CTA
     unsigned int* const img32 = reinterpret_cast<unsigned int*>(img) + 3 * h - 16;      // this lane's three words of a unit start here + 2 loc
     char* const xbh = reinterpret_cast<char*>(xb) + 16 * h;                            // ... and its 16 bytes of a unit here + 32 unit
     for (int i = 0; i < ns_per; ++i) {
-        const uint2 e = tab[i * npr + pr];
-        if (e.x != NO_UNIT) {                                          // strip points always lie inside the image: no masks
-            const unsigned int* const s = img32 + 2 * (e.y & 0xffffu);
-            st_half(xbh + 32 * (size_t)e.x, half_pack(s[0], s[1], s[2], tag));
+        const unsigned int e = tab[i * npr + pr];
+        if (e != NO_UNIT) {                                            // strip points always lie inside the image: no masks
+            const unsigned int* const s = img32 + 2 * entry_loc(e, SW);
+            st_half(xbh + 32 * (size_t)entry_unit(e, ox, oy, upitch), half_pack(s[0], s[1], s[2], tag));
         }
     }
     if (stamp != nullptr && tid_o == 0) *stamp = globaltimer_ns();
-    // All threads fetch ring half-units: NB per thread in flight at a time as 16-byte asynchronous copies into a landing
-    // zone in shared memory (no registers are held while they fly: an L2 round trip for data another SM has just written
-    // costs ~0.5 us here).  A copy is a weak load: it may bring the previous round's bytes, which the tags expose; such
-    // halves are then polled with strong loads: ONE lane of the warp polls one of them (waiting tiles do not load L2),
-    // then every lane fetches its missing halves again.
+    // All threads fetch ring half-units as 16-byte asynchronous copies into a landing zone in shared memory, NB slots per thread
+    // in flight together (no registers are held while they fly: an L2 round trip for data another SM has just written costs
+    // ~0.5 us here).  A copy is a weak load: it may bring the previous round's bytes, which the tags expose; the slots that did
+    // not validate are fetched again, all of them together, after ONE lane of the warp has polled one of them with strong loads
+    // until it carries the tag (waiting tiles do not load L2).
     constexpr int NB = CAV_RECV_BATCH;
-    const uint2* const tabr = tab + ns_per * npr + pr;
+    const unsigned int* const tabr = tab + ns_per * npr + pr;
     HalfUnit* const mine_land = reinterpret_cast<HalfUnit*>(land) + tid_o;                 // slot j of this thread: mine_land[j * nth_o]
     for (int i0 = 0; i0 < nr_per; i0 += NB) {
-        unsigned int bad = 0;
+        unsigned int pending = 0;                                       // slots of this batch that hold no valid half yet
 #pragma unroll
-        for (int j = 0; j < NB; ++j) {
-            const unsigned int u = i0 + j < nr_per ? tabr[(i0 + j) * npr].x : NO_UNIT;
-            if (u != NO_UNIT) {
-                const unsigned int dst = (unsigned int)__cvta_generic_to_shared(mine_land + j * nth_o);
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(xbh + 32 * (size_t)u) : "memory");
-            }
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        for (int j = 0; j < NB; ++j)
+            if (i0 + j < nr_per && tabr[(i0 + j) * npr] != NO_UNIT) pending |= 1u << j;
+        long long t0 = 0;
+        for (int attempt = 0;; ++attempt) {
 #pragma unroll
-        for (int j = 0; j < NB; ++j) {
-            const unsigned int u = i0 + j < nr_per ? tabr[(i0 + j) * npr].x : NO_UNIT;
-            if (u != NO_UNIT && !half_ok(mine_land[j * nth_o], tag)) bad |= 1u << j;
-        }
-        unsigned int waiting = __ballot_sync(0xffffffffu, bad != 0u);
-        if (waiting) {
-            const long long t0 = clock64();
-            while (waiting) {
-                int giveup = 0;
-                if ((int)threadIdx.x == __ffs((int)waiting) - 1) {
-                    const int j0 = __ffs((int)bad) - 1;            // the first missing half of this lane
-                    const unsigned int off = tabr[(i0 + j0) * npr].x;
-                    while (!half_ok(ld_half(xbh + 32 * (size_t)off), tag)) {
-                        if (*(volatile unsigned int*)err != 0u) { giveup = 1; break; }      // some tile gave up: do not wait again
-                        if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) {
-                            if (atomicExch(err, 1u) == 0u) {      // the first tile to give up says what it was waiting for (CAV_DEBUG)
-                                const HalfUnit w = ld_half(xbh + 32 * (size_t)off);
-                                err[1] = tile; err[2] = off; err[3] = round; err[4] = tag;
-                                err[5] = w.w1 >> 16; err[6] = w.w3 >> 16; err[7] = (unsigned int)h; err[8] = 0u;
-                                err[9] = (unsigned int)tid_o;
-                            }
-                            giveup = 1; break;
+            for (int j = 0; j < NB; ++j)
+                if ((pending >> j) & 1u) {
+                    const unsigned int dst = (unsigned int)__cvta_generic_to_shared(mine_land + j * nth_o);
+                    const char* const src = xbh + 32 * (size_t)entry_unit(tabr[(i0 + j) * npr], ox, oy, upitch);
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+                }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+#pragma unroll
+            for (int j = 0; j < NB; ++j)
+                if (((pending >> j) & 1u) && half_ok(mine_land[j * nth_o], tag)) pending &= ~(1u << j);
+            const unsigned int waiting = __ballot_sync(0xffffffffu, pending != 0u);
+            if (!waiting) break;
+            if (attempt == 0) t0 = clock64();
+            int giveup = 0;
+            if ((int)threadIdx.x == __ffs((int)waiting) - 1) {
+                const int j0 = __ffs((int)pending) - 1;                // the first missing half of this lane
+                const unsigned int off = entry_unit(tabr[(i0 + j0) * npr], ox, oy, upitch);
+                while (!half_ok(ld_half(xbh + 32 * (size_t)off), tag)) {
+                    if (*(volatile unsigned int*)err != 0u) { giveup = 1; break; }      // some tile gave up: do not wait again
+                    if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) {
+                        if (atomicExch(err, 1u) == 0u) {      // the first tile to give up says what it was waiting for (CAV_DEBUG)
+                            const HalfUnit w = ld_half(xbh + 32 * (size_t)off);
+                            err[1] = tile; err[2] = off; err[3] = round; err[4] = tag;
+                            err[5] = w.w1 >> 16; err[6] = w.w3 >> 16; err[7] = (unsigned int)h; err[8] = 0u;
+                            err[9] = (unsigned int)tid_o;
                         }
+                        giveup = 1; break;
                     }
                 }
-                if (__any_sync(0xffffffffu, giveup)) break;
-#pragma unroll
-                for (int j = 0; j < NB; ++j)
-                    if ((bad >> j) & 1u) {
-                        const HalfUnit v = ld_half(xbh + 32 * (size_t)tabr[(i0 + j) * npr].x);
-                        if (half_ok(v, tag)) { mine_land[j * nth_o] = v; bad &= ~(1u << j); }
-                    }
-                waiting = __ballot_sync(0xffffffffu, bad != 0u);
             }
+            if (__any_sync(0xffffffffu, giveup)) break;
         }
 #pragma unroll
         for (int j = 0; j < NB; ++j) {
-            const uint2 e = i0 + j < nr_per ? tabr[(i0 + j) * npr] : make_uint2(NO_UNIT, 0u);
-            if (e.x != NO_UNIT) {
+            const unsigned int e = i0 + j < nr_per ? tabr[(i0 + j) * npr] : NO_UNIT;
+            if (e != NO_UNIT) {
                 unsigned int A, B, C;
                 half_unpack(mine_land[j * nth_o], A, B, C);
-                unsigned int* const d = img32 + 2 * (e.y & 0xffffu);
+                unsigned int* const d = img32 + 2 * entry_loc(e, SW);
                 // words 0 1 | 2 of lane 0 belong to points 0 | 1 of the unit, words 0 | 1 2 of lane 1 to points 1 | 2; bits 16-18 of
                 // the entry say which points lie inside the image
-                const unsigned int m = e.y >> (16 + h);
+                const unsigned int m = e >> (16 + h);
                 if (m & 1u) d[0] = A;
                 if (h ? (m & 2u) : (m & 1u)) d[1] = B;
                 if (m & 2u) d[2] = C;
@@ -562,13 +558,12 @@ __device__ __forceinline__ double thom_lid(double c2h2, double lid, double p_adj
 // image holds the NEW vorticity on core + halo (+0.0 elsewhere) and the ring copy is refreshed; the caller turns it into q.
 // Not inlined: see exchange_units.
 template <int C, int R, int MAXW>
-__device__ __forceinline__ void rhs_phase(const ResArgs* __restrict__ ap, const double (&pp)[R][C], double* __restrict__ sm, const int stage,
+__device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R][C], double* __restrict__ sm, const int stage,
                                        const unsigned int round, const unsigned int fl) {
     constexpr int TOPOFF = (MAXW + 1) * C * 32;
     constexpr int SW = 32 * C;
-    constexpr int edge_doubles = (2 + CAV_QROWS) * TOPOFF;
+    constexpr int edge_doubles = 2 * TOPOFF + CAV_QROWS * (TOPOFF - C * 32);
     double* const sB = sm + (int)threadIdx.y * C * 32 + (int)threadIdx.x;
-    const ResArgs& a = *ap;           // the copy of the kernel parameters in shared memory: fields are re-read where they are used
     {
     const int z = opaque_zero();
     const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
@@ -720,9 +715,9 @@ __device__ __forceinline__ void rhs_phase(const ResArgs* __restrict__ ap, const 
     __syncthreads();
     if (a.ntx * a.nty > 1) {
         double* const land = img + H * SW + 2 * SW + 2 * H;
-        const uint2* const tab = reinterpret_cast<const uint2*>(land + 2 * CAV_RECV_BATCH * nth_o);
+        const unsigned int* const tab = reinterpret_cast<const unsigned int*>(land + 2 * CAV_RECV_BATCH * nth_o);
         exchange_units((round & 1u) ? a.x1 : a.x0, round, a.ns_per, a.nr_per, a.err, nullptr, img, tab, land, tid_o, nth_o,
-                       blockIdx.y * a.ntx + blockIdx.x);
+                       te.ox, te.oy, a.upitch, blockIdx.y * a.ntx + blockIdx.x);
         __syncthreads();
     }
     {   // first ring of the new vorticity around the core, kept for a3 of the next stage
@@ -748,7 +743,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
     mark(a, 0);
 
     // edge arrays; the slots no thread ever writes (warp -1, warp nwarps) stay +0.0
-    constexpr int edge_doubles = (2 + CAV_QROWS) * TOPOFF;       // bottom edges, top edges, q of the CAV_QROWS middle rows
+    constexpr int edge_doubles = 2 * TOPOFF + CAV_QROWS * (TOPOFF - C * 32);   // bottom edges, top edges (MAXW + 1 warps), q of the CAV_QROWS middle rows (MAXW warps)
     for (int k = tid; k < edge_doubles; k += nthreads) sm[k] = 0.0;
     double* const sB = sm + warp * C * 32 + lane;      // [MAXW + 1][C][32] bottom row of warp at [warp]; top rows TOPOFF further, at [warp + 1]
 
@@ -770,20 +765,12 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
     // ---- exchange tables (multi-tile plans only): copied from the per-plan tables in global memory ----
     {
         const int H = nwarps * R;
-        uint2* const tabs = reinterpret_cast<uint2*>(sm + edge_doubles + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nthreads);
+        unsigned int* const tabs = reinterpret_cast<unsigned int*>(sm + edge_doubles + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nthreads);
         if (a.ntx * a.nty > 1) {
-            const int n = (int)xtab_entries(nthreads, a.ns_per, a.nr_per);
-            const uint2* const src = a.tables + (size_t)(bj * a.ntx + bi) * n;
+            const int n = (int)xtab_words(nthreads, a.ns_per, a.nr_per);
+            const unsigned int* const src = a.tables + (size_t)(bj * a.ntx + bi) * n;
             for (int k = tid; k < n; k += nthreads) tabs[k] = src[k];
         }
-    }
-
-    {   // a copy of the kernel parameters in shared memory (for rhs_phase)
-        const int H = nwarps * R;
-        unsigned int* const dst = reinterpret_cast<unsigned int*>(sm + edge_doubles + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nthreads) +
-                                  2 * (a.ntx * a.nty > 1 ? xtab_entries(nthreads, a.ns_per, a.nr_per) : 0);
-        const unsigned int* const src = reinterpret_cast<const unsigned int*>(&a);
-        for (int k = tid; k < (int)(sizeof(ResArgs) / 4); k += nthreads) dst[k] = src[k];
     }
 
     // ---- load the micro-tile: psi, and the right-hand side q = cq w of the first stage ----
@@ -824,7 +811,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
 #pragma unroll
     for (int ci = 0; ci < C; ++ci) {      // q of the two middle rows moves to shared memory (read back by this thread only)
 #pragma unroll
-        for (int k = 0; k < CAV_QROWS; ++k) sB[(2 + k) * TOPOFF + ci * 32] = q[(R - CAV_QROWS) / 2 + k][ci];
+        for (int k = 0; k < CAV_QROWS; ++k) sB[2 * TOPOFF + k * (TOPOFF - C * 32) + ci * 32] = q[(R - CAV_QROWS) / 2 + k][ci];
     }
     publish_all<C, R, TOPOFF>(p, sB, fl);
     mark(a, 1);
@@ -858,13 +845,14 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
             const int nw = (int)blockDim.y + z, tid_o = wp * 32 + ln, nth_o = nw * 32, H = nw * R;
             double* const img = sm + edge_doubles;
             double* const land = img + H * SW + 2 * SW + 2 * H;
-            const uint2* const tab = reinterpret_cast<const uint2*>(land + 2 * CAV_RECV_BATCH * nth_o);
-            const unsigned int rows = reinterpret_cast<const unsigned int*>(tab + (a.ns_per + a.nr_per) * (nth_o >> 1))[tid_o];
+            const unsigned int* const tab = reinterpret_cast<const unsigned int*>(land + 2 * CAV_RECV_BATCH * nth_o);
+            const unsigned int rows = tab[(a.ns_per + a.nr_per) * (nth_o >> 1) + tid_o];
+            const TileGeom tx = tile_geom(a.N + z, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, H);
             stage_tile<C, R>(p, img, ln, wp, rows);
             __syncthreads();
             exchange_units((round & 1u) ? a.x1 : a.x0, round, a.ns_per, a.nr_per, a.err,
                            (a.trace != nullptr && tslot + 1 < a.trace_cap) ? a.trace + (size_t)(blockIdx.y * a.ntx + blockIdx.x) * a.trace_cap + tslot + 1 : nullptr,
-                           img, tab, land, tid_o, nth_o, blockIdx.y * a.ntx + blockIdx.x);
+                           img, tab, land, tid_o, nth_o, tx.ox, tx.oy, a.upitch, blockIdx.y * a.ntx + blockIdx.x);
             ++round;
             __syncthreads();
             mark(a, tslot + 2);
@@ -876,13 +864,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
 
         // ================= a2 + a3: wall vorticity, transport right-hand side, stage combination =================
         {
-            {
-                const int nth_ = (int)blockDim.y * 32, H_ = (int)blockDim.y * R;
-                const ResArgs* const ap = reinterpret_cast<const ResArgs*>(
-                    reinterpret_cast<const unsigned int*>(sm + edge_doubles + H_ * SW + 2 * SW + 2 * H_ + 2 * CAV_RECV_BATCH * nth_) +
-                    2 * (a.ntx * a.nty > 1 ? xtab_entries(nth_, a.ns_per, a.nr_per) : 0));
-                rhs_phase<C, R, MAXW>(ap, p, sm, stage, round, fl);
-            }
+            rhs_phase<C, R, MAXW>(a, p, sm, stage, round, fl);
             if (a.ntx * a.nty > 1) ++round;                                     // the vorticity exchange
             const int z = opaque_zero();
             const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
@@ -895,7 +877,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
 #pragma unroll
             for (int ci = 0; ci < C; ++ci) {
 #pragma unroll
-                for (int kq = 0; kq < CAV_QROWS; ++kq) sB[(2 + kq) * TOPOFF + ci * 32] = q[(R - CAV_QROWS) / 2 + kq][ci];
+                for (int kq = 0; kq < CAV_QROWS; ++kq) sB[2 * TOPOFF + kq * (TOPOFF - C * 32) + ci * 32] = q[(R - CAV_QROWS) / 2 + kq][ci];
             }
             __syncthreads();              // the ring copy is complete before the image is staged again
         }
@@ -1058,7 +1040,7 @@ void resident_describe(const ResidentPlan& pl, char* buf, int len) {
 int resident_variants() { return NVARIANTS; }
 
 size_t resident_table_bytes(const ResidentPlan& pl) {
-    return (pl.ok && pl.ntiles > 1) ? (size_t)pl.ntiles * xtab_entries(32 * pl.warps, pl.ns_per, pl.nr_per) * sizeof(uint2) : 0;
+    return (pl.ok && pl.ntiles > 1) ? (size_t)pl.ntiles * xtab_words(32 * pl.warps, pl.ns_per, pl.nr_per) * sizeof(unsigned int) : 0;
 }
 
 int resident_build_tables(const Params& P, const ResidentPlan& pl, void* tables_dev, cudaStream_t st) {
@@ -1068,7 +1050,7 @@ int resident_build_tables(const Params& P, const ResidentPlan& pl, void* tables_
     a.halo = pl.halo; a.CW = pl.CW; a.CH = pl.CH; a.ntx = pl.ntx; a.nty = pl.nty;
     a.ns_per = pl.ns_per; a.nr_per = pl.nr_per;
     const dim3 grid(pl.ntx, pl.nty), block(32, pl.warps);
-    if (pl.C == 4 && pl.R == 6) k_build_tables<4, 6><<<grid, block, 0, st>>>(a, (uint2*)tables_dev);
+    if (pl.C == 4 && pl.R == 6) k_build_tables<4, 6><<<grid, block, 0, st>>>(a, (unsigned int*)tables_dev);
     else return -(int)cudaErrorNotSupported;
     const cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? 1 : -(int)e;
@@ -1087,7 +1069,7 @@ int resident_launch(const Params& P, const ResidentPlan& pl, const double* psi_i
     if (nsteps < 0 || S < 0 || (nsteps == 0 && S == 0) || psi_in == psi_out || (pl.ntiles > 1 && (!tables || !xa || !xb)))
         return -(int)cudaErrorInvalidValue;
     ResArgs a{};
-    a.tables = (const uint2*)tables;
+    a.tables = (const unsigned int*)tables;
     a.N = P.N; a.pitch = P.pitch; a.cb = P.cb; a.omb = P.omb; a.cq = P.cq;
     a.i2h = P.i2h; a.ih2 = P.ih2; a.nu = P.nu; a.c2h2 = P.c2h2; a.lid = P.lid; a.dt = P.dt;
     a.psi_in = psi_in; a.psi_out = psi_out; a.wbase = wbase; a.fstride = fstride;
