@@ -135,7 +135,7 @@ int cav_get_diag(cav_ctx* ctx, cav_diag* out);
  * device.  The default is CAV_ENGINE_AUTO. */
 int cav_set_engine(cav_ctx* ctx, int engine);
 
-/* Resident engine only: forces T, the number of sweeps between two halo exchanges (1..8; the halo is 2T
+/* Resident engine only: forces T, the number of sweeps between two halo exchanges (1..10; the halo is 2T
  * points deep; 0 = the planner's own choice) and / or the kernel variant (0 = the only one built: one CTA of up to 16 warps per
  * SM; -1 = the planner's choice), and re-plans the tiling.  The result of every other call is unchanged bit for bit; this is a
  * tuning / testing knob.  CAV_ENOTSUP if no such plan exists (the previous plan is kept). */

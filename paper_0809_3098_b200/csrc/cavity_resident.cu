@@ -435,30 +435,42 @@ __device__ __forceinline__ void read_tile(double (&v)[R][C], const double* __res
             v[rj][0] = lo.x; v[rj][1] = lo.y; v[rj][2] = hi.x; v[rj][3] = hi.y;
         }
 }
-// image <- field g on the interior points of [x0, x1) x [y0, y1) (grid coordinates), +0.0 everywhere else.  Coalesced:
-// consecutive threads = consecutive x.  cg: the field may have been written by this CTA during this launch.
+// image <- field g on the interior points of [x0, x1) x [y0, y1) (grid coordinates), +0.0 everywhere else.  Coalesced: a warp
+// takes whole image rows (rows warp, warp + nwarps, ...: R of them), a lane the columns lane + 32 j.  cg: the field may have been
+// written by this CTA during this launch.  The loads are issued in two batches of R C / 2, all of a batch in flight together
+// (an L2 round trip per element, one after the other, would cost more than the whole stage combination).
 template <int C, int R>
 __device__ __forceinline__ void fill_image(double* __restrict__ img, const double* __restrict__ g, const int x0, const int x1,
-                                           const int y0, const int y1, const int ox, const int oy, const int H, const int N,
-                                           const int pitch, const int tid, const int nth) {
+                                           const int y0, const int y1, const int ox, const int oy, const int nwarps, const int N,
+                                           const int pitch, const int lane, const int warp) {
     constexpr int SW = 32 * C;
     const int xa = imax(x0, 1), xb = imin(x1, N), ya = imax(y0, 1), yb = imin(y1, N);
-    // H SW = R C nth elements: a fixed trip count, unrolled in batches so that the loads of a batch are in flight together
-    // (an L2 round trip per element, one after the other, would cost more than the whole stage combination)
-    constexpr int BATCH = R * C >= 12 ? 12 : R * C;
-    static_assert((R * C) % BATCH == 0, "whole batches");
-#pragma unroll 1
-    for (int it0 = 0; it0 < R * C; it0 += BATCH) {
-        double v[BATCH];
+    unsigned int colok = 0;
 #pragma unroll
-        for (int j = 0; j < BATCH; ++j) {
-            const int k = (it0 + j) * nth + tid;
-            const int gx = ox + k % SW, gy = oy + k / SW;
-            v[j] = 0.0;
-            if (gx >= xa && gx < xb && gy >= ya && gy < yb) v[j] = __ldcg(g + (size_t)gy * pitch + gx);
+    for (int j = 0; j < C; ++j)
+        if (ox + lane + 32 * j >= xa && ox + lane + 32 * j < xb) colok |= 1u << j;
+    const double* const gc = g + (ox + lane);                 // column of this lane, j = 0
+    double* const ic = img + lane;
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+        double v[R / 2][C];
+#pragma unroll
+        for (int i = 0; i < R / 2; ++i) {
+            const int row = warp + nwarps * (half * (R / 2) + i), gy = oy + row;
+            const bool rowok = gy >= ya && gy < yb;
+            const double* const gr = gc + (size_t)gy * pitch;
+#pragma unroll
+            for (int j = 0; j < C; ++j) {
+                v[i][j] = 0.0;
+                if (rowok && ((colok >> j) & 1u)) v[i][j] = __ldcg(gr + 32 * j);
+            }
         }
 #pragma unroll
-        for (int j = 0; j < BATCH; ++j) img[(it0 + j) * nth + tid] = v[j];
+        for (int i = 0; i < R / 2; ++i) {
+            const int row = warp + nwarps * (half * (R / 2) + i);
+#pragma unroll
+            for (int j = 0; j < C; ++j) ic[row * SW + 32 * j] = v[i][j];
+        }
     }
 }
 
@@ -585,22 +597,29 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
     // (0) the pointwise operand of the combination (omega^n for stages 2-4, T for stage 5) is requested now, for all points of
     //     the micro-tile at once, and used in (2): its L2 round trip hides behind (1).  The same registers then take the result.
     double ab[R][C];
+    unsigned int rowin = 0, colin = 0;                    // rows / columns of the micro-tile that hold interior points of the core
+#pragma unroll
+    for (int rj = 0; rj < R; ++rj)
+        if (gy0 + rj >= Y0 && gy0 + rj < Y1) rowin |= 1u << rj;
+#pragma unroll
+    for (int ci = 0; ci < C; ++ci)
+        if (gx0 + ci >= X0 && gx0 + ci < X1) colin |= 1u << ci;
     {
-        const double* const src = k == 5 ? tbuf : w0b;
+        const double* const src = (k == 5 ? tbuf : w0b) + ((size_t)gy0 * pitch + gx0);
+        const unsigned int rsel = k != 1 ? rowin : 0u;
 #pragma unroll
         for (int rj = 0; rj < R; ++rj)
 #pragma unroll
             for (int ci = 0; ci < C; ++ci) {
-                const int gx = gx0 + ci, gy = gy0 + rj;
                 ab[rj][ci] = 0.0;
-                if (k != 1 && gx >= X0 && gx < X1 && gy >= Y0 && gy < Y1) ab[rj][ci] = src[(size_t)gy * pitch + gx];
+                if (((rsel >> rj) & 1u) && ((colin >> ci) & 1u)) ab[rj][ci] = src[(size_t)rj * pitch + ci];
             }
     }
 
     // (1) the image receives the stage input: core from the tile's own global buffer, first ring from the copy kept
     //     since the last vorticity exchange, walls next to the core from Thom's formula (written by the owner of the
     //     adjacent point, who also stores it to the ring of the stage output: k_rk_stage does the same).
-    fill_image<C, R>(img, win, X0, X1, Y0, Y1, te.ox, te.oy, H, Ne, pitch, tid_o, nth_o);
+    fill_image<C, R>(img, win, X0, X1, Y0, Y1, te.ox, te.oy, nw, Ne, pitch, ln, wp);
     __syncthreads();              // fill_image writes zeros everywhere else: the ring and wall writers come after it
     {
         const int rB = Y0 - 1 - te.oy, rT = Y1 - te.oy, cL = X0 - 1 - te.ox, cR = X1 - te.ox;
@@ -648,13 +667,13 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
 #pragma unroll
     for (int rj = 0; rj < R; ++rj) {
         const int gy = gy0 + rj;
-        if (gy < Y0 || gy >= Y1) continue;                              // the same for the whole warp
+        if (!((rowin >> rj) & 1u)) continue;                            // the same for the whole warp
         const double* const ir = img + (row0 + rj) * SW + lx0;
         double lnb = __shfl_up_sync(0xffffffffu, pp[rj][C - 1], 1);
         double rnb = __shfl_down_sync(0xffffffffu, pp[rj][0], 1);
         if (fl & FL_ZERO_LEFT) lnb = 0.0;                               // the wall (or the end of the thread grid), as in the sweeps
         if (fl & FL_ZERO_RIGHT) rnb = 0.0;
-        if (gx0 + C - 1 < X0 || gx0 >= X1) continue;
+        if (colin == 0u) continue;
         double wc[C + 2], ws[C], wn[C];
         wc[0] = img[img_ix(row0 + rj, lx0 - 1, SW)]; wc[C + 1] = img[img_ix(row0 + rj, lx0 + C, SW)];
 #pragma unroll
@@ -668,7 +687,7 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
 #pragma unroll
         for (int ci = 0; ci < C; ++ci) {
             const int gx = gx0 + ci;
-            if (gx < X0 || gx >= X1) continue;
+            if (!((colin >> ci) & 1u)) continue;
             const double pW = ci > 0 ? pp[rj][ci - 1] : lnb;
             const double pE = ci < C - 1 ? pp[rj][ci + 1] : rnb;
             const double pS = rj > 0 ? pp[rj - 1][ci] : sB[TOPOFF + ci * 32];            // top row of the warp below
@@ -707,10 +726,8 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
 #pragma unroll
     for (int rj = 0; rj < R; ++rj)
 #pragma unroll
-        for (int ci = 0; ci < C; ++ci) {
-            const int gx = gx0 + ci, gy = gy0 + rj;
-            if (!(gx >= X0 && gx < X1 && gy >= Y0 && gy < Y1)) ab[rj][ci] = 0.0;
-        }
+        for (int ci = 0; ci < C; ++ci)
+            if (!(((rowin >> rj) & 1u) && ((colin >> ci) & 1u))) ab[rj][ci] = 0.0;
     stage_tile<C, R>(ab, img, ln, wp, 0x3fu);
     __syncthreads();
     if (a.ntx * a.nty > 1) {
@@ -779,11 +796,11 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
     {
         const int H = nwarps * R;
         double* const img = sm + edge_doubles;
-        fill_image<C, R>(img, a.psi_in, 0, N + 1, 0, N + 1, t.ox, t.oy, H, N, a.pitch, tid, nthreads);
+        fill_image<C, R>(img, a.psi_in, 0, N + 1, 0, N + 1, t.ox, t.oy, nwarps, N, a.pitch, lane, warp);
         __syncthreads();
         read_tile<C, R>(p, img, lane, warp, 0x3fu);
         __syncthreads();
-        fill_image<C, R>(img, a.wbase, 0, N + 1, 0, N + 1, t.ox, t.oy, H, N, a.pitch, tid, nthreads);
+        fill_image<C, R>(img, a.wbase, 0, N + 1, 0, N + 1, t.ox, t.oy, nwarps, N, a.pitch, lane, warp);
         __syncthreads();
         read_tile<C, R>(q, img, lane, warp, 0x3fu);
         if (a.nsteps > 0) {               // first ring of the stage input around the core, kept for a3
@@ -915,6 +932,7 @@ const Variant VARIANTS[] = {
 constexpr int NVARIANTS = sizeof(VARIANTS) / sizeof(VARIANTS[0]);
 
 inline int cdiv(int a, int b) { return (a + b - 1) / b; }
+inline double sweep_cycles(int warps) { return 2.0 * (cdiv(warps, 4) * 187.0 + 40.0); }      // one sweep = two colour half-sweeps
 
 // Checks that every tile of the candidate fits its thread grid and counts the exchange units per thread.
 bool finish_plan(ResidentPlan& pl, int N, int max_smem) {
@@ -986,22 +1004,21 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
             c.ok = true; c.variant = vi; c.C = v.C; c.R = v.R; c.warps = warps; c.regs = regs; c.sm_count = sms; c.per_sm = 1;
             // single tile: the whole grid in one CTA, no exchange at all
             if (G + v.C - 1 <= W && G + v.R - 1 <= H) {
-                const double cost = (double)H * W * 0.135 + 150.0;
+                const double cost = sweep_cycles(warps);
                 c.T = 1 << 30; c.halo = 0; c.CW = G; c.CH = G; c.ntx = c.nty = c.ntiles = 1;
                 if (cost < best_cost && finish_plan(c, P.N, smem_cap)) { best_cost = cost; best = c; }
                 continue;
             }
-            for (int T = 1; T <= 8; ++T) {
+            for (int T = 1; T <= 10; ++T) {
                 if (T_override > 0 && T != T_override) continue;
                 const int halo = 2 * T;
                 int CW, ntx, CH, nty;
                 if (!split(G, W, v.C - 1, halo, 3, CW, ntx) || !split(G, H, v.R - 1, halo, 1, CH, nty)) continue;
                 const int ntiles = ntx * nty;
                 if (ntiles < 2 || ntiles > sms) continue;
-                // Cost per sweep in SM cycles, calibrated on B200 (profiles/): 0.135 cycles per point of the thread grid
-                // plus one exchange per T sweeps whose cost is mostly latency (staging, store burst, L2 round trips) and grows
-                // with the halo depth.
-                const double cost = (double)H * W * 0.135 + (5000.0 + 600.0 * T) / T;
+                // Cost per sweep in SM cycles, calibrated on B200 (profiles/r2_*.md): a colour half-sweep takes ~187 cycles per warp
+                // of the busiest SM sub-partition (+ barrier), an exchange ~6500 cycles + 250 per sweep of halo depth, mostly latency.
+                const double cost = sweep_cycles(warps) + (6500.0 + 250.0 * T) / T;
                 c.T = T; c.halo = halo; c.CW = CW; c.CH = CH; c.ntx = ntx; c.nty = nty; c.ntiles = ntiles;
                 if (cost < best_cost && finish_plan(c, P.N, smem_cap)) { best_cost = cost; best = c; }
             }

@@ -28,7 +28,7 @@ struct ResidentPlan {
     int per_sm = 1;       // CTAs per SM
 };
 
-// T_override > 0 forces the sweeps per round (1..8; tests use it to exercise short and ragged rounds);
+// T_override > 0 forces the sweeps per round (1..10; tests use it to exercise short and ragged rounds);
 // variant_override >= 0 forces the micro-tile shape (index into the compiled variants).
 ResidentPlan resident_plan(const Params& P, int device, int T_override = 0, int variant_override = -1);
 int resident_variants();
