@@ -154,6 +154,11 @@ __device__ __forceinline__ void half_unpack(const HalfUnit& u, unsigned int& A, 
     C = __byte_perm(u.w2, u.w3, 0x5432);       // w2[31:16] | w3[15:0] << 16
 }
 __device__ __forceinline__ void st_half(void* p, const HalfUnit& u) {
+#ifdef CAV_EXPERIMENT_WEAK_STORE      // timing experiment only (a weak store racing with the readers' loads is a data race by the model)
+    asm volatile("st.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"((unsigned long long)u.w0 | ((unsigned long long)u.w1 << 32)),
+                 "l"((unsigned long long)u.w2 | ((unsigned long long)u.w3 << 32)) : "memory");
+    return;
+#endif
     asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"((unsigned long long)u.w0 | ((unsigned long long)u.w1 << 32)),
                  "l"((unsigned long long)u.w2 | ((unsigned long long)u.w3 << 32)) : "memory");
 }
@@ -351,10 +356,12 @@ __host__ __device__ inline URegion recv_units(const TileGeom& t, int N, int halo
 // 32-bit words per tile: one entry per pair of lanes and slot, then one word per thread: bits 0-5 = micro-tile rows that hold points of units this
 // tile sends (staged before an exchange), bits 8-13 = rows that hold points of units it receives (read back after it)
 __host__ __device__ inline size_t xtab_words(int nth, int ns_per, int nr_per) { return (size_t)(ns_per + nr_per) * (nth / 2) + (size_t)nth; }
+// ... and behind them, in shared memory only, the tile origin (ox, oy): the exchange needs it every round
+__host__ __device__ inline size_t xtab_smem_words(int nth, int ns_per, int nr_per) { return xtab_words(nth, ns_per, nr_per) + 4; }
 __host__ __device__ inline size_t smem_layout_bytes(int C, int R, int maxw, int warps, int ns_per, int nr_per) {
     const size_t nth = 32 * (size_t)warps, H = (size_t)R * warps, SW = 32 * (size_t)C;
     return 8 * ((2 * (size_t)(maxw + 1) + CAV_QROWS * (size_t)maxw) * C * 32 + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nth) +
-           4 * xtab_words((int)nth, ns_per, nr_per);
+           4 * xtab_smem_words((int)nth, ns_per, nr_per);
 }
 
 // table entry (32 bits; NO_UNIT = none): bits 0-7 = local x of the unit's first point + 8 (it may be -2: groups are aligned to
@@ -488,12 +495,19 @@ __device__ __noinline__ void exchange_units(ulonglong4* __restrict__ xb, const u
     const int h = tid_o & 1, pr = tid_o >> 1, npr = nth_o >> 1;       // half, pair index, pairs in the CTA
     unsigned int* const img32 = reinterpret_cast<unsigned int*>(img) + 3 * h - 16;      // this lane's three words of a unit start here + 2 loc
     char* const xbh = reinterpret_cast<char*>(xb) + 16 * h;                            // ... and its 16 bytes of a unit here + 32 unit
-    for (int i = 0; i < ns_per; ++i) {
-        const unsigned int e = tab[i * npr + pr];
-        if (e != NO_UNIT) {                                            // strip points always lie inside the image: no masks
-            const unsigned int* const s = img32 + 2 * entry_loc(e, SW);
-            st_half(xbh + 32 * (size_t)entry_unit(e, ox, oy, upitch), half_pack(s[0], s[1], s[2], tag));
-        }
+    for (int i0 = 0; i0 < ns_per; i0 += 3) {                           // three slots at a time: their loads overlap
+        unsigned int e[3], A[3], B[3], Cw[3];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) e[j] = i0 + j < ns_per ? tab[(i0 + j) * npr + pr] : NO_UNIT;
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+            if (e[j] != NO_UNIT) {                                     // strip points always lie inside the image: no masks
+                const unsigned int* const s = img32 + 2 * entry_loc(e[j], SW);
+                A[j] = s[0]; B[j] = s[1]; Cw[j] = s[2];
+            }
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+            if (e[j] != NO_UNIT) st_half(xbh + 32 * (size_t)entry_unit(e[j], ox, oy, upitch), half_pack(A[j], B[j], Cw[j], tag));
     }
     if (stamp != nullptr && tid_o == 0) *stamp = globaltimer_ns();
     // All threads fetch ring half-units as 16-byte asynchronous copies into a landing zone in shared memory, NB slots per thread
@@ -787,6 +801,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
             const int n = (int)xtab_words(nthreads, a.ns_per, a.nr_per);
             const unsigned int* const src = a.tables + (size_t)(bj * a.ntx + bi) * n;
             for (int k = tid; k < n; k += nthreads) tabs[k] = src[k];
+            if (tid == 0) { tabs[n] = (unsigned int)t.ox; tabs[n + 1] = (unsigned int)t.oy; }
         }
     }
 
@@ -864,12 +879,12 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
             double* const land = img + H * SW + 2 * SW + 2 * H;
             const unsigned int* const tab = reinterpret_cast<const unsigned int*>(land + 2 * CAV_RECV_BATCH * nth_o);
             const unsigned int rows = tab[(a.ns_per + a.nr_per) * (nth_o >> 1) + tid_o];
-            const TileGeom tx = tile_geom(a.N + z, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, H);
+            const int tox = (int)tab[(a.ns_per + a.nr_per) * (nth_o >> 1) + nth_o], toy = (int)tab[(a.ns_per + a.nr_per) * (nth_o >> 1) + nth_o + 1];
             stage_tile<C, R>(p, img, ln, wp, rows);
             __syncthreads();
             exchange_units((round & 1u) ? a.x1 : a.x0, round, a.ns_per, a.nr_per, a.err,
                            (a.trace != nullptr && tslot + 1 < a.trace_cap) ? a.trace + (size_t)(blockIdx.y * a.ntx + blockIdx.x) * a.trace_cap + tslot + 1 : nullptr,
-                           img, tab, land, tid_o, nth_o, tx.ox, tx.oy, a.upitch, blockIdx.y * a.ntx + blockIdx.x);
+                           img, tab, land, tid_o, nth_o, tox, toy, a.upitch, blockIdx.y * a.ntx + blockIdx.x);
             ++round;
             __syncthreads();
             mark(a, tslot + 2);
