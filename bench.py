@@ -60,6 +60,8 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (default 4, the metric's)")
     ap.add_argument("--engine", default="auto", choices=["auto", "stream", "resident"])
+    ap.add_argument("--sweep", default="redblack", choices=["redblack", "jacobi", "compact9"],
+                    help="a1 variant (default: the red-black sweeps the metric is quoted on; compact9 = the paper's own operator, NEXT-1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-others", action="store_true", help="skip the other configs and the Poisson-only run")
@@ -221,7 +223,10 @@ def run_ours(args, wl, rank, world, local_rank):
     G = (wl.N + 1) ** 2
     P = (wl.N - 1) ** 2
     S = wl.sweeps_per_stage
-    cav = binding.Cavity(wl.N, wl.Re, wl.dt, wl.sor_omega, S, engine=args.engine)
+    beta = wl.sor_omega if args.sweep == "redblack" else min(wl.sor_omega, 0.8)
+    cav = binding.Cavity(wl.N, wl.Re, wl.dt, beta, S, engine=args.engine)
+    if args.sweep != "redblack":
+        cav.set_sweep(args.sweep)          # beta <= 1: the paper's under-relaxed range for its operator; the work per sweep does not depend on it
     psi0, w0 = W.initial_fields(wl)
     cav.set_fields(psi0, w0)
     if wl.poisson_sweeps:
@@ -284,7 +289,8 @@ def run_ours(args, wl, rank, world, local_rank):
     dfma_peak, nominal_mhz = cav.measure_fp64_peak()
     fp64_nominal = SM_COUNT * FP64_LANES_PER_SM * sm_max_mhz * 1e6
     launches_per_step = launches / float(K)
-    instr_per_step = 5.0 * P * (FP64_INSTR_PER_POINT_SWEEP * S + FP64_INSTR_PER_POINT_STAGE)
+    ips = 9 if args.sweep == "compact9" else FP64_INSTR_PER_POINT_SWEEP      # compact operator: 6 DADD + 3 DFMA per point-sweep
+    instr_per_step = 5.0 * P * (ips * S + FP64_INSTR_PER_POINT_STAGE)
     step_s = statistics.mean(per_step_ms) * 1e-3
     achieved = instr_per_step / step_s
     # a1 alone: sweep-only launches of the step's own shape (S sweeps), timed by the library's events around the a1 launch
@@ -299,7 +305,7 @@ def run_ours(args, wl, rank, world, local_rank):
         cav.poisson(S, want_residual=False)
         tsw += cav.last_elapsed_ms() * 1e-3
         lsw += cav.launch_count() - l1 - extra
-    sweep_rate = FP64_INSTR_PER_POINT_SWEEP * P * S * reps / tsw
+    sweep_rate = ips * P * S * reps / tsw
     traffic = NCU_DRAM_BYTES_PER_STEP_LAUNCH if (wl.N == 1024 and S == 200 and resident) else None
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": dfma_peak / 1e12, "unit": "T fp64 instr/s",
                 "frac": achieved / dfma_peak, "traffic": traffic, "traffic_source": NCU_DRAM_SOURCE if traffic else None,
@@ -321,7 +327,7 @@ def run_ours(args, wl, rank, world, local_rank):
 
     # ---- the other configs (bounded step counts) and the Poisson-only run of config 5 (BASELINE.json configs[4]) ----
     others, poisson_only = None, None
-    if rank == 0 and world == 1 and not args.no_others:
+    if rank == 0 and world == 1 and not args.no_others and args.sweep == "redblack":
         cav.close()
         others = {}
         for kcfg in (1, 2, 3, 5):
@@ -352,15 +358,29 @@ def run_ours(args, wl, rank, world, local_rank):
                                       "device-resident, L2 not flushed (the working set is on chip)" % nst,
                                       "plan": c2.describe()}
             c2.close()
+        # NEXT-1: the paper's own operator (4th-order compact 9-point, four-colour SOR) on the metric's config, resident engine
+        w4 = W.config(args.config)
+        c9 = binding.Cavity(w4.N, w4.Re, w4.dt, 0.8, w4.sweeps_per_stage, engine=args.engine)
+        c9.set_sweep("compact9")
+        c9.set_fields(*W.initial_fields(w4))
+        c9.step(2)
+        ts = []
+        for _ in range(3):
+            c9.step(10)
+            ts.append(c9.last_elapsed_ms() * 1e-3 / 10)
+        others["compact9_" + "cfg%d" % args.config] = {"workload": w4.name + ", compact 9-point operator (eq 14-21), beta 0.8", "ms_per_step": 1e3 * min(ts),
+                                                       "GPSU_per_s": 5.0 * (w4.N + 1) ** 2 / min(ts), "ratio_to_5_point_path": min(ts) / step_s,
+                                                       "steps_timed": 10, "plan": c9.describe()}
+        c9.close()
     else:
         cav.close()
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": 1e3 * t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl.name if world == 1 else W.config(args.config).name + " (rank 0) + Table-1 Re replicas",
+            "config": {"sweep": args.sweep, "workload": wl.name if world == 1 else W.config(args.config).name + " (rank 0) + Table-1 Re replicas",
                        "grid": "%dx%d" % (wl.N + 1, wl.N + 1), "Re": wl.Re, "sweeps_per_stage": S,
-                       "sor_omega": wl.sor_omega, "dt": wl.dt, "parallelism": "replicas x%d" % world,
+                       "sor_omega": beta, "dt": wl.dt, "parallelism": "replicas x%d" % world,
                        "l2": "flushed before every timed step (256 MiB write, outside the per-step CUDA events)",
                        "timing": "sum of per-step CUDA-event times on the launch stream, max over ranks"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,

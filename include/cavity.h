@@ -113,8 +113,10 @@ int cav_poisson(cav_ctx* ctx, int nsweeps, double* res_inf_out);
  * values (it converges for beta <= 1; nothing is checked).  With CAV_SWEEP_COMPACT9 a sweep is eq 15 of the paper,
  *   psi <- (3/5)(beta/a)(A + B + C) + (1 - beta) psi,  A, B, C of eq 16-18, a = 2/h^2,
  * whose B reads omega on the walls: the stage input carries the wall vorticity a2 computed in the previous stage (for the
- * first stage after cav_set_fields: the ring as given; reading N2).  Both variants run as kernels over global
- * memory whatever the engine (one per Jacobi sweep, four per compact sweep), inside a CUDA graph of the whole time step. */
+ * first stage after cav_set_fields: the ring as given; reading N2).  The Jacobi sweeps run as one kernel per sweep
+ * over global memory whatever the engine (inside a CUDA graph of the time step).  The compact sweeps run in the resident engine's
+ * persistent kernel like the red-black ones (four colour passes per sweep, halo 4T deep; the tiling is planned anew when the
+ * sweep kind changes), or, with CAV_ENGINE_STREAM, as four kernels per sweep over global memory; both agree bit for bit. */
 int cav_set_sweep(cav_ctx* ctx, int kind);
 
 /* One time step, and the paper's steady-state monitors of that step (eq 26-27):

@@ -156,7 +156,11 @@ void resolve_engine(cav_ctx* c) {
     if (e != c->engine) { c->engine = e; drop_graph(c); }
 }
 
-inline bool resident_path(const cav_ctx* c) { return c->engine == CAV_ENGINE_RESIDENT && c->sweep == CAV_SWEEP_REDBLACK; }
+// the resident kernel runs the red-black sweeps (plan kind 0) and the compact operator's four-colour sweeps (kind 1)
+inline int plan_kind(int sweep) { return sweep == CAV_SWEEP_COMPACT9 ? 1 : 0; }
+inline bool resident_path(const cav_ctx* c) {
+    return c->engine == CAV_ENGINE_RESIDENT && c->sweep != CAV_SWEEP_JACOBI && c->plan.ok && c->plan.kind == plan_kind(c->sweep);
+}
 
 // one launch of the resident kernel: nsteps whole time steps, or (nsteps = 0) S sweeps of a1 with right-hand side omega^n
 int enqueue_resident(cav_ctx* c, int nsteps, int S, long long& nl, long long* trace_dev = nullptr, int trace_cap = 0) {
@@ -427,7 +431,15 @@ CAV_API int cav_set_sweep(cav_ctx* c, int kind) {
     if (!c || kind < CAV_SWEEP_REDBLACK || kind > CAV_SWEEP_COMPACT9) return CAV_EINVAL;
     DeviceGuard dg(c->device);
     CK(cudaStreamSynchronize(c->st));
-    if (kind != c->sweep) { c->sweep = kind; drop_graph(c); }
+    if (kind != c->sweep) {
+        c->sweep = kind;
+        drop_graph(c);
+        if (kind != CAV_SWEEP_JACOBI && c->plan.kind != plan_kind(kind)) {       // the halo depth per sweep differs: plan anew
+            c->plan = cavk::resident_plan(c->P, c->device, 0, -1, plan_kind(kind));
+            build_plan_tables(c);
+            resolve_engine(c);
+        }
+    }
     return CAV_OK;
 }
 
@@ -493,7 +505,7 @@ CAV_API int cav_set_resident_plan(cav_ctx* c, int sweeps_per_exchange, int varia
     if (!c || sweeps_per_exchange < 0 || variant >= cavk::resident_variants()) return CAV_EINVAL;
     DeviceGuard dg(c->device);
     CK(cudaStreamSynchronize(c->st));
-    cavk::ResidentPlan pl = cavk::resident_plan(c->P, c->device, sweeps_per_exchange, variant < 0 ? -1 : variant);
+    cavk::ResidentPlan pl = cavk::resident_plan(c->P, c->device, sweeps_per_exchange, variant < 0 ? -1 : variant, plan_kind(c->sweep));
     if (!pl.ok) return CAV_ENOTSUP;
     const cavk::ResidentPlan old = c->plan;
     c->plan = pl;

@@ -83,6 +83,7 @@ __device__ constexpr double RK5_A4 = 0.386708617503269, RK5_C4 = 0.2260074832369
 struct ResArgs {
     int N, pitch;
     double cb, omb, cq;                 // a1
+    double c9e, c9c, c9q;               // a1, compact 9-point operator (NEXT-1): 0.2 beta, 0.05 beta, (0.025 beta) h^2
     double i2h, ih2, nu, c2h2, lid, dt; // a2, a3
     const double* psi_in;   // stream function before the launch
     double* psi_out;        // ... and after (a different field)
@@ -97,6 +98,7 @@ struct ResArgs {
     int S;                  // sweeps per stage (nsteps > 0) or in total (nsteps == 0)
     int T, halo, CW, CH, ntx, nty;
     int ns_per, nr_per;     // table entries per thread: strip units to store / ring units to fetch
+    int walls;              // the exchanged regions include the wall points (compact operator)
     const unsigned int* tables;   // per-plan exchange tables, one block per tile (k_build_tables)
     long long* trace;       // profiling only (cav_trace_sweeps): per tile, %globaltimer at the phase boundaries; else null
     int trace_cap;          // slots per tile
@@ -274,6 +276,78 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
     __syncthreads();
 }
 
+// NEXT-1: one colour pass of the paper's 4th-order compact 9-point operator (eq 14-21) relaxed in four colours
+// (reading N1), on the register micro-tile.  (KX, KY) = LOCAL colour being updated: the points with ci & 1 == KX and
+// rj & 1 == KY (six per thread); all eight neighbours of such a point belong to the three other colours.
+//     se = (W + E) + (S + N);  sc = (SW + SE) + (NW + NE);  psi <- fma(1 - beta, psi, fma(0.2 beta, se, fma(0.05 beta, sc, qB)))
+// (the expression of k_compact_colour).  From the other threads a pass needs ONE side column (the lane to the left if KX == 0, to
+// the right if KX == 1: six doubles by shuffle) and ONE edge row of five values (the warp below if KY == 0, above if KY == 1: the
+// edge arrays, whose neighbouring lane slots give the two diagonal values).
+template <int C, int R, int KX, int KY, bool FIX, int TOPOFF>
+__device__ __forceinline__ void colour_pass(double (&p)[R][C], const double (&q)[R][C], const double c9e, const double c9c, const double omb,
+                                            double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl_) {
+    static_assert(C == 4 && R == 6 && CAV_QROWS == 2, "written for the 4 x 6 micro-tile with q of rows 2, 3 in shared memory");
+    unsigned int fl = fl_;
+    asm volatile("" : "+r"(fl));               // opaque: the bit tests below are redone here, not hoisted into registers of their own
+    double* const sT = sB + TOPOFF;
+    double qs[C], side[R], edge[C + 2];        // edge[1 + c] = column c of the row below (KY == 0) / above (KY == 1), c = -1 .. C
+#pragma unroll
+    for (int ci = KX; ci < C; ci += 2) qs[ci] = sB[2 * TOPOFF + KY * (TOPOFF - C * 32) + ci * 32];      // q of row 2 + KY
+    {
+        const double* const er = KY == 0 ? sT : sB + C * 32;       // top row of the warp below (slot warp) / bottom row of the warp above
+#pragma unroll
+        for (int c = 0; c < C; ++c) edge[1 + c] = er[c * 32];
+        if (KX == 0) {
+            const double v = er[(C - 1) * 32 - 1];                  // column C - 1 of the lane to the left
+            edge[0] = (fl & FL_ZERO_LEFT) ? 0.0 : v;
+        } else {
+            const double v = er[1];                                 // column 0 of the lane to the right
+            edge[C + 1] = (fl & FL_ZERO_RIGHT) ? 0.0 : v;
+        }
+    }
+#pragma unroll
+    for (int rj = 0; rj < R; ++rj) {
+        if (KX == 0) {
+            const double v = __shfl_up_sync(0xffffffffu, p[rj][C - 1], 1);
+            side[rj] = (fl & FL_ZERO_LEFT) ? 0.0 : v;
+        } else {
+            const double v = __shfl_down_sync(0xffffffffu, p[rj][0], 1);
+            side[rj] = (fl & FL_ZERO_RIGHT) ? 0.0 : v;
+        }
+    }
+    // value at (column c, row r) around the micro-tile, c in -1 .. C, r in -1 .. R (only what this colour needs is ever asked for)
+    auto at = [&](int c, int r) -> double {
+        if (r < 0 || r >= R) return edge[1 + c];
+        if (c < 0 || c >= C) return side[r];
+        return p[r][c];
+    };
+#pragma unroll
+    for (int rj = KY; rj < R; rj += 2) {
+#pragma unroll
+        for (int ci = KX; ci < C; ci += 2) {
+            const double se = (at(ci - 1, rj) + at(ci + 1, rj)) + (at(ci, rj - 1) + at(ci, rj + 1));
+            const double sc = (at(ci - 1, rj - 1) + at(ci + 1, rj - 1)) + (at(ci - 1, rj + 1) + at(ci + 1, rj + 1));
+            const double qv = (rj == 2 + KY) ? qs[ci] : q[rj][ci];
+            p[rj][ci] = fma(omb, p[rj][ci], fma(c9e, se, fma(c9c, sc, qv)));
+        }
+    }
+    unsigned int wm = FIX ? wallmask : 0u;
+    if (FIX) asm volatile("" : "+r"(wm));
+    if (FIX && wm) {
+#pragma unroll
+        for (int rj = KY; rj < R; rj += 2)
+#pragma unroll
+            for (int ci = KX; ci < C; ci += 2)
+                if ((wm >> (rj * C + ci)) & 1u) p[rj][ci] = 0.0;
+    }
+#pragma unroll
+    for (int ci = KX; ci < C; ci += 2) {
+        if (KY == 0 && (fl & FL_PUB_BOTTOM)) sB[ci * 32] = p[0][ci];
+        if (KY == 1 && (fl & FL_PUB_TOP)) sT[C * 32 + ci * 32] = p[R - 1][ci];
+    }
+    __syncthreads();
+}
+
 template <int C, int R, int TOPOFF>
 __device__ __forceinline__ void publish_all(const double (&p)[R][C], double* __restrict__ sB, const unsigned int fl) {
     double* const sT = sB + TOPOFF;
@@ -320,8 +394,10 @@ __host__ __device__ inline URect urect_of(int x0, int x1, int y0, int y1) {     
     return r;
 }
 // Interior points of the core within `halo` of a core edge that has a neighbour tile behind it (walls are never needed).
-__host__ __device__ inline URegion send_units(const TileGeom& t, int N, int halo, int bi, int bj, int ntx, int nty) {
-    const int X0 = imax(t.cx0, 1), X1 = imin(t.cx1, N), Y0 = imax(t.cy0, 1), Y1 = imin(t.cy1, N);
+// walls: the wall points too (compact operator: its right-hand side at the points next to a wall reads omega ON the wall, also in the ring)
+__host__ __device__ inline URegion send_units(const TileGeom& t, int N, int halo, int bi, int bj, int ntx, int nty, bool walls) {
+    const int lo = walls ? 0 : 1, hi = walls ? N + 1 : N;
+    const int X0 = imax(t.cx0, lo), X1 = imin(t.cx1, hi), Y0 = imax(t.cy0, lo), Y1 = imin(t.cy1, hi);
     const int hb = bj > 0 ? halo : 0, ht = bj < nty - 1 ? halo : 0, wl = bi > 0 ? halo : 0, wr = bi < ntx - 1 ? halo : 0;
     const int yB = imin(Y0 + hb, Y1), yT = imax(Y1 - ht, yB), xL = imin(X0 + wl, X1), xR = imax(X1 - wr, xL);
     URegion g;
@@ -333,8 +409,9 @@ __host__ __device__ inline URegion send_units(const TileGeom& t, int N, int halo
     return g;
 }
 // Interior points within `halo` of the core, outside it (the ring).
-__host__ __device__ inline URegion recv_units(const TileGeom& t, int N, int halo) {
-    const int xlo = imax(t.cx0 - halo, 1), xhi = imin(t.cx1 + halo, N), ylo = imax(t.cy0 - halo, 1), yhi = imin(t.cy1 + halo, N);
+__host__ __device__ inline URegion recv_units(const TileGeom& t, int N, int halo, bool walls) {
+    const int lo = walls ? 0 : 1, hi = walls ? N + 1 : N;
+    const int xlo = imax(t.cx0 - halo, lo), xhi = imin(t.cx1 + halo, hi), ylo = imax(t.cy0 - halo, lo), yhi = imin(t.cy1 + halo, hi);
     const int yc0 = imax(t.cy0, ylo), yc1 = imin(t.cy1, yhi), xc0 = imax(t.cx0, xlo), xc1 = imin(t.cx1, xhi);
     // Order = the order in which the neighbours STORE these units (send_units: bottom strip, top strip, left, right), so
     // that what was stored first is fetched first: the ring above comes from the northern tiles' bottom strips, etc.
@@ -389,7 +466,7 @@ __global__ void k_build_tables(const ResArgs a, unsigned int* __restrict__ out) 
     const int N = a.N, bi = blockIdx.x, bj = blockIdx.y;
     const TileGeom t = tile_geom(N, a.CW, a.CH, a.halo, a.ntx, a.nty, bi, bj, C, R, 32 * C, nwarps * R);
     unsigned int* const o = out + (size_t)(bj * a.ntx + bi) * xtab_words(nthreads, a.ns_per, a.nr_per);
-    const URegion gs = send_units(t, N, a.halo, bi, bj, a.ntx, a.nty), gr = recv_units(t, N, a.halo);
+    const URegion gs = send_units(t, N, a.halo, bi, bj, a.ntx, a.nty, a.walls != 0), gr = recv_units(t, N, a.halo, a.walls != 0);
     const int npr = nthreads / 2;                                              // one entry per pair of adjacent lanes
     for (int i = 0; i < a.ns_per + a.nr_per; ++i) {
         if (tid >= npr) break;
@@ -446,12 +523,13 @@ __device__ __forceinline__ void read_tile(double (&v)[R][C], const double* __res
 // takes whole image rows (rows warp, warp + nwarps, ...: R of them), a lane the columns lane + 32 j.  cg: the field may have been
 // written by this CTA during this launch.  The loads are issued in two batches of R C / 2, all of a batch in flight together
 // (an L2 round trip per element, one after the other, would cost more than the whole stage combination).
-template <int C, int R>
+template <int C, int R, bool WALLS = false>
 __device__ __forceinline__ void fill_image(double* __restrict__ img, const double* __restrict__ g, const int x0, const int x1,
                                            const int y0, const int y1, const int ox, const int oy, const int nwarps, const int N,
                                            const int pitch, const int lane, const int warp) {
     constexpr int SW = 32 * C;
-    const int xa = imax(x0, 1), xb = imin(x1, N), ya = imax(y0, 1), yb = imin(y1, N);
+    // WALLS: the wall points too (the compact operator's right-hand side reads omega on the walls)
+    const int xa = imax(x0, WALLS ? 0 : 1), xb = imin(x1, WALLS ? N + 1 : N), ya = imax(y0, WALLS ? 0 : 1), yb = imin(y1, WALLS ? N + 1 : N);
     unsigned int colok = 0;
 #pragma unroll
     for (int j = 0; j < C; ++j)
@@ -577,13 +655,37 @@ __device__ __noinline__ void exchange_units(ulonglong4* __restrict__ xb, const u
     }
 }
 
+// NEXT-1: the right-hand side of the compact sweeps from the image of omega (walls included):
+//     qB = ((0.025 beta) h^2) (((wW + wE) + (wS + wN)) + 8 w0) on interior points, +0.0 elsewhere   (k_compact_rhs)
+// The outermost ring of the tile gets a value computed from whatever lies beyond it: that ring is only ever read, never updated.
+template <int C, int R>
+__device__ __forceinline__ void qb_from_image(double (&q)[R][C], const double* __restrict__ img, const double c9q, const int gx0,
+                                              const int gy0, const int N, const int lane, const int warp) {
+    constexpr int SW = 32 * C;
+    const double* const s = img + (warp * R) * SW + lane * C;
+#pragma unroll
+    for (int rj = 0; rj < R; ++rj) {
+        double wc[C + 2];
+        wc[0] = s[rj * SW - 1]; wc[C + 1] = s[rj * SW + C];
+#pragma unroll
+        for (int ci = 0; ci < C; ++ci) wc[1 + ci] = s[rj * SW + ci];
+#pragma unroll
+        for (int ci = 0; ci < C; ++ci) {
+            const int gx = gx0 + ci, gy = gy0 + rj;
+            const bool inter = gx >= 1 && gx <= N - 1 && gy >= 1 && gy <= N - 1;
+            const double v = c9q * (((wc[ci] + wc[ci + 2]) + (s[(rj - 1) * SW + ci] + s[(rj + 1) * SW + ci])) + 8.0 * wc[1 + ci]);
+            q[rj][ci] = inter ? v : 0.0;
+        }
+    }
+}
+
 __device__ __forceinline__ double thom_wall(double c2h2, double p_adj) { return -(c2h2 * p_adj); }
 __device__ __forceinline__ double thom_lid(double c2h2, double lid, double p_adj) { return -(c2h2 * p_adj) - lid; }
 
 // a2 + a3 of one stage for this tile (see the file header).  pl: the thread's psi micro-tile, [rj * C + ci].  On return the
 // image holds the NEW vorticity on core + halo (+0.0 elsewhere) and the ring copy is refreshed; the caller turns it into q.
 // Not inlined: see exchange_units.
-template <int C, int R, int MAXW>
+template <int C, int R, int MAXW, int KIND>
 __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R][C], double* __restrict__ sm, const int stage,
                                        const unsigned int round, const unsigned int fl) {
     constexpr int TOPOFF = (MAXW + 1) * C * 32;
@@ -743,6 +845,26 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
         for (int ci = 0; ci < C; ++ci)
             if (!(((rowin >> rj) & 1u) && ((colin >> ci) & 1u))) ab[rj][ci] = 0.0;
     stage_tile<C, R>(ab, img, ln, wp, 0x3fu);
+    if (KIND == 1) {
+        // NEXT-1: B of eq 17 reads omega on the walls: the stage output carries the wall vorticity just computed (reading N2),
+        // so the image of the new vorticity gets it too (neighbours fetch it with the ring; corners are never read)
+        __syncthreads();              // the zeros staged by the owners of the wall points are in place
+        if ((gx0 <= 1 || gx0 + C - 1 >= Ne - 1 || gy0 <= 1 || gy0 + R - 1 >= Ne - 1)) {
+#pragma unroll
+            for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+                for (int ci = 0; ci < C; ++ci) {
+                    const int gx = gx0 + ci, gy = gy0 + rj;
+                    if (gx < X0 || gx >= X1 || gy < Y0 || gy >= Y1) continue;
+                    const int ir_ = row0 + rj, ix_ = lx0 + ci;
+                    const double pv = pp[rj][ci];
+                    if (gx == 1) img[img_ix(ir_, ix_ - 1, SW)] = thom_wall(a.c2h2, pv);
+                    if (gx == Ne - 1) img[img_ix(ir_, ix_ + 1, SW)] = thom_wall(a.c2h2, pv);
+                    if (gy == 1) img[img_ix(ir_ - 1, ix_, SW)] = thom_wall(a.c2h2, pv);
+                    if (gy == Ne - 1) img[img_ix(ir_ + 1, ix_, SW)] = thom_lid(a.c2h2, a.lid, pv);
+                }
+        }
+    }
     __syncthreads();
     if (a.ntx * a.nty > 1) {
         double* const land = img + H * SW + 2 * SW + 2 * H;
@@ -761,7 +883,8 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
 }
 
 // MAXW = most warps per CTA the kernel is launched with: 65536 / (32 MAXW) registers per thread are available.
-template <int C, int R, int MAXW, bool FIX>
+// KIND: 0 = red-black sweeps of the 5-point operator (a1), 1 = four-colour sweeps of the compact 9-point operator (NEXT-1)
+template <int C, int R, int MAXW, bool FIX, int KIND>
 __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant__ ResArgs a) {
     constexpr int TOPOFF = (MAXW + 1) * C * 32;
     constexpr int SW = 32 * C;
@@ -783,6 +906,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
     // local colour = global colour ^ odd_origin.  Computed from blockIdx only: the branch on it is uniform for the compiler
     // too, so the sweep loops stay convergent code (uniform registers for the coefficients, no divergence guards on the shuffles)
     const bool odd_origin = ((t.ox + t.oy) & 1) != 0;
+    const int par9 = (t.ox & 1) | ((t.oy & 1) << 1);            // compact operator: parity of the origin in x and y
     unsigned int fl = FL_PUB_BOTTOM | FL_PUB_TOP;
     {
         const int lzl = t.left_al ? 1 : 0;                                     // lane 0 holds x = -(C-1) .. 0
@@ -815,9 +939,10 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
         __syncthreads();
         read_tile<C, R>(p, img, lane, warp, 0x3fu);
         __syncthreads();
-        fill_image<C, R>(img, a.wbase, 0, N + 1, 0, N + 1, t.ox, t.oy, nwarps, N, a.pitch, lane, warp);
+        fill_image<C, R, KIND == 1>(img, a.wbase, 0, N + 1, 0, N + 1, t.ox, t.oy, nwarps, N, a.pitch, lane, warp);
         __syncthreads();
-        read_tile<C, R>(q, img, lane, warp, 0x3fu);
+        if (KIND == 1) qb_from_image<C, R>(q, img, a.c9q, gx0_, gy0_, N, lane, warp);
+        else read_tile<C, R>(q, img, lane, warp, 0x3fu);
         if (a.nsteps > 0) {               // first ring of the stage input around the core, kept for a3
             double* const wr = img + H * SW;
             const int rB = imax(t.cy0, 1) - 1 - t.oy, rT = imin(t.cy1, N) - t.oy, cL = imax(t.cx0, 1) - 1 - t.ox, cR = imin(t.cx1, N) - t.ox;
@@ -825,10 +950,12 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
             for (int k = tid; k < H; k += nthreads) { wr[2 * SW + k] = img[img_ix(k, cL, SW)]; wr[2 * SW + H + k] = img[img_ix(k, cR, SW)]; }
         }
     }
+    if (KIND == 0) {
 #pragma unroll
-    for (int rj = 0; rj < R; ++rj)
+        for (int rj = 0; rj < R; ++rj)
 #pragma unroll
-        for (int ci = 0; ci < C; ++ci) q[rj][ci] = a.cq * q[rj][ci];          // +0.0 where the point is not interior
+            for (int ci = 0; ci < C; ++ci) q[rj][ci] = a.cq * q[rj][ci];      // +0.0 where the point is not interior
+    }
     if (FIX) {
 #pragma unroll 1
         for (int k = 0; k < R * C; ++k) {
@@ -854,7 +981,18 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
     for (int stage = 0; stage < (a.nsteps > 0 ? 5 * a.nsteps : 1); ++stage) {
         // ================= a1: S sweeps, a halo exchange after every T of them =================
         for (int rem = a.S; rem > 0; rem -= a.T) {
-            if (odd_origin) {
+            if (KIND == 1) {
+                // four colours (i mod 2, j mod 2) in the order (0,0), (1,0), (0,1), (1,1) (reading N1); local colour = global ^ origin parity
+                for (int s = min(a.T, rem); s > 0; --s)
+                    for (int g = 0; g < 4; ++g) {
+                        switch (g ^ par9) {
+                            case 0: colour_pass<C, R, 0, 0, FIX, TOPOFF>(p, q, a.c9e, a.c9c, a.omb, sB, wallmask, fl); break;
+                            case 1: colour_pass<C, R, 1, 0, FIX, TOPOFF>(p, q, a.c9e, a.c9c, a.omb, sB, wallmask, fl); break;
+                            case 2: colour_pass<C, R, 0, 1, FIX, TOPOFF>(p, q, a.c9e, a.c9c, a.omb, sB, wallmask, fl); break;
+                            default: colour_pass<C, R, 1, 1, FIX, TOPOFF>(p, q, a.c9e, a.c9c, a.omb, sB, wallmask, fl); break;
+                        }
+                    }
+            } else if (odd_origin) {
                 for (int s = min(a.T, rem); s > 0; --s) {                         // red = (i + j) even first (G9): local colour 1 here
                     half_sweep<C, R, 1, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
                     half_sweep<C, R, 0, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
@@ -896,16 +1034,21 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
 
         // ================= a2 + a3: wall vorticity, transport right-hand side, stage combination =================
         {
-            rhs_phase<C, R, MAXW>(a, p, sm, stage, round, fl);
+            rhs_phase<C, R, MAXW, KIND>(a, p, sm, stage, round, fl);
             if (a.ntx * a.nty > 1) ++round;                                     // the vorticity exchange
             const int z = opaque_zero();
             const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
             double* const img = sm + edge_doubles;
-            read_tile<C, R>(q, img, ln, wp, 0x3fu);
+            if (KIND == 1) {
+                const TileGeom tq = tile_geom(a.N + z, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, ((int)blockDim.y + z) * R);
+                qb_from_image<C, R>(q, img, a.c9q, tq.ox + ln * C, tq.oy + wp * R, a.N + z, ln, wp);
+            } else {
+                read_tile<C, R>(q, img, ln, wp, 0x3fu);
 #pragma unroll
-            for (int rj = 0; rj < R; ++rj)
+                for (int rj = 0; rj < R; ++rj)
 #pragma unroll
-                for (int ci = 0; ci < C; ++ci) q[rj][ci] = a.cq * q[rj][ci];
+                    for (int ci = 0; ci < C; ++ci) q[rj][ci] = a.cq * q[rj][ci];
+            }
 #pragma unroll
             for (int ci = 0; ci < C; ++ci) {
 #pragma unroll
@@ -937,12 +1080,13 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
 // ---- compiled variants ------------------------------------------------------------------------------
 struct Variant {
     int C, R, maxw;
-    const void* fn;        // every wall isolated by alignment (the plans of large grids)
-    const void* fn_fix;    // with the wall-mask fix-up (a tile that holds both walls of one direction)
+    const void* fn[2];        // [kind] every wall isolated by alignment (the plans of large grids)
+    const void* fn_fix[2];    // [kind] with the wall-mask fix-up (a tile that holds both walls of one direction)
 };
 const Variant VARIANTS[] = {
-    // one CTA of up to 16 warps per SM (also the single-tile plans of small grids)
-    {4, 6, 16, (const void*)k_resident<4, 6, 16, false>, (const void*)k_resident<4, 6, 16, true>},
+    // one CTA of up to 16 warps per SM (also the single-tile plans of small grids); kind 0 = red-black 5-point, 1 = compact 9-point
+    {4, 6, 16, {(const void*)k_resident<4, 6, 16, false, 0>, (const void*)k_resident<4, 6, 16, false, 1>},
+               {(const void*)k_resident<4, 6, 16, true, 0>, (const void*)k_resident<4, 6, 16, true, 1>}},
 };
 constexpr int NVARIANTS = sizeof(VARIANTS) / sizeof(VARIANTS[0]);
 
@@ -958,8 +1102,8 @@ bool finish_plan(ResidentPlan& pl, int N, int max_smem) {
             const TileGeom t = tile_geom(N, pl.CW, pl.CH, pl.halo, pl.ntx, pl.nty, bi, bj, pl.C, pl.R, W, H);
             if (!t.fits) return false;
             if (pl.ntiles > 1) {
-                smax = std::max(smax, uregion_total(send_units(t, N, pl.halo, bi, bj, pl.ntx, pl.nty)));
-                rmax = std::max(rmax, uregion_total(recv_units(t, N, pl.halo)));
+                smax = std::max(smax, uregion_total(send_units(t, N, pl.halo, bi, bj, pl.ntx, pl.nty, pl.kind == 1)));
+                rmax = std::max(rmax, uregion_total(recv_units(t, N, pl.halo, pl.kind == 1)));
             }
         }
     pl.ns_per = cdiv(smax, nth / 2);         // units per PAIR of lanes (a lane moves one 16-byte half of each)
@@ -991,7 +1135,7 @@ bool split(int G, int L, int lead, int h, int align, int& core, int& n) {
 
 }  // namespace
 
-ResidentPlan resident_plan(const Params& P, int device, int T_override, int variant_override) {
+ResidentPlan resident_plan(const Params& P, int device, int T_override, int variant_override, int kind) {
     ResidentPlan best;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); return best; }
@@ -1006,7 +1150,7 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
         if (variant_override >= 0 && vi != variant_override) continue;
         const Variant& v = VARIANTS[vi];
         cudaFuncAttributes fa, fb;
-        if (cudaFuncGetAttributes(&fa, v.fn) != cudaSuccess || cudaFuncGetAttributes(&fb, v.fn_fix) != cudaSuccess) { cudaGetLastError(); continue; }
+        if (cudaFuncGetAttributes(&fa, v.fn[kind]) != cudaSuccess || cudaFuncGetAttributes(&fb, v.fn_fix[kind]) != cudaSuccess) { cudaGetLastError(); continue; }
         const int regs = std::max(fa.numRegs, fb.numRegs);
         const int max_threads = std::min(fa.maxThreadsPerBlock, fb.maxThreadsPerBlock);
         const int max_warps = std::min(v.maxw, std::min(max_threads / 32, (int)(prop.regsPerBlock / (32 * std::max(regs, 1)))));
@@ -1016,31 +1160,32 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
         for (int warps = 1; warps <= max_warps; ++warps) {
             const int H = warps * v.R;           // tile height in points
             ResidentPlan c;
-            c.ok = true; c.variant = vi; c.C = v.C; c.R = v.R; c.warps = warps; c.regs = regs; c.sm_count = sms; c.per_sm = 1;
+            c.ok = true; c.variant = vi; c.C = v.C; c.R = v.R; c.warps = warps; c.regs = regs; c.sm_count = sms; c.per_sm = 1; c.kind = kind;
+            const double sweep_cost = (kind == 1 ? 2.2 : 1.0) * sweep_cycles(warps);      // four colour passes of 54 fp64 instructions instead of two of 60
             // single tile: the whole grid in one CTA, no exchange at all
             if (G + v.C - 1 <= W && G + v.R - 1 <= H) {
-                const double cost = sweep_cycles(warps);
+                const double cost = sweep_cost;
                 c.T = 1 << 30; c.halo = 0; c.CW = G; c.CH = G; c.ntx = c.nty = c.ntiles = 1;
                 if (cost < best_cost && finish_plan(c, P.N, smem_cap)) { best_cost = cost; best = c; }
                 continue;
             }
             for (int T = 1; T <= 10; ++T) {
                 if (T_override > 0 && T != T_override) continue;
-                const int halo = 2 * T;
+                const int halo = (kind == 1 ? 4 : 2) * T;      // one ring is consumed per colour pass
                 int CW, ntx, CH, nty;
                 if (!split(G, W, v.C - 1, halo, 3, CW, ntx) || !split(G, H, v.R - 1, halo, 1, CH, nty)) continue;
                 const int ntiles = ntx * nty;
                 if (ntiles < 2 || ntiles > sms) continue;
                 // Cost per sweep in SM cycles, calibrated on B200 (profiles/r2_*.md): a colour half-sweep takes ~187 cycles per warp
                 // of the busiest SM sub-partition (+ barrier), an exchange ~6500 cycles + 250 per sweep of halo depth, mostly latency.
-                const double cost = sweep_cycles(warps) + (6500.0 + 250.0 * T) / T;
+                const double cost = sweep_cost + (6500.0 + 125.0 * halo) / T;
                 c.T = T; c.halo = halo; c.CW = CW; c.CH = CH; c.ntx = ntx; c.nty = nty; c.ntiles = ntiles;
                 if (cost < best_cost && finish_plan(c, P.N, smem_cap)) { best_cost = cost; best = c; }
             }
         }
     }
     if (best.ok) {
-        const void* fn = best.fixup ? VARIANTS[best.variant].fn_fix : VARIANTS[best.variant].fn;
+        const void* fn = best.fixup ? VARIANTS[best.variant].fn_fix[kind] : VARIANTS[best.variant].fn[kind];
         if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin) != cudaSuccess) {
             cudaGetLastError();
             best.ok = false;
@@ -1059,13 +1204,13 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
 void resident_describe(const ResidentPlan& pl, char* buf, int len) {
     if (!pl.ok) { std::snprintf(buf, (size_t)len, "none"); return; }
     if (pl.ntiles == 1)
-        std::snprintf(buf, (size_t)len, "1 tile, %d warps x (%dx%d micro-tiles), whole time steps on chip, %d regs, %d B smem",
-                      pl.warps, pl.C, pl.R, pl.regs, pl.smem_bytes);
+        std::snprintf(buf, (size_t)len, "%s1 tile, %d warps x (%dx%d micro-tiles), whole time steps on chip, %d regs, %d B smem",
+                      pl.kind == 1 ? "compact 9-point operator, " : "", pl.warps, pl.C, pl.R, pl.regs, pl.smem_bytes);
     else
         std::snprintf(buf, (size_t)len,
-                      "%dx%d tiles of %dx%d core + halo %d, T=%d sweeps per exchange, %d warps x (%dx%d micro-tiles), "
+                      "%s%dx%d tiles of %dx%d core + halo %d, T=%d sweeps per exchange, %d warps x (%dx%d micro-tiles), "
                       "%d+%d exchange half-units (16 B) per thread, %d regs, %d B smem, one CTA per SM on %d SMs",
-                      pl.ntx, pl.nty, pl.CW, pl.CH, pl.halo, pl.T, pl.warps, pl.C, pl.R, pl.ns_per, pl.nr_per, pl.regs,
+                      pl.kind == 1 ? "compact 9-point operator, " : "", pl.ntx, pl.nty, pl.CW, pl.CH, pl.halo, pl.T, pl.warps, pl.C, pl.R, pl.ns_per, pl.nr_per, pl.regs,
                       pl.smem_bytes, pl.sm_count);
 }
 
@@ -1080,7 +1225,7 @@ int resident_build_tables(const Params& P, const ResidentPlan& pl, void* tables_
     ResArgs a{};
     a.N = P.N; a.pitch = P.pitch; a.upitch = resident_unit_pitch(P.N);
     a.halo = pl.halo; a.CW = pl.CW; a.CH = pl.CH; a.ntx = pl.ntx; a.nty = pl.nty;
-    a.ns_per = pl.ns_per; a.nr_per = pl.nr_per;
+    a.ns_per = pl.ns_per; a.nr_per = pl.nr_per; a.walls = pl.kind == 1;
     const dim3 grid(pl.ntx, pl.nty), block(32, pl.warps);
     if (pl.C == 4 && pl.R == 6) k_build_tables<4, 6><<<grid, block, 0, st>>>(a, (unsigned int*)tables_dev);
     else return -(int)cudaErrorNotSupported;
@@ -1103,6 +1248,7 @@ int resident_launch(const Params& P, const ResidentPlan& pl, const double* psi_i
     ResArgs a{};
     a.tables = (const unsigned int*)tables;
     a.N = P.N; a.pitch = P.pitch; a.cb = P.cb; a.omb = P.omb; a.cq = P.cq;
+    a.c9e = P.c9e; a.c9c = P.c9c; a.c9q = P.c9q;
     a.i2h = P.i2h; a.ih2 = P.ih2; a.nu = P.nu; a.c2h2 = P.c2h2; a.lid = P.lid; a.dt = P.dt;
     a.psi_in = psi_in; a.psi_out = psi_out; a.wbase = wbase; a.fstride = fstride;
     a.x0 = (ulonglong4*)xa; a.x1 = (ulonglong4*)xb; a.upitch = resident_unit_pitch(P.N);
@@ -1116,7 +1262,7 @@ int resident_launch(const Params& P, const ResidentPlan& pl, const double* psi_i
     *epoch += (unsigned int)resident_rounds(pl, nsteps, S);      // wraps harmlessly: tags only tell round r from round r - 2
     void* args[] = {&a};
     const dim3 grid(pl.ntx, pl.nty), block(32, pl.warps);
-    const void* fn = pl.fixup ? VARIANTS[pl.variant].fn_fix : VARIANTS[pl.variant].fn;
+    const void* fn = pl.fixup ? VARIANTS[pl.variant].fn_fix[pl.kind] : VARIANTS[pl.variant].fn[pl.kind];
     const cudaError_t e = cudaLaunchCooperativeKernel(fn, grid, block, args, (size_t)pl.smem_bytes, st);
     if (e != cudaSuccess) { cudaGetLastError(); return -(int)e; }
     return 1;

@@ -16,7 +16,7 @@ struct ResidentPlan {
     int C = 0, R = 0;     // micro-tile: each thread owns C consecutive x-points times R rows, in registers
     int warps = 0;        // warps per CTA; a warp spans 32 C points in x and R rows in y
     int T = 0;            // sweeps per round (between two halo exchanges); single tile: unused
-    int halo = 0;         // 2 T (one ring is consumed per colour half-sweep); 0 for a single tile
+    int halo = 0;         // 2 T, compact operator 4 T (one ring is consumed per colour pass); 0 for a single tile
     int CW = 0, CH = 0;   // core (owned) points per tile in x and y; tile (bi, bj) owns [bi CW, (bi+1) CW) x [bj CH, (bj+1) CH)
     int ntx = 0, nty = 0; // tiles in x and y
     int ntiles = 0;
@@ -26,11 +26,12 @@ struct ResidentPlan {
     int regs = 0;         // registers per thread of the chosen variant (as compiled)
     int sm_count = 0;
     int per_sm = 1;       // CTAs per SM
+    int kind = 0;         // 0 = red-black sweeps of the 5-point operator (halo 2T), 1 = four-colour sweeps of the compact 9-point operator (halo 4T)
 };
 
 // T_override > 0 forces the sweeps per round (1..10; tests use it to exercise short and ragged rounds);
 // variant_override >= 0 forces the micro-tile shape (index into the compiled variants).
-ResidentPlan resident_plan(const Params& P, int device, int T_override = 0, int variant_override = -1);
+ResidentPlan resident_plan(const Params& P, int device, int T_override = 0, int variant_override = -1, int kind = 0);
 int resident_variants();
 void resident_describe(const ResidentPlan& plan, char* buf, int len);
 

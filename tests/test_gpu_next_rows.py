@@ -205,3 +205,37 @@ def test_compact9_config1_contract_and_cavity_physics(cav, orc):
     assert relerr(gp, op) <= TOL and relerr(gw, ow) <= TOL
     assert gp.min() < -0.05 and np.isfinite(gw).all()
     g.close(); o.close()
+
+
+@pytest.mark.parametrize("N,S", [(257, 7), (513, 5), (1024, 4)])
+@pytest.mark.parametrize("T", [0, 1, 2, 3])
+def test_compact9_resident_engine_matches_the_stream_kernels(cav, N, S, T):
+    """NEXT-1 on the resident engine (four colour passes per sweep in the persistent kernel, halo 4T, wall vorticity exchanged
+    with the ring) against the four-kernels-per-sweep path over global memory: bit for bit, sweeps-only launches and whole
+    time steps, forced and planned exchange periods (ragged last rounds included)."""
+    psi0, w0 = random_fields(N, 1357 + N + T)
+    g = cav.Cavity(N, 1500.0, 0.4 / N, 1.1, S, engine="resident")
+    g.set_sweep("compact9")
+    if T:
+        try:
+            g.set_resident_plan(T)
+        except cav.CavityError:
+            g.close()
+            pytest.skip("no compact plan with T=%d for N=%d" % (T, N))
+    assert "compact 9-point operator" in g.describe() and "engine resident" in g.describe()
+    s = cav.Cavity(N, 1500.0, 0.4 / N, 1.1, S, engine="stream")
+    s.set_sweep("compact9")
+    for c in (g, s):
+        c.set_fields(psi0, w0)
+        c.poisson(2 * max(T, 1) + 1)
+        c.step(2)
+    (gp, gw), (sp, sw) = g.get_fields(), s.get_fields()
+    assert np.array_equal(gp, sp) and np.array_equal(gw, sw), (N, S, T)
+    # switching back to the red-black sweeps re-plans the tiling (halo 2T) and still agrees
+    for c in (g, s):
+        c.set_sweep("redblack")
+        c.step(1)
+    (gp, gw), (sp, sw) = g.get_fields(), s.get_fields()
+    assert np.array_equal(gp, sp) and np.array_equal(gw, sw)
+    assert "compact" not in g.describe()
+    g.close(); s.close()
