@@ -43,6 +43,7 @@ def lib():
         L.orc_set_sweep.argtypes = [C.c_void_p, C.c_int]
         L.orc_jacobi.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, C.c_int]
         L.orc_compact.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, C.c_int]
+        L.orc_compact_lex.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, C.c_int]
         L.orc_step_res.argtypes = [C.c_void_p, dp, dp]
         L.orc_run_to_steady.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int), dp, dp,
                                         C.POINTER(C.c_int)]
@@ -168,6 +169,14 @@ def compact(N, beta, psi, omega, nsweeps, mode=MODE_PLAIN):
     p = _field(psi, N, "psi").copy()
     omega = _field(omega, N, "omega")
     _chk(lib().orc_compact(N, beta, mode, _p(p), _p(omega), nsweeps), "orc_compact")
+    return p
+
+
+def compact_lex(N, beta, psi, omega, nsweeps, mode=MODE_PLAIN):
+    """Lexicographic sweeps of the compact operator, the paper's own order; oracle only (NEXT-3)."""
+    p = _field(psi, N, "psi").copy()
+    omega = _field(omega, N, "omega")
+    _chk(lib().orc_compact_lex(N, beta, mode, _p(p), _p(omega), nsweeps), "orc_compact_lex")
     return p
 
 

@@ -39,8 +39,9 @@
 // Pins (tests/test_oracle_pins.py, run with -m "not gpu"): manufactured Poisson solution and its
 // closed-form discrete eigenvalue, exactness on quadratics, Thom on a quadratic wall profile,
 // SSPRK(5,4) stability polynomial + 4th-order convergence, Young's SOR rate, dense direct solve
-// on 9x9, wall/fixed-point invariants.  The composed whole step has no external pin (the paper
-// prints no field values): "parity unpinned" beyond the composition of the pinned pieces.
+// on 9x9, wall/fixed-point invariants, and the composed whole step: bit-exact recomposition in numpy from the
+// operator-level entry points (orc_sor / orc_jacobi / orc_compact, orc_thom, orc_rhs) in the order above.
+// No function of this file is "parity unpinned".
 
 #include <cmath>
 #include <cstdlib>
@@ -212,6 +213,18 @@ void compact_sweeps(int N, int mode, double beta, std::vector<double>& psi, cons
                     psi[idx(N, i, j)] = (mode == ORC_MODE_FMA) ? compact_point_fma(psi, w, N, i, j, beta)
                                                                 : compact_point_plain(psi, w, N, i, j, beta);
                 }
+}
+
+// NEXT-3 (oracle only): the sweep order the paper itself describes: lexicographic, "use the current estimates of
+// psi when they become available" (Gauss-Seidel with relaxation factor beta, eq 15), here i inner, j outer.  A serial
+// recurrence: it has no GPU counterpart (reading N1 replaces it by four colours on both sides); it exists so that the paper's
+// own order and its under-relaxed range beta = 0.8 ... 0.1 can be exercised and compared with the four-colour order.
+void compact_sweeps_lex(int N, int mode, double beta, std::vector<double>& psi, const std::vector<double>& w, int nsweeps) {
+    for (int s = 0; s < nsweeps; ++s)
+        for (int j = 1; j <= N - 1; ++j)
+            for (int i = 1; i <= N - 1; ++i)
+                psi[idx(N, i, j)] = (mode == ORC_MODE_FMA) ? compact_point_fma(psi, w, N, i, j, beta)
+                                                            : compact_point_plain(psi, w, N, i, j, beta);
 }
 
 void poisson_sweeps(const orc_ctx* c, std::vector<double>& psi, const std::vector<double>& w, int nsweeps) {
@@ -512,6 +525,16 @@ ORC_API int orc_compact(int N, double beta, int mode, double* psi, const double*
     const size_t G = (size_t)(N + 1) * (size_t)(N + 1);
     std::vector<double> p(psi, psi + G), w(omega, omega + G);
     compact_sweeps(N, mode, beta, p, w, nsweeps);
+    std::memcpy(psi, p.data(), G * sizeof(double));
+    return ORC_OK;
+}
+
+// nsweeps LEXICOGRAPHIC sweeps of the compact operator (the paper's own order; NEXT-3, oracle only).
+ORC_API int orc_compact_lex(int N, double beta, int mode, double* psi, const double* omega, int nsweeps) {
+    if (N < 2 || !psi || !omega || nsweeps < 0) return ORC_EINVAL;
+    const size_t G = (size_t)(N + 1) * (size_t)(N + 1);
+    std::vector<double> p(psi, psi + G), w(omega, omega + G);
+    compact_sweeps_lex(N, mode, beta, p, w, nsweeps);
     std::memcpy(psi, p.data(), G * sizeof(double));
     return ORC_OK;
 }

@@ -7,6 +7,7 @@
 #include <c10/cuda/CUDACachingAllocator.h>
 #include <c10/cuda/CUDAStream.h>
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>      // header-only; ranges show up in Nsight timelines, cost nothing otherwise
 
 #include <algorithm>
 #include <cmath>
@@ -61,6 +62,11 @@ struct cav_ctx {
 };
 
 namespace {
+
+struct NvtxRange {                 // one range per entry point that enqueues work (tracing)
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 struct DeviceGuard {
     int prev = -1;
@@ -239,6 +245,7 @@ void try_build_graph(cav_ctx* c) {
 
 int step_impl(cav_ctx* c, int nsteps, bool sync) {
     if (!c || nsteps < 0) return CAV_EINVAL;
+    NvtxRange nv("cav_step: SSPRK(5,4) time steps (a1 + a2 + a3)");
     DeviceGuard dg(c->device);
     if (nsteps == 0) return CAV_OK;
     resolve_engine(c);
@@ -392,6 +399,7 @@ CAV_API int cav_sync(cav_ctx* c) {
 
 CAV_API int cav_poisson(cav_ctx* c, int nsweeps, double* res_inf_out) {
     if (!c || nsweeps < 0) return CAV_EINVAL;
+    NvtxRange nv("cav_poisson: a1 sweeps + a2");
     DeviceGuard dg(c->device);
     resolve_engine(c);
     long long nl = 0;
@@ -414,6 +422,7 @@ CAV_API int cav_poisson(cav_ctx* c, int nsweeps, double* res_inf_out) {
 
 CAV_API int cav_get_diag(cav_ctx* c, cav_diag* out) {
     if (!c || !out) return CAV_EINVAL;
+    NvtxRange nv("cav_get_diag: a4 reductions");
     DeviceGuard dg(c->device);
     long long nl = 0;
     double r[4] = {0, 0, 0, 0};
@@ -445,6 +454,7 @@ CAV_API int cav_set_sweep(cav_ctx* c, int kind) {
 
 CAV_API int cav_step_res(cav_ctx* c, double* res_psi_out, double* res_omega_out) {
     if (!c) return CAV_EINVAL;
+    NvtxRange nv("cav_step_res: time step + RES monitors");
     DeviceGuard dg(c->device);
     const size_t nb = c->field_doubles * sizeof(double);
     if (!c->prev) {

@@ -239,3 +239,21 @@ def test_compact9_resident_engine_matches_the_stream_kernels(cav, N, S, T):
     assert np.array_equal(gp, sp) and np.array_equal(gw, sw)
     assert "compact" not in g.describe()
     g.close(); s.close()
+
+
+def test_table1_workload_spot_check_against_the_oracle(cav, orc):
+    """The paper's production grid and time step (Table 1: 1024 x 1024 points, dt = 0.001, Re = 5 000) with the
+    sweep count and relaxation factor of the run to steady state reported in DESIGN.md section 10 (S = 20, beta = 1.97): a few
+    steps from rest, monitors included, bit for bit against the FMA oracle."""
+    N, Re, dt, beta, S = 1023, 5000.0, 0.001, 1.97, 20
+    g = cav.Cavity(N, Re, dt, beta, S)
+    o = orc.OracleCavity(N, Re, dt, beta, S, orc.MODE_FMA)
+    z = np.zeros((N + 1, N + 1))
+    g.set_fields(None, z); o.set_fields(None, z)
+    g.step(3); o.step(3)
+    grp, grw = g.step_res(); orp, orw = o.step_res()
+    (gp, gw), (op, ow) = g.get_fields(), o.get_fields()
+    assert np.array_equal(gp, op) and np.array_equal(gw, ow)
+    assert abs(grp - orp) <= 1e-11 * orp and abs(grw - orw) <= 1e-11 * orw
+    assert gp.min() < 0.0                                     # clockwise from the first steps on
+    g.close(); o.close()

@@ -757,3 +757,60 @@ def test_full_configs_against_survey_appendix_b_third_opinion(cfg, ke, ens, psi_
     assert abs(d["kinetic_energy"] / ke - 1.0) < 1e-11
     assert abs(d["enstrophy"] / ens - 1.0) < 1e-11
     assert abs(psi[1:wl.N, 1:wl.N].min() / psi_min - 1.0) < 1e-11
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-3 remainder: the paper's own sweep order (lexicographic, "use the current estimates when they become
+# available") and its under-relaxed range beta = 0.8 ... 0.1, oracle only
+# --------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("mode", MODES)
+def test_lexicographic_compact_sweep_uses_new_values_as_they_become_available(mode):
+    # delta at (5, 5), omega = 0, beta = 1, one sweep (i inner, j outer): a point swept BEFORE the delta's neighbours sees old
+    # values only, a point swept after sees the new ones: hand-computed from eq 15 collected (weights 1/5 edge, 1/20 corner)
+    N = 10
+    psi = np.zeros((N + 1, N + 1)); psi[5, 5] = 1.0
+    out = oracle.compact_lex(N, 1.0, psi, np.zeros_like(psi), 1, mode)
+    a44 = 0.05                                                  # (i=4, j=4): corner neighbour (5,5) = 1, nothing new yet
+    a54 = 0.2 * (1.0 + a44)                                     # (5,4): edge (5,5) old = 1, edge (4,4) NEW
+    a64 = 0.2 * a54 + 0.05 * 1.0                                # (6,4): edge (5,4) NEW, corner (5,5) old
+    a35 = 0.05 * a44                                            # (3,5): corner (4,4) NEW
+    a45 = 0.2 * (1.0 + a44 + a35) + 0.05 * a54                  # (4,5): edge (5,5) old, edges (4,4), (3,5) NEW, corner (5,4) NEW
+    assert abs(out[4, 4] - a44) < 1e-16 and abs(out[4, 5] - a54) < 1e-16 and abs(out[4, 6] - a64) < 1e-16
+    assert abs(out[5, 3] - a35) < 1e-16 and abs(out[5, 4] - a45) < 1e-16
+    # the delta itself is replaced by the combination of its 8 neighbours, four of them new
+    a55 = 0.2 * (out[5, 4] + 0.0 + out[4, 5] + 0.0) + 0.05 * (out[4, 4] + out[4, 6] + 0.0 + 0.0)
+    assert abs(out[5, 5] - a55) < 1e-16
+    # and it differs from the four-colour order after one sweep, but has the same fixed point (next test)
+    assert np.max(np.abs(out - oracle.compact(N, 1.0, psi, np.zeros_like(psi), 1, mode))) > 1e-3
+
+
+@pytest.mark.parametrize("beta", [0.8, 0.5, 0.3, 0.1])
+def test_lexicographic_order_converges_to_the_same_discrete_solution_over_the_papers_beta_range(beta):
+    # "the relaxation parameter varies from 0.8 to 0.1".  The fixed point of eq 15 does not depend on beta or on the
+    # sweep order: the closed-form discrete solution of the compact scheme for a sine mode (pinned above for four colours)
+    N, k, l = 12, 1, 2
+    X, Y = grid(N)
+    w = np.sin(k * np.pi * X) * np.sin(l * np.pi * Y)
+    w[0] = w[-1] = 0.0; w[:, 0] = w[:, -1] = 0.0
+    target = compact_ratio(N, k, l) * w
+    psi = np.zeros_like(w)
+    errs = []
+    for _ in range(6):
+        psi = oracle.compact_lex(N, beta, psi, w, int(60 / beta))
+        errs.append(np.max(np.abs(psi - target)))
+    assert all(errs[i + 1] < errs[i] for i in range(5) if errs[i] > 1e-15), errs   # monotone decay: under-relaxation is stable
+    psi = oracle.compact_lex(N, beta, psi, w, int(4000 / beta))
+    assert np.max(np.abs(psi - target)) < 1e-13
+    four = oracle.compact(N, beta, np.zeros_like(w), w, int(6000 / beta))
+    assert np.max(np.abs(four - psi)) < 1e-13
+
+
+def test_under_relaxation_slows_convergence_monotonically():
+    # the smaller beta, the slower the paper's iteration (why the sweep count, which the paper never states, matters: D3)
+    N = 12
+    X, Y = grid(N)
+    w = np.sin(np.pi * X) * np.sin(np.pi * Y); w[0] = w[-1] = 0.0; w[:, 0] = w[:, -1] = 0.0
+    target = compact_ratio(N, 1, 1) * w
+    left = [np.max(np.abs(oracle.compact_lex(N, b, np.zeros_like(w), w, 100) - target)) for b in (0.8, 0.5, 0.3, 0.1)]
+    assert left[0] < left[1] < left[2] < left[3]
