@@ -156,11 +156,6 @@ __device__ __forceinline__ void half_unpack(const HalfUnit& u, unsigned int& A, 
     C = __byte_perm(u.w2, u.w3, 0x5432);       // w2[31:16] | w3[15:0] << 16
 }
 __device__ __forceinline__ void st_half(void* p, const HalfUnit& u) {
-#ifdef CAV_EXPERIMENT_WEAK_STORE      // timing experiment only (a weak store racing with the readers' loads is a data race by the model)
-    asm volatile("st.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"((unsigned long long)u.w0 | ((unsigned long long)u.w1 << 32)),
-                 "l"((unsigned long long)u.w2 | ((unsigned long long)u.w3 << 32)) : "memory");
-    return;
-#endif
     asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"((unsigned long long)u.w0 | ((unsigned long long)u.w1 << 32)),
                  "l"((unsigned long long)u.w2 | ((unsigned long long)u.w3 << 32)) : "memory");
 }
