@@ -4,6 +4,7 @@ dt = 0.001, Re = 5 000 ... 30 000) stepped until RES_psi and RES_omega (eq 26-27
 
     python -m paper_0809_3098_b200.run_to_steady --Re 5000 [--points 1024] [--dt 0.001] [--sweeps 20] [--beta 1.97]
                                                  [--max-steps 3000000] [--check-every 1000] [--budget-s 1100] [--report-every 50]
+                                                 [--sweep redblack|compact9]
 
 The paper states neither its sweep count nor its stopping rule for the inner iteration (D3); S and beta here are this build's.
 Prints one JSON line per report and a final summary line.  GPU only: there is no CPU fallback.
@@ -26,14 +27,18 @@ def main():
     ap.add_argument("--check-every", type=int, default=1000)
     ap.add_argument("--budget-s", type=float, default=1100.0, help="stop after this much wall time even if not converged")
     ap.add_argument("--report-every", type=int, default=50, help="print every this many checks")
+    ap.add_argument("--sweep", default="redblack", choices=["redblack", "compact9"],
+                    help="Poisson operator / sweep: the 5-point red-black SOR of BASELINE.json, or the paper's own compact 9-point operator")
     args = ap.parse_args()
     from . import binding
     N = args.points - 1
     tol_psi, tol_w = (1e-12, 1e-10) if args.Re <= 20000 else (1e-10, 1e-8)
     cav = binding.Cavity(N, args.Re, args.dt, args.beta, args.sweeps)
+    if args.sweep != "redblack":
+        cav.set_sweep(args.sweep)
     cav.set_fields(None, np.zeros((N + 1, N + 1)))                               # fluid at rest, impulsive lid start (G11)
     print(json.dumps({"plan": cav.describe(), "Re": args.Re, "points": args.points, "dt": args.dt, "S": args.sweeps,
-                      "beta": args.beta, "tol": [tol_psi, tol_w]}), flush=True)
+                      "beta": args.beta, "sweep": args.sweep, "tol": [tol_psi, tol_w]}), flush=True)
     t0 = time.perf_counter()
     steps, nchk, m = 0, 0, None
     chunk = args.check_every * args.report_every
