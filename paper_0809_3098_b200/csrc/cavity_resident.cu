@@ -27,18 +27,22 @@
 // sweep of a stage, and once per stage for the new vorticity, the CTAs refresh their halos through L2 WITHOUT any fence,
 // flag or barrier between CTAs: the validity tag travels inside the data.  Three consecutive points of a row (x = 3g,
 // 3g + 1, 3g + 2: core widths are multiples of 3, so a group has one owner) travel as one 32-byte unit of four 64-bit
-// words, each word = 48 payload bits | 16-bit tag, written by two st.relaxed.gpu.v2.b64 and read by two
-// ld.relaxed.gpu.v2.b64.  The PTX memory model treats a vector access as a set of scalar accesses of the element
+// words, each word = 48 payload bits | 16-bit tag, moved by a PAIR of adjacent lanes, 16 bytes each (one st / ld.relaxed.gpu
+// .v2.b64 per lane: a warp instruction covers whole sectors).  The PTX memory model treats a vector access as a set of scalar accesses of the element
 // type in unspecified order; every 64-bit element is single-copy atomic and carries its own tag, so a reader that finds the
 // tag of the round it waits for in all four words holds that round's three values, however the four were ordered or
 // torn.  At a given location a reader can only ever find the round it waits for or the one two rounds earlier (two buffers
 // alternate by round parity: a tile writes round r + 1 only after it has received round r from every neighbour, and a
 // neighbour posts round r only after it has consumed round r - 1), so 16-bit tags 1 + r mod 65535 never alias; 0 = never
-// valid (freshly cleared buffers).  The exchange is cooperative and coalesced: every thread copies its micro-tile into a
-// shared-memory image of the tile (row-major), then ALL threads of the CTA store the strip units (consecutive threads =
-// consecutive units) and fetch the ring units the same way (a unit that does not carry the tag yet is polled by one lane
-// of the warp), unpack them into the image, and every thread reads its micro-tile back.  Which unit a thread moves is
+// valid (freshly cleared buffers).  The exchange is cooperative and coalesced: the threads copy the micro-tile rows that hold
+// strip points into a shared-memory image of the tile (row-major), then ALL threads of the CTA store the strip units
+// (consecutive lane pairs = consecutive units) and fetch the ring units the same way, as asynchronous 16-byte copies into a
+// landing zone, all of a thread's slots in flight together (a half that does not carry the tag yet is polled by one lane
+// of the warp), unpack them into the image, and the rows that hold ring points are read back.  Which unit a pair moves is
 // precomputed once per plan (k_build_tables) and copied to shared memory at launch.
+//
+// NEXT-1 (KIND = 1): the same kernel runs the paper's own compact 9-point operator, relaxed in four colours (colour_pass):
+// four passes per sweep, halo 4T, right-hand side qB from the image of omega including the wall vorticity.
 //
 // a2 + a3 in the tile.  After the last sweep of a stage and one more psi exchange the tile holds psi on core + halo; the
 // stage input vorticity of the core is re-read from the tile's own global buffer into the shared-memory image, its first
@@ -677,9 +681,9 @@ __device__ __forceinline__ void qb_from_image(double (&q)[R][C], const double* _
 __device__ __forceinline__ double thom_wall(double c2h2, double p_adj) { return -(c2h2 * p_adj); }
 __device__ __forceinline__ double thom_lid(double c2h2, double lid, double p_adj) { return -(c2h2 * p_adj) - lid; }
 
-// a2 + a3 of one stage for this tile (see the file header).  pl: the thread's psi micro-tile, [rj * C + ci].  On return the
+// a2 + a3 of one stage for this tile (see the file header).  pp: the thread's psi micro-tile (registers).  On return the
 // image holds the NEW vorticity on core + halo (+0.0 elsewhere) and the ring copy is refreshed; the caller turns it into q.
-// Not inlined: see exchange_units.
+// Inlined: with psi passed through local memory to a non-inlined version the phase took 33 us per stage instead of 24.
 template <int C, int R, int MAXW, int KIND>
 __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R][C], double* __restrict__ sm, const int stage,
                                        const unsigned int round, const unsigned int fl) {

@@ -1,5 +1,5 @@
 // cavity_resident.cuh — the resident engine: one persistent CTA per tile, psi and the scaled right-hand side held in
-// registers, temporal blocking with a 2T-deep halo that is refreshed through L2 every T sweeps as self-validating tagged
+// registers, temporal blocking with a 2T-deep halo (4T: compact operator) that is refreshed through L2 every T sweeps as self-validating tagged
 // data (no fence, flag or grid barrier), a2 + a3 of every stage evaluated in the tile: whole time steps in one launch.
 // See DESIGN.md "Resident engine".  Plain CUDA: no torch types.
 #pragma once
@@ -20,7 +20,7 @@ struct ResidentPlan {
     int CW = 0, CH = 0;   // core (owned) points per tile in x and y; tile (bi, bj) owns [bi CW, (bi+1) CW) x [bj CH, (bj+1) CH)
     int ntx = 0, nty = 0; // tiles in x and y
     int ntiles = 0;
-    int ns_per = 0, nr_per = 0;   // 32-byte exchange units each thread stores / fetches per round (0 for a single tile)
+    int ns_per = 0, nr_per = 0;   // 16-byte halves of 32-byte exchange units each thread stores / fetches per round (0 for a single tile)
     bool fixup = false;           // some tile holds both walls of one direction: the kernel variant with the wall-mask fix-up
     int smem_bytes = 0;
     int regs = 0;         // registers per thread of the chosen variant (as compiled)
