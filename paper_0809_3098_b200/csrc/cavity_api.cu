@@ -44,7 +44,6 @@ struct cav_ctx {
     int sweep = CAV_SWEEP_REDBLACK;  // a1 variant
     double* scratch = nullptr;       // diagnostics partials
     double* out4 = nullptr;          // diagnostics result (device)
-    void* tables = nullptr;          // resident engine: per-plan exchange tables (own allocation, rebuilt on re-plan)
     unsigned int* err_word = nullptr;// resident engine: device error word (a tile gave up waiting for a neighbour)
     unsigned int epoch = 0;          // resident engine: exchange rounds done so far (host side; the tag of a round derives from it)
     bool resident_ran = false;       // a resident launch has been enqueued since the error word was last cleared
@@ -129,22 +128,16 @@ void drop_graph(cav_ctx* c) {
     c->graph_launches = 0;
 }
 
-// (re)builds the exchange tables and (re)allocates / clears the exchange buffers of c->plan; on failure the plan is marked
-// unusable.  Cleared buffers carry tag 0 = never valid, so units of another plan can never be taken for this one's.
-void build_plan_tables(cav_ctx* c) {
-    dev_free(c->tables);
-    const size_t nb = cavk::resident_table_bytes(c->plan);
-    if (!c->plan.ok || nb == 0) { dev_free(c->xbuf); c->xa = c->xb = nullptr; return; }
-    const size_t xbytes = (cavk::resident_exchange_bytes(c->N) + 255) / 256 * 256;
+// (re)allocates / clears the exchange buffers of c->plan; on failure the plan is marked unusable.  Cleared buffers carry
+// tag 0 = never valid, so units of another plan can never be taken for this one's.
+void build_plan_buffers(cav_ctx* c) {
+    if (!c->plan.ok || c->plan.ntiles <= 1) { dev_free(c->xbuf); c->xa = c->xb = nullptr; return; }
+    const size_t xbytes = cavk::resident_exchange_bytes(c->N);
     if (!c->xbuf) c->xbuf = dev_alloc(c, 2 * xbytes);
-    c->tables = dev_alloc(c, nb);
-    if (!c->tables || !c->xbuf) { c->plan.ok = false; return; }
+    if (!c->xbuf) { c->plan.ok = false; return; }
     c->xa = c->xbuf;
     c->xb = (char*)c->xbuf + xbytes;
     if (cudaMemsetAsync(c->xbuf, 0, 2 * xbytes, c->st) != cudaSuccess) { cudaGetLastError(); c->plan.ok = false; return; }
-    const int nl = cavk::resident_build_tables(c->P, c->plan, c->tables, c->st);
-    if (nl < 0 || cudaStreamSynchronize(c->st) != cudaSuccess) { cudaGetLastError(); c->plan.ok = false; return; }
-    c->launches += nl;
 }
 
 // The resident engine's tiles give up (and say so) instead of spinning forever on a neighbour that never arrives.  The word
@@ -171,7 +164,7 @@ inline bool resident_path(const cav_ctx* c) {
 // one launch of the resident kernel: nsteps whole time steps, or (nsteps = 0) S sweeps of a1 with right-hand side omega^n
 int enqueue_resident(cav_ctx* c, int nsteps, int S, long long& nl, long long* trace_dev = nullptr, int trace_cap = 0) {
     if (nsteps == 0 && S <= 0) return CAV_OK;
-    LAUNCH(cavk::resident_launch(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, c->tables, c->w[0], c->field_doubles, c->err_word,
+    LAUNCH(cavk::resident_launch(c->P, c->plan, c->psi, c->psi2, c->xa, c->xb, c->w[0], c->field_doubles, c->err_word,
                                  &c->epoch, nsteps, S, c->st, trace_dev, trace_cap));
     std::swap(c->psi, c->psi2);
     c->resident_ran = true;
@@ -321,7 +314,7 @@ CAV_API int cav_create(cav_ctx** out, int N, double Re, double dt, double sor_om
         c->err_word = (unsigned int*)p;
         if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) throw (int)CAV_ECUDA;
         if (cudaStreamSynchronize(c->st) != cudaSuccess) throw (int)CAV_ECUDA;
-        build_plan_tables(c);
+        build_plan_buffers(c);
         resolve_engine(c);
     } catch (int code) {
         rc = code;
@@ -349,7 +342,6 @@ CAV_API void cav_destroy(cav_ctx* c) {
         if (c->slab) {
             try { c10::cuda::CUDACachingAllocator::raw_delete(c->slab); } catch (...) {}
         }
-        dev_free(c->tables);
         dev_free(c->xbuf);
         void* qv = c->q; dev_free(qv); c->q = nullptr;
         void* pv = c->prev; dev_free(pv); c->prev = nullptr;
@@ -445,7 +437,7 @@ CAV_API int cav_set_sweep(cav_ctx* c, int kind) {
         drop_graph(c);
         if (kind != CAV_SWEEP_JACOBI && c->plan.kind != plan_kind(kind)) {       // the halo depth per sweep differs: plan anew
             c->plan = cavk::resident_plan(c->P, c->device, 0, -1, plan_kind(kind));
-            build_plan_tables(c);
+            build_plan_buffers(c);
             resolve_engine(c);
         }
     }
@@ -519,8 +511,8 @@ CAV_API int cav_set_resident_plan(cav_ctx* c, int sweeps_per_exchange, int varia
     if (!pl.ok) return CAV_ENOTSUP;
     const cavk::ResidentPlan old = c->plan;
     c->plan = pl;
-    build_plan_tables(c);
-    if (!c->plan.ok) { c->plan = old; build_plan_tables(c); resolve_engine(c); return CAV_ENOMEM; }
+    build_plan_buffers(c);
+    if (!c->plan.ok) { c->plan = old; build_plan_buffers(c); resolve_engine(c); return CAV_ENOMEM; }
     return clear_resident_error(c);
 }
 
@@ -552,7 +544,7 @@ CAV_API int cav_debug_set_epoch(cav_ctx* c, unsigned int epoch) {
     DeviceGuard dg(c->device);
     CK(cudaStreamSynchronize(c->st));
     // a jump of the round counter breaks the "this round or the one two before" invariant of the tags: start from cleared buffers
-    if (c->xbuf) CK(cudaMemsetAsync(c->xbuf, 0, 2 * ((cavk::resident_exchange_bytes(c->N) + 255) / 256 * 256), c->st));
+    if (c->xbuf) CK(cudaMemsetAsync(c->xbuf, 0, 2 * cavk::resident_exchange_bytes(c->N), c->st));
     c->epoch = epoch;
     return CAV_OK;
 }

@@ -67,12 +67,8 @@ namespace {
 #define CAV_SPIN_TIMEOUT 20000000000LL      // ~10 s at 2 GHz: a neighbour whose data never arrives is a bug, not a wait
 #endif
 constexpr long long SPIN_TIMEOUT_CYCLES = CAV_SPIN_TIMEOUT;
-constexpr unsigned int NO_UNIT = 0xffffffffu;
 #ifndef CAV_QROWS
 #define CAV_QROWS 2             // rows of the micro-tile whose q lives in shared memory instead of registers
-#endif
-#ifndef CAV_RECV_BATCH
-#define CAV_RECV_BATCH 6        // ring half-units (16 bytes) a thread keeps in flight at a time, as asynchronous copies into shared memory
 #endif
 
 // SSPRK(5,4) in Shu-Osher form, eq 9-13, readings G1 / G2 (the same table as cavity_kernels.cu, typed here again
@@ -93,43 +89,57 @@ struct ResArgs {
     double* psi_out;        // ... and after (a different field)
     double* wbase;          // omega^n, omega^(1..4), T: six fields, `fstride` doubles apart; sweeps-only launches read field 0
     size_t fstride;
-    ulonglong4* x0;         // exchange buffer of even rounds: one 32-byte unit per group of 3 points, upitch units per grid row
-    ulonglong4* x1;         // exchange buffer of odd rounds
+    char* x0;               // exchange buffer of even rounds: three planes (16 + 16 + 8 bytes per unit of four points), upitch units per grid row
+    char* x1;               // exchange buffer of odd rounds
+    size_t p1off, p2off;    // byte offsets of the second and third plane inside a buffer
     int upitch;
     unsigned int* err;      // error word: set if a tile gave up waiting for a neighbour
-    unsigned int base;      // exchange rounds done by earlier launches (tag of round r: 1 + r mod 65535; buffer: r & 1)
+    unsigned int base;      // exchange rounds done by earlier launches (tag of round r: 1 + r mod 4095; buffer: r & 1)
     int nsteps;             // > 0: that many whole time steps (a1 + a2 + a3, five stages each); 0: S sweeps of a1 only
     int S;                  // sweeps per stage (nsteps > 0) or in total (nsteps == 0)
     int T, halo, CW, CH, ntx, nty;
-    int ns_per, nr_per;     // table entries per thread: strip units to store / ring units to fetch
     int walls;              // the exchanged regions include the wall points (compact operator)
-    const unsigned int* tables;   // per-plan exchange tables, one block per tile (k_build_tables)
     long long* trace;       // profiling only (cav_trace_sweeps): per tile, %globaltimer at the phase boundaries; else null
     int trace_cap;          // slots per tile
 };
 
 // Geometry of tile (bi, bj): owned core, origin of the thread grid, wall alignment.  Shared by the planner (host) and the
 // kernel so that both agree on what fits.
+// Exchange units are groups of four consecutive points of a grid row, unit k = the columns 4k - 3 .. 4k (so that the wall
+// column x = 0 is the last column of unit 0, as it is the last column of lane 0 of a left-edge tile).  With more than one tile
+// in x the cores are [0, CW + 1), [CW + 1, 2 CW + 1), ... with CW a multiple of 4: every core boundary is a unit boundary (a
+// unit has exactly one owner), and every tile but those of the last column puts its origin at a unit boundary, so that the
+// four columns of a lane ARE a unit (D = 0).  A tile of the last column must put the wall x = N into the first column of a
+// lane; its lanes then start D = (N - 1) mod 4 columns after a unit boundary, and it moves its units through a warp shuffle.
 struct TileGeom {
     int cx0, cx1, cy0, cy1;        // core [cx0, cx1) x [cy0, cy1)
     int ox, oy;                    // grid coordinates of local point (0, 0)
+    int D;                         // (ox - 1) mod 4: columns between a unit boundary and the first column of a lane
     bool left_al, right_al, bot_al, top_al;   // wall isolated in a lane / warp that owns no interior point
     bool fits;                     // the W x H thread grid covers core + halo (clipped to the grid) and the aligned walls
 };
+__host__ __device__ inline int round_up4(int v) { return (v + 3) / 4 * 4; }
 
 __host__ __device__ inline TileGeom tile_geom(int N, int CW, int CH, int halo, int ntx, int nty, int bi, int bj, int C, int R,
                                               int W, int H) {
     TileGeom g;
-    g.cx0 = bi * CW; g.cy0 = bj * CH;
-    g.cx1 = g.cx0 + CW < N + 1 ? g.cx0 + CW : N + 1;
+    g.cx0 = (ntx > 1 && bi > 0) ? bi * CW + 1 : 0;
+    g.cy0 = bj * CH;
+    g.cx1 = (ntx > 1 && (bi + 1) * CW + 1 < N + 1) ? (bi + 1) * CW + 1 : N + 1;
     g.cy1 = g.cy0 + CH < N + 1 ? g.cy0 + CH : N + 1;
     g.left_al = bi == 0;
     g.right_al = bi == ntx - 1 && ntx > 1;
     g.bot_al = bj == 0;
     g.top_al = bj == nty - 1 && nty > 1;
+    g.D = 0;
     if (g.left_al) g.ox = -(C - 1);                                   // x = 0 is column C - 1 of lane 0
-    else if (g.right_al) g.ox = g.cx0 - halo - (C - (N - g.cx0 + halo) % C) % C;      // (N - ox) % C == 0
-    else g.ox = g.cx0 - halo;
+    else if (g.right_al) {
+        // (N - ox) % C == 0: x = N is the first column of a lane.  If the lanes are not units (D > 0) lane 0 receives its
+        // first C - D columns from nobody: they must lie outside the halo.
+        g.D = (N - 1) & 3;
+        const int lim = g.cx0 - halo - (g.D ? C - g.D : 0);
+        g.ox = lim - (((lim - N) % C) + C) % C;
+    } else g.ox = g.cx0 - round_up4(halo);
     if (g.bot_al) g.oy = -(R - 1);                                    // y = 0 is row R - 1 of warp 0
     else if (g.top_al) g.oy = g.cy0 - halo - (R - (N - g.cy0 + halo) % R) % R;        // (N - oy) % R == 0
     else g.oy = g.cy0 - halo;
@@ -139,39 +149,61 @@ __host__ __device__ inline TileGeom tile_geom(int N, int CW, int CH, int halo, i
     return g;
 }
 
-// ---- one exchanged unit: three consecutive doubles of an image row = six 32-bit words c0 .. c5, moved by a PAIR of adjacent
-// lanes, 16 bytes each (one warp instruction covers 512 contiguous bytes: whole 32-byte sectors).  Lane h = 0 takes
-// (A, B, C) = (c0, c1, c2), lane h = 1 takes (c3, c4, c5), and each packs its three words with two copies of the 16-bit tag into
-// two 64-bit elements, tag in the top 16 bits of each:
-//     element 0 = A | (B[15:0] | tag << 16) << 32        element 1 = (B[31:16] | C[15:0] << 16) | (C[31:16] | tag << 16) << 32
-// No word straddles the two lanes, so packing and unpacking are three byte permutes each and need no shuffle.
-struct HalfUnit { unsigned int w0, w1, w2, w3; };      // elements {w0, w1} and {w2, w3}, little endian
-__device__ __forceinline__ HalfUnit half_pack(unsigned int A, unsigned int B, unsigned int C, unsigned int tag) {
-    HalfUnit u;
-    u.w0 = A;
-    u.w1 = __byte_perm(B, tag, 0x5410);        // B[15:0] | tag << 16
-    u.w2 = __byte_perm(B, C, 0x5432);          // B[31:16] | C[15:0] << 16
-    u.w3 = __byte_perm(C, tag, 0x5432);        // C[31:16] | tag << 16
+// ---- one exchanged unit: four consecutive doubles d0 .. d3 of a grid row as five 64-bit words, each carrying a 12-bit tag:
+//     word i (i < 4) = d_i with the low 12 bits of its mantissa replaced by the tag
+//     word 4         = the four displaced 12-bit pieces in bits 0-47, the tag in bits 48-59
+// Words 0, 1 live in plane 0 of the exchange buffer (16 bytes per unit), words 2, 3 in plane 1, word 4 in plane 2 (8 bytes
+// per unit): the 32 lanes of a warp move 32 consecutive units with three instructions that cover 512 + 512 + 256
+// contiguous bytes (whole 32-byte sectors).  They are moved with st / ld.relaxed.gpu.global.v2.b64 and .b64; the PTX memory
+// model treats a vector access as a set of scalar accesses of the element type, and every 64-bit element is single-copy
+// atomic and carries its own tag, so a reader that finds the tag it waits for in all five words holds that round's four values.
+struct Unit { unsigned long long w0, w1, w2, w3, w4; };
+__device__ __forceinline__ Unit unit_pack(double d0, double d1, double d2, double d3, unsigned int tag) {
+    const unsigned int l0 = (unsigned int)__double2loint(d0), l1 = (unsigned int)__double2loint(d1);
+    const unsigned int l2 = (unsigned int)__double2loint(d2), l3 = (unsigned int)__double2loint(d3);
+    Unit u;
+    u.w0 = ((unsigned long long)(unsigned int)__double2hiint(d0) << 32) | ((l0 & 0xfffff000u) | tag);
+    u.w1 = ((unsigned long long)(unsigned int)__double2hiint(d1) << 32) | ((l1 & 0xfffff000u) | tag);
+    u.w2 = ((unsigned long long)(unsigned int)__double2hiint(d2) << 32) | ((l2 & 0xfffff000u) | tag);
+    u.w3 = ((unsigned long long)(unsigned int)__double2hiint(d3) << 32) | ((l3 & 0xfffff000u) | tag);
+    const unsigned int m = (l0 & 0xfffu) | ((l1 & 0xfffu) << 12) | (l2 << 24);
+    const unsigned int h = ((l2 >> 8) & 0xfu) | ((l3 & 0xfffu) << 4) | (tag << 16);
+    u.w4 = ((unsigned long long)h << 32) | m;
     return u;
 }
-__device__ __forceinline__ void half_unpack(const HalfUnit& u, unsigned int& A, unsigned int& B, unsigned int& C) {
-    A = u.w0;
-    B = __byte_perm(u.w1, u.w2, 0x5410);       // w1[15:0] | w2[15:0] << 16
-    C = __byte_perm(u.w2, u.w3, 0x5432);       // w2[31:16] | w3[15:0] << 16
+__device__ __forceinline__ bool unit_ok(const Unit& u, unsigned int tag) {
+    const unsigned int x = (((unsigned int)u.w0 ^ tag) | ((unsigned int)u.w1 ^ tag) | ((unsigned int)u.w2 ^ tag) | ((unsigned int)u.w3 ^ tag)) & 0xfffu;
+    return x == 0u && ((unsigned int)(u.w4 >> 48) & 0xfffu) == tag;
 }
-__device__ __forceinline__ void st_half(void* p, const HalfUnit& u) {
-    asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"((unsigned long long)u.w0 | ((unsigned long long)u.w1 << 32)),
-                 "l"((unsigned long long)u.w2 | ((unsigned long long)u.w3 << 32)) : "memory");
+__device__ __forceinline__ void unit_unpack(const Unit& u, double& d0, double& d1, double& d2, double& d3) {
+    const unsigned int m = (unsigned int)u.w4, h = (unsigned int)(u.w4 >> 32);
+    d0 = __hiloint2double((int)(u.w0 >> 32), (int)(((unsigned int)u.w0 & 0xfffff000u) | (m & 0xfffu)));
+    d1 = __hiloint2double((int)(u.w1 >> 32), (int)(((unsigned int)u.w1 & 0xfffff000u) | ((m >> 12) & 0xfffu)));
+    d2 = __hiloint2double((int)(u.w2 >> 32), (int)(((unsigned int)u.w2 & 0xfffff000u) | (m >> 24) | ((h & 0xfu) << 8)));
+    d3 = __hiloint2double((int)(u.w3 >> 32), (int)(((unsigned int)u.w3 & 0xfffff000u) | ((h >> 4) & 0xfffu)));
 }
-__device__ __forceinline__ HalfUnit ld_half(const void* p) {
-    unsigned long long a, b;
+__device__ __forceinline__ void st_v2(void* p, unsigned long long a, unsigned long long b) {
+    asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
+}
+__device__ __forceinline__ void st_b64(void* p, unsigned long long a) {
+    asm volatile("st.relaxed.gpu.global.b64 [%0], %1;" ::"l"(p), "l"(a) : "memory");
+}
+__device__ __forceinline__ void ld_v2(const void* p, unsigned long long& a, unsigned long long& b) {
     asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
-    HalfUnit u;
-    u.w0 = (unsigned int)a; u.w1 = (unsigned int)(a >> 32); u.w2 = (unsigned int)b; u.w3 = (unsigned int)(b >> 32);
-    return u;
 }
-__device__ __forceinline__ bool half_ok(const HalfUnit& u, unsigned int tag) { return (u.w1 >> 16) == tag && (u.w3 >> 16) == tag; }
-__host__ __device__ inline unsigned int round_tag(unsigned int round) { return 1u + round % 65535u; }
+__device__ __forceinline__ void ld_b64(const void* p, unsigned long long& a) {
+    asm volatile("ld.relaxed.gpu.global.b64 %0, [%1];" : "=l"(a) : "l"(p) : "memory");
+}
+// predicated forms that load straight into the registers of the doubles they replace (left untouched if !on)
+__device__ __forceinline__ void ld_v2_if(const int on, const void* p, double& a, double& b) {
+    unsigned long long x = (unsigned long long)__double_as_longlong(a), y = (unsigned long long)__double_as_longlong(b);
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %3, 0;\n\t@q ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];\n\t}" : "+l"(x), "+l"(y) : "l"(p), "r"(on) : "memory");
+    a = __longlong_as_double((long long)x); b = __longlong_as_double((long long)y);
+}
+__device__ __forceinline__ void ld_b64_if(const int on, const void* p, unsigned long long& a) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %2, 0;\n\t@q ld.relaxed.gpu.global.b64 %0, [%1];\n\t}" : "+l"(a) : "l"(p), "r"(on) : "memory");
+}
+__host__ __device__ inline unsigned int round_tag(unsigned int round) { return 1u + round % 4095u; }
 
 __device__ __forceinline__ long long globaltimer_ns() {
     unsigned long long t;
@@ -358,135 +390,203 @@ __device__ __forceinline__ void publish_all(const double (&p)[R][C], double* __r
     __syncthreads();
 }
 
-// ---- the units a tile sends (border strips of its core) and receives (its ring): four disjoint rectangles each -------
-// A unit is the group g of a grid row y: the points x = 3g, 3g + 1, 3g + 2.  Core widths are multiples of 3 whenever a tile
-// has a neighbour in x, so every group lies in exactly one core.
-struct URect { int g0, g1, y0, y1; };                    // groups [g0, g1) x rows [y0, y1)
-struct URegion { URect r[4]; };
 __host__ __device__ inline int imax(int a, int b) { return a > b ? a : b; }
 __host__ __device__ inline int imin(int a, int b) { return a < b ? a : b; }
-__host__ __device__ inline int urect_count(const URect& r) {
-    const int w = r.g1 - r.g0, h = r.y1 - r.y0;
-    return (w > 0 && h > 0) ? w * h : 0;
-}
-__host__ __device__ inline int uregion_total(const URegion& g) {
-    return urect_count(g.r[0]) + urect_count(g.r[1]) + urect_count(g.r[2]) + urect_count(g.r[3]);
-}
-// u-th unit of the region (row-major inside each rectangle, rectangles in order); false if u is past the end
-__host__ __device__ inline bool uregion_unit(const URegion& g, int u, int& gi, int& y) {
-    for (int k = 0; k < 4; ++k) {
-        const int n = urect_count(g.r[k]);
-        if (u < n) {
-            const int w = g.r[k].g1 - g.r[k].g0;
-            y = g.r[k].y0 + u / w;
-            gi = g.r[k].g0 + u % w;
-            return true;
-        }
-        u -= n;
-    }
-    return false;
-}
-__host__ __device__ inline URect urect_of(int x0, int x1, int y0, int y1) {      // the groups that meet the points [x0, x1)
-    URect r;
-    r.y0 = y0; r.y1 = y1;
-    if (x1 > x0) { r.g0 = x0 / 3; r.g1 = (x1 - 1) / 3 + 1; } else { r.g0 = r.g1 = 0; }
-    return r;
-}
-// Interior points of the core within `halo` of a core edge that has a neighbour tile behind it (walls are never needed).
-// walls: the wall points too (compact operator: its right-hand side at the points next to a wall reads omega ON the wall, also in the ring)
-__host__ __device__ inline URegion send_units(const TileGeom& t, int N, int halo, int bi, int bj, int ntx, int nty, bool walls) {
-    const int lo = walls ? 0 : 1, hi = walls ? N + 1 : N;
-    const int X0 = imax(t.cx0, lo), X1 = imin(t.cx1, hi), Y0 = imax(t.cy0, lo), Y1 = imin(t.cy1, hi);
-    const int hb = bj > 0 ? halo : 0, ht = bj < nty - 1 ? halo : 0, wl = bi > 0 ? halo : 0, wr = bi < ntx - 1 ? halo : 0;
-    const int yB = imin(Y0 + hb, Y1), yT = imax(Y1 - ht, yB), xL = imin(X0 + wl, X1), xR = imax(X1 - wr, xL);
-    URegion g;
-    g.r[0] = urect_of(X0, X1, Y0, yB);
-    g.r[1] = urect_of(X0, X1, yT, Y1);
-    g.r[2] = urect_of(X0, xL, yB, yT);
-    g.r[3] = urect_of(xR, X1, yB, yT);
-    if (urect_count(g.r[2]) > 0 && urect_count(g.r[3]) > 0 && g.r[3].g0 < g.r[2].g1) g.r[3].g0 = imin(g.r[2].g1, g.r[3].g1);   // narrow core: no unit twice
-    return g;
-}
-// Interior points within `halo` of the core, outside it (the ring).
-__host__ __device__ inline URegion recv_units(const TileGeom& t, int N, int halo, bool walls) {
-    const int lo = walls ? 0 : 1, hi = walls ? N + 1 : N;
-    const int xlo = imax(t.cx0 - halo, lo), xhi = imin(t.cx1 + halo, hi), ylo = imax(t.cy0 - halo, lo), yhi = imin(t.cy1 + halo, hi);
-    const int yc0 = imax(t.cy0, ylo), yc1 = imin(t.cy1, yhi), xc0 = imax(t.cx0, xlo), xc1 = imin(t.cx1, xhi);
-    // Order = the order in which the neighbours STORE these units (send_units: bottom strip, top strip, left, right), so
-    // that what was stored first is fetched first: the ring above comes from the northern tiles' bottom strips, etc.
-    URegion g;
-    g.r[0] = urect_of(xlo, xhi, yc1, yhi);      // ring above   <- bottom strips of the tiles above
-    g.r[1] = urect_of(xlo, xhi, ylo, yc0);      // ring below   <- top strips of the tiles below
-    g.r[2] = urect_of(xc1, xhi, yc0, yc1);      // ring right   <- left strip of the tile to the right (xc1 = its cx0: a multiple of 3)
-    g.r[3] = urect_of(xlo, xc0, yc0, yc1);      // ring left    <- right strip of the tile to the left (xc0 = cx0: a multiple of 3)
-    return g;
-}
 
 // Shared-memory layout (doubles unless said otherwise), nthreads = 32 nwarps, H = R nwarps, SW = 32 C:
 //   edges   (2 (MAXW + 1) + 2 MAXW) C 32   bottom / top rows of the micro-tiles, q of the two middle rows (sized for MAXW warps)
-//   image   H SW                         the tile, row-major: staging area of every exchange, and omega of the stage input during a3
+//   image   H SW                         the tile, row-major: initial load, final store, omega of the stage input during a3
 //   wring   2 SW + 2 H                   first ring of the stage input vorticity around the core (rows below / above, columns left / right)
-//   land    2 CAV_RECV_BATCH nthreads    landing zone of the asynchronous ring fetches: 16 bytes per thread and slot
-//   table   (ns_per + nr_per) nthreads / 2 u32   per pair of lanes and slot: where the unit's points sit in the image (loc_pack; NO_UNIT: none),
-//           then nthreads u32: the rows of the micro-tile that are staged / read back around an exchange
-// 32-bit words per tile: one entry per pair of lanes and slot, then one word per thread: bits 0-5 = micro-tile rows that hold points of units this
-// tile sends (staged before an exchange), bits 8-13 = rows that hold points of units it receives (read back after it)
-__host__ __device__ inline size_t xtab_words(int nth, int ns_per, int nr_per) { return (size_t)(ns_per + nr_per) * (nth / 2) + (size_t)nth; }
-// ... and behind them, in shared memory only, the tile origin (ox, oy): the exchange needs it every round
-__host__ __device__ inline size_t xtab_smem_words(int nth, int ns_per, int nr_per) { return xtab_words(nth, ns_per, nr_per) + 4; }
-__host__ __device__ inline size_t smem_layout_bytes(int C, int R, int maxw, int warps, int ns_per, int nr_per) {
+//   xinfo   2 nthreads u32               per thread: which rows of its micro-tile it sends / receives, and its unit index (xchg_setup)
+__host__ __device__ inline size_t smem_layout_bytes(int C, int R, int maxw, int warps) {
     const size_t nth = 32 * (size_t)warps, H = (size_t)R * warps, SW = 32 * (size_t)C;
-    return 8 * ((2 * (size_t)(maxw + 1) + CAV_QROWS * (size_t)maxw) * C * 32 + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nth) +
-           4 * xtab_smem_words((int)nth, ns_per, nr_per);
+    return 8 * ((2 * (size_t)(maxw + 1) + CAV_QROWS * (size_t)maxw) * C * 32 + H * SW + 2 * SW + 2 * H) + 4 * 2 * nth;
 }
 
-// table entry (32 bits; NO_UNIT = none): bits 0-7 = local x of the unit's first point + 8 (it may be -2: groups are aligned to
-// the grid, not to the tile), bits 8-14 = local row, bits 16-18 = which of the three points lie inside the image row.
-// The unit's place in the exchange buffer follows from the tile origin: row oy + row, group (ox + lx) / 3.
-__host__ __device__ inline unsigned int loc_pack(int lx0, int row, int W) {
-    unsigned int m = 0;
-    for (int j = 0; j < 3; ++j)
-        if (lx0 + j >= 0 && lx0 + j < W) m |= 1u << j;
-    return (unsigned int)(lx0 + 8) | ((unsigned int)row << 8) | (m << 16);
-}
-// image index of the first point + 8, and unit index, of an entry
-__device__ __forceinline__ unsigned int entry_loc(unsigned int e, int SW) { return ((e >> 8) & 0x7fu) * (unsigned int)SW + (e & 0xffu); }
-__device__ __forceinline__ unsigned int entry_unit(unsigned int e, int ox, int oy, int upitch) {
-    const unsigned int x = (unsigned int)(ox + (int)(e & 0xffu) - 8);           // = 3 g, below 2^15
-    return (unsigned int)(oy + (int)((e >> 8) & 0x7fu)) * (unsigned int)upitch + ((x * 43691u) >> 17);
-}
-
-// Builds, once per plan, the exchange tables of every tile in global memory (in the layout the kernel copies to shared
-// memory at launch): which unit each thread stores / fetches and where its three points sit in the image.
+// Which units a thread moves in an exchange.  Its OWN unit of micro-tile row rj is (k, y = gy0 + rj): k = the unit its four
+// columns are (D = 0), or the unit made of its last D columns and the first 4 - D columns of the lane to its right (D > 0).
+//   info bits 0-5:   rows whose own unit it STORES: the unit lies in the tile's core, within `halo` of a core edge that has
+//                    a neighbour behind it
+//   info bits 8-13:  rows whose own unit it FETCHES: the unit lies outside the core, within `halo` of it (the ring)
+//   info bits 16-21: (D > 0) rows whose first 4 - D columns come from the unit the lane to the LEFT fetches
+//   ubase:           index of the own unit of row 0 in the exchange planes (row rj: + rj upitch); may be negative for
+//                    rows below the grid, which are never moved
+// Points: interior rows / columns only; with `walls` (compact operator: its right-hand side reads omega ON the walls, also in
+// the ring) the wall rows / columns too.  A unit counts if at least one of its columns does.
 template <int C, int R>
-__global__ void k_build_tables(const ResArgs a, unsigned int* __restrict__ out) {
-    const int lane = threadIdx.x, warp = threadIdx.y, nwarps = blockDim.y;
-    const int tid = warp * 32 + lane, nthreads = nwarps * 32;
-    const int N = a.N, bi = blockIdx.x, bj = blockIdx.y;
-    const TileGeom t = tile_geom(N, a.CW, a.CH, a.halo, a.ntx, a.nty, bi, bj, C, R, 32 * C, nwarps * R);
-    unsigned int* const o = out + (size_t)(bj * a.ntx + bi) * xtab_words(nthreads, a.ns_per, a.nr_per);
-    const URegion gs = send_units(t, N, a.halo, bi, bj, a.ntx, a.nty, a.walls != 0), gr = recv_units(t, N, a.halo, a.walls != 0);
-    const int npr = nthreads / 2;                                              // one entry per pair of adjacent lanes
-    for (int i = 0; i < a.ns_per + a.nr_per; ++i) {
-        if (tid >= npr) break;
-        const bool snd = i < a.ns_per;
-        const int u = (snd ? i : i - a.ns_per) * npr + tid;
-        int g = 0, y = 0;
-        unsigned int e = NO_UNIT;
-        if (uregion_unit(snd ? gs : gr, u, g, y)) e = loc_pack(3 * g - t.ox, y - t.oy, 32 * C);
-        o[(size_t)i * npr + tid] = e;
+__device__ __forceinline__ void xchg_setup(const ResArgs& a, const TileGeom& t, const int lane, const int warp, const int bi,
+                                           const int bj, unsigned int& info, int& ubase) {
+    static_assert(C == 4, "units are groups of four columns");
+    const int N = a.N, halo = a.halo, D = t.D;
+    const int kown = (t.ox + 3 - D) / 4 + lane + (D ? 1 : 0);       // ox + 3 - D is a non-negative multiple of 4
+    const int gy0 = t.oy + warp * R;
+    const int xf = 4 * kown - 3, xl = 4 * kown, xr = imax(xf, 0);   // first / last column of the unit, its first column inside the grid
+    const int lo = a.walls ? 0 : 1, hi = a.walls ? N : N - 1;       // the rows / columns that are exchanged
+    const bool colok = xl >= lo && xf <= hi;
+    const bool incx = xr >= t.cx0 && xr < t.cx1;
+    const bool bandx = (bi > 0 && xr < t.cx0 + halo) || (bi < a.ntx - 1 && xl >= t.cx1 - halo);
+    const bool nearx = xl >= t.cx0 - halo && xf < t.cx1 + halo;
+    unsigned int send = 0, recv = 0;
+    for (int rj = 0; rj < R; ++rj) {
+        const int y = gy0 + rj;
+        const bool rowok = y >= lo && y <= hi;
+        const bool incy = y >= t.cy0 && y < t.cy1;
+        const bool bandy = (bj > 0 && y < t.cy0 + halo) || (bj < a.nty - 1 && y >= t.cy1 - halo);
+        const bool neary = y >= t.cy0 - halo && y < t.cy1 + halo;
+        if (colok && rowok && incx && incy && (bandx || bandy) && (D == 0 || lane < 31)) send |= 1u << rj;
+        if (colok && rowok && nearx && neary && !(incx && incy)) recv |= 1u << rj;
     }
-    unsigned int rows = 0;
-    for (int rj = 0; rj < R; ++rj)
-        for (int ci = 0; ci < C; ++ci) {
-            const int gx = t.ox + lane * C + ci, gy = t.oy + warp * R + rj;
-            if (gx < 0) continue;
-            for (int k = 0; k < 4; ++k) {
-                if (gx / 3 >= gs.r[k].g0 && gx / 3 < gs.r[k].g1 && gy >= gs.r[k].y0 && gy < gs.r[k].y1) rows |= 1u << rj;
-                if (gx / 3 >= gr.r[k].g0 && gx / 3 < gr.r[k].g1 && gy >= gr.r[k].y0 && gy < gr.r[k].y1) rows |= 1u << (8 + rj);
+    const unsigned int rprev = __shfl_up_sync(0xffffffffu, recv, 1);
+    info = send | (recv << 8) | ((D && lane > 0) ? rprev << 16 : 0u);
+    ubase = gy0 * a.upitch + kown;
+}
+
+// The halo exchange of one field held in registers (psi after a round of sweeps; the new vorticity once per stage): every
+// thread stores the units of its micro-tile that lie in the border strips of the core, straight from its registers, and
+// fetches the units of its ring rows straight into them.  No shared memory, no table, no barrier.  A unit that does not
+// carry the tag of this round yet is fetched again (three rows of a thread are in flight together).
+// D > 0 (tiles of the last column when (N - 1) mod 4 != 0): a unit is the last D columns of a lane and the first 4 - D of the
+// next one; the sender collects them by shuffle, the receiver hands the second part on by shuffle.  All control flow around
+// the shuffles is warp-uniform.
+template <int C, int R, int D>
+__device__ __forceinline__ void xchg_units(double (&v)[R][C], char* __restrict__ xb, const size_t p1off, const size_t p2off,
+                                           const unsigned int round, const unsigned int info, const int ubase, const int upitch,
+                                           unsigned int* __restrict__ err, long long* __restrict__ stamp, const unsigned int tile) {
+    static_assert(C == 4 && R == 6, "written for the 4 x 6 micro-tile");
+    const unsigned int tag = round_tag(round);
+    const unsigned int send = info & 0x3fu;
+    const unsigned int wsend = D ? __reduce_or_sync(0xffffffffu, send) : 0u;
+#pragma unroll
+    for (int rj = 0; rj < R; ++rj) {
+        double u0, u1, u2, u3;
+        if (D == 0) {
+            u0 = v[rj][0]; u1 = v[rj][1]; u2 = v[rj][2]; u3 = v[rj][3];
+        } else {
+            if (!((wsend >> rj) & 1u)) continue;                        // the same for the whole warp
+            double mine[2 * C];
+#pragma unroll
+            for (int c = 0; c < C; ++c) mine[c] = v[rj][c];
+#pragma unroll
+            for (int c = 0; c < C - D; ++c) mine[C + c] = __shfl_down_sync(0xffffffffu, v[rj][c], 1);
+            u0 = mine[C - D]; u1 = mine[C - D + 1]; u2 = mine[C - D + 2]; u3 = mine[C - D + 3];
+        }
+        if ((send >> rj) & 1u) {
+            const Unit u = unit_pack(u0, u1, u2, u3, tag);
+            const size_t ui = (size_t)(ubase + rj * upitch);
+            st_v2(xb + 16 * ui, u.w0, u.w1);
+            st_v2(xb + p1off + 16 * ui, u.w2, u.w3);
+            st_b64(xb + p2off + 8 * ui, u.w4);
+        }
+    }
+    if (stamp != nullptr && threadIdx.x == 0 && threadIdx.y == 0) *stamp = globaltimer_ns();
+
+    // ---- fetch.  Word i of a row's own unit belongs into v[rj][C - OWN + i] for i < OWN (OWN = 4 if D = 0, else D), the other
+    // NF = 4 - OWN words into the first columns of the lane to the right.  The own words are loaded straight into the
+    // registers they replace (those ring values are dead), so that all rows of a thread can be in flight together.
+    constexpr int OWN = D == 0 ? C : D, NF = C - OWN;
+    // rows in flight together: with all six the sweep loops lose registers to this phase (q spills into them), measured
+#ifndef CAV_RB0
+#define CAV_RB0 (R / 2)
+#endif
+    constexpr int RB = D == 0 ? CAV_RB0 : R / 2;
+    unsigned int pending = (info >> 8) & 0x3fu;
+    const unsigned int rprev = (info >> 16) & 0x3fu;
+    long long t0 = 0;
+    int giveup = 0;
+    // The neighbours store while this tile does: fetching at once would mostly bring the previous round's bytes.  The first and
+    // the last lane of the warp that wait for anything poll the last word of their last row (what their neighbour stores
+    // last) until it carries the tag; only then does the warp fetch.  A heuristic for WHEN to fetch: the tags decide validity.
+    {
+        const unsigned int waiting = __ballot_sync(0xffffffffu, pending != 0u);
+        if (waiting != 0u && ((int)threadIdx.x == __ffs((int)waiting) - 1 || (int)threadIdx.x == 31 - __clz((int)waiting))) {
+            const int rj = 31 - __clz((int)pending);
+            const char* const pw = xb + p2off + 8 * (size_t)(ubase + rj * upitch);
+            unsigned long long w4;
+            ld_b64(pw, w4);
+            if (((unsigned int)(w4 >> 48) & 0xfffu) != tag) {
+                t0 = clock64();
+                do {
+                    ld_b64(pw, w4);
+                    if (*(volatile unsigned int*)err != 0u || clock64() - t0 > SPIN_TIMEOUT_CYCLES) break;      // decided below
+                } while (((unsigned int)(w4 >> 48) & 0xfffu) != tag);
             }
         }
-    o[(size_t)(a.ns_per + a.nr_per) * npr + tid] = rows;
+        __syncwarp();
+    }
+    for (int attempt = 0;; ++attempt) {
+#pragma unroll
+        for (int b0 = 0; b0 < R; b0 += RB) {
+            unsigned long long w4[RB];
+            double tmp[RB][NF > 0 ? NF : 1];
+#pragma unroll
+            for (int j = 0; j < RB; ++j) {
+                const int rj = b0 + j;
+                const int on = (int)((pending >> rj) & 1u);
+                const size_t ui = (size_t)(ubase + rj * upitch);
+                w4[j] = 0ull;
+#pragma unroll
+                for (int c = 0; c < NF; ++c) tmp[j][c] = 0.0;
+                // words 0, 1 / 2, 3: each goes to its own register (v) or to tmp
+                double& d0 = OWN > 0 ? v[rj][C - OWN] : tmp[j][0];
+                double& d1 = OWN > 1 ? v[rj][C - OWN + 1 < C ? C - OWN + 1 : C - 1] : tmp[j][1 - OWN < 0 ? 0 : (1 - OWN < NF ? 1 - OWN : 0)];
+                double& d2 = OWN > 2 ? v[rj][C - OWN + 2 < C ? C - OWN + 2 : C - 1] : tmp[j][2 - OWN < 0 ? 0 : (2 - OWN < NF ? 2 - OWN : 0)];
+                double& d3 = OWN > 3 ? v[rj][C - 1] : tmp[j][3 - OWN < 0 ? 0 : (3 - OWN < NF ? 3 - OWN : 0)];
+                ld_v2_if(on, xb + 16 * ui, d0, d1);
+                ld_v2_if(on, xb + p1off + 16 * ui, d2, d3);
+                ld_b64_if(on, xb + p2off + 8 * ui, w4[j]);
+            }
+#pragma unroll
+            for (int j = 0; j < RB; ++j) {
+                const int rj = b0 + j;
+                double& d0 = OWN > 0 ? v[rj][C - OWN] : tmp[j][0];
+                double& d1 = OWN > 1 ? v[rj][C - OWN + 1 < C ? C - OWN + 1 : C - 1] : tmp[j][1 - OWN < 0 ? 0 : (1 - OWN < NF ? 1 - OWN : 0)];
+                double& d2 = OWN > 2 ? v[rj][C - OWN + 2 < C ? C - OWN + 2 : C - 1] : tmp[j][2 - OWN < 0 ? 0 : (2 - OWN < NF ? 2 - OWN : 0)];
+                double& d3 = OWN > 3 ? v[rj][C - 1] : tmp[j][3 - OWN < 0 ? 0 : (3 - OWN < NF ? 3 - OWN : 0)];
+                const unsigned int tg = (((unsigned int)__double2loint(d0) ^ tag) | ((unsigned int)__double2loint(d1) ^ tag) |
+                                         ((unsigned int)__double2loint(d2) ^ tag) | ((unsigned int)__double2loint(d3) ^ tag)) & 0xfffu;
+                const unsigned int m = (unsigned int)w4[j], h = (unsigned int)(w4[j] >> 32);
+                const bool ok = ((pending >> rj) & 1u) && tg == 0u && ((h >> 16) & 0xfffu) == tag;
+                if (ok) {
+                    pending &= ~(1u << rj);
+                    // in place: only the low word of each double changes
+                    d0 = __hiloint2double(__double2hiint(d0), (int)(((unsigned int)__double2loint(d0) & 0xfffff000u) | (m & 0xfffu)));
+                    d1 = __hiloint2double(__double2hiint(d1), (int)(((unsigned int)__double2loint(d1) & 0xfffff000u) | ((m >> 12) & 0xfffu)));
+                    d2 = __hiloint2double(__double2hiint(d2), (int)(((unsigned int)__double2loint(d2) & 0xfffff000u) | (m >> 24) | ((h & 0xfu) << 8)));
+                    d3 = __hiloint2double(__double2hiint(d3), (int)(((unsigned int)__double2loint(d3) & 0xfffff000u) | ((h >> 4) & 0xfffu)));
+                }
+                if (D != 0) {
+                    const unsigned int got = __ballot_sync(0xffffffffu, ok);
+                    if (got) {                                          // the same for the whole warp
+                        const bool take = ((got << 1) >> threadIdx.x) & 1u & (rprev >> rj);
+#pragma unroll
+                        for (int c = 0; c < NF; ++c) {
+                            const double x = __shfl_up_sync(0xffffffffu, tmp[j][c], 1);
+                            if (take) v[rj][c] = x;
+                        }
+                    }
+                }
+            }
+        }
+        if (!__ballot_sync(0xffffffffu, pending != 0u)) break;
+        if (attempt == 0 && t0 == 0) t0 = clock64();
+        if (pending != 0u) {
+            if (*(volatile unsigned int*)err != 0u) giveup = 1;        // some tile gave up: do not wait again
+            else if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) {
+                if (atomicExch(err, 1u) == 0u) {      // the first tile to give up says what it was waiting for (CAV_DEBUG)
+                    const int rj = __ffs((int)pending) - 1;
+                    const size_t ui = (size_t)(ubase + rj * upitch);
+                    unsigned long long f0, f1, f4;
+                    ld_v2(xb + 16 * ui, f0, f1);
+                    ld_b64(xb + p2off + 8 * ui, f4);
+                    err[1] = tile; err[2] = (unsigned int)ui; err[3] = round; err[4] = tag;
+                    err[5] = (unsigned int)f0 & 0xfffu; err[6] = (unsigned int)f1 & 0xfffu; err[7] = (unsigned int)(f4 >> 48) & 0xfffu; err[8] = pending;
+                    err[9] = threadIdx.y * 32 + threadIdx.x;
+                }
+                giveup = 1;
+            }
+        }
+        if (__any_sync(0xffffffffu, giveup)) break;
+    }
 }
 
 // ---- the tile image in shared memory ----------------------------------------------------------------------------
@@ -554,102 +654,6 @@ __device__ __forceinline__ void fill_image(double* __restrict__ img, const doubl
             const int row = warp + nwarps * (half * (R / 2) + i);
 #pragma unroll
             for (int j = 0; j < C; ++j) ic[row * SW + 32 * j] = v[i][j];
-        }
-    }
-}
-
-// Stores this tile's strip units from the image, fetches its ring units into the image.  All threads; no barrier inside.
-// Not inlined (like rhs_phase below): its registers are allocated apart from the sweep loops, which hold psi and q in
-// registers and have none to spare.
-// Scalar arguments only: a reference to the kernel parameters would be re-read through generic loads after every store.
-// xb: the exchange buffer of this round; stamp: where thread 0 records the time between storing and fetching (or null).
-__device__ __noinline__ void exchange_units(ulonglong4* __restrict__ xb, const unsigned int round, const int ns_per, const int nr_per,
-                                               unsigned int* __restrict__ err, long long* __restrict__ stamp, double* __restrict__ img,
-                                               const unsigned int* __restrict__ tab, double* __restrict__ land, const int tid_o,
-                                               const int nth_o, const int ox, const int oy, const int upitch, const unsigned int tile) {
-    constexpr int SW = 128;                                             // image row = 32 lanes x 4 points
-    const unsigned int tag = round_tag(round);
-    const int h = tid_o & 1, pr = tid_o >> 1, npr = nth_o >> 1;       // half, pair index, pairs in the CTA
-    unsigned int* const img32 = reinterpret_cast<unsigned int*>(img) + 3 * h - 16;      // this lane's three words of a unit start here + 2 loc
-    char* const xbh = reinterpret_cast<char*>(xb) + 16 * h;                            // ... and its 16 bytes of a unit here + 32 unit
-    for (int i0 = 0; i0 < ns_per; i0 += 3) {                           // three slots at a time: their loads overlap
-        unsigned int e[3], A[3], B[3], Cw[3];
-#pragma unroll
-        for (int j = 0; j < 3; ++j) e[j] = i0 + j < ns_per ? tab[(i0 + j) * npr + pr] : NO_UNIT;
-#pragma unroll
-        for (int j = 0; j < 3; ++j)
-            if (e[j] != NO_UNIT) {                                     // strip points always lie inside the image: no masks
-                const unsigned int* const s = img32 + 2 * entry_loc(e[j], SW);
-                A[j] = s[0]; B[j] = s[1]; Cw[j] = s[2];
-            }
-#pragma unroll
-        for (int j = 0; j < 3; ++j)
-            if (e[j] != NO_UNIT) st_half(xbh + 32 * (size_t)entry_unit(e[j], ox, oy, upitch), half_pack(A[j], B[j], Cw[j], tag));
-    }
-    if (stamp != nullptr && tid_o == 0) *stamp = globaltimer_ns();
-    // All threads fetch ring half-units as 16-byte asynchronous copies into a landing zone in shared memory, NB slots per thread
-    // in flight together (no registers are held while they fly: an L2 round trip for data another SM has just written costs
-    // ~0.5 us here).  A copy is a weak load: it may bring the previous round's bytes, which the tags expose; the slots that did
-    // not validate are fetched again, all of them together, after ONE lane of the warp has polled one of them with strong loads
-    // until it carries the tag (waiting tiles do not load L2).
-    constexpr int NB = CAV_RECV_BATCH;
-    const unsigned int* const tabr = tab + ns_per * npr + pr;
-    HalfUnit* const mine_land = reinterpret_cast<HalfUnit*>(land) + tid_o;                 // slot j of this thread: mine_land[j * nth_o]
-    for (int i0 = 0; i0 < nr_per; i0 += NB) {
-        unsigned int pending = 0;                                       // slots of this batch that hold no valid half yet
-#pragma unroll
-        for (int j = 0; j < NB; ++j)
-            if (i0 + j < nr_per && tabr[(i0 + j) * npr] != NO_UNIT) pending |= 1u << j;
-        long long t0 = 0;
-        for (int attempt = 0;; ++attempt) {
-#pragma unroll
-            for (int j = 0; j < NB; ++j)
-                if ((pending >> j) & 1u) {
-                    const unsigned int dst = (unsigned int)__cvta_generic_to_shared(mine_land + j * nth_o);
-                    const char* const src = xbh + 32 * (size_t)entry_unit(tabr[(i0 + j) * npr], ox, oy, upitch);
-                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-                }
-            asm volatile("cp.async.commit_group;" ::: "memory");
-            asm volatile("cp.async.wait_group 0;" ::: "memory");
-#pragma unroll
-            for (int j = 0; j < NB; ++j)
-                if (((pending >> j) & 1u) && half_ok(mine_land[j * nth_o], tag)) pending &= ~(1u << j);
-            const unsigned int waiting = __ballot_sync(0xffffffffu, pending != 0u);
-            if (!waiting) break;
-            if (attempt == 0) t0 = clock64();
-            int giveup = 0;
-            if ((int)threadIdx.x == __ffs((int)waiting) - 1) {
-                const int j0 = __ffs((int)pending) - 1;                // the first missing half of this lane
-                const unsigned int off = entry_unit(tabr[(i0 + j0) * npr], ox, oy, upitch);
-                while (!half_ok(ld_half(xbh + 32 * (size_t)off), tag)) {
-                    if (*(volatile unsigned int*)err != 0u) { giveup = 1; break; }      // some tile gave up: do not wait again
-                    if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) {
-                        if (atomicExch(err, 1u) == 0u) {      // the first tile to give up says what it was waiting for (CAV_DEBUG)
-                            const HalfUnit w = ld_half(xbh + 32 * (size_t)off);
-                            err[1] = tile; err[2] = off; err[3] = round; err[4] = tag;
-                            err[5] = w.w1 >> 16; err[6] = w.w3 >> 16; err[7] = (unsigned int)h; err[8] = 0u;
-                            err[9] = (unsigned int)tid_o;
-                        }
-                        giveup = 1; break;
-                    }
-                }
-            }
-            if (__any_sync(0xffffffffu, giveup)) break;
-        }
-#pragma unroll
-        for (int j = 0; j < NB; ++j) {
-            const unsigned int e = i0 + j < nr_per ? tabr[(i0 + j) * npr] : NO_UNIT;
-            if (e != NO_UNIT) {
-                unsigned int A, B, C;
-                half_unpack(mine_land[j * nth_o], A, B, C);
-                unsigned int* const d = img32 + 2 * entry_loc(e, SW);
-                // words 0 1 | 2 of lane 0 belong to points 0 | 1 of the unit, words 0 | 1 2 of lane 1 to points 1 | 2; bits 16-18 of
-                // the entry say which points lie inside the image
-                const unsigned int m = e >> (16 + h);
-                if (m & 1u) d[0] = A;
-                if (h ? (m & 2u) : (m & 1u)) d[1] = B;
-                if (m & 2u) d[2] = C;
-            }
         }
     }
 }
@@ -866,10 +870,20 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
     }
     __syncthreads();
     if (a.ntx * a.nty > 1) {
-        double* const land = img + H * SW + 2 * SW + 2 * H;
-        const unsigned int* const tab = reinterpret_cast<const unsigned int*>(land + 2 * CAV_RECV_BATCH * nth_o);
-        exchange_units((round & 1u) ? a.x1 : a.x0, round, a.ns_per, a.nr_per, a.err, nullptr, img, tab, land, tid_o, nth_o,
-                       te.ox, te.oy, a.upitch, blockIdx.y * a.ntx + blockIdx.x);
+        // the new vorticity of core + walls goes back to the registers (the walls were written into the image by the owners
+        // of the adjacent points), is exchanged like psi, and the ring it brought goes into the image
+        read_tile<C, R>(ab, img, ln, wp, 0x3fu);
+        const unsigned int* const xi = reinterpret_cast<const unsigned int*>(img + H * SW + 2 * SW + 2 * H) + 2 * tid_o;
+        const unsigned int info = xi[0];
+        const int ubase = (int)xi[1];
+        char* const xb = (round & 1u) ? a.x1 : a.x0;
+        switch (te.D) {
+            case 0: xchg_units<C, R, 0>(ab, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, nullptr, blockIdx.y * a.ntx + blockIdx.x); break;
+            case 1: xchg_units<C, R, 1>(ab, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, nullptr, blockIdx.y * a.ntx + blockIdx.x); break;
+            case 2: xchg_units<C, R, 2>(ab, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, nullptr, blockIdx.y * a.ntx + blockIdx.x); break;
+            default: xchg_units<C, R, 3>(ab, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, nullptr, blockIdx.y * a.ntx + blockIdx.x); break;
+        }
+        stage_tile<C, R>(ab, img, ln, wp, (info >> 8) | (info >> 16));
         __syncthreads();
     }
     {   // first ring of the new vorticity around the core, kept for a3 of the next stage
@@ -916,16 +930,14 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
         if (t.top_al && warp == (N - t.oy) / R) fl &= ~FL_PUB_BOTTOM;          // that warp holds y = N .. N + R - 1
     }
 
-    // ---- exchange tables (multi-tile plans only): copied from the per-plan tables in global memory ----
-    {
+    // ---- what this thread moves in an exchange (multi-tile plans only), kept in shared memory: the sweeps have no register to spare ----
+    if (a.ntx * a.nty > 1) {
         const int H = nwarps * R;
-        unsigned int* const tabs = reinterpret_cast<unsigned int*>(sm + edge_doubles + H * SW + 2 * SW + 2 * H + 2 * CAV_RECV_BATCH * nthreads);
-        if (a.ntx * a.nty > 1) {
-            const int n = (int)xtab_words(nthreads, a.ns_per, a.nr_per);
-            const unsigned int* const src = a.tables + (size_t)(bj * a.ntx + bi) * n;
-            for (int k = tid; k < n; k += nthreads) tabs[k] = src[k];
-            if (tid == 0) { tabs[n] = (unsigned int)t.ox; tabs[n + 1] = (unsigned int)t.oy; }
-        }
+        unsigned int* const xi = reinterpret_cast<unsigned int*>(sm + edge_doubles + H * SW + 2 * SW + 2 * H) + 2 * tid;
+        unsigned int info;
+        int ubase;
+        xchg_setup<C, R>(a, t, lane, warp, bi, bj, info, ubase);
+        xi[0] = info; xi[1] = (unsigned int)ubase;
     }
 
     // ---- load the micro-tile: psi, and the right-hand side q = cq w of the first stage ----
@@ -1006,26 +1018,29 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
             mark(a, tslot);
             if (a.ntx * a.nty == 1 || (a.nsteps == 0 && rem <= a.T)) continue;  // sweeps only: the last round needs no exchange
 
-            // ---- halo exchange of psi through L2: tagged data, no fence, no flag ----
+            // ---- halo exchange of psi through L2, register to register: tagged data, no fence, no flag, no barrier ----
             // Opaque copies: everything derived from them is recomputed here every round instead of being hoisted out of
             // the round loop, where it would stay live across the sweeps and push q into local memory.
-            const int z = opaque_zero();
-            const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
-            const int nw = (int)blockDim.y + z, tid_o = wp * 32 + ln, nth_o = nw * 32, H = nw * R;
-            double* const img = sm + edge_doubles;
-            double* const land = img + H * SW + 2 * SW + 2 * H;
-            const unsigned int* const tab = reinterpret_cast<const unsigned int*>(land + 2 * CAV_RECV_BATCH * nth_o);
-            const unsigned int rows = tab[(a.ns_per + a.nr_per) * (nth_o >> 1) + tid_o];
-            const int tox = (int)tab[(a.ns_per + a.nr_per) * (nth_o >> 1) + nth_o], toy = (int)tab[(a.ns_per + a.nr_per) * (nth_o >> 1) + nth_o + 1];
-            stage_tile<C, R>(p, img, ln, wp, rows);
-            __syncthreads();
-            exchange_units((round & 1u) ? a.x1 : a.x0, round, a.ns_per, a.nr_per, a.err,
-                           (a.trace != nullptr && tslot + 1 < a.trace_cap) ? a.trace + (size_t)(blockIdx.y * a.ntx + blockIdx.x) * a.trace_cap + tslot + 1 : nullptr,
-                           img, tab, land, tid_o, nth_o, tox, toy, a.upitch, blockIdx.y * a.ntx + blockIdx.x);
+            {
+                const int z = opaque_zero();
+                const int nw = (int)blockDim.y + z, tid_o = ((int)threadIdx.y + z) * 32 + (int)threadIdx.x;
+                const unsigned int* const xi = reinterpret_cast<const unsigned int*>(sm + edge_doubles + nw * R * SW + 2 * SW + 2 * nw * R) + 2 * tid_o;
+                const unsigned int info = xi[0];
+                const int ubase = (int)xi[1];
+                char* const xb = (round & 1u) ? a.x1 : a.x0;
+                long long* const stamp = (a.trace != nullptr && tslot + 1 < a.trace_cap) ? a.trace + (size_t)(blockIdx.y * a.ntx + blockIdx.x) * a.trace_cap + tslot + 1 : nullptr;
+                const unsigned int tile = blockIdx.y * a.ntx + blockIdx.x;
+                // D of this tile, from blockIdx and the parameters only: a uniform branch
+                const int Dt = ((int)blockIdx.x == a.ntx - 1 && a.ntx > 1) ? ((a.N - 1) & 3) : 0;
+                switch (Dt) {
+                    case 0: xchg_units<C, R, 0>(p, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, stamp, tile); break;
+                    case 1: xchg_units<C, R, 1>(p, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, stamp, tile); break;
+                    case 2: xchg_units<C, R, 2>(p, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, stamp, tile); break;
+                    default: xchg_units<C, R, 3>(p, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, stamp, tile); break;
+                }
+            }
             ++round;
-            __syncthreads();
             mark(a, tslot + 2);
-            read_tile<C, R>(p, img, ln, wp, rows >> 8);
             publish_all<C, R, TOPOFF>(p, sB, fl);
             mark(a, tslot + 3);
         }
@@ -1092,42 +1107,48 @@ constexpr int NVARIANTS = sizeof(VARIANTS) / sizeof(VARIANTS[0]);
 inline int cdiv(int a, int b) { return (a + b - 1) / b; }
 inline double sweep_cycles(int warps) { return 2.0 * (cdiv(warps, 4) * 187.0 + 40.0); }      // one sweep = two colour half-sweeps
 
-// Checks that every tile of the candidate fits its thread grid and counts the exchange units per thread.
+// Checks that every tile of the candidate fits its thread grid.
 bool finish_plan(ResidentPlan& pl, int N, int max_smem) {
-    const int W = 32 * pl.C, H = pl.warps * pl.R, nth = 32 * pl.warps;
-    int smax = 0, rmax = 0;
+    const int W = 32 * pl.C, H = pl.warps * pl.R;
     for (int bj = 0; bj < pl.nty; ++bj)
         for (int bi = 0; bi < pl.ntx; ++bi) {
             const TileGeom t = tile_geom(N, pl.CW, pl.CH, pl.halo, pl.ntx, pl.nty, bi, bj, pl.C, pl.R, W, H);
             if (!t.fits) return false;
-            if (pl.ntiles > 1) {
-                smax = std::max(smax, uregion_total(send_units(t, N, pl.halo, bi, bj, pl.ntx, pl.nty, pl.kind == 1)));
-                rmax = std::max(rmax, uregion_total(recv_units(t, N, pl.halo, pl.kind == 1)));
-            }
         }
-    pl.ns_per = cdiv(smax, nth / 2);         // units per PAIR of lanes (a lane moves one 16-byte half of each)
-    pl.nr_per = cdiv(rmax, nth / 2);
     const int maxw = VARIANTS[pl.variant].maxw;
-    const size_t smem = smem_layout_bytes(pl.C, pl.R, maxw, pl.warps, pl.ns_per, pl.nr_per);
+    const size_t smem = smem_layout_bytes(pl.C, pl.R, maxw, pl.warps);
     pl.fixup = pl.ntx == 1 || pl.nty == 1;
     if (smem > (size_t)max_smem) return false;
     pl.smem_bytes = (int)smem;
     return true;
 }
 
-// One direction of the tiling: G points, thread grid of L points, halo h; core sizes are multiples of `align` when there
-// is more than one tile.  false if no uniform core size works.
-bool split(int G, int L, int lead, int h, int align, int& core, int& n) {
+// Tiling in y: G points, thread grid of L rows, halo h.  false if no uniform core size works.
+bool split(int G, int L, int lead, int h, int& core, int& n) {
     if (G + lead <= L) { core = G; n = 1; return true; }       // one tile holds both walls (lead = alignment slack of the first wall)
-    const int cmax = (L - 2 * h) / align * align;
+    const int cmax = L - 2 * h;
     if (cmax <= h) return false;
     for (n = cdiv(G, cmax); n <= G; ++n) {
-        core = cdiv(cdiv(G, n), align) * align;
+        core = cdiv(G, n);
         if (core > cmax) continue;
         n = cdiv(G, core);
         // the halo must come from adjacent tiles only, and must not reach a wall through an edge tile (only an
         // edge tile isolates the wall; elsewhere nothing keeps a wall point inside the thread grid at 0)
         return n >= 2 && core > h && G - (n - 1) * core > h;
+    }
+    return false;
+}
+// Tiling in x (tile_geom): cores [0, CW + 1), [CW + 1, 2 CW + 1), ..., CW a multiple of 4; an inner tile holds
+// round_up4(h) + CW + h columns.
+bool split_x(int N, int L, int lead, int h, int& core, int& n) {
+    if (N + 1 + lead <= L) { core = N + 1; n = 1; return true; }
+    const int cmax = (L - round_up4(h) - h) / 4 * 4;
+    if (cmax <= h) return false;
+    for (n = std::max(cdiv(N, cmax), 2); n <= N; ++n) {
+        core = round_up4(cdiv(N, n));
+        if (core > cmax) continue;
+        n = cdiv(N, core);
+        return n >= 2 && core > h && N - (n - 1) * core > h;
     }
     return false;
 }
@@ -1172,7 +1193,7 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
                 if (T_override > 0 && T != T_override) continue;
                 const int halo = (kind == 1 ? 4 : 2) * T;      // one ring is consumed per colour pass
                 int CW, ntx, CH, nty;
-                if (!split(G, W, v.C - 1, halo, 3, CW, ntx) || !split(G, H, v.R - 1, halo, 1, CH, nty)) continue;
+                if (!split_x(P.N, W, v.C - 1, halo, CW, ntx) || !split(G, H, v.R - 1, halo, CH, nty)) continue;
                 const int ntiles = ntx * nty;
                 if (ntiles < 2 || ntiles > sms) continue;
                 // Cost per sweep in SM cycles, calibrated on B200 (profiles/r2_*.md): a colour half-sweep takes ~187 cycles per warp
@@ -1208,29 +1229,12 @@ void resident_describe(const ResidentPlan& pl, char* buf, int len) {
     else
         std::snprintf(buf, (size_t)len,
                       "%s%dx%d tiles of %dx%d core + halo %d, T=%d sweeps per exchange, %d warps x (%dx%d micro-tiles), "
-                      "%d+%d exchange half-units (16 B) per thread, %d regs, %d B smem, one CTA per SM on %d SMs",
-                      pl.kind == 1 ? "compact 9-point operator, " : "", pl.ntx, pl.nty, pl.CW, pl.CH, pl.halo, pl.T, pl.warps, pl.C, pl.R, pl.ns_per, pl.nr_per, pl.regs,
+                      "register-to-register exchange of 40-byte units of four points, %d regs, %d B smem, one CTA per SM on %d SMs",
+                      pl.kind == 1 ? "compact 9-point operator, " : "", pl.ntx, pl.nty, pl.CW, pl.CH, pl.halo, pl.T, pl.warps, pl.C, pl.R, pl.regs,
                       pl.smem_bytes, pl.sm_count);
 }
 
 int resident_variants() { return NVARIANTS; }
-
-size_t resident_table_bytes(const ResidentPlan& pl) {
-    return (pl.ok && pl.ntiles > 1) ? (size_t)pl.ntiles * xtab_words(32 * pl.warps, pl.ns_per, pl.nr_per) * sizeof(unsigned int) : 0;
-}
-
-int resident_build_tables(const Params& P, const ResidentPlan& pl, void* tables_dev, cudaStream_t st) {
-    if (!pl.ok || pl.ntiles <= 1) return 0;
-    ResArgs a{};
-    a.N = P.N; a.pitch = P.pitch; a.upitch = resident_unit_pitch(P.N);
-    a.halo = pl.halo; a.CW = pl.CW; a.CH = pl.CH; a.ntx = pl.ntx; a.nty = pl.nty;
-    a.ns_per = pl.ns_per; a.nr_per = pl.nr_per; a.walls = pl.kind == 1;
-    const dim3 grid(pl.ntx, pl.nty), block(32, pl.warps);
-    if (pl.C == 4 && pl.R == 6) k_build_tables<4, 6><<<grid, block, 0, st>>>(a, (unsigned int*)tables_dev);
-    else return -(int)cudaErrorNotSupported;
-    const cudaError_t e = cudaGetLastError();
-    return e == cudaSuccess ? 1 : -(int)e;
-}
 
 long long resident_rounds(const ResidentPlan& pl, int nsteps, int S) {
     if (!pl.ok || pl.ntiles <= 1) return 0;
@@ -1239,24 +1243,24 @@ long long resident_rounds(const ResidentPlan& pl, int nsteps, int S) {
 }
 
 int resident_launch(const Params& P, const ResidentPlan& pl, const double* psi_in, double* psi_out, void* xa, void* xb,
-                    const void* tables, double* wbase, size_t fstride, unsigned int* err_word, unsigned int* epoch,
+                    double* wbase, size_t fstride, unsigned int* err_word, unsigned int* epoch,
                     int nsteps, int S, cudaStream_t st, long long* trace_dev, int trace_cap) {
     if (!pl.ok) return -(int)cudaErrorNotSupported;
-    if (nsteps < 0 || S < 0 || (nsteps == 0 && S == 0) || psi_in == psi_out || (pl.ntiles > 1 && (!tables || !xa || !xb)))
+    if (nsteps < 0 || S < 0 || (nsteps == 0 && S == 0) || psi_in == psi_out || (pl.ntiles > 1 && (!xa || !xb)))
         return -(int)cudaErrorInvalidValue;
     ResArgs a{};
-    a.tables = (const unsigned int*)tables;
     a.N = P.N; a.pitch = P.pitch; a.cb = P.cb; a.omb = P.omb; a.cq = P.cq;
     a.c9e = P.c9e; a.c9c = P.c9c; a.c9q = P.c9q;
     a.i2h = P.i2h; a.ih2 = P.ih2; a.nu = P.nu; a.c2h2 = P.c2h2; a.lid = P.lid; a.dt = P.dt;
     a.psi_in = psi_in; a.psi_out = psi_out; a.wbase = wbase; a.fstride = fstride;
-    a.x0 = (ulonglong4*)xa; a.x1 = (ulonglong4*)xb; a.upitch = resident_unit_pitch(P.N);
+    a.x0 = (char*)xa; a.x1 = (char*)xb; a.upitch = resident_unit_pitch(P.N);
+    a.p1off = resident_plane_bytes(P.N, 16); a.p2off = 2 * resident_plane_bytes(P.N, 16);
+    a.walls = pl.kind == 1;
     a.err = err_word;
     a.base = *epoch;
     a.nsteps = nsteps; a.S = S;
     a.T = pl.ntiles == 1 ? std::max(S, 1) : pl.T;
     a.halo = pl.halo; a.CW = pl.CW; a.CH = pl.CH; a.ntx = pl.ntx; a.nty = pl.nty;
-    a.ns_per = pl.ns_per; a.nr_per = pl.nr_per;
     a.trace = trace_dev; a.trace_cap = trace_cap;
     *epoch += (unsigned int)resident_rounds(pl, nsteps, S);      // wraps harmlessly: tags only tell round r from round r - 2
     void* args[] = {&a};

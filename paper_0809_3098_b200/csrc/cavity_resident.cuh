@@ -17,10 +17,9 @@ struct ResidentPlan {
     int warps = 0;        // warps per CTA; a warp spans 32 C points in x and R rows in y
     int T = 0;            // sweeps per round (between two halo exchanges); single tile: unused
     int halo = 0;         // 2 T, compact operator 4 T (one ring is consumed per colour pass); 0 for a single tile
-    int CW = 0, CH = 0;   // core (owned) points per tile in x and y; tile (bi, bj) owns [bi CW, (bi+1) CW) x [bj CH, (bj+1) CH)
+    int CW = 0, CH = 0;   // core (owned) points per tile in x and y: rows [bj CH, (bj+1) CH); columns [0, CW + 1), [CW + 1, 2 CW + 1), ... (CW a multiple of 4)
     int ntx = 0, nty = 0; // tiles in x and y
     int ntiles = 0;
-    int ns_per = 0, nr_per = 0;   // 16-byte halves of 32-byte exchange units each thread stores / fetches per round (0 for a single tile)
     bool fixup = false;           // some tile holds both walls of one direction: the kernel variant with the wall-mask fix-up
     int smem_bytes = 0;
     int regs = 0;         // registers per thread of the chosen variant (as compiled)
@@ -35,14 +34,13 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override = 0, int 
 int resident_variants();
 void resident_describe(const ResidentPlan& plan, char* buf, int len);
 
-// ONE exchange buffer (the engine needs two, zero-filled before first use and whenever the plan changes): a 32-byte unit
-// per group of three consecutive points of a grid row.
-inline int resident_unit_pitch(int N) { return (N + 1 + 2) / 3; }
-inline size_t resident_exchange_bytes(int N) { return (size_t)resident_unit_pitch(N) * (size_t)(N + 1) * 32; }
-
-// Per-plan exchange tables (device memory, built once per plan): their size, and the kernel that fills them.
-size_t resident_table_bytes(const ResidentPlan& plan);
-int resident_build_tables(const Params& P, const ResidentPlan& plan, void* tables_dev, cudaStream_t st);
+// ONE exchange buffer (the engine needs two, zero-filled before first use and whenever the plan changes): a unit per group
+// of four consecutive points of a grid row (unit k = columns 4k - 3 .. 4k), stored as three planes of 16, 16 and 8 bytes per unit.
+inline int resident_unit_pitch(int N) { return (N + 3) / 4 + 2; }
+inline size_t resident_plane_bytes(int N, int bytes_per_unit) {
+    return ((size_t)resident_unit_pitch(N) * (size_t)(N + 1) * (size_t)bytes_per_unit + 255) / 256 * 256;
+}
+inline size_t resident_exchange_bytes(int N) { return 2 * resident_plane_bytes(N, 16) + resident_plane_bytes(N, 8); }
 
 // Halo-exchange rounds one launch performs (the host-side round counter advances by this).
 long long resident_rounds(const ResidentPlan& plan, int nsteps, int S);
@@ -51,14 +49,13 @@ long long resident_rounds(const ResidentPlan& plan, int nsteps, int S);
 //   nsteps > 0: nsteps whole SSPRK(5,4) time steps, each 5 x [S sweeps of a1, a2, a3].  wbase points at six fields fstride
 //               doubles apart: omega^n (in: the state; out: the new state, ring = stage-5 Thom ring), omega^(1..4), T.
 //   nsteps = 0: S sweeps of a1 with right-hand side cq * (field 0 of wbase); nothing but psi is written.
-// Reads psi_in, writes psi_out (two different fields).  xa, xb: the two exchange buffers; tables: what resident_build_tables
-// wrote for this plan (all three may be null for a single-tile plan).  err_word: one device word, zero-filled; non-zero
+// Reads psi_in, writes psi_out (two different fields).  xa, xb: the two exchange buffers (may be null for a single-tile plan).  err_word: one device word, zero-filled; non-zero
 // afterwards = a tile gave up waiting for a neighbour.  *epoch is the host-side count of exchange rounds, advanced by this call.
 // trace_dev (profiling only, sweeps-only launches): device array of ntiles x trace_cap %globaltimer stamps (ns), slot 0 = start,
 // 1 = inputs loaded, then per round r: 2 + 4r sweeps done, 3 + 4r border strips stored, 4 + 4r ring received, 5 + 4r edges republished.
 // Returns the number of kernel launches (1), or a negative cudaError_t.
 int resident_launch(const Params& P, const ResidentPlan& plan, const double* psi_in, double* psi_out, void* xa, void* xb,
-                    const void* tables, double* wbase, size_t fstride, unsigned int* err_word, unsigned int* epoch,
+                    double* wbase, size_t fstride, unsigned int* err_word, unsigned int* epoch,
                     int nsteps, int S, cudaStream_t st, long long* trace_dev = nullptr, int trace_cap = 0);
 
 }  // namespace cavk
