@@ -151,8 +151,18 @@ int cav_set_resident_plan(cav_ctx* ctx, int sweeps_per_exchange, int variant);
  * with the capacity of a plan's tile count (at most 1023). */
 int cav_trace_sweeps(cav_ctx* ctx, int nsweeps, long long* stamps_out, int slots_per_tile, int* ntiles_out);
 
-/* Testing aid, resident engine: sets the host-side count of halo-exchange rounds (the 16-bit tag of a round is 1 + round mod
- * 65535, the buffer round mod 2) and clears the exchange buffers, so that a test can run across the wrap of the tags and of the
+/* Host logic of the resident engine, no device and no context needed: plans the tiling of an (N + 1)^2 grid for a device with
+ * `sms` multiprocessors, `smem_bytes` of shared memory per block and 65536 registers (sweep: CAV_SWEEP_REDBLACK or
+ * CAV_SWEEP_COMPACT9; T > 0 forces the sweeps per exchange round) and checks its halo-exchange pattern: every unit of four
+ * points a tile fetches must be stored by exactly one tile, every stored unit must be fetched, every tile must fit its thread
+ * grid.  plan_out[8] (may be NULL) = ntx, nty, CW, CH, halo, T, warps, shared-memory bytes; counts_out[5] (may be NULL) = units
+ * fetched, units stored, fetches without exactly one store, stores nobody fetches, tiles that do not fit.
+ * Returns CAV_OK if the plan is consistent (also for a single-tile plan, which exchanges nothing), CAV_ENOTSUP if the grid
+ * has no resident plan under these figures, CAV_EINVAL for bad arguments or an inconsistent pattern. */
+int cav_plan_check(int N, int sweep, int T, int sms, int smem_bytes, int* plan_out, long long* counts_out);
+
+/* Testing aid, resident engine: sets the host-side count of halo-exchange rounds (the 12-bit tag of a round is 1 + round mod
+ * 4095, the buffer round mod 2) and clears the exchange buffers, so that a test can run across the wrap of the tags and of the
  * 32-bit counter.  Neither wrap needs any action in normal use: a reader can only ever meet the round it waits for or the one
  * two rounds earlier. */
 int cav_debug_set_epoch(cav_ctx* ctx, unsigned int epoch);

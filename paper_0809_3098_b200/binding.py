@@ -17,7 +17,7 @@ _ENGINES = {"auto": ENGINE_AUTO, "stream": ENGINE_STREAM, "resident": ENGINE_RES
 SYMBOLS = ("cav_create", "cav_destroy", "cav_set_fields", "cav_get_fields", "cav_step", "cav_step_async", "cav_sync",
            "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_set_resident_plan", "cav_trace_sweeps", "cav_describe", "cav_launch_count",
            "cav_last_elapsed_ms", "cav_strerror", "cav_set_sweep", "cav_step_res", "cav_run_to_steady", "cav_debug_set_epoch",
-           "cav_measure_fp64_peak")
+           "cav_measure_fp64_peak", "cav_plan_check")
 
 SWEEP_REDBLACK, SWEEP_JACOBI, SWEEP_COMPACT9 = 0, 1, 2
 _SWEEPS = {"redblack": SWEEP_REDBLACK, "jacobi": SWEEP_JACOBI, "compact9": SWEEP_COMPACT9}
@@ -81,6 +81,7 @@ def lib():
     L.cav_run_to_steady.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(CavMonitor)]
     L.cav_debug_set_epoch.argtypes = [C.c_void_p, C.c_uint]
     L.cav_measure_fp64_peak.argtypes = [C.c_void_p, dp, dp]
+    L.cav_plan_check.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
     L.cav_strerror.argtypes = [C.c_int]
     L.cav_strerror.restype = C.c_char_p
     _lib = L
@@ -101,6 +102,17 @@ def _field(a, N, name):
     if a.shape != (N + 1, N + 1):
         raise ValueError("%s must have shape (N+1, N+1) = (%d, %d), row j = y index" % (name, N + 1, N + 1))
     return a
+
+
+def plan_check(N, sweep="redblack", T=0, sms=148, smem_bytes=232448):
+    """Host logic only (no device): the resident plan of an (N + 1)^2 grid and the consistency of its halo-exchange pattern.
+    Returns (rc, plan dict or None, counts dict)."""
+    plan = (C.c_int * 8)()
+    counts = (C.c_longlong * 5)()
+    rc = lib().cav_plan_check(int(N), _SWEEPS[sweep], int(T), int(sms), int(smem_bytes), plan, counts)
+    names = ("ntx", "nty", "CW", "CH", "halo", "T", "warps", "smem_bytes")
+    cn = ("fetched", "stored", "unmatched", "unfetched", "misfit")
+    return rc, (dict(zip(names, plan)) if rc != -4 else None), dict(zip(cn, counts))
 
 
 class Cavity:

@@ -539,6 +539,18 @@ CAV_API int cav_trace_sweeps(cav_ctx* c, int nsweeps, long long* stamps_out, int
     return rc == CAV_OK ? check_resident_error(c) : rc;
 }
 
+CAV_API int cav_plan_check(int N, int sweep, int T, int sms, int smem_bytes, int* plan_out, long long* counts_out) {
+    if (N < 2 || (sweep != CAV_SWEEP_REDBLACK && sweep != CAV_SWEEP_COMPACT9) || T < 0 || sms < 1 || smem_bytes < 1) return CAV_EINVAL;
+    const cavk::ResidentPlan pl = cavk::resident_plan_for(N, plan_kind(sweep), T, -1, sms, smem_bytes, 65536);
+    if (counts_out) for (int k = 0; k < 5; ++k) counts_out[k] = 0;
+    if (!pl.ok) return CAV_ENOTSUP;
+    if (plan_out) {
+        plan_out[0] = pl.ntx; plan_out[1] = pl.nty; plan_out[2] = pl.CW; plan_out[3] = pl.CH; plan_out[4] = pl.halo;
+        plan_out[5] = pl.ntiles > 1 ? pl.T : 0; plan_out[6] = pl.warps; plan_out[7] = pl.smem_bytes;
+    }
+    return cavk::resident_check_exchange(pl, N, counts_out) == 0 ? CAV_OK : CAV_EINVAL;
+}
+
 CAV_API int cav_debug_set_epoch(cav_ctx* c, unsigned int epoch) {
     if (!c) return CAV_EINVAL;
     DeviceGuard dg(c->device);

@@ -58,6 +58,7 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <vector>
 
 namespace cavk {
 
@@ -67,6 +68,9 @@ namespace {
 #define CAV_SPIN_TIMEOUT 20000000000LL      // ~10 s at 2 GHz: a neighbour whose data never arrives is a bug, not a wait
 #endif
 constexpr long long SPIN_TIMEOUT_CYCLES = CAV_SPIN_TIMEOUT;
+#ifndef CAV_RB
+#define CAV_RB 6             // rows of a thread in flight together in the psi exchange
+#endif
 #ifndef CAV_QROWS
 #define CAV_QROWS 2             // rows of the micro-tile whose q lives in shared memory instead of registers
 #endif
@@ -108,14 +112,15 @@ struct ResArgs {
 // Exchange units are groups of four consecutive points of a grid row, unit k = the columns 4k - 3 .. 4k (so that the wall
 // column x = 0 is the last column of unit 0, as it is the last column of lane 0 of a left-edge tile).  With more than one tile
 // in x the cores are [0, CW + 1), [CW + 1, 2 CW + 1), ... with CW a multiple of 4: every core boundary is a unit boundary (a
-// unit has exactly one owner), and every tile but those of the last column puts its origin at a unit boundary, so that the
-// four columns of a lane ARE a unit (D = 0).  A tile of the last column must put the wall x = N into the first column of a
-// lane; its lanes then start D = (N - 1) mod 4 columns after a unit boundary, and it moves its units through a warp shuffle.
+// unit has exactly one owner), and every tile puts its origin at a unit boundary: the four columns of a lane ARE a unit.
+// A tile of the last column then finds the wall x = N in column wc = (N - 1) mod 4 of a lane: wc = 0 isolates it as on the
+// other three sides; wc > 0 leaves interior points in the same lane, and the sweeps of those tiles (a uniform branch) read
+// +0.0 in place of that column (WC variant of half_sweep / colour_pass).
 struct TileGeom {
     int cx0, cx1, cy0, cy1;        // core [cx0, cx1) x [cy0, cy1)
     int ox, oy;                    // grid coordinates of local point (0, 0)
-    int D;                         // (ox - 1) mod 4: columns between a unit boundary and the first column of a lane
-    bool left_al, right_al, bot_al, top_al;   // wall isolated in a lane / warp that owns no interior point
+    int wc;                        // tiles of the last column: the column of a lane that holds x = N (0: isolated by alignment)
+    bool left_al, right_al, bot_al, top_al;   // wall isolated in a lane / warp that owns no interior point, or (right, wc > 0) read as +0.0
     bool fits;                     // the W x H thread grid covers core + halo (clipped to the grid) and the aligned walls
 };
 __host__ __device__ inline int round_up4(int v) { return (v + 3) / 4 * 4; }
@@ -131,15 +136,10 @@ __host__ __device__ inline TileGeom tile_geom(int N, int CW, int CH, int halo, i
     g.right_al = bi == ntx - 1 && ntx > 1;
     g.bot_al = bj == 0;
     g.top_al = bj == nty - 1 && nty > 1;
-    g.D = 0;
+    g.wc = 0;
     if (g.left_al) g.ox = -(C - 1);                                   // x = 0 is column C - 1 of lane 0
-    else if (g.right_al) {
-        // (N - ox) % C == 0: x = N is the first column of a lane.  If the lanes are not units (D > 0) lane 0 receives its
-        // first C - D columns from nobody: they must lie outside the halo.
-        g.D = (N - 1) & 3;
-        const int lim = g.cx0 - halo - (g.D ? C - g.D : 0);
-        g.ox = lim - (((lim - N) % C) + C) % C;
-    } else g.ox = g.cx0 - round_up4(halo);
+    else g.ox = g.cx0 - round_up4(halo);                              // = 1 (mod 4)
+    if (g.right_al) g.wc = (N - g.ox) % C;
     if (g.bot_al) g.oy = -(R - 1);                                    // y = 0 is row R - 1 of warp 0
     else if (g.top_al) g.oy = g.cy0 - halo - (R - (N - g.cy0 + halo) % R) % R;        // (N - oy) % R == 0
     else g.oy = g.cy0 - halo;
@@ -227,6 +227,7 @@ constexpr unsigned int FL_ZERO_LEFT = 1u;     // the left neighbour column is a 
 constexpr unsigned int FL_ZERO_RIGHT = 2u;    // same on the right
 constexpr unsigned int FL_PUB_BOTTOM = 4u;    // publish the bottom row of the micro-tile to the warp below
 constexpr unsigned int FL_PUB_TOP = 8u;       // publish the top row to the warp above
+constexpr unsigned int FL_WALL_LANE = 16u;    // this lane holds the wall x = N in column WC > 0, behind interior points: that column reads as +0.0
 
 // One colour half-sweep on the register micro-tile.  K = LOCAL colour being updated: local point (ci, rj) has local colour
 // (ci + rj) & 1 (C, R even); the kernel maps the global colour to the local one through the parity of the tile origin.
@@ -234,7 +235,7 @@ constexpr unsigned int FL_PUB_TOP = 8u;       // publish the top row to the warp
 // the rows above / below live in the adjacent warps and come through the sB / sT edge arrays.
 // wallmask: bit rj * C + ci set = that point lies ON a wall that could not be isolated by alignment and is put back to
 // +0.0 after the update (eq 23-24).
-template <int C, int R, int K, bool FIX, int TOPOFF>
+template <int C, int R, int K, bool FIX, int TOPOFF, int WC>
 __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[R][C], const double cb, const double omb,
                                            double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl_) {
     unsigned int fl = fl_;
@@ -274,7 +275,8 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
         for (int ci = 0; ci < C; ++ci) {
             if (((ci + rj) & 1) != K) continue;
             const double pW = ci > 0 ? p[rj][ci - 1] : Lnb[rj];
-            const double pE = ci < C - 1 ? p[rj][ci + 1] : Rnb[rj];
+            double pE = ci < C - 1 ? p[rj][ci + 1] : Rnb[rj];
+            if (WC > 0 && ci == WC - 1 && (fl & FL_WALL_LANE)) pE = 0.0;       // the wall x = N inside this lane
             const double pS = rj > 0 ? p[rj - 1][ci] : Bnb[ci];
             const double pN = rj < R - 1 ? p[rj + 1][ci] : Tnb[ci];
             const double nb = (pW + pE) + (pS + pN);
@@ -314,7 +316,7 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
 // (the expression of k_compact_colour).  From the other threads a pass needs ONE side column (the lane to the left if KX == 0, to
 // the right if KX == 1: six doubles by shuffle) and ONE edge row of five values (the warp below if KY == 0, above if KY == 1: the
 // edge arrays, whose neighbouring lane slots give the two diagonal values).
-template <int C, int R, int KX, int KY, bool FIX, int TOPOFF>
+template <int C, int R, int KX, int KY, bool FIX, int TOPOFF, int WC>
 __device__ __forceinline__ void colour_pass(double (&p)[R][C], const double (&q)[R][C], const double c9e, const double c9c, const double omb,
                                             double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl_) {
     static_assert(C == 4 && R == 6 && CAV_QROWS == 2, "written for the 4 x 6 micro-tile with q of rows 2, 3 in shared memory");
@@ -348,9 +350,12 @@ __device__ __forceinline__ void colour_pass(double (&p)[R][C], const double (&q)
     }
     // value at (column c, row r) around the micro-tile, c in -1 .. C, r in -1 .. R (only what this colour needs is ever asked for)
     auto at = [&](int c, int r) -> double {
-        if (r < 0 || r >= R) return edge[1 + c];
-        if (c < 0 || c >= C) return side[r];
-        return p[r][c];
+        double x;
+        if (r < 0 || r >= R) x = edge[1 + c];
+        else if (c < 0 || c >= C) x = side[r];
+        else x = p[r][c];
+        if (WC > 0 && c == WC && (fl & FL_WALL_LANE)) x = 0.0;         // the wall x = N inside this lane
+        return x;
     };
 #pragma unroll
     for (int rj = KY; rj < R; rj += 2) {
@@ -379,6 +384,35 @@ __device__ __forceinline__ void colour_pass(double (&p)[R][C], const double (&q)
     __syncthreads();
 }
 
+// ns sweeps on the register micro-tile.  WC: the column of a lane that holds the wall x = N behind interior points (0: none).
+template <int C, int R, bool FIX, int TOPOFF, int KIND, int WC>
+__device__ __forceinline__ void run_sweeps(double (&p)[R][C], const double (&q)[R][C], const double cb, const double omb, const double c9e,
+                                           const double c9c, double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl, const int ns,
+                                           const bool odd_origin, const int par9) {
+    if (KIND == 1) {
+        // four colours (i mod 2, j mod 2) in the order (0,0), (1,0), (0,1), (1,1) (reading N1); local colour = global ^ origin parity
+        for (int s = ns; s > 0; --s)
+            for (int g = 0; g < 4; ++g) {
+                switch (g ^ par9) {
+                    case 0: colour_pass<C, R, 0, 0, FIX, TOPOFF, WC>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
+                    case 1: colour_pass<C, R, 1, 0, FIX, TOPOFF, WC>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
+                    case 2: colour_pass<C, R, 0, 1, FIX, TOPOFF, WC>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
+                    default: colour_pass<C, R, 1, 1, FIX, TOPOFF, WC>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
+                }
+            }
+    } else if (odd_origin) {
+        for (int s = ns; s > 0; --s) {                                     // red = (i + j) even first (G9): local colour 1 here
+            half_sweep<C, R, 1, FIX, TOPOFF, WC>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 0, FIX, TOPOFF, WC>(p, q, cb, omb, sB, wallmask, fl);
+        }
+    } else {
+        for (int s = ns; s > 0; --s) {
+            half_sweep<C, R, 0, FIX, TOPOFF, WC>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 1, FIX, TOPOFF, WC>(p, q, cb, omb, sB, wallmask, fl);
+        }
+    }
+}
+
 template <int C, int R, int TOPOFF>
 __device__ __forceinline__ void publish_all(const double (&p)[R][C], double* __restrict__ sB, const unsigned int fl) {
     double* const sT = sB + TOPOFF;
@@ -403,75 +437,57 @@ __host__ __device__ inline size_t smem_layout_bytes(int C, int R, int maxw, int 
     return 8 * ((2 * (size_t)(maxw + 1) + CAV_QROWS * (size_t)maxw) * C * 32 + H * SW + 2 * SW + 2 * H) + 4 * 2 * nth;
 }
 
-// Which units a thread moves in an exchange.  Its OWN unit of micro-tile row rj is (k, y = gy0 + rj): k = the unit its four
-// columns are (D = 0), or the unit made of its last D columns and the first 4 - D columns of the lane to its right (D > 0).
+// Which units a thread moves in an exchange.  Row rj of its micro-tile is the unit (k, y = gy0 + rj), k = (ox + 3) / 4 + lane.
 //   info bits 0-5:   rows whose own unit it STORES: the unit lies in the tile's core, within `halo` of a core edge that has
 //                    a neighbour behind it
 //   info bits 8-13:  rows whose own unit it FETCHES: the unit lies outside the core, within `halo` of it (the ring)
-//   info bits 16-21: (D > 0) rows whose first 4 - D columns come from the unit the lane to the LEFT fetches
 //   ubase:           index of the own unit of row 0 in the exchange planes (row rj: + rj upitch); may be negative for
 //                    rows below the grid, which are never moved
 // Points: interior rows / columns only; with `walls` (compact operator: its right-hand side reads omega ON the walls, also in
 // the ring) the wall rows / columns too.  A unit counts if at least one of its columns does.
 template <int C, int R>
-__device__ __forceinline__ void xchg_setup(const ResArgs& a, const TileGeom& t, const int lane, const int warp, const int bi,
-                                           const int bj, unsigned int& info, int& ubase) {
+__host__ __device__ inline void xchg_setup(const int N, const int halo, const bool walls, const int ntx, const int nty, const int upitch,
+                                           const TileGeom& t, const int lane, const int warp, const int bi, const int bj,
+                                           unsigned int& info, int& ubase) {
     static_assert(C == 4, "units are groups of four columns");
-    const int N = a.N, halo = a.halo, D = t.D;
-    const int kown = (t.ox + 3 - D) / 4 + lane + (D ? 1 : 0);       // ox + 3 - D is a non-negative multiple of 4
+    const int kown = (t.ox + 3) / 4 + lane;                         // ox + 3 is a non-negative multiple of 4
     const int gy0 = t.oy + warp * R;
     const int xf = 4 * kown - 3, xl = 4 * kown, xr = imax(xf, 0);   // first / last column of the unit, its first column inside the grid
-    const int lo = a.walls ? 0 : 1, hi = a.walls ? N : N - 1;       // the rows / columns that are exchanged
+    const int lo = walls ? 0 : 1, hi = walls ? N : N - 1;           // the rows / columns that are exchanged
     const bool colok = xl >= lo && xf <= hi;
     const bool incx = xr >= t.cx0 && xr < t.cx1;
-    const bool bandx = (bi > 0 && xr < t.cx0 + halo) || (bi < a.ntx - 1 && xl >= t.cx1 - halo);
+    const bool bandx = (bi > 0 && xr < t.cx0 + halo) || (bi < ntx - 1 && xl >= t.cx1 - halo);
     const bool nearx = xl >= t.cx0 - halo && xf < t.cx1 + halo;
     unsigned int send = 0, recv = 0;
     for (int rj = 0; rj < R; ++rj) {
         const int y = gy0 + rj;
         const bool rowok = y >= lo && y <= hi;
         const bool incy = y >= t.cy0 && y < t.cy1;
-        const bool bandy = (bj > 0 && y < t.cy0 + halo) || (bj < a.nty - 1 && y >= t.cy1 - halo);
+        const bool bandy = (bj > 0 && y < t.cy0 + halo) || (bj < nty - 1 && y >= t.cy1 - halo);
         const bool neary = y >= t.cy0 - halo && y < t.cy1 + halo;
-        if (colok && rowok && incx && incy && (bandx || bandy) && (D == 0 || lane < 31)) send |= 1u << rj;
+        if (colok && rowok && incx && incy && (bandx || bandy)) send |= 1u << rj;
         if (colok && rowok && nearx && neary && !(incx && incy)) recv |= 1u << rj;
     }
-    const unsigned int rprev = __shfl_up_sync(0xffffffffu, recv, 1);
-    info = send | (recv << 8) | ((D && lane > 0) ? rprev << 16 : 0u);
-    ubase = gy0 * a.upitch + kown;
+    info = send | (recv << 8);
+    ubase = gy0 * upitch + kown;
 }
 
 // The halo exchange of one field held in registers (psi after a round of sweeps; the new vorticity once per stage): every
-// thread stores the units of its micro-tile that lie in the border strips of the core, straight from its registers, and
-// fetches the units of its ring rows straight into them.  No shared memory, no table, no barrier.  A unit that does not
-// carry the tag of this round yet is fetched again (three rows of a thread are in flight together).
-// D > 0 (tiles of the last column when (N - 1) mod 4 != 0): a unit is the last D columns of a lane and the first 4 - D of the
-// next one; the sender collects them by shuffle, the receiver hands the second part on by shuffle.  All control flow around
-// the shuffles is warp-uniform.
-template <int C, int R, int D>
+// thread stores the rows of its micro-tile that lie in the border strips of the core, straight from its registers, and
+// fetches its ring rows straight into them.  No shared memory, no table, no barrier.
+// RB rows of a thread are in flight together; the words of a unit are loaded into the very registers of the doubles they
+// replace (those ring values are dead), so that only word 4 of each row needs registers of its own.
+template <int C, int R, int RB>
 __device__ __forceinline__ void xchg_units(double (&v)[R][C], char* __restrict__ xb, const size_t p1off, const size_t p2off,
                                            const unsigned int round, const unsigned int info, const int ubase, const int upitch,
                                            unsigned int* __restrict__ err, long long* __restrict__ stamp, const unsigned int tile) {
-    static_assert(C == 4 && R == 6, "written for the 4 x 6 micro-tile");
+    static_assert(C == 4 && R % RB == 0, "a unit is the four columns of a lane");
     const unsigned int tag = round_tag(round);
     const unsigned int send = info & 0x3fu;
-    const unsigned int wsend = D ? __reduce_or_sync(0xffffffffu, send) : 0u;
 #pragma unroll
     for (int rj = 0; rj < R; ++rj) {
-        double u0, u1, u2, u3;
-        if (D == 0) {
-            u0 = v[rj][0]; u1 = v[rj][1]; u2 = v[rj][2]; u3 = v[rj][3];
-        } else {
-            if (!((wsend >> rj) & 1u)) continue;                        // the same for the whole warp
-            double mine[2 * C];
-#pragma unroll
-            for (int c = 0; c < C; ++c) mine[c] = v[rj][c];
-#pragma unroll
-            for (int c = 0; c < C - D; ++c) mine[C + c] = __shfl_down_sync(0xffffffffu, v[rj][c], 1);
-            u0 = mine[C - D]; u1 = mine[C - D + 1]; u2 = mine[C - D + 2]; u3 = mine[C - D + 3];
-        }
         if ((send >> rj) & 1u) {
-            const Unit u = unit_pack(u0, u1, u2, u3, tag);
+            const Unit u = unit_pack(v[rj][0], v[rj][1], v[rj][2], v[rj][3], tag);
             const size_t ui = (size_t)(ubase + rj * upitch);
             st_v2(xb + 16 * ui, u.w0, u.w1);
             st_v2(xb + p1off + 16 * ui, u.w2, u.w3);
@@ -480,19 +496,8 @@ __device__ __forceinline__ void xchg_units(double (&v)[R][C], char* __restrict__
     }
     if (stamp != nullptr && threadIdx.x == 0 && threadIdx.y == 0) *stamp = globaltimer_ns();
 
-    // ---- fetch.  Word i of a row's own unit belongs into v[rj][C - OWN + i] for i < OWN (OWN = 4 if D = 0, else D), the other
-    // NF = 4 - OWN words into the first columns of the lane to the right.  The own words are loaded straight into the
-    // registers they replace (those ring values are dead), so that all rows of a thread can be in flight together.
-    constexpr int OWN = D == 0 ? C : D, NF = C - OWN;
-    // rows in flight together: with all six the sweep loops lose registers to this phase (q spills into them), measured
-#ifndef CAV_RB0
-#define CAV_RB0 (R / 2)
-#endif
-    constexpr int RB = D == 0 ? CAV_RB0 : R / 2;
     unsigned int pending = (info >> 8) & 0x3fu;
-    const unsigned int rprev = (info >> 16) & 0x3fu;
     long long t0 = 0;
-    int giveup = 0;
     // The neighbours store while this tile does: fetching at once would mostly bring the previous round's bytes.  The first and
     // the last lane of the warp that wait for anything poll the last word of their last row (what their neighbour stores
     // last) until it carries the tag; only then does the warp fetch.  A heuristic for WHEN to fetch: the tags decide validity.
@@ -513,40 +518,28 @@ __device__ __forceinline__ void xchg_units(double (&v)[R][C], char* __restrict__
         }
         __syncwarp();
     }
-    for (int attempt = 0;; ++attempt) {
+    while (__any_sync(0xffffffffu, pending != 0u)) {
 #pragma unroll
         for (int b0 = 0; b0 < R; b0 += RB) {
             unsigned long long w4[RB];
-            double tmp[RB][NF > 0 ? NF : 1];
 #pragma unroll
             for (int j = 0; j < RB; ++j) {
                 const int rj = b0 + j;
                 const int on = (int)((pending >> rj) & 1u);
                 const size_t ui = (size_t)(ubase + rj * upitch);
                 w4[j] = 0ull;
-#pragma unroll
-                for (int c = 0; c < NF; ++c) tmp[j][c] = 0.0;
-                // words 0, 1 / 2, 3: each goes to its own register (v) or to tmp
-                double& d0 = OWN > 0 ? v[rj][C - OWN] : tmp[j][0];
-                double& d1 = OWN > 1 ? v[rj][C - OWN + 1 < C ? C - OWN + 1 : C - 1] : tmp[j][1 - OWN < 0 ? 0 : (1 - OWN < NF ? 1 - OWN : 0)];
-                double& d2 = OWN > 2 ? v[rj][C - OWN + 2 < C ? C - OWN + 2 : C - 1] : tmp[j][2 - OWN < 0 ? 0 : (2 - OWN < NF ? 2 - OWN : 0)];
-                double& d3 = OWN > 3 ? v[rj][C - 1] : tmp[j][3 - OWN < 0 ? 0 : (3 - OWN < NF ? 3 - OWN : 0)];
-                ld_v2_if(on, xb + 16 * ui, d0, d1);
-                ld_v2_if(on, xb + p1off + 16 * ui, d2, d3);
+                ld_v2_if(on, xb + 16 * ui, v[rj][0], v[rj][1]);
+                ld_v2_if(on, xb + p1off + 16 * ui, v[rj][2], v[rj][3]);
                 ld_b64_if(on, xb + p2off + 8 * ui, w4[j]);
             }
 #pragma unroll
             for (int j = 0; j < RB; ++j) {
                 const int rj = b0 + j;
-                double& d0 = OWN > 0 ? v[rj][C - OWN] : tmp[j][0];
-                double& d1 = OWN > 1 ? v[rj][C - OWN + 1 < C ? C - OWN + 1 : C - 1] : tmp[j][1 - OWN < 0 ? 0 : (1 - OWN < NF ? 1 - OWN : 0)];
-                double& d2 = OWN > 2 ? v[rj][C - OWN + 2 < C ? C - OWN + 2 : C - 1] : tmp[j][2 - OWN < 0 ? 0 : (2 - OWN < NF ? 2 - OWN : 0)];
-                double& d3 = OWN > 3 ? v[rj][C - 1] : tmp[j][3 - OWN < 0 ? 0 : (3 - OWN < NF ? 3 - OWN : 0)];
+                double& d0 = v[rj][0]; double& d1 = v[rj][1]; double& d2 = v[rj][2]; double& d3 = v[rj][3];
                 const unsigned int tg = (((unsigned int)__double2loint(d0) ^ tag) | ((unsigned int)__double2loint(d1) ^ tag) |
                                          ((unsigned int)__double2loint(d2) ^ tag) | ((unsigned int)__double2loint(d3) ^ tag)) & 0xfffu;
                 const unsigned int m = (unsigned int)w4[j], h = (unsigned int)(w4[j] >> 32);
-                const bool ok = ((pending >> rj) & 1u) && tg == 0u && ((h >> 16) & 0xfffu) == tag;
-                if (ok) {
+                if (((pending >> rj) & 1u) && tg == 0u && ((h >> 16) & 0xfffu) == tag) {
                     pending &= ~(1u << rj);
                     // in place: only the low word of each double changes
                     d0 = __hiloint2double(__double2hiint(d0), (int)(((unsigned int)__double2loint(d0) & 0xfffff000u) | (m & 0xfffu)));
@@ -554,39 +547,29 @@ __device__ __forceinline__ void xchg_units(double (&v)[R][C], char* __restrict__
                     d2 = __hiloint2double(__double2hiint(d2), (int)(((unsigned int)__double2loint(d2) & 0xfffff000u) | (m >> 24) | ((h & 0xfu) << 8)));
                     d3 = __hiloint2double(__double2hiint(d3), (int)(((unsigned int)__double2loint(d3) & 0xfffff000u) | ((h >> 4) & 0xfffu)));
                 }
-                if (D != 0) {
-                    const unsigned int got = __ballot_sync(0xffffffffu, ok);
-                    if (got) {                                          // the same for the whole warp
-                        const bool take = ((got << 1) >> threadIdx.x) & 1u & (rprev >> rj);
-#pragma unroll
-                        for (int c = 0; c < NF; ++c) {
-                            const double x = __shfl_up_sync(0xffffffffu, tmp[j][c], 1);
-                            if (take) v[rj][c] = x;
-                        }
-                    }
-                }
             }
         }
-        if (!__ballot_sync(0xffffffffu, pending != 0u)) break;
-        if (attempt == 0 && t0 == 0) t0 = clock64();
+        int gu = 0;
         if (pending != 0u) {
-            if (*(volatile unsigned int*)err != 0u) giveup = 1;        // some tile gave up: do not wait again
-            else if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) {
-                if (atomicExch(err, 1u) == 0u) {      // the first tile to give up says what it was waiting for (CAV_DEBUG)
-                    const int rj = __ffs((int)pending) - 1;
-                    const size_t ui = (size_t)(ubase + rj * upitch);
-                    unsigned long long f0, f1, f4;
-                    ld_v2(xb + 16 * ui, f0, f1);
-                    ld_b64(xb + p2off + 8 * ui, f4);
-                    err[1] = tile; err[2] = (unsigned int)ui; err[3] = round; err[4] = tag;
-                    err[5] = (unsigned int)f0 & 0xfffu; err[6] = (unsigned int)f1 & 0xfffu; err[7] = (unsigned int)(f4 >> 48) & 0xfffu; err[8] = pending;
-                    err[9] = threadIdx.y * 32 + threadIdx.x;
-                }
-                giveup = 1;
+        if (t0 == 0) t0 = clock64();
+        if (*(volatile unsigned int*)err != 0u) gu = 1;
+        else if (clock64() - t0 > SPIN_TIMEOUT_CYCLES) {
+            if (atomicExch(err, 1u) == 0u) {          // the first tile to give up says what it was waiting for (CAV_DEBUG)
+                const int rj = __ffs((int)pending) - 1;
+                const size_t ui = (size_t)(ubase + rj * upitch);
+                unsigned long long f0, f1, f4;
+                ld_v2(xb + 16 * ui, f0, f1);
+                ld_b64(xb + p2off + 8 * ui, f4);
+                err[1] = tile; err[2] = (unsigned int)ui; err[3] = round; err[4] = tag;
+                err[5] = (unsigned int)f0 & 0xfffu; err[6] = (unsigned int)f1 & 0xfffu; err[7] = (unsigned int)(f4 >> 48) & 0xfffu; err[8] = pending;
+                err[9] = threadIdx.y * 32 + threadIdx.x;
             }
+            gu = 1;
         }
-        if (__any_sync(0xffffffffu, giveup)) break;
+        }
+        if (__any_sync(0xffffffffu, gu)) break;
     }
+    __syncwarp();
 }
 
 // ---- the tile image in shared memory ----------------------------------------------------------------------------
@@ -808,7 +791,7 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
             const int gx = gx0 + ci;
             if (!((colin >> ci) & 1u)) continue;
             const double pW = ci > 0 ? pp[rj][ci - 1] : lnb;
-            const double pE = ci < C - 1 ? pp[rj][ci + 1] : rnb;
+            const double pE = gx == Ne - 1 ? 0.0 : (ci < C - 1 ? pp[rj][ci + 1] : rnb);      // psi = 0 on the wall x = N, wherever it sits
             const double pS = rj > 0 ? pp[rj - 1][ci] : sB[TOPOFF + ci * 32];            // top row of the warp below
             const double pN = rj < R - 1 ? pp[rj + 1][ci] : sB[C * 32 + ci * 32];        // bottom row of the warp above
             const double w0 = wc[1 + ci], wW = wc[ci], wE = wc[2 + ci], wS = ws[ci], wN = wn[ci];
@@ -877,13 +860,8 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
         const unsigned int info = xi[0];
         const int ubase = (int)xi[1];
         char* const xb = (round & 1u) ? a.x1 : a.x0;
-        switch (te.D) {
-            case 0: xchg_units<C, R, 0>(ab, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, nullptr, blockIdx.y * a.ntx + blockIdx.x); break;
-            case 1: xchg_units<C, R, 1>(ab, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, nullptr, blockIdx.y * a.ntx + blockIdx.x); break;
-            case 2: xchg_units<C, R, 2>(ab, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, nullptr, blockIdx.y * a.ntx + blockIdx.x); break;
-            default: xchg_units<C, R, 3>(ab, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, nullptr, blockIdx.y * a.ntx + blockIdx.x); break;
-        }
-        stage_tile<C, R>(ab, img, ln, wp, (info >> 8) | (info >> 16));
+        xchg_units<C, R, R / 2>(ab, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, nullptr, blockIdx.y * a.ntx + blockIdx.x);
+        stage_tile<C, R>(ab, img, ln, wp, info >> 8);
         __syncthreads();
     }
     {   // first ring of the new vorticity around the core, kept for a3 of the next stage
@@ -923,7 +901,8 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
     unsigned int fl = FL_PUB_BOTTOM | FL_PUB_TOP;
     {
         const int lzl = t.left_al ? 1 : 0;                                     // lane 0 holds x = -(C-1) .. 0
-        const int lzr = t.right_al ? (N - t.ox) / C - 1 : 31;                  // lane (N - ox) / C holds x = N .. N + C - 1
+        const int lzr = (t.right_al && t.wc == 0) ? (N - t.ox) / C - 1 : 31;   // lane (N - ox) / C holds x = N .. N + C - 1
+        if (t.right_al && t.wc > 0 && lane == (N - t.ox) / C) fl |= FL_WALL_LANE;
         if (lane == lzl) fl |= FL_ZERO_LEFT;
         if (lane == lzr) fl |= FL_ZERO_RIGHT;
         if (t.bot_al && warp == 0) fl &= ~FL_PUB_TOP;                          // warp 0 holds y = -(R-1) .. 0
@@ -936,7 +915,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
         unsigned int* const xi = reinterpret_cast<unsigned int*>(sm + edge_doubles + H * SW + 2 * SW + 2 * H) + 2 * tid;
         unsigned int info;
         int ubase;
-        xchg_setup<C, R>(a, t, lane, warp, bi, bj, info, ubase);
+        xchg_setup<C, R>(N, a.halo, a.walls != 0, a.ntx, a.nty, a.upitch, t, lane, warp, bi, bj, info, ubase);
         xi[0] = info; xi[1] = (unsigned int)ubase;
     }
 
@@ -992,26 +971,16 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
     for (int stage = 0; stage < (a.nsteps > 0 ? 5 * a.nsteps : 1); ++stage) {
         // ================= a1: S sweeps, a halo exchange after every T of them =================
         for (int rem = a.S; rem > 0; rem -= a.T) {
-            if (KIND == 1) {
-                // four colours (i mod 2, j mod 2) in the order (0,0), (1,0), (0,1), (1,1) (reading N1); local colour = global ^ origin parity
-                for (int s = min(a.T, rem); s > 0; --s)
-                    for (int g = 0; g < 4; ++g) {
-                        switch (g ^ par9) {
-                            case 0: colour_pass<C, R, 0, 0, FIX, TOPOFF>(p, q, a.c9e, a.c9c, a.omb, sB, wallmask, fl); break;
-                            case 1: colour_pass<C, R, 1, 0, FIX, TOPOFF>(p, q, a.c9e, a.c9c, a.omb, sB, wallmask, fl); break;
-                            case 2: colour_pass<C, R, 0, 1, FIX, TOPOFF>(p, q, a.c9e, a.c9c, a.omb, sB, wallmask, fl); break;
-                            default: colour_pass<C, R, 1, 1, FIX, TOPOFF>(p, q, a.c9e, a.c9c, a.omb, sB, wallmask, fl); break;
-                        }
-                    }
-            } else if (odd_origin) {
-                for (int s = min(a.T, rem); s > 0; --s) {                         // red = (i + j) even first (G9): local colour 1 here
-                    half_sweep<C, R, 1, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
-                    half_sweep<C, R, 0, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
-                }
-            } else {
-                for (int s = min(a.T, rem); s > 0; --s) {
-                    half_sweep<C, R, 0, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
-                    half_sweep<C, R, 1, FIX, TOPOFF>(p, q, a.cb, a.omb, sB, wallmask, fl);
+            {
+                // the column of a lane that holds the wall x = N (tiles of the last column), from blockIdx and the parameters
+                // only: a uniform branch, like the colour order
+                const int wct = ((int)blockIdx.x == a.ntx - 1 && a.ntx > 1) ? ((a.N - 1) & 3) : 0;
+                const int ns = min(a.T, rem);
+                switch (wct) {
+                    case 0: run_sweeps<C, R, FIX, TOPOFF, KIND, 0>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                    case 1: run_sweeps<C, R, FIX, TOPOFF, KIND, 1>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                    case 2: run_sweeps<C, R, FIX, TOPOFF, KIND, 2>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                    default: run_sweeps<C, R, FIX, TOPOFF, KIND, 3>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
                 }
             }
             const int tslot = 2 + 4 * (int)(round - a.base);                    // trace slot (meaningful in sweeps-only launches)
@@ -1030,14 +999,7 @@ __global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant
                 char* const xb = (round & 1u) ? a.x1 : a.x0;
                 long long* const stamp = (a.trace != nullptr && tslot + 1 < a.trace_cap) ? a.trace + (size_t)(blockIdx.y * a.ntx + blockIdx.x) * a.trace_cap + tslot + 1 : nullptr;
                 const unsigned int tile = blockIdx.y * a.ntx + blockIdx.x;
-                // D of this tile, from blockIdx and the parameters only: a uniform branch
-                const int Dt = ((int)blockIdx.x == a.ntx - 1 && a.ntx > 1) ? ((a.N - 1) & 3) : 0;
-                switch (Dt) {
-                    case 0: xchg_units<C, R, 0>(p, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, stamp, tile); break;
-                    case 1: xchg_units<C, R, 1>(p, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, stamp, tile); break;
-                    case 2: xchg_units<C, R, 2>(p, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, stamp, tile); break;
-                    default: xchg_units<C, R, 3>(p, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, stamp, tile); break;
-                }
+                xchg_units<C, R, CAV_RB>(p, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, stamp, tile);
             }
             ++round;
             mark(a, tslot + 2);
@@ -1155,28 +1117,17 @@ bool split_x(int N, int L, int lead, int h, int& core, int& n) {
 
 }  // namespace
 
-ResidentPlan resident_plan(const Params& P, int device, int T_override, int variant_override, int kind) {
+ResidentPlan resident_plan_for(int N, int kind, int T_override, int variant_override, int sms, int smem_cap, int regs_per_block) {
     ResidentPlan best;
-    cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); return best; }
-    int coop = 0;
-    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device);
-    if (!coop) return best;
-    const int sms = prop.multiProcessorCount;
-    const int G = P.N + 1;                       // points per side, walls included
+    const int G = N + 1;                         // points per side, walls included
     double best_cost = 1e300;
-
+    if (kind < 0 || kind > 1 || N < 2) return best;
     for (int vi = 0; vi < NVARIANTS; ++vi) {
         if (variant_override >= 0 && vi != variant_override) continue;
         const Variant& v = VARIANTS[vi];
-        cudaFuncAttributes fa, fb;
-        if (cudaFuncGetAttributes(&fa, v.fn[kind]) != cudaSuccess || cudaFuncGetAttributes(&fb, v.fn_fix[kind]) != cudaSuccess) { cudaGetLastError(); continue; }
-        const int regs = std::max(fa.numRegs, fb.numRegs);
-        const int max_threads = std::min(fa.maxThreadsPerBlock, fb.maxThreadsPerBlock);
-        const int max_warps = std::min(v.maxw, std::min(max_threads / 32, (int)(prop.regsPerBlock / (32 * std::max(regs, 1)))));
+        const int regs = 65536 / (32 * v.maxw);  // __launch_bounds__(32 maxw, 1): what the kernels are compiled for
+        const int max_warps = std::min(v.maxw, regs_per_block / (32 * regs));
         const int W = 32 * v.C;                  // tile width in points
-        const int smem_cap = std::min((int)prop.sharedMemPerBlockOptin,
-                                      (int)prop.sharedMemPerMultiprocessor - (int)prop.reservedSharedMemPerBlock);
         for (int warps = 1; warps <= max_warps; ++warps) {
             const int H = warps * v.R;           // tile height in points
             ResidentPlan c;
@@ -1186,31 +1137,47 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
             if (G + v.C - 1 <= W && G + v.R - 1 <= H) {
                 const double cost = sweep_cost;
                 c.T = 1 << 30; c.halo = 0; c.CW = G; c.CH = G; c.ntx = c.nty = c.ntiles = 1;
-                if (cost < best_cost && finish_plan(c, P.N, smem_cap)) { best_cost = cost; best = c; }
+                if (cost < best_cost && finish_plan(c, N, smem_cap)) { best_cost = cost; best = c; }
                 continue;
             }
             for (int T = 1; T <= 10; ++T) {
                 if (T_override > 0 && T != T_override) continue;
                 const int halo = (kind == 1 ? 4 : 2) * T;      // one ring is consumed per colour pass
                 int CW, ntx, CH, nty;
-                if (!split_x(P.N, W, v.C - 1, halo, CW, ntx) || !split(G, H, v.R - 1, halo, CH, nty)) continue;
+                if (!split_x(N, W, v.C - 1, halo, CW, ntx) || !split(G, H, v.R - 1, halo, CH, nty)) continue;
                 const int ntiles = ntx * nty;
                 if (ntiles < 2 || ntiles > sms) continue;
                 // Cost per sweep in SM cycles, calibrated on B200 (profiles/r2_*.md): a colour half-sweep takes ~187 cycles per warp
                 // of the busiest SM sub-partition (+ barrier), an exchange ~6500 cycles + 250 per sweep of halo depth, mostly latency.
                 const double cost = sweep_cost + (6500.0 + 125.0 * halo) / T;
                 c.T = T; c.halo = halo; c.CW = CW; c.CH = CH; c.ntx = ntx; c.nty = nty; c.ntiles = ntiles;
-                if (cost < best_cost && finish_plan(c, P.N, smem_cap)) { best_cost = cost; best = c; }
+                if (cost < best_cost && finish_plan(c, N, smem_cap)) { best_cost = cost; best = c; }
             }
         }
     }
+    return best;
+}
+
+ResidentPlan resident_plan(const Params& P, int device, int T_override, int variant_override, int kind) {
+    ResidentPlan best;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); return best; }
+    int coop = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device);
+    if (!coop) return best;
+    const int sms = prop.multiProcessorCount;
+    const int smem_cap = std::min((int)prop.sharedMemPerBlockOptin, (int)prop.sharedMemPerMultiprocessor - (int)prop.reservedSharedMemPerBlock);
+    best = resident_plan_for(P.N, kind, T_override, variant_override, sms, smem_cap, (int)prop.regsPerBlock);
     if (best.ok) {
         const void* fn = best.fixup ? VARIANTS[best.variant].fn_fix[kind] : VARIANTS[best.variant].fn[kind];
-        if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin) != cudaSuccess) {
+        cudaFuncAttributes fa;
+        if (cudaFuncGetAttributes(&fa, fn) != cudaSuccess || fa.numRegs * 32 * best.warps > (int)prop.regsPerBlock ||
+            cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin) != cudaSuccess) {
             cudaGetLastError();
             best.ok = false;
             return best;
         }
+        best.regs = fa.numRegs;
         int per_sm = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 32 * best.warps, best.smem_bytes) != cudaSuccess ||
             per_sm * sms < best.ntiles) {
@@ -1219,6 +1186,42 @@ ResidentPlan resident_plan(const Params& P, int device, int T_override, int vari
         }
     }
     return best;
+}
+
+// Host-side check of the exchange pattern of a plan (no device needed): every unit a tile fetches must be stored by
+// exactly one tile, its owner, and lie in the rows / columns both agree on; every stored unit must be fetched by someone.
+// counts[0] = units fetched, [1] = units stored, [2] = fetched but stored by nobody or by more than one, [3] = stored but
+// fetched by nobody, [4] = tiles that do not fit their thread grid.  Returns 0 if [2] = [3] = [4] = 0.
+int resident_check_exchange(const ResidentPlan& pl, int N, long long* counts) {
+    long long c[5] = {0, 0, 0, 0, 0};
+    if (pl.ok && pl.ntiles > 1 && pl.C == 4 && pl.R == 6) {
+        const int upitch = resident_unit_pitch(N);
+        const size_t nunits = (size_t)upitch * (size_t)(N + 1);
+        std::vector<unsigned char> stored(nunits, 0), fetched(nunits, 0);
+        const bool walls = pl.kind == 1;
+        for (int bj = 0; bj < pl.nty; ++bj)
+            for (int bi = 0; bi < pl.ntx; ++bi) {
+                const TileGeom t = tile_geom(N, pl.CW, pl.CH, pl.halo, pl.ntx, pl.nty, bi, bj, 4, 6, 128, pl.warps * 6);
+                if (!t.fits) ++c[4];
+                for (int warp = 0; warp < pl.warps; ++warp)
+                    for (int lane = 0; lane < 32; ++lane) {
+                        unsigned int info; int ubase;
+                        xchg_setup<4, 6>(N, pl.halo, walls, pl.ntx, pl.nty, upitch, t, lane, warp, bi, bj, info, ubase);
+                        for (int rj = 0; rj < 6; ++rj) {
+                            const long long u = (long long)ubase + (long long)rj * upitch;
+                            if ((info >> rj) & 1u) { if (u < 0 || (size_t)u >= nunits) ++c[2]; else { ++c[1]; if (stored[(size_t)u] < 255) ++stored[(size_t)u]; } }
+                            if ((info >> (8 + rj)) & 1u) { if (u < 0 || (size_t)u >= nunits) ++c[2]; else { ++c[0]; if (fetched[(size_t)u] < 255) ++fetched[(size_t)u]; } }
+                        }
+                    }
+            }
+        for (size_t u = 0; u < nunits; ++u) {
+            if (fetched[u] && stored[u] != 1) ++c[2];
+            if (stored[u] > 1) ++c[2];
+            if (stored[u] && !fetched[u]) ++c[3];
+        }
+    }
+    if (counts) for (int k = 0; k < 5; ++k) counts[k] = c[k];
+    return (c[2] || c[3] || c[4]) ? 1 : 0;
 }
 
 void resident_describe(const ResidentPlan& pl, char* buf, int len) {

@@ -31,6 +31,11 @@ struct ResidentPlan {
 // T_override > 0 forces the sweeps per round (1..10; tests use it to exercise short and ragged rounds);
 // variant_override >= 0 forces the micro-tile shape (index into the compiled variants).
 ResidentPlan resident_plan(const Params& P, int device, int T_override = 0, int variant_override = -1, int kind = 0);
+// The same planner for given device figures (no device needed: host logic, testable on CPU)
+ResidentPlan resident_plan_for(int N, int kind, int T_override, int variant_override, int sms, int smem_cap, int regs_per_block);
+// Host-side check of a plan's exchange pattern (every fetched unit stored by exactly one tile, every stored unit fetched);
+// counts[5]: fetched, stored, unmatched fetches / double stores, stores nobody fetches, tiles that do not fit.  0 = consistent.
+int resident_check_exchange(const ResidentPlan& plan, int N, long long* counts);
 int resident_variants();
 void resident_describe(const ResidentPlan& plan, char* buf, int len);
 
