@@ -71,8 +71,11 @@ constexpr long long SPIN_TIMEOUT_CYCLES = CAV_SPIN_TIMEOUT;
 #ifndef CAV_RB
 #define CAV_RB 6             // rows of a thread in flight together in the psi exchange
 #endif
+#ifndef CAV_EDGE_FIRST
+#define CAV_EDGE_FIRST 1      // half-sweep: edge rows, publish, barrier, inner rows (0: all rows, publish, barrier)
+#endif
 #ifndef CAV_QROWS
-#define CAV_QROWS 2             // rows of the micro-tile whose q lives in shared memory instead of registers
+#define CAV_QROWS 0             // rows of the micro-tile whose q lives in shared memory instead of registers (0: the register-to-register exchange left room for all of q)
 #endif
 
 // SSPRK(5,4) in Shu-Osher form, eq 9-13, readings G1 / G2 (the same table as cavity_kernels.cu, typed here again
@@ -246,7 +249,7 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
     // arrays (same address register): 16 registers fewer held across the whole kernel.
     double* const sT = sB + TOPOFF;
     constexpr int QR = CAV_QROWS, Q0 = (R - QR) / 2;
-    double Lnb[R], Rnb[R], Bnb[C], Tnb[C], qs[QR][C];
+    double Lnb[R], Rnb[R], Bnb[C], Tnb[C], qs[QR > 0 ? QR : 1][C];
 #pragma unroll
     for (int ci = 0; ci < C; ++ci) {
 #pragma unroll
@@ -269,8 +272,7 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
             Rnb[rj] = (fl & FL_ZERO_RIGHT) ? 0.0 : v;
         }
     }
-#pragma unroll
-    for (int rj = 0; rj < R; ++rj) {
+    auto update_row = [&](const int rj) {
 #pragma unroll
         for (int ci = 0; ci < C; ++ci) {
             if (((ci + rj) & 1) != K) continue;
@@ -283,7 +285,26 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
             const double qv = (rj >= Q0 && rj < Q0 + QR) ? qs[rj - Q0 < 0 ? 0 : (rj - Q0 >= QR ? QR - 1 : rj - Q0)][ci] : q[rj][ci];
             p[rj][ci] = fma(omb, p[rj][ci], fma(cb, nb, qv));
         }
+    };
+#if CAV_EDGE_FIRST
+    if (!FIX) {
+        // The two rows other warps wait for come first and are published at once; the four inner rows, which need nothing
+        // from other warps, follow BEHIND the barrier: they cover its skew and the latency of the next half-sweep's edge loads.
+        update_row(0);
+        update_row(R - 1);
+#pragma unroll
+        for (int ci = 0; ci < C; ++ci) {
+            if ((ci & 1) == K && (fl & FL_PUB_BOTTOM)) sB[ci * 32] = p[0][ci];
+            if (((ci + R - 1) & 1) == K && (fl & FL_PUB_TOP)) sT[C * 32 + ci * 32] = p[R - 1][ci];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int rj = 1; rj < R - 1; ++rj) update_row(rj);
+        return;
     }
+#endif
+#pragma unroll
+    for (int rj = 0; rj < R; ++rj) update_row(rj);
     unsigned int wm = FIX ? wallmask : 0u;
     if (FIX) asm volatile("" : "+r"(wm));      // opaque: keeps the bit tests from being hoisted into live registers
     if (FIX && wm) {
@@ -319,13 +340,16 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
 template <int C, int R, int KX, int KY, bool FIX, int TOPOFF, int WC>
 __device__ __forceinline__ void colour_pass(double (&p)[R][C], const double (&q)[R][C], const double c9e, const double c9c, const double omb,
                                             double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl_) {
-    static_assert(C == 4 && R == 6 && CAV_QROWS == 2, "written for the 4 x 6 micro-tile with q of rows 2, 3 in shared memory");
+    static_assert(C == 4 && R == 6 && CAV_QROWS <= 2, "written for the 4 x 6 micro-tile with q of at most two middle rows in shared memory");
+    constexpr int QR = CAV_QROWS, Q0 = (R - QR) / 2;
+    // the row of parity KY whose q lives in shared memory (-1: none), and which of the QR arrays holds it
+    constexpr int QROW = (QR >= 1 && (Q0 & 1) == KY) ? Q0 : ((QR >= 2 && ((Q0 + 1) & 1) == KY) ? Q0 + 1 : -1);
     unsigned int fl = fl_;
     asm volatile("" : "+r"(fl));               // opaque: the bit tests below are redone here, not hoisted into registers of their own
     double* const sT = sB + TOPOFF;
     double qs[C], side[R], edge[C + 2];        // edge[1 + c] = column c of the row below (KY == 0) / above (KY == 1), c = -1 .. C
 #pragma unroll
-    for (int ci = KX; ci < C; ci += 2) qs[ci] = sB[2 * TOPOFF + KY * (TOPOFF - C * 32) + ci * 32];      // q of row 2 + KY
+    for (int ci = KX; ci < C; ci += 2) qs[ci] = QROW >= 0 ? sB[2 * TOPOFF + (QROW - Q0 < 0 ? 0 : QROW - Q0) * (TOPOFF - C * 32) + ci * 32] : 0.0;      // q of row QROW
     {
         const double* const er = KY == 0 ? sT : sB + C * 32;       // top row of the warp below (slot warp) / bottom row of the warp above
 #pragma unroll
@@ -363,7 +387,7 @@ __device__ __forceinline__ void colour_pass(double (&p)[R][C], const double (&q)
         for (int ci = KX; ci < C; ci += 2) {
             const double se = (at(ci - 1, rj) + at(ci + 1, rj)) + (at(ci, rj - 1) + at(ci, rj + 1));
             const double sc = (at(ci - 1, rj - 1) + at(ci + 1, rj - 1)) + (at(ci - 1, rj + 1) + at(ci + 1, rj + 1));
-            const double qv = (rj == 2 + KY) ? qs[ci] : q[rj][ci];
+            const double qv = (rj == QROW) ? qs[ci] : q[rj][ci];
             p[rj][ci] = fma(omb, p[rj][ci], fma(c9e, se, fma(c9c, sc, qv)));
         }
     }
