@@ -900,7 +900,7 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
 // MAXW = most warps per CTA the kernel is launched with: 65536 / (32 MAXW) registers per thread are available.
 // KIND: 0 = red-black sweeps of the 5-point operator (a1), 1 = four-colour sweeps of the compact 9-point operator (NEXT-1)
 template <int C, int R, int MAXW, bool FIX, int KIND>
-__global__ void __launch_bounds__(32 * MAXW, 1) k_resident(const __grid_constant__ ResArgs a) {
+__global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_constant__ ResArgs a) {
     constexpr int TOPOFF = (MAXW + 1) * C * 32;
     constexpr int SW = 32 * C;
     static_assert(C % 2 == 0 && R % 2 == 0 && R * C <= 32, "even micro-tile that fits the 32-bit point masks");
@@ -1149,19 +1149,21 @@ ResidentPlan resident_plan_for(int N, int kind, int T_override, int variant_over
     for (int vi = 0; vi < NVARIANTS; ++vi) {
         if (variant_override >= 0 && vi != variant_override) continue;
         const Variant& v = VARIANTS[vi];
-        const int regs = 65536 / (32 * v.maxw);  // __launch_bounds__(32 maxw, 1): what the kernels are compiled for
-        const int max_warps = std::min(v.maxw, regs_per_block / (32 * regs));
+        const int per_sm = 16 / v.maxw;          // CTAs per SM the variant is compiled for (__launch_bounds__(32 maxw, 16 / maxw))
+        const int regs = 128;
+        const int max_warps = std::min(v.maxw, regs_per_block / (32 * regs) / per_sm);
+        const int smem_cta = per_sm == 1 ? smem_cap : (smem_cap + 1024) / per_sm - 1024;      // 1 KB per CTA is reserved by the system
         const int W = 32 * v.C;                  // tile width in points
         for (int warps = 1; warps <= max_warps; ++warps) {
             const int H = warps * v.R;           // tile height in points
             ResidentPlan c;
-            c.ok = true; c.variant = vi; c.C = v.C; c.R = v.R; c.warps = warps; c.regs = regs; c.sm_count = sms; c.per_sm = 1; c.kind = kind;
+            c.ok = true; c.variant = vi; c.C = v.C; c.R = v.R; c.warps = warps; c.regs = regs; c.sm_count = sms; c.per_sm = per_sm; c.kind = kind;
             const double sweep_cost = (kind == 1 ? 2.2 : 1.0) * sweep_cycles(warps);      // four colour passes of 54 fp64 instructions instead of two of 60
             // single tile: the whole grid in one CTA, no exchange at all
             if (G + v.C - 1 <= W && G + v.R - 1 <= H) {
                 const double cost = sweep_cost;
                 c.T = 1 << 30; c.halo = 0; c.CW = G; c.CH = G; c.ntx = c.nty = c.ntiles = 1;
-                if (cost < best_cost && finish_plan(c, N, smem_cap)) { best_cost = cost; best = c; }
+                if (per_sm == 1 && cost < best_cost && finish_plan(c, N, smem_cta)) { best_cost = cost; best = c; }
                 continue;
             }
             for (int T = 1; T <= 10; ++T) {
@@ -1170,12 +1172,12 @@ ResidentPlan resident_plan_for(int N, int kind, int T_override, int variant_over
                 int CW, ntx, CH, nty;
                 if (!split_x(N, W, v.C - 1, halo, CW, ntx) || !split(G, H, v.R - 1, halo, CH, nty)) continue;
                 const int ntiles = ntx * nty;
-                if (ntiles < 2 || ntiles > sms) continue;
-                // Cost per sweep in SM cycles, calibrated on B200 (profiles/r2_*.md): a colour half-sweep takes ~187 cycles per warp
-                // of the busiest SM sub-partition (+ barrier), an exchange ~6500 cycles + 250 per sweep of halo depth, mostly latency.
-                const double cost = sweep_cost + (6500.0 + 125.0 * halo) / T;
+                if (ntiles < 2 || ntiles > sms * per_sm) continue;
+                // Cost per sweep in SM cycles, calibrated on B200 (profiles/r2b_*.md): a colour half-sweep takes ~187 cycles per warp
+                // of the busiest SM sub-partition (+ barrier), an exchange ~5000 cycles of latency + 130 per point of halo depth.
+                const double cost = sweep_cost + (5000.0 + 130.0 * halo) / T;
                 c.T = T; c.halo = halo; c.CW = CW; c.CH = CH; c.ntx = ntx; c.nty = nty; c.ntiles = ntiles;
-                if (cost < best_cost && finish_plan(c, N, smem_cap)) { best_cost = cost; best = c; }
+                if (cost < best_cost && finish_plan(c, N, smem_cta)) { best_cost = cost; best = c; }
             }
         }
     }
@@ -1256,9 +1258,9 @@ void resident_describe(const ResidentPlan& pl, char* buf, int len) {
     else
         std::snprintf(buf, (size_t)len,
                       "%s%dx%d tiles of %dx%d core + halo %d, T=%d sweeps per exchange, %d warps x (%dx%d micro-tiles), "
-                      "register-to-register exchange of 40-byte units of four points, %d regs, %d B smem, one CTA per SM on %d SMs",
+                      "register-to-register exchange of 40-byte units of four points, %d regs, %d B smem, %d CTA(s) per SM on %d SMs",
                       pl.kind == 1 ? "compact 9-point operator, " : "", pl.ntx, pl.nty, pl.CW, pl.CH, pl.halo, pl.T, pl.warps, pl.C, pl.R, pl.regs,
-                      pl.smem_bytes, pl.sm_count);
+                      pl.smem_bytes, pl.per_sm, pl.sm_count);
 }
 
 int resident_variants() { return NVARIANTS; }

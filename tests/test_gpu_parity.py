@@ -374,7 +374,7 @@ def test_resident_variants_agree_with_stream_engine(cav, N, S, variant, T):
     except cav.CavityError:
         g.close()
         pytest.skip("no plan with T=%d, variant %d for N=%d" % (T, variant, N))
-    assert "T=%d " % T in g.describe() and "one CTA per SM" in g.describe()
+    assert "T=%d " % T in g.describe() and "CTA(s) per SM" in g.describe()
     s = cav.Cavity(N, 2000.0, 0.5 / N, 1.97, S, engine="stream")
     for c in (g, s):
         c.set_fields(psi0, w0)
