@@ -522,25 +522,23 @@ __device__ __forceinline__ void xchg_units(double (&v)[R][C], char* __restrict__
 
     unsigned int pending = (info >> 8) & 0x3fu;
     long long t0 = 0;
-    // The neighbours store while this tile does: fetching at once would mostly bring the previous round's bytes.  The first and
-    // the last lane of the warp that wait for anything poll the last word of their last row (what their neighbour stores
-    // last) until it carries the tag; only then does the warp fetch.  A heuristic for WHEN to fetch: the tags decide validity.
+    // The neighbours store while this tile does: fetching at once would mostly bring the previous round's bytes.  Every lane
+    // that waits for anything polls the last word of its last row (what its neighbour stores last; the lanes of a warp read
+    // neighbouring words: one coalesced access) until it carries the tag; only then does the warp fetch.  A heuristic for
+    // WHEN to fetch: the tags decide validity.
     {
-        const unsigned int waiting = __ballot_sync(0xffffffffu, pending != 0u);
-        if (waiting != 0u && ((int)threadIdx.x == __ffs((int)waiting) - 1 || (int)threadIdx.x == 31 - __clz((int)waiting))) {
-            const int rj = 31 - __clz((int)pending);
-            const char* const pw = xb + p2off + 8 * (size_t)(ubase + rj * upitch);
-            unsigned long long w4;
-            ld_b64(pw, w4);
-            if (((unsigned int)(w4 >> 48) & 0xfffu) != tag) {
-                t0 = clock64();
-                do {
-                    ld_b64(pw, w4);
-                    if (*(volatile unsigned int*)err != 0u || clock64() - t0 > SPIN_TIMEOUT_CYCLES) break;      // decided below
-                } while (((unsigned int)(w4 >> 48) & 0xfffu) != tag);
+        bool need = pending != 0u;
+        const char* const pw = xb + p2off + 8 * (size_t)(ubase + (need ? 31 - __clz((int)pending) : 0) * upitch);
+        for (;;) {
+            if (need) {
+                unsigned long long w4;
+                ld_b64(pw, w4);
+                if (((unsigned int)(w4 >> 48) & 0xfffu) == tag) need = false;
             }
+            if (!__any_sync(0xffffffffu, need)) break;
+            if (t0 == 0) t0 = clock64();
+            if (__any_sync(0xffffffffu, need && (*(volatile unsigned int*)err != 0u || clock64() - t0 > SPIN_TIMEOUT_CYCLES))) break;      // decided below
         }
-        __syncwarp();
     }
     while (__any_sync(0xffffffffu, pending != 0u)) {
 #pragma unroll
