@@ -690,6 +690,58 @@ __device__ __forceinline__ void qb_from_image(double (&q)[R][C], const double* _
 __device__ __forceinline__ double thom_wall(double c2h2, double p_adj) { return -(c2h2 * p_adj); }
 __device__ __forceinline__ double thom_lid(double c2h2, double lid, double p_adj) { return -(c2h2 * p_adj) - lid; }
 
+// a2 (eq 25) for the points of this thread's micro-tile that lie next to a wall and inside the tile's core
+// [X0, X1) x [Y0, Y1): the wall value goes into the image next to the point and, with TO_GLOBAL, into the ring of the stage
+// output (the bottom and top rows own the corners, G10).  A thread holds at most one column next to the left / right wall and
+// one row next to the bottom / top wall; which one is a run-time index, resolved by selects (most threads hold none and skip
+// everything: the fully unrolled point-by-point form of this took 2500 instructions per thread and stage).
+template <int C, int R, bool TO_GLOBAL>
+__device__ __forceinline__ void thom_walls(const double (&pp)[R][C], double* __restrict__ img, double* __restrict__ wout, const int gx0,
+                                           const int gy0, const int X0, const int X1, const int Y0, const int Y1, const int Ne,
+                                           const int pitch, const int row0, const int lx0, const double c2h2, const double lid) {
+    constexpr int SW = 32 * C;
+    static_assert(C == 4 && R == 6, "select chains written for the 4 x 6 micro-tile");
+    auto col = [&](const int rj, const int c) -> double {
+        return c == 0 ? pp[rj][0] : (c == 1 ? pp[rj][1] : (c == 2 ? pp[rj][2] : pp[rj][3]));
+    };
+    auto row = [&](const int r, const int ci) -> double {
+        return r == 0 ? pp[0][ci] : (r == 1 ? pp[1][ci] : (r == 2 ? pp[2][ci] : (r == 3 ? pp[3][ci] : (r == 4 ? pp[4][ci] : pp[5][ci]))));
+    };
+#pragma unroll
+    for (int side = 0; side < 2; ++side) {                    // x = 1 (wall x = 0) and x = Ne - 1 (wall x = Ne)
+        const int xa = side == 0 ? 1 : Ne - 1, c = xa - gx0;
+        if (c < 0 || c >= C || xa < X0 || xa >= X1) continue;
+#pragma unroll
+        for (int rj = 0; rj < R; ++rj) {
+            const int gy = gy0 + rj;
+            if (gy < Y0 || gy >= Y1) continue;
+            const double v = thom_wall(c2h2, col(rj, c));
+            img[img_ix(row0 + rj, lx0 + c + (side == 0 ? -1 : 1), SW)] = v;
+            if (TO_GLOBAL) wout[(size_t)gy * pitch + (side == 0 ? 0 : Ne)] = v;
+        }
+    }
+#pragma unroll
+    for (int side = 0; side < 2; ++side) {                    // y = 1 (wall y = 0) and y = Ne - 1 (the lid y = Ne)
+        const int ya = side == 0 ? 1 : Ne - 1, r = ya - gy0;
+        if (r < 0 || r >= R || ya < Y0 || ya >= Y1) continue;
+#pragma unroll
+        for (int ci = 0; ci < C; ++ci) {
+            const int gx = gx0 + ci;
+            if (gx < X0 || gx >= X1) continue;
+            const double pv = row(r, ci);
+            const double v = side == 0 ? thom_wall(c2h2, pv) : thom_lid(c2h2, lid, pv);
+            img[img_ix(row0 + r + (side == 0 ? -1 : 1), lx0 + ci, SW)] = v;
+            if (TO_GLOBAL) {
+                double* const wrow = wout + (side == 0 ? (size_t)0 : (size_t)Ne * pitch);
+                wrow[gx] = v;
+                const double vc = side == 0 ? thom_wall(c2h2, 0.0) : thom_lid(c2h2, lid, 0.0);
+                if (gx == 1) wrow[0] = vc;
+                if (gx == Ne - 1) wrow[Ne] = vc;
+            }
+        }
+    }
+}
+
 // a2 + a3 of one stage for this tile (see the file header).  pp: the thread's psi micro-tile (registers).  On return the
 // image holds the NEW vorticity on core + halo (+0.0 elsewhere) and the ring copy is refreshed; the caller turns it into q.
 // Inlined: with psi passed through local memory to a non-inlined version the phase took 33 us per stage instead of 24.
@@ -762,32 +814,13 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
             }
         }
     }
-    if ((gx0 <= 1 || gx0 + C - 1 >= Ne - 1 || gy0 <= 1 || gy0 + R - 1 >= Ne - 1)) {
-#pragma unroll
-        for (int rj = 0; rj < R; ++rj)
-#pragma unroll
-            for (int ci = 0; ci < C; ++ci) {
-                const int gx = gx0 + ci, gy = gy0 + rj;
-                if (gx < X0 || gx >= X1 || gy < Y0 || gy >= Y1) continue;
-                const int ir_ = row0 + rj, ix_ = lx0 + ci;
-                const double pv = pp[rj][ci];
-                if (gx == 1) { const double v = thom_wall(a.c2h2, pv); img[img_ix(ir_, ix_ - 1, SW)] = v; wout[(size_t)gy * pitch] = v; }
-                if (gx == Ne - 1) { const double v = thom_wall(a.c2h2, pv); img[img_ix(ir_, ix_ + 1, SW)] = v; wout[(size_t)gy * pitch + Ne] = v; }
-                if (gy == 1) {
-                    const double v = thom_wall(a.c2h2, pv); img[img_ix(ir_ - 1, ix_, SW)] = v; wout[gx] = v;
-                    if (gx == 1) wout[0] = thom_wall(a.c2h2, 0.0);                      // the bottom and top rows own the corners (G10)
-                    if (gx == Ne - 1) wout[Ne] = thom_wall(a.c2h2, 0.0);
-                }
-                if (gy == Ne - 1) {
-                    const double v = thom_lid(a.c2h2, a.lid, pv); img[img_ix(ir_ + 1, ix_, SW)] = v; wout[(size_t)Ne * pitch + gx] = v;
-                    if (gx == 1) wout[(size_t)Ne * pitch] = thom_lid(a.c2h2, a.lid, 0.0);
-                    if (gx == Ne - 1) wout[(size_t)Ne * pitch + Ne] = thom_lid(a.c2h2, a.lid, 0.0);
-                }
-            }
-    }
+    thom_walls<C, R, true>(pp, img, wout, gx0, gy0, X0, X1, Y0, Y1, Ne, pitch, row0, lx0, a.c2h2, a.lid);
     __syncthreads();
 
     // (2) eq 8 + eq 22 and the combination of eq 9-13 for the core points of this thread, row by row
+    const double rk_c = k == 1 ? RK1_C : (k == 2 ? RK2_C : (k == 3 ? RK3_C : (k == 4 ? RK4_C : RK5_C4)));
+    const double rk_a1 = k == 2 ? RK2_A1 : (k == 3 ? RK3_A2 : (k == 4 ? RK4_A3 : RK5_A4));
+    const double rk_a0 = k == 2 ? RK2_A0 : (k == 3 ? RK3_A0 : (k == 4 ? RK4_A0 : 1.0));
 #pragma unroll
     for (int rj = 0; rj < R; ++rj) {
         const int gy = gy0 + rj;
@@ -827,19 +860,10 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
             const double dL = a.dt * L;
             const size_t gk = (size_t)gy * pitch + gx;
             const double av = ab[rj][ci];
-            double out;
-            if (k == 1) {
-                out = fma(RK1_C, dL, w0);                                               // eq 9
-            } else if (k == 2) {
-                out = fma(RK2_C, dL, fma(RK2_A1, w0, RK2_A0 * av));                     // eq 10 (w0 here is omega^(1), av = omega^n)
-            } else if (k == 3) {
-                out = fma(RK3_C, dL, fma(RK3_A2, w0, RK3_A0 * av));                     // eq 11
-            } else if (k == 4) {
-                out = fma(RK4_C, dL, fma(RK4_A3, w0, RK4_A0 * av));                     // eq 12
-                tbuf[gk] = fma(RK5_C3, dL, fma(RK5_A3, w0, RK5_A2 * w2b[gk]));          // eq 13, first three terms
-            } else {
-                out = fma(RK5_C4, dL, fma(RK5_A4, w0, av));                             // eq 13, the rest (av = T)
-            }
+            // eq 9-13 in one form: out = fma(c, dL, fma(a1, w0, a0 av)) (eq 13: a0 = 1, av = T; eq 9: the inner term is w0 itself)
+            const double inner = k == 1 ? w0 : fma(rk_a1, w0, rk_a0 * av);
+            const double out = fma(rk_c, dL, inner);
+            if (k == 4) tbuf[gk] = fma(RK5_C3, dL, fma(RK5_A3, w0, RK5_A2 * w2b[gk]));      // eq 13, first three terms
             wout[gk] = out;
             ab[rj][ci] = out;
         }
@@ -857,21 +881,7 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
         // NEXT-1: B of eq 17 reads omega on the walls: the stage output carries the wall vorticity just computed (reading N2),
         // so the image of the new vorticity gets it too (neighbours fetch it with the ring; corners are never read)
         __syncthreads();              // the zeros staged by the owners of the wall points are in place
-        if ((gx0 <= 1 || gx0 + C - 1 >= Ne - 1 || gy0 <= 1 || gy0 + R - 1 >= Ne - 1)) {
-#pragma unroll
-            for (int rj = 0; rj < R; ++rj)
-#pragma unroll
-                for (int ci = 0; ci < C; ++ci) {
-                    const int gx = gx0 + ci, gy = gy0 + rj;
-                    if (gx < X0 || gx >= X1 || gy < Y0 || gy >= Y1) continue;
-                    const int ir_ = row0 + rj, ix_ = lx0 + ci;
-                    const double pv = pp[rj][ci];
-                    if (gx == 1) img[img_ix(ir_, ix_ - 1, SW)] = thom_wall(a.c2h2, pv);
-                    if (gx == Ne - 1) img[img_ix(ir_, ix_ + 1, SW)] = thom_wall(a.c2h2, pv);
-                    if (gy == 1) img[img_ix(ir_ - 1, ix_, SW)] = thom_wall(a.c2h2, pv);
-                    if (gy == Ne - 1) img[img_ix(ir_ + 1, ix_, SW)] = thom_lid(a.c2h2, a.lid, pv);
-                }
-        }
+        thom_walls<C, R, false>(pp, img, nullptr, gx0, gy0, X0, X1, Y0, Y1, Ne, pitch, row0, lx0, a.c2h2, a.lid);
     }
     __syncthreads();
     if (a.ntx * a.nty > 1) {
