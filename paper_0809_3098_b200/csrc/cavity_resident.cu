@@ -453,12 +453,13 @@ __host__ __device__ inline int imin(int a, int b) { return a < b ? a : b; }
 
 // Shared-memory layout (doubles unless said otherwise), nthreads = 32 nwarps, H = R nwarps, SW = 32 C:
 //   edges   (2 (MAXW + 1) + 2 MAXW) C 32   bottom / top rows of the micro-tiles, q of the two middle rows (sized for MAXW warps)
-//   image   H SW                         the tile, row-major: initial load, final store, omega of the stage input during a3
-//   wring   2 SW + 2 H                   first ring of the stage input vorticity around the core (rows below / above, columns left / right)
+//   image   (H + 1) SW                   the tile, row-major (+ one row: the compact operator's right-hand side reads one row past
+//                                        the tile, values it never uses): initial load, final store; between the stages it keeps the vorticity
+//                                        of core + halo (the input of the next stage's a3): the psi rounds never touch it
 //   xinfo   2 nthreads u32               per thread: which rows of its micro-tile it sends / receives, and its unit index (xchg_setup)
 __host__ __device__ inline size_t smem_layout_bytes(int C, int R, int maxw, int warps) {
     const size_t nth = 32 * (size_t)warps, H = (size_t)R * warps, SW = 32 * (size_t)C;
-    return 8 * ((2 * (size_t)(maxw + 1) + CAV_QROWS * (size_t)maxw) * C * 32 + H * SW + 2 * SW + 2 * H) + 4 * 2 * nth;
+    return 8 * ((2 * (size_t)(maxw + 1) + CAV_QROWS * (size_t)maxw) * C * 32 + (H + 1) * SW) + 4 * 2 * nth;
 }
 
 // Which units a thread moves in an exchange.  Row rj of its micro-tile is the unit (k, y = gy0 + rj), k = (ox + 3) / 4 + lane.
@@ -759,13 +760,11 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
     const int Ne = a.N + z, pitch = a.pitch;
     const TileGeom te = tile_geom(Ne, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, H);
     const int k = stage % 5 + 1;                                    // RK stage 1..5
-    const double* const win = a.wbase + (size_t)(k - 1) * a.fstride;    // omega^(k-1)
     double* const wout = a.wbase + (size_t)(k % 5) * a.fstride;         // omega^(k); stage 5 writes omega^{n+1} over omega^n
     double* const tbuf = a.wbase + (size_t)(5 + z) * a.fstride;         // T: first three terms of eq 13 (+ z: not hoisted)
     const double* const w0b = a.wbase + (size_t)z * a.fstride;          // omega^n
     const double* const w2b = a.wbase + (size_t)(2 + z) * a.fstride;
     double* const img = sm + edge_doubles;
-    const double* const wr = img + H * SW;
     // interior points of the core, in grid and in local coordinates
     const int X0 = imax(te.cx0, 1), X1 = imin(te.cx1, Ne), Y0 = imax(te.cy0, 1), Y1 = imin(te.cy1, Ne);
     const int lx0 = ln * C, row0 = wp * R, gx0 = te.ox + lx0, gy0 = te.oy + row0;
@@ -792,28 +791,10 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
             }
     }
 
-    // (1) the image receives the stage input: core from the tile's own global buffer, first ring from the copy kept
-    //     since the last vorticity exchange, walls next to the core from Thom's formula (written by the owner of the
-    //     adjacent point, who also stores it to the ring of the stage output: k_rk_stage does the same).
-    fill_image<C, R>(img, win, X0, X1, Y0, Y1, te.ox, te.oy, nw, Ne, pitch, ln, wp);
-    __syncthreads();              // fill_image writes zeros everywhere else: the ring and wall writers come after it
-    {
-        const int rB = Y0 - 1 - te.oy, rT = Y1 - te.oy, cL = X0 - 1 - te.ox, cR = X1 - te.ox;
-        for (int c = tid_o; c < SW; c += nth_o) {
-            const int gx = te.ox + c;
-            if (gx >= X0 && gx < X1) {
-                if (Y0 - 1 >= 1) img[img_ix(rB, c, SW)] = wr[c];
-                if (Y1 <= Ne - 1) img[img_ix(rT, c, SW)] = wr[SW + c];
-            }
-        }
-        for (int r2 = tid_o; r2 < H; r2 += nth_o) {
-            const int gy = te.oy + r2;
-            if (gy >= Y0 && gy < Y1) {
-                if (X0 - 1 >= 1) img[img_ix(r2, cL, SW)] = wr[2 * SW + r2];
-                if (X1 <= Ne - 1) img[img_ix(r2, cR, SW)] = wr[2 * SW + H + r2];
-            }
-        }
-    }
+    // (1) the image still holds the stage input on core + halo: nothing has written it since the end of the previous stage
+    //     (the psi rounds move registers only), at the first stage of a launch it holds omega^n as loaded.  Only the walls next to
+    //     the core change: Thom's formula on the new psi, written by the owner of the adjacent point, who also stores it to the
+    //     ring of the stage output (k_rk_stage does the same).
     thom_walls<C, R, true>(pp, img, wout, gx0, gy0, X0, X1, Y0, Y1, Ne, pitch, row0, lx0, a.c2h2, a.lid);
     __syncthreads();
 
@@ -888,19 +869,13 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
         // the new vorticity of core + walls goes back to the registers (the walls were written into the image by the owners
         // of the adjacent points), is exchanged like psi, and the ring it brought goes into the image
         read_tile<C, R>(ab, img, ln, wp, 0x3fu);
-        const unsigned int* const xi = reinterpret_cast<const unsigned int*>(img + H * SW + 2 * SW + 2 * H) + 2 * tid_o;
+        const unsigned int* const xi = reinterpret_cast<const unsigned int*>(img + (H + 1) * SW) + 2 * tid_o;
         const unsigned int info = xi[0];
         const int ubase = (int)xi[1];
         char* const xb = (round & 1u) ? a.x1 : a.x0;
         xchg_units<C, R, R / 2>(ab, xb, a.p1off, a.p2off, round, info, ubase, a.upitch, a.err, nullptr, blockIdx.y * a.ntx + blockIdx.x);
         stage_tile<C, R>(ab, img, ln, wp, info >> 8);
         __syncthreads();
-    }
-    {   // first ring of the new vorticity around the core, kept for a3 of the next stage
-        double* const wrw = img + H * SW;
-        const int rB = Y0 - 1 - te.oy, rT = Y1 - te.oy, cL = X0 - 1 - te.ox, cR = X1 - te.ox;
-        for (int c = tid_o; c < SW; c += nth_o) { wrw[c] = img[img_ix(rB, c, SW)]; wrw[SW + c] = img[img_ix(rT, c, SW)]; }
-        for (int r2 = tid_o; r2 < H; r2 += nth_o) { wrw[2 * SW + r2] = img[img_ix(r2, cL, SW)]; wrw[2 * SW + H + r2] = img[img_ix(r2, cR, SW)]; }
     }
     }
 }
@@ -944,7 +919,7 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
     // ---- what this thread moves in an exchange (multi-tile plans only), kept in shared memory: the sweeps have no register to spare ----
     if (a.ntx * a.nty > 1) {
         const int H = nwarps * R;
-        unsigned int* const xi = reinterpret_cast<unsigned int*>(sm + edge_doubles + H * SW + 2 * SW + 2 * H) + 2 * tid;
+        unsigned int* const xi = reinterpret_cast<unsigned int*>(sm + edge_doubles + (H + 1) * SW) + 2 * tid;
         unsigned int info;
         int ubase;
         xchg_setup<C, R>(N, a.halo, a.walls != 0, a.ntx, a.nty, a.upitch, t, lane, warp, bi, bj, info, ubase);
@@ -965,12 +940,6 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
         __syncthreads();
         if (KIND == 1) qb_from_image<C, R>(q, img, a.c9q, gx0_, gy0_, N, lane, warp);
         else read_tile<C, R>(q, img, lane, warp, 0x3fu);
-        if (a.nsteps > 0) {               // first ring of the stage input around the core, kept for a3
-            double* const wr = img + H * SW;
-            const int rB = imax(t.cy0, 1) - 1 - t.oy, rT = imin(t.cy1, N) - t.oy, cL = imax(t.cx0, 1) - 1 - t.ox, cR = imin(t.cx1, N) - t.ox;
-            for (int k = tid; k < SW; k += nthreads) { wr[k] = img[img_ix(rB, k, SW)]; wr[SW + k] = img[img_ix(rT, k, SW)]; }
-            for (int k = tid; k < H; k += nthreads) { wr[2 * SW + k] = img[img_ix(k, cL, SW)]; wr[2 * SW + H + k] = img[img_ix(k, cR, SW)]; }
-        }
     }
     if (KIND == 0) {
 #pragma unroll
@@ -1025,7 +994,7 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
             {
                 const int z = opaque_zero();
                 const int nw = (int)blockDim.y + z, tid_o = ((int)threadIdx.y + z) * 32 + (int)threadIdx.x;
-                const unsigned int* const xi = reinterpret_cast<const unsigned int*>(sm + edge_doubles + nw * R * SW + 2 * SW + 2 * nw * R) + 2 * tid_o;
+                const unsigned int* const xi = reinterpret_cast<const unsigned int*>(sm + edge_doubles + (nw * R + 1) * SW) + 2 * tid_o;
                 const unsigned int info = xi[0];
                 const int ubase = (int)xi[1];
                 char* const xb = (round & 1u) ? a.x1 : a.x0;
