@@ -230,6 +230,7 @@ constexpr unsigned int FL_ZERO_LEFT = 1u;     // the left neighbour column is a 
 constexpr unsigned int FL_ZERO_RIGHT = 2u;    // same on the right
 constexpr unsigned int FL_PUB_BOTTOM = 4u;    // publish the bottom row of the micro-tile to the warp below
 constexpr unsigned int FL_PUB_TOP = 8u;       // publish the top row to the warp above
+constexpr unsigned int FL_MASK = 32u;         // 5-point sweeps: this lane reads the wall x = 0 / x = N as one of its west / east neighbours (see half_sweep, CLS)
 constexpr unsigned int FL_WALL_LANE = 16u;    // this lane holds the wall x = N in column WC > 0, behind interior points: that column reads as +0.0
 
 // One colour half-sweep on the register micro-tile.  K = LOCAL colour being updated: local point (ci, rj) has local colour
@@ -238,7 +239,13 @@ constexpr unsigned int FL_WALL_LANE = 16u;    // this lane holds the wall x = N 
 // the rows above / below live in the adjacent warps and come through the sB / sT edge arrays.
 // wallmask: bit rj * C + ci set = that point lies ON a wall that could not be isolated by alignment and is put back to
 // +0.0 after the update (eq 23-24).
-template <int C, int R, int K, bool FIX, int TOPOFF, int WC>
+// CLS: where a wall column sits for the tiles of this class (a uniform branch in the kernel picks the class from blockIdx):
+//   0 none; 1 x = 0 is the last column of the lane to the LEFT of the flagged lane; 2 x = N is the first column of the lane to its
+//   RIGHT; 3, 4, 5 x = N is column 1, 2, 3 of the flagged lane itself, behind interior points.
+// The flagged lane (FL_MASK) must read +0.0 there (eq 23-24) although the register holds something else.  No select:
+// the pair sum that contains the term is written fma(m, term, other) with m = 0.0 in the flagged lane and 1.0 elsewhere, which
+// rounds exactly like term + other (m = 1) or gives other (m = 0): same fp64 instruction count, no integer work in the loop.
+template <int C, int R, int K, bool FIX, int TOPOFF, int CLS>
 __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[R][C], const double cb, const double omb,
                                            double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl_) {
     unsigned int fl = fl_;
@@ -265,23 +272,27 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
     for (int rj = 0; rj < R; ++rj) {
         if ((rj & 1) == K) {                                               // right edge of lane - 1
             const double v = __shfl_up_sync(0xffffffffu, p[rj][C - 1], 1);
-            Lnb[rj] = (fl & FL_ZERO_LEFT) ? 0.0 : v;
+            Lnb[rj] = v;
         }
         if (((C - 1 + rj) & 1) == K) {                                     // left edge of lane + 1
             const double v = __shfl_down_sync(0xffffffffu, p[rj][0], 1);
-            Rnb[rj] = (fl & FL_ZERO_RIGHT) ? 0.0 : v;
+            Rnb[rj] = v;
         }
     }
+    const double m = (CLS != 0 && (fl & FL_MASK)) ? 0.0 : 1.0;
     auto update_row = [&](const int rj) {
 #pragma unroll
         for (int ci = 0; ci < C; ++ci) {
             if (((ci + rj) & 1) != K) continue;
             const double pW = ci > 0 ? p[rj][ci - 1] : Lnb[rj];
-            double pE = ci < C - 1 ? p[rj][ci + 1] : Rnb[rj];
-            if (WC > 0 && ci == WC - 1 && (fl & FL_WALL_LANE)) pE = 0.0;       // the wall x = N inside this lane
+            const double pE = ci < C - 1 ? p[rj][ci + 1] : Rnb[rj];
             const double pS = rj > 0 ? p[rj - 1][ci] : Bnb[ci];
             const double pN = rj < R - 1 ? p[rj + 1][ci] : Tnb[ci];
-            const double nb = (pW + pE) + (pS + pN);
+            double we;
+            if (CLS == 1 && ci == 0) we = fma(m, pW, pE);                      // pW is the wall x = 0 in the flagged lane
+            else if ((CLS == 2 && ci == C - 1) || (CLS >= 3 && ci == CLS - 3)) we = fma(m, pE, pW);      // pE is the wall x = N there
+            else we = pW + pE;
+            const double nb = we + (pS + pN);
             const double qv = (rj >= Q0 && rj < Q0 + QR) ? qs[rj - Q0 < 0 ? 0 : (rj - Q0 >= QR ? QR - 1 : rj - Q0)][ci] : q[rj][ci];
             p[rj][ci] = fma(omb, p[rj][ci], fma(cb, nb, qv));
         }
@@ -408,8 +419,9 @@ __device__ __forceinline__ void colour_pass(double (&p)[R][C], const double (&q)
     __syncthreads();
 }
 
-// ns sweeps on the register micro-tile.  WC: the column of a lane that holds the wall x = N behind interior points (0: none).
-template <int C, int R, bool FIX, int TOPOFF, int KIND, int WC>
+// ns sweeps on the register micro-tile.  CLS: the tile's class (half_sweep); the compact operator's passes take WC, the column of a
+// lane that holds the wall x = N behind interior points (0: none), and the select flags.
+template <int C, int R, bool FIX, int TOPOFF, int KIND, int CLS>
 __device__ __forceinline__ void run_sweeps(double (&p)[R][C], const double (&q)[R][C], const double cb, const double omb, const double c9e,
                                            const double c9c, double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl, const int ns,
                                            const bool odd_origin, const int par9) {
@@ -418,21 +430,21 @@ __device__ __forceinline__ void run_sweeps(double (&p)[R][C], const double (&q)[
         for (int s = ns; s > 0; --s)
             for (int g = 0; g < 4; ++g) {
                 switch (g ^ par9) {
-                    case 0: colour_pass<C, R, 0, 0, FIX, TOPOFF, WC>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
-                    case 1: colour_pass<C, R, 1, 0, FIX, TOPOFF, WC>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
-                    case 2: colour_pass<C, R, 0, 1, FIX, TOPOFF, WC>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
-                    default: colour_pass<C, R, 1, 1, FIX, TOPOFF, WC>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
+                    case 0: colour_pass<C, R, 0, 0, FIX, TOPOFF, (CLS >= 3 ? CLS - 2 : 0)>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
+                    case 1: colour_pass<C, R, 1, 0, FIX, TOPOFF, (CLS >= 3 ? CLS - 2 : 0)>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
+                    case 2: colour_pass<C, R, 0, 1, FIX, TOPOFF, (CLS >= 3 ? CLS - 2 : 0)>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
+                    default: colour_pass<C, R, 1, 1, FIX, TOPOFF, (CLS >= 3 ? CLS - 2 : 0)>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
                 }
             }
     } else if (odd_origin) {
         for (int s = ns; s > 0; --s) {                                     // red = (i + j) even first (G9): local colour 1 here
-            half_sweep<C, R, 1, FIX, TOPOFF, WC>(p, q, cb, omb, sB, wallmask, fl);
-            half_sweep<C, R, 0, FIX, TOPOFF, WC>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 1, FIX, TOPOFF, CLS>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 0, FIX, TOPOFF, CLS>(p, q, cb, omb, sB, wallmask, fl);
         }
     } else {
         for (int s = ns; s > 0; --s) {
-            half_sweep<C, R, 0, FIX, TOPOFF, WC>(p, q, cb, omb, sB, wallmask, fl);
-            half_sweep<C, R, 1, FIX, TOPOFF, WC>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 0, FIX, TOPOFF, CLS>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 1, FIX, TOPOFF, CLS>(p, q, cb, omb, sB, wallmask, fl);
         }
     }
 }
@@ -912,6 +924,8 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
         if (t.right_al && t.wc > 0 && lane == (N - t.ox) / C) fl |= FL_WALL_LANE;
         if (lane == lzl) fl |= FL_ZERO_LEFT;
         if (lane == lzr) fl |= FL_ZERO_RIGHT;
+        // the lane of the 5-point sweeps' mask (half_sweep, CLS 1 / 2 / 3-5); a tile has one class, so one flag serves all
+        if (t.left_al ? lane == 1 : (t.right_al && lane == (N - t.ox) / C - (t.wc == 0 ? 1 : 0))) fl |= FL_MASK;
         if (t.bot_al && warp == 0) fl &= ~FL_PUB_TOP;                          // warp 0 holds y = -(R-1) .. 0
         if (t.top_al && warp == (N - t.oy) / R) fl &= ~FL_PUB_BOTTOM;          // that warp holds y = N .. N + R - 1
     }
@@ -973,15 +987,17 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
         // ================= a1: S sweeps, a halo exchange after every T of them =================
         for (int rem = a.S; rem > 0; rem -= a.T) {
             {
-                // the column of a lane that holds the wall x = N (tiles of the last column), from blockIdx and the parameters
-                // only: a uniform branch, like the colour order
-                const int wct = ((int)blockIdx.x == a.ntx - 1 && a.ntx > 1) ? ((a.N - 1) & 3) : 0;
+                // the class of the tile (where a wall column sits: first column of tiles, last column, none), from blockIdx and the
+                // parameters only: a uniform branch, like the colour order
+                const int cls = (int)blockIdx.x == 0 ? 1 : (((int)blockIdx.x == a.ntx - 1) ? 2 + ((a.N - 1) & 3) : 0);
                 const int ns = min(a.T, rem);
-                switch (wct) {
+                switch (cls) {
                     case 0: run_sweeps<C, R, FIX, TOPOFF, KIND, 0>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
                     case 1: run_sweeps<C, R, FIX, TOPOFF, KIND, 1>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
                     case 2: run_sweeps<C, R, FIX, TOPOFF, KIND, 2>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
-                    default: run_sweeps<C, R, FIX, TOPOFF, KIND, 3>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                    case 3: run_sweeps<C, R, FIX, TOPOFF, KIND, 3>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                    case 4: run_sweeps<C, R, FIX, TOPOFF, KIND, 4>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                    default: run_sweeps<C, R, FIX, TOPOFF, KIND, 5>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
                 }
             }
             const int tslot = 2 + 4 * (int)(round - a.base);                    // trace slot (meaningful in sweeps-only launches)
