@@ -155,7 +155,7 @@ int cav_trace_sweeps(cav_ctx* ctx, int nsweeps, long long* stamps_out, int slots
  * `sms` multiprocessors, `smem_bytes` of shared memory per block and 65536 registers (sweep: CAV_SWEEP_REDBLACK or
  * CAV_SWEEP_COMPACT9; T > 0 forces the sweeps per exchange round) and checks its halo-exchange pattern: every unit of four
  * points a tile fetches must be stored by exactly one tile, every stored unit must be fetched, every tile must fit its thread
- * grid.  plan_out[8] (may be NULL) = ntx, nty, CW, CH, halo, T, warps, shared-memory bytes; counts_out[5] (may be NULL) = units
+ * grid.  plan_out[9] (may be NULL) = ntx, nty, CW, CH, halo, T, warps, shared-memory bytes, EB (rows the first row of tiles owns beyond CH); counts_out[5] (may be NULL) = units
  * fetched, units stored, fetches without exactly one store, stores nobody fetches, tiles that do not fit.
  * Returns CAV_OK if the plan is consistent (also for a single-tile plan, which exchanges nothing), CAV_ENOTSUP if the grid
  * has no resident plan under these figures, CAV_EINVAL for bad arguments or an inconsistent pattern. */

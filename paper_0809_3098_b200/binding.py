@@ -107,10 +107,10 @@ def _field(a, N, name):
 def plan_check(N, sweep="redblack", T=0, sms=148, smem_bytes=232448):
     """Host logic only (no device): the resident plan of an (N + 1)^2 grid and the consistency of its halo-exchange pattern.
     Returns (rc, plan dict or None, counts dict)."""
-    plan = (C.c_int * 8)()
+    plan = (C.c_int * 9)()
     counts = (C.c_longlong * 5)()
     rc = lib().cav_plan_check(int(N), _SWEEPS[sweep], int(T), int(sms), int(smem_bytes), plan, counts)
-    names = ("ntx", "nty", "CW", "CH", "halo", "T", "warps", "smem_bytes")
+    names = ("ntx", "nty", "CW", "CH", "halo", "T", "warps", "smem_bytes", "EB")
     cn = ("fetched", "stored", "unmatched", "unfetched", "misfit")
     return rc, (dict(zip(names, plan)) if rc != -4 else None), dict(zip(cn, counts))
 

@@ -546,7 +546,7 @@ CAV_API int cav_plan_check(int N, int sweep, int T, int sms, int smem_bytes, int
     if (!pl.ok) return CAV_ENOTSUP;
     if (plan_out) {
         plan_out[0] = pl.ntx; plan_out[1] = pl.nty; plan_out[2] = pl.CW; plan_out[3] = pl.CH; plan_out[4] = pl.halo;
-        plan_out[5] = pl.ntiles > 1 ? pl.T : 0; plan_out[6] = pl.warps; plan_out[7] = pl.smem_bytes;
+        plan_out[5] = pl.ntiles > 1 ? pl.T : 0; plan_out[6] = pl.warps; plan_out[7] = pl.smem_bytes; plan_out[8] = pl.EB;
     }
     return cavk::resident_check_exchange(pl, N, counts_out) == 0 ? CAV_OK : CAV_EINVAL;
 }

@@ -104,7 +104,7 @@ struct ResArgs {
     unsigned int base;      // exchange rounds done by earlier launches (tag of round r: 1 + r mod 4095; buffer: r & 1)
     int nsteps;             // > 0: that many whole time steps (a1 + a2 + a3, five stages each); 0: S sweeps of a1 only
     int S;                  // sweeps per stage (nsteps > 0) or in total (nsteps == 0)
-    int T, halo, CW, CH, ntx, nty;
+    int T, halo, CW, CH, EB, ntx, nty;
     int walls;              // the exchanged regions include the wall points (compact operator)
     long long* trace;       // profiling only (cav_trace_sweeps): per tile, %globaltimer at the phase boundaries; else null
     int trace_cap;          // slots per tile
@@ -124,26 +124,29 @@ struct TileGeom {
     int ox, oy;                    // grid coordinates of local point (0, 0)
     int wc;                        // tiles of the last column: the column of a lane that holds x = N (0: isolated by alignment)
     bool left_al, right_al, bot_al, top_al;   // wall isolated in a lane / warp that owns no interior point, or (right, wc > 0) read as +0.0
+    bool bot_in;                   // the wall y = 0 is row 0 of warp 0, read as +0.0 by row 1 (plans with EB > 0: five more rows for the core)
     bool fits;                     // the W x H thread grid covers core + halo (clipped to the grid) and the aligned walls
 };
 __host__ __device__ inline int round_up4(int v) { return (v + 3) / 4 * 4; }
 
-__host__ __device__ inline TileGeom tile_geom(int N, int CW, int CH, int halo, int ntx, int nty, int bi, int bj, int C, int R,
+__host__ __device__ inline TileGeom tile_geom(int N, int CW, int CH, int EB, int halo, int ntx, int nty, int bi, int bj, int C, int R,
                                               int W, int H) {
     TileGeom g;
     g.cx0 = (ntx > 1 && bi > 0) ? bi * CW + 1 : 0;
-    g.cy0 = bj * CH;
+    g.cy0 = bj == 0 ? 0 : EB + bj * CH;       // EB > 0: the bottom tiles own EB more rows (see bot_in below)
     g.cx1 = (ntx > 1 && (bi + 1) * CW + 1 < N + 1) ? (bi + 1) * CW + 1 : N + 1;
-    g.cy1 = g.cy0 + CH < N + 1 ? g.cy0 + CH : N + 1;
+    g.cy1 = (bj < nty - 1 && EB + (bj + 1) * CH < N + 1) ? EB + (bj + 1) * CH : N + 1;      // the last tile takes what is left
     g.left_al = bi == 0;
     g.right_al = bi == ntx - 1 && ntx > 1;
-    g.bot_al = bj == 0;
+    g.bot_al = bj == 0 && EB == 0;
+    g.bot_in = bj == 0 && EB > 0;
     g.top_al = bj == nty - 1 && nty > 1;
     g.wc = 0;
     if (g.left_al) g.ox = -(C - 1);                                   // x = 0 is column C - 1 of lane 0
     else g.ox = g.cx0 - round_up4(halo);                              // = 1 (mod 4)
     if (g.right_al) g.wc = (N - g.ox) % C;
     if (g.bot_al) g.oy = -(R - 1);                                    // y = 0 is row R - 1 of warp 0
+    else if (g.bot_in) g.oy = 0;                                      // y = 0 is row 0 of warp 0, below interior rows of the same warp
     else if (g.top_al) g.oy = g.cy0 - halo - (R - (N - g.cy0 + halo) % R) % R;        // (N - oy) % R == 0
     else g.oy = g.cy0 - halo;
     const int xneed = (g.cx1 + halo < N + 1 ? g.cx1 + halo : N + 1);  // one past the last column the tile must hold
@@ -231,6 +234,7 @@ constexpr unsigned int FL_ZERO_RIGHT = 2u;    // same on the right
 constexpr unsigned int FL_PUB_BOTTOM = 4u;    // publish the bottom row of the micro-tile to the warp below
 constexpr unsigned int FL_PUB_TOP = 8u;       // publish the top row to the warp above
 constexpr unsigned int FL_MASK = 32u;         // 5-point sweeps: this lane reads the wall x = 0 / x = N as one of its west / east neighbours (see half_sweep, CLS)
+constexpr unsigned int FL_MASKB = 64u;        // 5-point sweeps: row 0 of this warp is the wall y = 0 (bot_in tiles): row 1 reads +0.0 below it
 constexpr unsigned int FL_WALL_LANE = 16u;    // this lane holds the wall x = N in column WC > 0, behind interior points: that column reads as +0.0
 
 // One colour half-sweep on the register micro-tile.  K = LOCAL colour being updated: local point (ci, rj) has local colour
@@ -245,7 +249,8 @@ constexpr unsigned int FL_WALL_LANE = 16u;    // this lane holds the wall x = N 
 // The flagged lane (FL_MASK) must read +0.0 there (eq 23-24) although the register holds something else.  No select:
 // the pair sum that contains the term is written fma(m, term, other) with m = 0.0 in the flagged lane and 1.0 elsewhere, which
 // rounds exactly like term + other (m = 1) or gives other (m = 0): same fp64 instruction count, no integer work in the loop.
-template <int C, int R, int K, bool FIX, int TOPOFF, int CLS>
+// CLSY = 1: tiles of the first row whose wall y = 0 is row 0 of warp 0 (bot_in): the flagged warp (FL_MASKB) masks it the same way.
+template <int C, int R, int K, bool FIX, int TOPOFF, int CLS, int CLSY>
 __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[R][C], const double cb, const double omb,
                                            double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl_) {
     unsigned int fl = fl_;
@@ -280,6 +285,7 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
         }
     }
     const double m = (CLS != 0 && (fl & FL_MASK)) ? 0.0 : 1.0;
+    const double mb = (CLSY != 0 && (fl & FL_MASKB)) ? 0.0 : 1.0;
     auto update_row = [&](const int rj) {
 #pragma unroll
         for (int ci = 0; ci < C; ++ci) {
@@ -292,7 +298,8 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
             if (CLS == 1 && ci == 0) we = fma(m, pW, pE);                      // pW is the wall x = 0 in the flagged lane
             else if ((CLS == 2 && ci == C - 1) || (CLS >= 3 && ci == CLS - 3)) we = fma(m, pE, pW);      // pE is the wall x = N there
             else we = pW + pE;
-            const double nb = we + (pS + pN);
+            const double sn = (CLSY == 1 && rj == 1) ? fma(mb, pS, pN) : pS + pN;      // pS is the wall y = 0 in the flagged warp
+            const double nb = we + sn;
             const double qv = (rj >= Q0 && rj < Q0 + QR) ? qs[rj - Q0 < 0 ? 0 : (rj - Q0 >= QR ? QR - 1 : rj - Q0)][ci] : q[rj][ci];
             p[rj][ci] = fma(omb, p[rj][ci], fma(cb, nb, qv));
         }
@@ -421,7 +428,7 @@ __device__ __forceinline__ void colour_pass(double (&p)[R][C], const double (&q)
 
 // ns sweeps on the register micro-tile.  CLS: the tile's class (half_sweep); the compact operator's passes take WC, the column of a
 // lane that holds the wall x = N behind interior points (0: none), and the select flags.
-template <int C, int R, bool FIX, int TOPOFF, int KIND, int CLS>
+template <int C, int R, bool FIX, int TOPOFF, int KIND, int CLS, int CLSY>
 __device__ __forceinline__ void run_sweeps(double (&p)[R][C], const double (&q)[R][C], const double cb, const double omb, const double c9e,
                                            const double c9c, double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl, const int ns,
                                            const bool odd_origin, const int par9) {
@@ -438,13 +445,13 @@ __device__ __forceinline__ void run_sweeps(double (&p)[R][C], const double (&q)[
             }
     } else if (odd_origin) {
         for (int s = ns; s > 0; --s) {                                     // red = (i + j) even first (G9): local colour 1 here
-            half_sweep<C, R, 1, FIX, TOPOFF, CLS>(p, q, cb, omb, sB, wallmask, fl);
-            half_sweep<C, R, 0, FIX, TOPOFF, CLS>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 1, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 0, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl);
         }
     } else {
         for (int s = ns; s > 0; --s) {
-            half_sweep<C, R, 0, FIX, TOPOFF, CLS>(p, q, cb, omb, sB, wallmask, fl);
-            half_sweep<C, R, 1, FIX, TOPOFF, CLS>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 0, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 1, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl);
         }
     }
 }
@@ -770,7 +777,7 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
     const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
     const int nw = (int)blockDim.y + z, tid_o = wp * 32 + ln, nth_o = nw * 32, H = nw * R;
     const int Ne = a.N + z, pitch = a.pitch;
-    const TileGeom te = tile_geom(Ne, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, H);
+    const TileGeom te = tile_geom(Ne, a.CW, a.CH, a.EB, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, H);
     const int k = stage % 5 + 1;                                    // RK stage 1..5
     double* const wout = a.wbase + (size_t)(k % 5) * a.fstride;         // omega^(k); stage 5 writes omega^{n+1} over omega^n
     double* const tbuf = a.wbase + (size_t)(5 + z) * a.fstride;         // T: first three terms of eq 13 (+ z: not hoisted)
@@ -840,7 +847,7 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
             if (!((colin >> ci) & 1u)) continue;
             const double pW = ci > 0 ? pp[rj][ci - 1] : lnb;
             const double pE = gx == Ne - 1 ? 0.0 : (ci < C - 1 ? pp[rj][ci + 1] : rnb);      // psi = 0 on the wall x = N, wherever it sits
-            const double pS = rj > 0 ? pp[rj - 1][ci] : sB[TOPOFF + ci * 32];            // top row of the warp below
+            const double pS = gy == 1 ? 0.0 : (rj > 0 ? pp[rj - 1][ci] : sB[TOPOFF + ci * 32]);      // psi = 0 on the wall y = 0; else the top row of the warp below
             const double pN = rj < R - 1 ? pp[rj + 1][ci] : sB[C * 32 + ci * 32];        // bottom row of the warp above
             const double w0 = wc[1 + ci], wW = wc[ci], wE = wc[2 + ci], wS = ws[ci], wN = wn[ci];
             // eq 22: u = dpsi/dy, v = -dpsi/dx;  eq 8
@@ -911,7 +918,7 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
     for (int k = tid; k < edge_doubles; k += nthreads) sm[k] = 0.0;
     double* const sB = sm + warp * C * 32 + lane;      // [MAXW + 1][C][32] bottom row of warp at [warp]; top rows TOPOFF further, at [warp + 1]
 
-    const TileGeom t = tile_geom(N, a.CW, a.CH, a.halo, a.ntx, a.nty, bi, bj, C, R, SW, nwarps * R);
+    const TileGeom t = tile_geom(N, a.CW, a.CH, a.EB, a.halo, a.ntx, a.nty, bi, bj, C, R, SW, nwarps * R);
     const int gx0_ = t.ox + lane * C, gy0_ = t.oy + warp * R;
     // local colour = global colour ^ odd_origin.  Computed from blockIdx only: the branch on it is uniform for the compiler
     // too, so the sweep loops stay convergent code (uniform registers for the coefficients, no divergence guards on the shuffles)
@@ -926,6 +933,7 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
         if (lane == lzr) fl |= FL_ZERO_RIGHT;
         // the lane of the 5-point sweeps' mask (half_sweep, CLS 1 / 2 / 3-5); a tile has one class, so one flag serves all
         if (t.left_al ? lane == 1 : (t.right_al && lane == (N - t.ox) / C - (t.wc == 0 ? 1 : 0))) fl |= FL_MASK;
+        if (t.bot_in && warp == 0) fl |= FL_MASKB;
         if (t.bot_al && warp == 0) fl &= ~FL_PUB_TOP;                          // warp 0 holds y = -(R-1) .. 0
         if (t.top_al && warp == (N - t.oy) / R) fl &= ~FL_PUB_BOTTOM;          // that warp holds y = N .. N + R - 1
     }
@@ -991,13 +999,24 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
                 // parameters only: a uniform branch, like the colour order
                 const int cls = (int)blockIdx.x == 0 ? 1 : (((int)blockIdx.x == a.ntx - 1) ? 2 + ((a.N - 1) & 3) : 0);
                 const int ns = min(a.T, rem);
-                switch (cls) {
-                    case 0: run_sweeps<C, R, FIX, TOPOFF, KIND, 0>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
-                    case 1: run_sweeps<C, R, FIX, TOPOFF, KIND, 1>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
-                    case 2: run_sweeps<C, R, FIX, TOPOFF, KIND, 2>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
-                    case 3: run_sweeps<C, R, FIX, TOPOFF, KIND, 3>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
-                    case 4: run_sweeps<C, R, FIX, TOPOFF, KIND, 4>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
-                    default: run_sweeps<C, R, FIX, TOPOFF, KIND, 5>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                if (KIND == 0 && (int)blockIdx.y == 0 && a.EB > 0) {       // bot_in tiles (uniform branch)
+                    switch (cls) {
+                        case 0: run_sweeps<C, R, FIX, TOPOFF, KIND, 0, 1>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                        case 1: run_sweeps<C, R, FIX, TOPOFF, KIND, 1, 1>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                        case 2: run_sweeps<C, R, FIX, TOPOFF, KIND, 2, 1>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                        case 3: run_sweeps<C, R, FIX, TOPOFF, KIND, 3, 1>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                        case 4: run_sweeps<C, R, FIX, TOPOFF, KIND, 4, 1>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                        default: run_sweeps<C, R, FIX, TOPOFF, KIND, 5, 1>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                    }
+                } else {
+                    switch (cls) {
+                        case 0: run_sweeps<C, R, FIX, TOPOFF, KIND, 0, 0>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                        case 1: run_sweeps<C, R, FIX, TOPOFF, KIND, 1, 0>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                        case 2: run_sweeps<C, R, FIX, TOPOFF, KIND, 2, 0>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                        case 3: run_sweeps<C, R, FIX, TOPOFF, KIND, 3, 0>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                        case 4: run_sweeps<C, R, FIX, TOPOFF, KIND, 4, 0>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                        default: run_sweeps<C, R, FIX, TOPOFF, KIND, 5, 0>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
+                    }
                 }
             }
             const int tslot = 2 + 4 * (int)(round - a.base);                    // trace slot (meaningful in sweeps-only launches)
@@ -1033,7 +1052,7 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
             const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
             double* const img = sm + edge_doubles;
             if (KIND == 1) {
-                const TileGeom tq = tile_geom(a.N + z, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, ((int)blockDim.y + z) * R);
+                const TileGeom tq = tile_geom(a.N + z, a.CW, a.CH, a.EB, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, ((int)blockDim.y + z) * R);
                 qb_from_image<C, R>(q, img, a.c9q, tq.ox + ln * C, tq.oy + wp * R, a.N + z, ln, wp);
             } else {
                 read_tile<C, R>(q, img, ln, wp, 0x3fu);
@@ -1057,7 +1076,7 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
         const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
         const int nw = (int)blockDim.y + z, tid_o = wp * 32 + ln, nth_o = nw * 32, H = nw * R;
         const int Ne = a.N + z;
-        const TileGeom te = tile_geom(Ne, a.CW, a.CH, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, H);
+        const TileGeom te = tile_geom(Ne, a.CW, a.CH, a.EB, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, H);
         double* const img = sm + edge_doubles;
         stage_tile<C, R>(p, img, ln, wp, 0x3fu);
         __syncthreads();
@@ -1091,7 +1110,7 @@ bool finish_plan(ResidentPlan& pl, int N, int max_smem) {
     const int W = 32 * pl.C, H = pl.warps * pl.R;
     for (int bj = 0; bj < pl.nty; ++bj)
         for (int bi = 0; bi < pl.ntx; ++bi) {
-            const TileGeom t = tile_geom(N, pl.CW, pl.CH, pl.halo, pl.ntx, pl.nty, bi, bj, pl.C, pl.R, W, H);
+            const TileGeom t = tile_geom(N, pl.CW, pl.CH, pl.EB, pl.halo, pl.ntx, pl.nty, bi, bj, pl.C, pl.R, W, H);
             if (!t.fits) return false;
         }
     const int maxw = VARIANTS[pl.variant].maxw;
@@ -1114,6 +1133,22 @@ bool split(int G, int L, int lead, int h, int& core, int& n) {
         // the halo must come from adjacent tiles only, and must not reach a wall through an edge tile (only an
         // edge tile isolates the wall; elsewhere nothing keeps a wall point inside the thread grid at 0)
         return n >= 2 && core > h && G - (n - 1) * core > h;
+    }
+    return false;
+}
+// Tiling in y with the wall y = 0 INSIDE warp 0 of the first row of tiles (tile_geom: bot_in): that row can own up to `h` more
+// rows than the others (it needs no halo below and no warp to isolate the wall), the last row takes what is left (at most
+// L - h - (R - 1) rows: its wall is aligned to a warp).  n tiles, cores CH + EB, CH, ..., CH, rest.  false if impossible.
+bool split_wb(int G, int L, int R, int h, int n, int& core, int& eb) {
+    const int cmax = L - 2 * h, ctmax = L - h - (R - 1);
+    if (n < 3 || cmax <= h) return false;
+    for (core = h + 1; core <= cmax; ++core) {
+        // the first row takes as much of the excess as it may, the last row the remainder
+        const int rest = G - (n - 1) * core;            // rows left for EB + the last core
+        if (rest <= h) continue;
+        eb = std::min(h, std::max(rest - core, 1));
+        const int last = rest - eb;
+        if (last > h && last <= ctmax && last <= core + h) return true;
     }
     return false;
 }
@@ -1163,13 +1198,21 @@ ResidentPlan resident_plan_for(int N, int kind, int T_override, int variant_over
                 if (T_override > 0 && T != T_override) continue;
                 const int halo = (kind == 1 ? 4 : 2) * T;      // one ring is consumed per colour pass
                 int CW, ntx, CH, nty;
-                if (!split_x(N, W, v.C - 1, halo, CW, ntx) || !split(G, H, v.R - 1, halo, CH, nty)) continue;
+                if (!split_x(N, W, v.C - 1, halo, CW, ntx)) continue;
+                int EB = 0;
+                bool okY = split(G, H, v.R - 1, halo, CH, nty) && ntx * nty <= sms * per_sm;
+                if (!okY && kind == 0 && ntx <= sms * per_sm) {
+                    // one row of tiles fewer with the wall y = 0 inside warp 0 of the first row (5-point sweeps only)
+                    for (nty = 3; nty * ntx <= sms * per_sm && !okY; ++nty) okY = split_wb(G, H, v.R, halo, nty, CH, EB);
+                    if (okY) --nty;
+                }
+                if (!okY) continue;
                 const int ntiles = ntx * nty;
                 if (ntiles < 2 || ntiles > sms * per_sm) continue;
                 // Cost per sweep in SM cycles, calibrated on B200 (profiles/r2b_*.md): a colour half-sweep takes ~187 cycles per warp
                 // of the busiest SM sub-partition (+ barrier), an exchange ~5000 cycles of latency + 130 per point of halo depth.
                 const double cost = sweep_cost + (5000.0 + 130.0 * halo) / T;
-                c.T = T; c.halo = halo; c.CW = CW; c.CH = CH; c.ntx = ntx; c.nty = nty; c.ntiles = ntiles;
+                c.T = T; c.halo = halo; c.CW = CW; c.CH = CH; c.EB = EB; c.ntx = ntx; c.nty = nty; c.ntiles = ntiles;
                 if (cost < best_cost && finish_plan(c, N, smem_cta)) { best_cost = cost; best = c; }
             }
         }
@@ -1220,7 +1263,7 @@ int resident_check_exchange(const ResidentPlan& pl, int N, long long* counts) {
         const bool walls = pl.kind == 1;
         for (int bj = 0; bj < pl.nty; ++bj)
             for (int bi = 0; bi < pl.ntx; ++bi) {
-                const TileGeom t = tile_geom(N, pl.CW, pl.CH, pl.halo, pl.ntx, pl.nty, bi, bj, 4, 6, 128, pl.warps * 6);
+                const TileGeom t = tile_geom(N, pl.CW, pl.CH, pl.EB, pl.halo, pl.ntx, pl.nty, bi, bj, 4, 6, 128, pl.warps * 6);
                 if (!t.fits) ++c[4];
                 for (int warp = 0; warp < pl.warps; ++warp)
                     for (int lane = 0; lane < 32; ++lane) {
@@ -1282,7 +1325,7 @@ int resident_launch(const Params& P, const ResidentPlan& pl, const double* psi_i
     a.base = *epoch;
     a.nsteps = nsteps; a.S = S;
     a.T = pl.ntiles == 1 ? std::max(S, 1) : pl.T;
-    a.halo = pl.halo; a.CW = pl.CW; a.CH = pl.CH; a.ntx = pl.ntx; a.nty = pl.nty;
+    a.halo = pl.halo; a.CW = pl.CW; a.CH = pl.CH; a.EB = pl.EB; a.ntx = pl.ntx; a.nty = pl.nty;
     a.trace = trace_dev; a.trace_cap = trace_cap;
     *epoch += (unsigned int)resident_rounds(pl, nsteps, S);      // wraps harmlessly: tags only tell round r from round r - 2
     void* args[] = {&a};

@@ -18,6 +18,8 @@ struct ResidentPlan {
     int T = 0;            // sweeps per round (between two halo exchanges); single tile: unused
     int halo = 0;         // 2 T, compact operator 4 T (one ring is consumed per colour pass); 0 for a single tile
     int CW = 0, CH = 0;   // core (owned) points per tile in x and y: rows [bj CH, (bj+1) CH); columns [0, CW + 1), [CW + 1, 2 CW + 1), ... (CW a multiple of 4)
+    int EB = 0;           // > 0: the bottom tiles own EB more rows, [0, CH + EB), the others [EB + bj CH, EB + (bj + 1) CH), the last one the rest;
+                          //      the wall y = 0 then sits inside warp 0 instead of being isolated in a warp of its own (5-point operator only)
     int ntx = 0, nty = 0; // tiles in x and y
     int ntiles = 0;
     bool fixup = false;           // some tile holds both walls of one direction: the kernel variant with the wall-mask fix-up

@@ -388,6 +388,7 @@ def test_resident_variants_agree_with_stream_engine(cav, N, S, variant, T):
 def test_trace_sweeps_reports_ordered_phases(cav):
     wl = W.config(4)
     g = cav.Cavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage)
+    g.set_resident_plan(5)                                            # five sweeps per exchange round, whatever the planner prefers
     g.set_fields(*W.initial_fields(wl))
     ref = cav.Cavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage, engine="stream")
     ref.set_fields(*W.initial_fields(wl))
@@ -401,9 +402,9 @@ def test_trace_sweeps_reports_ordered_phases(cav):
     g.close(); ref.close()
 
 
-@pytest.mark.parametrize("epoch", [65535 - 20, 2 * 65535 - 7, 0xFFFFFFF0 - 10, 0x80000000 - 3])
+@pytest.mark.parametrize("epoch", [4095 - 20, 2 * 4095 - 7, 65535 - 20, 0xFFFFFFF0 - 10, 0x80000000 - 3])
 def test_tag_epoch_restart_near_wrap(cav, epoch):
-    """Exchange tags are 16-bit (1 + round mod 65535) and the round counter is 32-bit: runs across the wrap of either (45
+    """Exchange tags are 12-bit (1 + round mod 4095) and the round counter is 32-bit: runs across the wrap of either (45
     exchange rounds follow the point the counter is set to) must stay bit-exact."""
     wl = W.config(3)                                   # 513 x 513, multi-tile plan; 9 sweeps per stage: two rounds per launch
     psi0, w0 = W.initial_fields(wl)
