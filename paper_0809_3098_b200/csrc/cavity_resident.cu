@@ -252,7 +252,8 @@ constexpr unsigned int FL_WALL_LANE = 16u;    // this lane holds the wall x = N 
 // CLSY = 1: tiles of the first row whose wall y = 0 is row 0 of warp 0 (bot_in): the flagged warp (FL_MASKB) masks it the same way.
 template <int C, int R, int K, bool FIX, int TOPOFF, int CLS, int CLSY>
 __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[R][C], const double cb, const double omb,
-                                           double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl_) {
+                                           double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl_, const double m,
+                                           const double mb) {
     unsigned int fl = fl_;
     asm volatile("" : "+r"(fl));               // opaque: the bit tests below are redone here, not hoisted into registers of their own
     // sB / sT point at [warp][0][lane] of the bottom / top edge arrays (stride 32 per ci, C * 32 per warp);
@@ -284,8 +285,6 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
             Rnb[rj] = v;
         }
     }
-    const double m = (CLS != 0 && (fl & FL_MASK)) ? 0.0 : 1.0;
-    const double mb = (CLSY != 0 && (fl & FL_MASKB)) ? 0.0 : 1.0;
     auto update_row = [&](const int rj) {
 #pragma unroll
         for (int ci = 0; ci < C; ++ci) {
@@ -443,15 +442,20 @@ __device__ __forceinline__ void run_sweeps(double (&p)[R][C], const double (&q)[
                     default: colour_pass<C, R, 1, 1, FIX, TOPOFF, (CLS >= 3 ? CLS - 2 : 0)>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
                 }
             }
-    } else if (odd_origin) {
+        return;
+    }
+    // the masks of half_sweep (CLS, CLSY), once per round: two registers each while the sweeps run
+    const double m = (CLS != 0 && (fl & FL_MASK)) ? 0.0 : 1.0;
+    const double mb = (CLSY != 0 && (fl & FL_MASKB)) ? 0.0 : 1.0;
+    if (odd_origin) {
         for (int s = ns; s > 0; --s) {                                     // red = (i + j) even first (G9): local colour 1 here
-            half_sweep<C, R, 1, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl);
-            half_sweep<C, R, 0, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 1, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl, m, mb);
+            half_sweep<C, R, 0, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl, m, mb);
         }
     } else {
         for (int s = ns; s > 0; --s) {
-            half_sweep<C, R, 0, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl);
-            half_sweep<C, R, 1, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl);
+            half_sweep<C, R, 0, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl, m, mb);
+            half_sweep<C, R, 1, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl, m, mb);
         }
     }
 }
