@@ -146,7 +146,7 @@ int cav_set_resident_plan(cav_ctx* ctx, int sweeps_per_exchange, int variant);
 /* Profiling aid, resident engine with the red-black sweeps only (CAV_ENOTSUP otherwise): runs nsweeps of a1 on the current
  * (psi, omega) like cav_poisson (without the a2 pass) and returns, for every tile, %globaltimer stamps (ns, one clock for all
  * tiles) at the phase boundaries: stamps_out is a HOST array of ntiles x slots_per_tile; slot 0 = kernel start, 1 = inputs
- * loaded, then for exchange round r: 2 + 4r = sweeps done, 3 + 4r = border strips stored, 4 + 4r = ring received from the
+ * loaded, then for exchange round r: 2 + 4r = sweeps done, 3 + 4r = border strips stored (by warp 0 of the tile), 4 + 4r = ring received from the
  * neighbours, 5 + 4r = edges republished.  Unused slots are 0; *ntiles_out (if non-NULL) receives the tile count; call once
  * with the capacity of a plan's tile count (at most 1023). */
 int cav_trace_sweeps(cav_ctx* ctx, int nsweeps, long long* stamps_out, int slots_per_tile, int* ntiles_out);

@@ -8,49 +8,51 @@
 // cavity_kernels.cu.  Inside one colour every update reads only the other colour and a3 is pointwise in its output, so the
 // schedule below cannot change a bit of the result; the tests compare with the FMA-mode oracle bit for bit.
 //
-// Schedule.  The (N+1)^2 grid is cut into ntx x nty tiles; tile (bi, bj) OWNS the core [bi CW, (bi+1) CW) x
-// [bj CH, (bj+1) CH) and additionally carries a halo of `halo` = 2T points on every side.  One CTA per tile, all CTAs
+// Schedule.  The (N+1)^2 grid is cut into ntx x nty tiles; tile (bi, bj) OWNS a core of about CW x CH points (tile_geom)
+// and additionally carries a halo of `halo` = 2T points on every side.  One CTA per tile, all CTAs
 // co-resident (cooperative launch).  A thread owns a C x R micro-tile (C consecutive x, R rows) of psi AND q in
 // registers for the whole launch; a warp spans 32 C points of R rows.  Threads exchange only the perimeter of their
 // micro-tile: left / right columns by warp shuffle, bottom / top rows through shared memory (edge arrays laid out so
 // that every access is unit-stride over the lanes), one __syncthreads per colour half-sweep.
 //
-// Walls cost nothing inside the sweeps.  The origin of an edge tile is shifted so that the wall column x = 0 is the LAST
-// column of a lane (x = N: the FIRST column of a lane) and the wall row y = 0 the LAST row of a warp (y = N: the FIRST row
-// of a warp).  Such a lane / warp owns no interior point; what it computes is never used: the adjacent lane substitutes
-// 0 for what the shuffle brings (the select that the tile edge needs anyway), and the warp never publishes that edge row,
-// so the shared-memory slot keeps the +0.0 it was initialised with (eq 23-24: psi = 0 on the walls).  A tile
-// whose origin parity is odd sweeps its local colour 1 first.  Walls that cannot be aligned (both walls of one direction in the same
-// tile: small grids) fall back to a bit mask of points that are put back to +0.0 after every half-sweep (FIX variant).
+// Walls cost nothing inside the sweeps.  Left wall: the origin of a tile of the first column is shifted so that x = 0 is the LAST
+// column of lane 0, which then owns no interior point.  Right wall: x = N lies in column (N - 1) mod 4 of a lane of the last
+// column of tiles (every tile's lanes start on a multiple of four plus one, see the exchange).  Bottom wall: y = 0 is the last row of
+// warp 0 (or, plans with EB > 0, the first row of warp 0, with interior rows above it in the same warp); top wall: y = N is the
+// first row of a warp.  Wherever a live point would read the wall through a register that holds something else, the pair sum
+// that contains the term is written fma(m, term, other) with m = 0.0 in that one lane / warp and 1.0 elsewhere (it rounds like
+// term + other, or gives other): no select, no extra fp64 instruction; the variant is picked per tile class by a uniform
+// branch (half_sweep: CLS, CLSY).  A warp that holds the isolated wall row never publishes it, so the shared-memory slot keeps
+// the +0.0 it was initialised with (eq 23-24: psi = 0 on the walls).  A tile whose origin parity is odd sweeps its
+// local colour 1 first.  Walls that cannot be aligned (both walls of one direction in the same tile: small grids) fall back
+// to a bit mask of points that are put back to +0.0 after every half-sweep (FIX variant).
 //
-// Halo exchange: every T sweeps (2T half-sweeps, each of which invalidates one more ring of the halo), after the last
-// sweep of a stage, and once per stage for the new vorticity, the CTAs refresh their halos through L2 WITHOUT any fence,
-// flag or barrier between CTAs: the validity tag travels inside the data.  Three consecutive points of a row (x = 3g,
-// 3g + 1, 3g + 2: core widths are multiples of 3, so a group has one owner) travel as one 32-byte unit of four 64-bit
-// words, each word = 48 payload bits | 16-bit tag, moved by a PAIR of adjacent lanes, 16 bytes each (one st / ld.relaxed.gpu
-// .v2.b64 per lane: a warp instruction covers whole sectors).  The PTX memory model treats a vector access as a set of scalar accesses of the element
-// type in unspecified order; every 64-bit element is single-copy atomic and carries its own tag, so a reader that finds the
-// tag of the round it waits for in all four words holds that round's three values, however the four were ordered or
-// torn.  At a given location a reader can only ever find the round it waits for or the one two rounds earlier (two buffers
-// alternate by round parity: a tile writes round r + 1 only after it has received round r from every neighbour, and a
-// neighbour posts round r only after it has consumed round r - 1), so 16-bit tags 1 + r mod 65535 never alias; 0 = never
-// valid (freshly cleared buffers).  The exchange is cooperative and coalesced: the threads copy the micro-tile rows that hold
-// strip points into a shared-memory image of the tile (row-major), then ALL threads of the CTA store the strip units
-// (consecutive lane pairs = consecutive units) and fetch the ring units the same way, as asynchronous 16-byte copies into a
-// landing zone, all of a thread's slots in flight together (a half that does not carry the tag yet is polled by one lane
-// of the warp), unpack them into the image, and the rows that hold ring points are read back.  Which unit a pair moves is
-// precomputed once per plan (k_build_tables) and copied to shared memory at launch.
+// Halo exchange, register to register: every T sweeps (2T half-sweeps, each of which invalidates one more ring of the halo),
+// after the last sweep of a stage, and once per stage for the new vorticity, the CTAs refresh their halos through L2 WITHOUT
+// any fence, flag or barrier between CTAs: the validity tag travels inside the data.  A unit is four consecutive points of a
+// grid row, x = 4k - 3 .. 4k: core boundaries in x and tile origins are unit boundaries, so a unit is exactly the four columns
+// one lane holds of that row, in the owner tile and in every tile that has it in its halo.  It travels as five 64-bit words,
+// each carrying a 12-bit tag (word i < 4: the double with the low 12 mantissa bits replaced by the tag; word 4: the four
+// displaced pieces and the tag), stored in three planes of 16 + 16 + 8 bytes per unit so that the three accesses of a warp
+// cover whole sectors (st / ld.relaxed.gpu.global.v2.b64 and .b64).  The PTX memory model treats a vector access as a set of
+// scalar accesses of the element type; every 64-bit element is single-copy atomic and carries its own tag, so a reader that
+// finds the tag it waits for in all five words holds that round's four values, however they were ordered or torn.  At a given
+// location a reader can only ever find the round it waits for or the one two rounds earlier (two buffers alternate by round
+// parity: a tile writes round r + 1 only after it has received round r from every neighbour, and a neighbour posts round r
+// only after it has consumed round r - 1), so tags 1 + r mod 4095 never alias; 0 = never valid (freshly cleared buffers).
+// A thread stores the rows of its micro-tile that lie in the border strips of the core straight from its psi registers,
+// polls the last word of its last ring row until the neighbour's data is there, and loads its ring rows straight into the
+// registers they replace: no shared memory, no table, no barrier inside the exchange (xchg_setup, xchg_units).
 //
 // NEXT-1 (KIND = 1): the same kernel runs the paper's own compact 9-point operator, relaxed in four colours (colour_pass):
 // four passes per sweep, halo 4T, right-hand side qB from the image of omega including the wall vorticity.
 //
-// a2 + a3 in the tile.  After the last sweep of a stage and one more psi exchange the tile holds psi on core + halo; the
-// stage input vorticity of the core is re-read from the tile's own global buffer into the shared-memory image, its first
-// ring comes from a small shared-memory copy kept since the vorticity exchange of the previous stage, the wall values next
-// to the core are Thom's formula applied to the adjacent psi (which also goes to the ring of the stage output in global
-// memory, G16).  Each thread evaluates eq 8 / 22 and the stage combination for its core points, stores them to the global
-// stage buffer (pointwise operands of later stages are read back from there by the same tile), the new vorticity is then
-// exchanged like psi and scaled into q for the next stage's sweeps.
+// a2 + a3 in the tile.  The shared-memory image of the tile keeps the vorticity of core + halo from one stage to the next (the
+// psi rounds never touch it; at launch it is loaded from omega^n).  After the last sweep of a stage and one more psi exchange
+// the wall values next to the core are Thom's formula applied to the adjacent psi (which also goes to the ring of the stage
+// output in global memory, G16); each thread evaluates eq 8 / 22 and the stage combination for its core points from the image,
+// stores them to the global stage buffer (pointwise operands of later stages are read back from there by the same tile), the
+// new vorticity is exchanged like psi, written into the image, and scaled into q for the next stage's sweeps.
 //
 // The kernel reads psi_in and writes psi_out (the API ping-pongs two fields), so no tile ever overwrites input a
 // neighbour has not loaded yet.
