@@ -447,8 +447,10 @@ __device__ __forceinline__ void run_sweeps(double (&p)[R][C], const double (&q)[
         return;
     }
     // the masks of half_sweep (CLS, CLSY), once per round: two registers each while the sweeps run
-    const double m = (CLS != 0 && (fl & FL_MASK)) ? 0.0 : 1.0;
-    const double mb = (CLSY != 0 && (fl & FL_MASKB)) ? 0.0 : 1.0;
+    double m = (CLS != 0 && (fl & FL_MASK)) ? 0.0 : 1.0;
+    double mb = (CLSY != 0 && (fl & FL_MASKB)) ? 0.0 : 1.0;
+    if (CLS != 0) asm volatile("" : "+d"(m));          // opaque: kept in two registers, not recomputed from the flags in every half-sweep
+    if (CLSY != 0) asm volatile("" : "+d"(mb));
     if (odd_origin) {
         for (int s = ns; s > 0; --s) {                                     // red = (i + j) even first (G9): local colour 1 here
             half_sweep<C, R, 1, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl, m, mb);
