@@ -356,9 +356,11 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
 // (the expression of k_compact_colour).  From the other threads a pass needs ONE side column (the lane to the left if KX == 0, to
 // the right if KX == 1: six doubles by shuffle) and ONE edge row of five values (the warp below if KY == 0, above if KY == 1: the
 // edge arrays, whose neighbouring lane slots give the two diagonal values).
-template <int C, int R, int KX, int KY, bool FIX, int TOPOFF, int WC>
+// CLS / CLSY and the masks m / mb as in half_sweep: the wall terms are masked inside the pair sums of se and sc.
+template <int C, int R, int KX, int KY, bool FIX, int TOPOFF, int CLS, int CLSY>
 __device__ __forceinline__ void colour_pass(double (&p)[R][C], const double (&q)[R][C], const double c9e, const double c9c, const double omb,
-                                            double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl_) {
+                                            double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl_, const double m,
+                                            const double mb) {
     static_assert(C == 4 && R == 6 && CAV_QROWS <= 2, "written for the 4 x 6 micro-tile with q of at most two middle rows in shared memory");
     constexpr int QR = CAV_QROWS, Q0 = (R - QR) / 2;
     // the row of parity KY whose q lives in shared memory (-1: none), and which of the QR arrays holds it
@@ -375,20 +377,20 @@ __device__ __forceinline__ void colour_pass(double (&p)[R][C], const double (&q)
         for (int c = 0; c < C; ++c) edge[1 + c] = er[c * 32];
         if (KX == 0) {
             const double v = er[(C - 1) * 32 - 1];                  // column C - 1 of the lane to the left
-            edge[0] = (fl & FL_ZERO_LEFT) ? 0.0 : v;
+            edge[0] = v;
         } else {
             const double v = er[1];                                 // column 0 of the lane to the right
-            edge[C + 1] = (fl & FL_ZERO_RIGHT) ? 0.0 : v;
+            edge[C + 1] = v;
         }
     }
 #pragma unroll
     for (int rj = 0; rj < R; ++rj) {
         if (KX == 0) {
             const double v = __shfl_up_sync(0xffffffffu, p[rj][C - 1], 1);
-            side[rj] = (fl & FL_ZERO_LEFT) ? 0.0 : v;
+            side[rj] = v;
         } else {
             const double v = __shfl_down_sync(0xffffffffu, p[rj][0], 1);
-            side[rj] = (fl & FL_ZERO_RIGHT) ? 0.0 : v;
+            side[rj] = v;
         }
     }
     // value at (column c, row r) around the micro-tile, c in -1 .. C, r in -1 .. R (only what this colour needs is ever asked for)
@@ -397,15 +399,24 @@ __device__ __forceinline__ void colour_pass(double (&p)[R][C], const double (&q)
         if (r < 0 || r >= R) x = edge[1 + c];
         else if (c < 0 || c >= C) x = side[r];
         else x = p[r][c];
-        if (WC > 0 && c == WC && (fl & FL_WALL_LANE)) x = 0.0;         // the wall x = N inside this lane
         return x;
+    };
+    // a + b of the columns ci - 1 and ci + 1, one of which may be a wall column that must read +0.0 in the flagged lane
+    auto xpair = [&](const int ci, const double a, const double b) -> double {
+        if (CLS == 1 && ci == 0) return fma(m, a, b);
+        if ((CLS == 2 && ci == C - 1) || (CLS >= 3 && ci == CLS - 3)) return fma(m, b, a);
+        return a + b;
     };
 #pragma unroll
     for (int rj = KY; rj < R; rj += 2) {
 #pragma unroll
         for (int ci = KX; ci < C; ci += 2) {
-            const double se = (at(ci - 1, rj) + at(ci + 1, rj)) + (at(ci, rj - 1) + at(ci, rj + 1));
-            const double sc = (at(ci - 1, rj - 1) + at(ci + 1, rj - 1)) + (at(ci - 1, rj + 1) + at(ci + 1, rj + 1));
+            const bool wy = CLSY == 1 && rj == 1;                       // row 0 of the flagged warp is the wall y = 0
+            const double we = xpair(ci, at(ci - 1, rj), at(ci + 1, rj));
+            const double sn = wy ? fma(mb, at(ci, rj - 1), at(ci, rj + 1)) : at(ci, rj - 1) + at(ci, rj + 1);
+            const double se = we + sn;
+            const double d1 = xpair(ci, at(ci - 1, rj - 1), at(ci + 1, rj - 1)), d2 = xpair(ci, at(ci - 1, rj + 1), at(ci + 1, rj + 1));
+            const double sc = wy ? fma(mb, d1, d2) : d1 + d2;
             const double qv = (rj == QROW) ? qs[ci] : q[rj][ci];
             p[rj][ci] = fma(omb, p[rj][ci], fma(c9e, se, fma(c9c, sc, qv)));
         }
@@ -433,24 +444,24 @@ template <int C, int R, bool FIX, int TOPOFF, int KIND, int CLS, int CLSY>
 __device__ __forceinline__ void run_sweeps(double (&p)[R][C], const double (&q)[R][C], const double cb, const double omb, const double c9e,
                                            const double c9c, double* __restrict__ sB, const unsigned int wallmask, const unsigned int fl, const int ns,
                                            const bool odd_origin, const int par9) {
-    if (KIND == 1) {
-        // four colours (i mod 2, j mod 2) in the order (0,0), (1,0), (0,1), (1,1) (reading N1); local colour = global ^ origin parity
-        for (int s = ns; s > 0; --s)
-            for (int g = 0; g < 4; ++g) {
-                switch (g ^ par9) {
-                    case 0: colour_pass<C, R, 0, 0, FIX, TOPOFF, (CLS >= 3 ? CLS - 2 : 0)>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
-                    case 1: colour_pass<C, R, 1, 0, FIX, TOPOFF, (CLS >= 3 ? CLS - 2 : 0)>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
-                    case 2: colour_pass<C, R, 0, 1, FIX, TOPOFF, (CLS >= 3 ? CLS - 2 : 0)>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
-                    default: colour_pass<C, R, 1, 1, FIX, TOPOFF, (CLS >= 3 ? CLS - 2 : 0)>(p, q, c9e, c9c, omb, sB, wallmask, fl); break;
-                }
-            }
-        return;
-    }
     // the masks of half_sweep (CLS, CLSY), once per round: two registers each while the sweeps run
     double m = (CLS != 0 && (fl & FL_MASK)) ? 0.0 : 1.0;
     double mb = (CLSY != 0 && (fl & FL_MASKB)) ? 0.0 : 1.0;
     if (CLS != 0) asm volatile("" : "+d"(m));          // opaque: kept in two registers, not recomputed from the flags in every half-sweep
     if (CLSY != 0) asm volatile("" : "+d"(mb));
+    if (KIND == 1) {
+        // four colours (i mod 2, j mod 2) in the order (0,0), (1,0), (0,1), (1,1) (reading N1); local colour = global ^ origin parity
+        for (int s = ns; s > 0; --s)
+            for (int g = 0; g < 4; ++g) {
+                switch (g ^ par9) {
+                    case 0: colour_pass<C, R, 0, 0, FIX, TOPOFF, CLS, CLSY>(p, q, c9e, c9c, omb, sB, wallmask, fl, m, mb); break;
+                    case 1: colour_pass<C, R, 1, 0, FIX, TOPOFF, CLS, CLSY>(p, q, c9e, c9c, omb, sB, wallmask, fl, m, mb); break;
+                    case 2: colour_pass<C, R, 0, 1, FIX, TOPOFF, CLS, CLSY>(p, q, c9e, c9c, omb, sB, wallmask, fl, m, mb); break;
+                    default: colour_pass<C, R, 1, 1, FIX, TOPOFF, CLS, CLSY>(p, q, c9e, c9c, omb, sB, wallmask, fl, m, mb); break;
+                }
+            }
+        return;
+    }
     if (odd_origin) {
         for (int s = ns; s > 0; --s) {                                     // red = (i + j) even first (G9): local colour 1 here
             half_sweep<C, R, 1, FIX, TOPOFF, CLS, CLSY>(p, q, cb, omb, sB, wallmask, fl, m, mb);
@@ -1007,7 +1018,7 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
                 // parameters only: a uniform branch, like the colour order
                 const int cls = (int)blockIdx.x == 0 ? 1 : (((int)blockIdx.x == a.ntx - 1) ? 2 + ((a.N - 1) & 3) : 0);
                 const int ns = min(a.T, rem);
-                if (KIND == 0 && (int)blockIdx.y == 0 && a.EB > 0) {       // bot_in tiles (uniform branch)
+                if ((int)blockIdx.y == 0 && a.EB > 0) {       // bot_in tiles (uniform branch)
                     switch (cls) {
                         case 0: run_sweeps<C, R, FIX, TOPOFF, KIND, 0, 1>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
                         case 1: run_sweeps<C, R, FIX, TOPOFF, KIND, 1, 1>(p, q, a.cb, a.omb, a.c9e, a.c9c, sB, wallmask, fl, ns, odd_origin, par9); break;
@@ -1209,8 +1220,8 @@ ResidentPlan resident_plan_for(int N, int kind, int T_override, int variant_over
                 if (!split_x(N, W, v.C - 1, halo, CW, ntx)) continue;
                 int EB = 0;
                 bool okY = split(G, H, v.R - 1, halo, CH, nty) && ntx * nty <= sms * per_sm;
-                if (!okY && kind == 0 && ntx <= sms * per_sm) {
-                    // one row of tiles fewer with the wall y = 0 inside warp 0 of the first row (5-point sweeps only)
+                if (!okY && ntx <= sms * per_sm) {
+                    // one row of tiles fewer with the wall y = 0 inside warp 0 of the first row
                     for (nty = 3; nty * ntx <= sms * per_sm && !okY; ++nty) okY = split_wb(G, H, v.R, halo, nty, CH, EB);
                     if (okY) --nty;
                 }
