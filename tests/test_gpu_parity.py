@@ -420,3 +420,32 @@ def test_tag_epoch_restart_near_wrap(cav, epoch):
     assert np.isfinite(gp).all() and np.isfinite(gw).all() and np.abs(gp).max() > 0
     assert np.array_equal(gp, sp) and np.array_equal(gw, sw)
     g.close(); s.close()
+
+
+@pytest.mark.parametrize("N", [1021, 1022, 1023, 1024])
+def test_wall_column_classes_and_first_row_extension_bit_exact(cav, orc, N):
+    """(N - 1) mod 4 = 0 .. 3 puts the wall x = N into column 0 .. 3 of a lane of the last column of tiles (four sweep-loop
+    classes, masked pair sums), and the planner's own plan at these sizes keeps the wall y = 0 inside warp 0 of the first row of
+    tiles (EB > 0, T = 6).  Sweeps alone and one whole time step against the FMA-mode oracle, bit for bit; the compact operator
+    (four-colour passes, T = 3, same geometry) likewise."""
+    rc, plan, counts = cav.plan_check(N, "redblack")
+    assert rc == 0 and plan["EB"] > 0 and plan["T"] == 6
+    psi0, w0 = random_fields(N, 4242 + N)
+    for sweep, beta, S in (("redblack", 1.9, 7), ("compact9", 0.8, 4)):
+        g = cav.Cavity(N, 5000.0, 0.4 / N, beta, S, engine="resident")
+        o = orc.OracleCavity(N, 5000.0, 0.4 / N, beta, S, orc.MODE_FMA)
+        if sweep == "compact9":
+            g.set_sweep("compact9")
+            o.set_sweep(orc.SWEEP_COMPACT9)
+        assert "core + halo 12" in g.describe(), g.describe()
+        g.set_fields(psi0, w0)
+        o.set_fields(psi0, w0)
+        g.poisson(S + 2)
+        o.poisson(S + 2)
+        assert np.array_equal(g.get_fields()[0], o.get_fields()[0]), (N, sweep, "sweeps")
+        g.step(1)
+        o.step(1)
+        (gp, gw), (op, ow) = g.get_fields(), o.get_fields()
+        assert np.array_equal(gp, op) and np.array_equal(gw, ow), (N, sweep, "step")
+        g.close()
+        o.close()
