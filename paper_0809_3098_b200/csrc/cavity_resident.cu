@@ -179,17 +179,7 @@ __device__ __forceinline__ Unit unit_pack(double d0, double d1, double d2, doubl
     u.w4 = ((unsigned long long)h << 32) | m;
     return u;
 }
-__device__ __forceinline__ bool unit_ok(const Unit& u, unsigned int tag) {
-    const unsigned int x = (((unsigned int)u.w0 ^ tag) | ((unsigned int)u.w1 ^ tag) | ((unsigned int)u.w2 ^ tag) | ((unsigned int)u.w3 ^ tag)) & 0xfffu;
-    return x == 0u && ((unsigned int)(u.w4 >> 48) & 0xfffu) == tag;
-}
-__device__ __forceinline__ void unit_unpack(const Unit& u, double& d0, double& d1, double& d2, double& d3) {
-    const unsigned int m = (unsigned int)u.w4, h = (unsigned int)(u.w4 >> 32);
-    d0 = __hiloint2double((int)(u.w0 >> 32), (int)(((unsigned int)u.w0 & 0xfffff000u) | (m & 0xfffu)));
-    d1 = __hiloint2double((int)(u.w1 >> 32), (int)(((unsigned int)u.w1 & 0xfffff000u) | ((m >> 12) & 0xfffu)));
-    d2 = __hiloint2double((int)(u.w2 >> 32), (int)(((unsigned int)u.w2 & 0xfffff000u) | (m >> 24) | ((h & 0xfu) << 8)));
-    d3 = __hiloint2double((int)(u.w3 >> 32), (int)(((unsigned int)u.w3 & 0xfffff000u) | ((h >> 4) & 0xfffu)));
-}
+// (the receiver checks the tags and puts the displaced bits back in place, in the registers the words were loaded into: xchg_units)
 __device__ __forceinline__ void st_v2(void* p, unsigned long long a, unsigned long long b) {
     asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
 }
@@ -319,9 +309,9 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
         __syncthreads();
 #pragma unroll
         for (int rj = 1; rj < R - 1; ++rj) update_row(rj);
-        return;
-    }
+    } else
 #endif
+    {
 #pragma unroll
     for (int rj = 0; rj < R; ++rj) update_row(rj);
     unsigned int wm = FIX ? wallmask : 0u;
@@ -347,6 +337,7 @@ __device__ __forceinline__ void half_sweep(double (&p)[R][C], const double (&q)[
         if (((ci + R - 1) & 1) == K && (fl & FL_PUB_TOP)) sT[C * 32 + ci * 32] = p[R - 1][ci];
     }
     __syncthreads();
+    }
 }
 
 // NEXT-1: one colour pass of the paper's 4th-order compact 9-point operator (eq 14-21) relaxed in four colours
@@ -794,7 +785,7 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
     {
     const int z = opaque_zero();
     const int ln = (int)threadIdx.x + z, wp = (int)threadIdx.y + z;
-    const int nw = (int)blockDim.y + z, tid_o = wp * 32 + ln, nth_o = nw * 32, H = nw * R;
+    const int nw = (int)blockDim.y + z, tid_o = wp * 32 + ln, H = nw * R;
     const int Ne = a.N + z, pitch = a.pitch;
     const TileGeom te = tile_geom(Ne, a.CW, a.CH, a.EB, a.halo, a.ntx, a.nty, (int)blockIdx.x + z, (int)blockIdx.y + z, C, R, SW, H);
     const int k = stage % 5 + 1;                                    // RK stage 1..5
@@ -971,7 +962,6 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
     double p[R][C], q[R][C];
     unsigned int wallmask = 0;            // wall points that alignment could not isolate (psi = 0 there, eq 23-24)
     {
-        const int H = nwarps * R;
         double* const img = sm + edge_doubles;
         fill_image<C, R>(img, a.psi_in, 0, N + 1, 0, N + 1, t.ox, t.oy, nwarps, N, a.pitch, lane, warp);
         __syncthreads();
