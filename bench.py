@@ -48,7 +48,7 @@ FP64_INSTR_PER_POINT_SWEEP = 5     # 3 DADD + 2 DFMA (DESIGN.md "Canonical arith
 FP64_INSTR_PER_POINT_STAGE = 30    # a2 + a3 ("5 S + 30 fp64 instructions per grid-point-stage")
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE k_resident launch (one time step of config 4) from the ncu --set full
 # capture summarised in profiles/ (cold L2 under ncu); None until that capture exists for the build
-NCU_DRAM_BYTES_PER_STEP_LAUNCH = 47.0e6
+NCU_DRAM_BYTES_PER_STEP_LAUNCH = 43.9e6
 NCU_DRAM_SOURCE = "profiles/r2c_final.md (ncu --set full, one launch = one time step of config 4)"
 
 
