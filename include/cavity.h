@@ -161,6 +161,13 @@ int cav_trace_sweeps(cav_ctx* ctx, int nsweeps, long long* stamps_out, int slots
  * has no resident plan under these figures, CAV_EINVAL for bad arguments or an inconsistent pattern. */
 int cav_plan_check(int N, int sweep, int T, int sms, int smem_bytes, int* plan_out, long long* counts_out);
 
+/* Testing aid, resident engine (no context; current device): the exchange unit of the halo exchange (four doubles as five
+ * 64-bit words, each with a 12-bit tag) as a round trip.  in_host holds nunits x 4 doubles (any bit patterns: NaN payloads, infinities,
+ * denormals, signed zeros); they are packed with `tag` (1 .. 4095), stored and loaded with the accesses of the exchange, validated and
+ * restored on the device into out_host, which must then equal in_host bit for bit.  *bad_out (may be NULL) = units whose five tags did not
+ * validate for `tag`, or validated for a different tag.  Errors: CAV_EINVAL (null pointers, nunits < 1, tag out of range), CAV_ECUDA. */
+int cav_debug_unit_roundtrip(const double* in_host, double* out_host, int nunits, unsigned int tag, int* bad_out);
+
 /* Testing aid, resident engine: sets the host-side count of halo-exchange rounds (the 12-bit tag of a round is 1 + round mod
  * 4095, the buffer round mod 2) and clears the exchange buffers, so that a test can run across the wrap of the tags and of the
  * 32-bit counter.  Neither wrap needs any action in normal use: a reader can only ever meet the round it waits for or the one

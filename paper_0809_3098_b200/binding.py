@@ -17,7 +17,7 @@ _ENGINES = {"auto": ENGINE_AUTO, "stream": ENGINE_STREAM, "resident": ENGINE_RES
 SYMBOLS = ("cav_create", "cav_destroy", "cav_set_fields", "cav_get_fields", "cav_step", "cav_step_async", "cav_sync",
            "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_set_resident_plan", "cav_trace_sweeps", "cav_describe", "cav_launch_count",
            "cav_last_elapsed_ms", "cav_strerror", "cav_set_sweep", "cav_step_res", "cav_run_to_steady", "cav_debug_set_epoch",
-           "cav_measure_fp64_peak", "cav_plan_check")
+           "cav_measure_fp64_peak", "cav_plan_check", "cav_debug_unit_roundtrip")
 
 SWEEP_REDBLACK, SWEEP_JACOBI, SWEEP_COMPACT9 = 0, 1, 2
 _SWEEPS = {"redblack": SWEEP_REDBLACK, "jacobi": SWEEP_JACOBI, "compact9": SWEEP_COMPACT9}
@@ -82,6 +82,7 @@ def lib():
     L.cav_debug_set_epoch.argtypes = [C.c_void_p, C.c_uint]
     L.cav_measure_fp64_peak.argtypes = [C.c_void_p, dp, dp]
     L.cav_plan_check.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
+    L.cav_debug_unit_roundtrip.argtypes = [dp, dp, C.c_int, C.c_uint, C.POINTER(C.c_int)]
     L.cav_strerror.argtypes = [C.c_int]
     L.cav_strerror.restype = C.c_char_p
     _lib = L
@@ -102,6 +103,17 @@ def _field(a, N, name):
     if a.shape != (N + 1, N + 1):
         raise ValueError("%s must have shape (N+1, N+1) = (%d, %d), row j = y index" % (name, N + 1, N + 1))
     return a
+
+
+def unit_roundtrip(values, tag):
+    """Testing aid: values (float64, length a multiple of 4, any bit patterns) through the exchange-unit encoding on the device.
+    Returns (restored values, number of units whose tags did not validate)."""
+    v = np.ascontiguousarray(values, dtype=np.float64)
+    assert v.ndim == 1 and v.size % 4 == 0 and v.size > 0
+    out = np.empty_like(v)
+    bad = C.c_int()
+    _chk(lib().cav_debug_unit_roundtrip(_p(v), _p(out), v.size // 4, int(tag), C.byref(bad)), "cav_debug_unit_roundtrip")
+    return out, bad.value
 
 
 def plan_check(N, sweep="redblack", T=0, sms=148, smem_bytes=232448):

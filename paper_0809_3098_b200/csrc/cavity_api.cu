@@ -551,6 +551,27 @@ CAV_API int cav_plan_check(int N, int sweep, int T, int sms, int smem_bytes, int
     return cavk::resident_check_exchange(pl, N, counts_out) == 0 ? CAV_OK : CAV_EINVAL;
 }
 
+CAV_API int cav_debug_unit_roundtrip(const double* in_host, double* out_host, int nunits, unsigned int tag, int* bad_out) {
+    if (!in_host || !out_host || nunits < 1 || tag < 1u || tag > 4095u) return CAV_EINVAL;
+    const size_t nb = (size_t)nunits * 4 * sizeof(double), sb = (((size_t)nunits * 16 + 255) / 256 * 256) * 2 + (size_t)nunits * 8 + 256;
+    double *din = nullptr, *dout = nullptr;
+    void* scratch = nullptr;
+    unsigned int* bad = nullptr;
+    unsigned int hbad = 0;
+    int rc = CAV_OK;
+    if (cudaMalloc(&din, nb) != cudaSuccess || cudaMalloc(&dout, nb) != cudaSuccess || cudaMalloc(&scratch, sb) != cudaSuccess ||
+        cudaMalloc(&bad, sizeof(unsigned int)) != cudaSuccess) rc = CAV_ECUDA;
+    if (rc == CAV_OK && (cudaMemcpy(din, in_host, nb, cudaMemcpyHostToDevice) != cudaSuccess || cudaMemset(scratch, 0, sb) != cudaSuccess ||
+                         cudaMemset(bad, 0, sizeof(unsigned int)) != cudaSuccess)) rc = CAV_ECUDA;
+    if (rc == CAV_OK && cavk::resident_unit_roundtrip(din, dout, scratch, nunits, tag, bad, 0) < 0) rc = CAV_ECUDA;
+    if (rc == CAV_OK && (cudaMemcpy(out_host, dout, nb, cudaMemcpyDeviceToHost) != cudaSuccess ||
+                         cudaMemcpy(&hbad, bad, sizeof(unsigned int), cudaMemcpyDeviceToHost) != cudaSuccess)) rc = CAV_ECUDA;
+    if (rc != CAV_OK) cudaGetLastError();
+    cudaFree(din); cudaFree(dout); cudaFree(scratch); cudaFree(bad);
+    if (bad_out) *bad_out = (int)hbad;
+    return rc;
+}
+
 CAV_API int cav_debug_set_epoch(cav_ctx* c, unsigned int epoch) {
     if (!c) return CAV_EINVAL;
     DeviceGuard dg(c->device);

@@ -179,7 +179,21 @@ __device__ __forceinline__ Unit unit_pack(double d0, double d1, double d2, doubl
     u.w4 = ((unsigned long long)h << 32) | m;
     return u;
 }
-// (the receiver checks the tags and puts the displaced bits back in place, in the registers the words were loaded into: xchg_units)
+// The receiver loads words 0-3 into the very registers of the doubles they replace and word 4 beside them: do all five carry the tag?
+__device__ __forceinline__ bool unit_tags_ok(const double d0, const double d1, const double d2, const double d3, const unsigned long long w4,
+                                             const unsigned int tag) {
+    const unsigned int tg = (((unsigned int)__double2loint(d0) ^ tag) | ((unsigned int)__double2loint(d1) ^ tag) |
+                             ((unsigned int)__double2loint(d2) ^ tag) | ((unsigned int)__double2loint(d3) ^ tag)) & 0xfffu;
+    return tg == 0u && ((unsigned int)(w4 >> 48) & 0xfffu) == tag;
+}
+// ... and the displaced 12-bit pieces go back in place: only the low word of each double changes
+__device__ __forceinline__ void unit_restore(double& d0, double& d1, double& d2, double& d3, const unsigned long long w4) {
+    const unsigned int m = (unsigned int)w4, h = (unsigned int)(w4 >> 32);
+    d0 = __hiloint2double(__double2hiint(d0), (int)(((unsigned int)__double2loint(d0) & 0xfffff000u) | (m & 0xfffu)));
+    d1 = __hiloint2double(__double2hiint(d1), (int)(((unsigned int)__double2loint(d1) & 0xfffff000u) | ((m >> 12) & 0xfffu)));
+    d2 = __hiloint2double(__double2hiint(d2), (int)(((unsigned int)__double2loint(d2) & 0xfffff000u) | (m >> 24) | ((h & 0xfu) << 8)));
+    d3 = __hiloint2double(__double2hiint(d3), (int)(((unsigned int)__double2loint(d3) & 0xfffff000u) | ((h >> 4) & 0xfffu)));
+}
 __device__ __forceinline__ void st_v2(void* p, unsigned long long a, unsigned long long b) {
     asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
 }
@@ -589,16 +603,9 @@ __device__ __forceinline__ void xchg_units(double (&v)[R][C], char* __restrict__
             for (int j = 0; j < RB; ++j) {
                 const int rj = b0 + j;
                 double& d0 = v[rj][0]; double& d1 = v[rj][1]; double& d2 = v[rj][2]; double& d3 = v[rj][3];
-                const unsigned int tg = (((unsigned int)__double2loint(d0) ^ tag) | ((unsigned int)__double2loint(d1) ^ tag) |
-                                         ((unsigned int)__double2loint(d2) ^ tag) | ((unsigned int)__double2loint(d3) ^ tag)) & 0xfffu;
-                const unsigned int m = (unsigned int)w4[j], h = (unsigned int)(w4[j] >> 32);
-                if (((pending >> rj) & 1u) && tg == 0u && ((h >> 16) & 0xfffu) == tag) {
+                if (((pending >> rj) & 1u) && unit_tags_ok(d0, d1, d2, d3, w4[j], tag)) {
                     pending &= ~(1u << rj);
-                    // in place: only the low word of each double changes
-                    d0 = __hiloint2double(__double2hiint(d0), (int)(((unsigned int)__double2loint(d0) & 0xfffff000u) | (m & 0xfffu)));
-                    d1 = __hiloint2double(__double2hiint(d1), (int)(((unsigned int)__double2loint(d1) & 0xfffff000u) | ((m >> 12) & 0xfffu)));
-                    d2 = __hiloint2double(__double2hiint(d2), (int)(((unsigned int)__double2loint(d2) & 0xfffff000u) | (m >> 24) | ((h & 0xfu) << 8)));
-                    d3 = __hiloint2double(__double2hiint(d3), (int)(((unsigned int)__double2loint(d3) & 0xfffff000u) | ((h >> 4) & 0xfffu)));
+                    unit_restore(d0, d1, d2, d3, w4[j]);
                 }
             }
         }
@@ -1199,7 +1206,35 @@ bool split_x(int N, int L, int lead, int h, int& core, int& n) {
     return false;
 }
 
+// Testing aid (cav_debug_unit_roundtrip): every thread packs four doubles into a unit with the given tag, stores it to the three planes
+// with the accesses of the exchange, loads it back the way the receiver does, checks the tags and restores the doubles.
+__global__ void k_unit_roundtrip(const double* __restrict__ in, double* __restrict__ out, char* __restrict__ xb, const size_t p1off,
+                                 const size_t p2off, const int nunits, const unsigned int tag, unsigned int* __restrict__ bad) {
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= nunits) return;
+    const Unit w = unit_pack(in[4 * u], in[4 * u + 1], in[4 * u + 2], in[4 * u + 3], tag);
+    st_v2(xb + 16 * (size_t)u, w.w0, w.w1);
+    st_v2(xb + p1off + 16 * (size_t)u, w.w2, w.w3);
+    st_b64(xb + p2off + 8 * (size_t)u, w.w4);
+    double d0 = 0.0, d1 = 0.0, d2 = 0.0, d3 = 0.0;
+    unsigned long long w4 = 0ull;
+    ld_v2_if(1, xb + 16 * (size_t)u, d0, d1);
+    ld_v2_if(1, xb + p1off + 16 * (size_t)u, d2, d3);
+    ld_b64_if(1, xb + p2off + 8 * (size_t)u, w4);
+    if (!unit_tags_ok(d0, d1, d2, d3, w4, tag) || unit_tags_ok(d0, d1, d2, d3, w4, tag == 1u ? 2u : tag - 1u)) atomicAdd(bad, 1u);
+    unit_restore(d0, d1, d2, d3, w4);
+    out[4 * u] = d0; out[4 * u + 1] = d1; out[4 * u + 2] = d2; out[4 * u + 3] = d3;
+}
+
 }  // namespace
+
+int resident_unit_roundtrip(const double* in_dev, double* out_dev, void* scratch_dev, int nunits, unsigned int tag, unsigned int* bad_dev,
+                             cudaStream_t st) {
+    const size_t p1 = ((size_t)nunits * 16 + 255) / 256 * 256;
+    k_unit_roundtrip<<<(nunits + 255) / 256, 256, 0, st>>>(in_dev, out_dev, (char*)scratch_dev, p1, 2 * p1, nunits, tag, bad_dev);
+    const cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? 1 : -(int)e;
+}
 
 ResidentPlan resident_plan_for(int N, int kind, int T_override, int variant_override, int sms, int smem_cap, int regs_per_block) {
     ResidentPlan best;

@@ -38,6 +38,10 @@ ResidentPlan resident_plan_for(int N, int kind, int T_override, int variant_over
 // Host-side check of a plan's exchange pattern (every fetched unit stored by exactly one tile, every stored unit fetched);
 // counts[5]: fetched, stored, unmatched fetches / double stores, stores nobody fetches, tiles that do not fit.  0 = consistent.
 int resident_check_exchange(const ResidentPlan& plan, int N, long long* counts);
+// Testing aid: packs nunits x 4 doubles into exchange units with `tag`, moves them through scratch_dev (>= 48 nunits + 512 bytes) with the
+// accesses of the exchange, and restores them into out_dev; *bad_dev counts units whose tags did not validate (or validated for another tag).
+int resident_unit_roundtrip(const double* in_dev, double* out_dev, void* scratch_dev, int nunits, unsigned int tag, unsigned int* bad_dev,
+                            cudaStream_t st);
 int resident_variants();
 void resident_describe(const ResidentPlan& plan, char* buf, int len);
 
