@@ -814,3 +814,43 @@ def test_under_relaxation_slows_convergence_monotonically():
     target = compact_ratio(N, 1, 1) * w
     left = [np.max(np.abs(oracle.compact_lex(N, b, np.zeros_like(w), w, 100) - target)) for b in (0.8, 0.5, 0.3, 0.1)]
     assert left[0] < left[1] < left[2] < left[3]
+
+
+# ---- the composition of orc_poisson (SURVEY S8(b) "poisson": nsweeps of a1, THEN one a2; eq 25) ----
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("kind,beta", [(oracle.SWEEP_REDBLACK, 1.7), (oracle.SWEEP_JACOBI, 0.9), (oracle.SWEEP_COMPACT9, 0.8)])
+@pytest.mark.parametrize("nsweeps", [0, 1, 7])
+def test_poisson_is_the_sweeps_then_thom_of_the_swept_psi(mode, kind, beta, nsweeps):
+    # Pins the ORDER and the presence of the trailing a2 (a Thom pass before the sweeps, or none at all, must fail here):
+    #   psi after   = the operator-level sweeps (pinned above by closed forms) of psi0 with the vorticity AS GIVEN, ring included
+    #                 (the compact operator's B term reads that ring: an early Thom pass would change psi itself);
+    #   omega ring  = Thom's formula of THAT psi, by the oracle's own a2 and, to rounding, typed out here from eq 25;
+    #   omega interior untouched;  return value = the max-norm residual of the returned state.
+    N, U = 13, 1.0
+    h = 1.0 / N
+    rng = np.random.default_rng(100 * kind + 10 * mode + nsweeps)
+    psi0 = rng.standard_normal((N + 1, N + 1))
+    psi0[0] = psi0[-1] = 0.0; psi0[:, 0] = psi0[:, -1] = 0.0
+    w0 = 5.0 * rng.standard_normal((N + 1, N + 1))            # random ring as well
+    o = oracle.OracleCavity(N, 100.0, 1e-3, beta, 3, mode)
+    o.set_sweep(kind)
+    o.set_fields(psi0, w0)
+    ret = o.poisson(nsweeps)
+    psi, w = o.get_fields()
+    res_inf = o.diag()["res_inf"]
+    o.close()
+    sweeps = {oracle.SWEEP_REDBLACK: oracle.sor, oracle.SWEEP_JACOBI: oracle.jacobi, oracle.SWEEP_COMPACT9: oracle.compact}[kind]
+    assert np.array_equal(psi, sweeps(N, beta, psi0, w0, nsweeps, mode))
+    assert np.array_equal(w, oracle.thom(N, U, psi, w0, mode))
+    assert np.array_equal(w[1:-1, 1:-1], w0[1:-1, 1:-1])
+    # eq 25 typed out: omega_wall = -2 psi_adjacent / h^2, minus 2U/h on the lid; the top and bottom rows own the corners (G10)
+    ring = w0.copy()
+    ring[1:-1, 0] = -2.0 * psi[1:-1, 1] / h**2
+    ring[1:-1, -1] = -2.0 * psi[1:-1, -2] / h**2
+    ring[0, :] = -2.0 * psi[1, :] / h**2
+    ring[-1, :] = -2.0 * psi[-2, :] / h**2 - 2.0 * U / h
+    assert np.allclose(w, ring, rtol=1e-13, atol=1e-12)
+    assert np.max(np.abs(w[0] - w0[0])) > 1.0 and np.max(np.abs(w[-1] - w0[-1])) > 1.0     # the ring did change
+    assert ret == res_inf
+    lap = (psi[1:-1, :-2] + psi[1:-1, 2:] + psi[:-2, 1:-1] + psi[2:, 1:-1] - 4.0 * psi[1:-1, 1:-1]) / h**2
+    assert abs(ret - np.max(np.abs(lap + w[1:-1, 1:-1]))) <= 1e-10 * ret
