@@ -39,6 +39,7 @@ extern "C" {
 #define CAV_ENOMEM  (-2)   /* host or device allocation failed */
 #define CAV_ECUDA   (-3)   /* CUDA runtime error, or no usable device */
 #define CAV_ENOTSUP (-4)   /* requested engine cannot run this problem on this device */
+#define CAV_ELIMIT  (-5)   /* problem larger than a fixed-size buffer of the library (cav_diag_noalloc: N > CAV_NOALLOC_MAX_N) */
 
 /* Sweep engines (all compute the same red-black SOR, bit for bit; they differ in how it is scheduled). */
 #define CAV_ENGINE_AUTO     0   /* pick by grid size (default) */
@@ -191,6 +192,46 @@ long long cav_launch_count(cav_ctx* ctx);
  * sweeps alone, without the a2 pass and the residual) on the context's stream (events recorded around the enqueued
  * work); blocks until that work has finished.  Writes 0 if none has run. */
 int cav_last_elapsed_ms(cav_ctx* ctx, float* ms_out);
+
+/* ---- The one entry point that allocates nothing -------------------------------------------------------------------------
+ *
+ * Every call above works on a context, and cav_create takes its fields and work buffers from PyTorch's caching allocator.
+ * That rules the library out for callers that may not allocate device memory at the moment they need a number from it:
+ * a thread that runs while some stream of the process is being captured in the global capture mode (cudaMalloc is refused
+ * there and invalidates the capture), a solver that lives inside a fixed slice of HBM handed out by a host application
+ * (the rest of the GPU belongs to somebody else's pool, so asking the driver for more can fail at any time), and loops that
+ * cannot afford the device-wide synchronisation cudaMalloc / cudaFree imply.  For them:
+ *
+ * cav_diag_noalloc computes the a4 diagnostics (the same four numbers cav_get_diag reports: res_inf, res_l2, kinetic_energy,
+ * enstrophy, in that order; definitions at struct cav_diag) of a state the CALLER holds in device memory, without a context
+ * and without calling cudaMalloc, cudaFree, PyTorch's allocator or any other routine that allocates.
+ *   N          intervals per side, 2 <= N <= CAV_NOALLOC_MAX_N
+ *   pitch      doubles per row of both fields, >= N + 1 (N + 1 for dense arrays; the padded pitch for rows that are padded)
+ *   psi_dev, omega_dev   DEVICE pointers, (N + 1) rows of `pitch` doubles, element (i, j) at j * pitch + i; read only.  psi is
+ *              read as given, walls included (cav_set_fields forces them to 0; here that is the caller's business).
+ *   out4_dev   DEVICE pointer to 4 doubles, written by the kernel
+ *   stream     a cudaStream_t passed as a plain pointer (NULL = the default stream) of the CURRENT device, which must be the
+ *              device the three buffers live on.
+ * The call returns once the work is enqueued on `stream`: out4_dev holds the result when the stream has got that far, and
+ * the input buffers must stay untouched until then.  It agrees with cav_get_diag to rounding (the sums are taken in another
+ * order: relative differences of a few 1e-16 per sum), not bit for bit; repeated calls on the same input agree bit for bit.
+ *
+ * The memory it does need (one partial result per grid row, and a counter) is a fixed 256.25 KiB array inside the library's
+ * device image.  Consequences a user must know:
+ *   - LIMIT: N > CAV_NOALLOC_MAX_N (8192) does not fit and is refused with CAV_ELIMIT; nothing is launched.
+ *   - Every GPU on which the library's device code gets loaded carries those 256.25 KiB until the process exits.
+ *   - The array is ONE per device, shared by all calls from all threads and streams.  Two calls whose kernels can overlap on
+ *     the GPU (different streams without an ordering between them) race on it and both results are garbage: order them.
+ *     Calls on one stream are safe back to back; each call clears the counter it needs to start from zero.
+ *   - The FIRST call on each device looks up the array's device address (cudaGetSymbolAddress, which makes the runtime load
+ *     the library's device image there).  Make that first call at start-up, before any stream capture begins.
+ * Errors: CAV_EINVAL (null pointer, N < 2, pitch < N + 1), CAV_ELIMIT (N too large), CAV_ENOTSUP (device ordinal >= 64),
+ * CAV_ECUDA (the runtime refused the lookup, the clear or the launch; CAV_DEBUG=1 prints which). */
+#define CAV_NOALLOC_MAX_N 8192
+int cav_diag_noalloc(int N, int pitch, const double* psi_dev, const double* omega_dev, double* out4_dev, void* stream);
+
+/* CAV_NOALLOC_MAX_N as the loaded library was built with. */
+int cav_noalloc_max_n(void);
 
 /* Static string for an error code. */
 const char* cav_strerror(int code);

@@ -17,7 +17,7 @@ _ENGINES = {"auto": ENGINE_AUTO, "stream": ENGINE_STREAM, "resident": ENGINE_RES
 SYMBOLS = ("cav_create", "cav_destroy", "cav_set_fields", "cav_get_fields", "cav_step", "cav_step_async", "cav_sync",
            "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_set_resident_plan", "cav_trace_sweeps", "cav_describe", "cav_launch_count",
            "cav_last_elapsed_ms", "cav_strerror", "cav_set_sweep", "cav_step_res", "cav_run_to_steady", "cav_debug_set_epoch",
-           "cav_measure_fp64_peak", "cav_plan_check", "cav_debug_unit_roundtrip")
+           "cav_measure_fp64_peak", "cav_plan_check", "cav_debug_unit_roundtrip", "cav_diag_noalloc", "cav_noalloc_max_n")
 
 SWEEP_REDBLACK, SWEEP_JACOBI, SWEEP_COMPACT9 = 0, 1, 2
 _SWEEPS = {"redblack": SWEEP_REDBLACK, "jacobi": SWEEP_JACOBI, "compact9": SWEEP_COMPACT9}
@@ -83,6 +83,8 @@ def lib():
     L.cav_measure_fp64_peak.argtypes = [C.c_void_p, dp, dp]
     L.cav_plan_check.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
     L.cav_debug_unit_roundtrip.argtypes = [dp, dp, C.c_int, C.c_uint, C.POINTER(C.c_int)]
+    L.cav_diag_noalloc.argtypes = [C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.cav_noalloc_max_n.argtypes = []
     L.cav_strerror.argtypes = [C.c_int]
     L.cav_strerror.restype = C.c_char_p
     _lib = L
@@ -114,6 +116,24 @@ def unit_roundtrip(values, tag):
     bad = C.c_int()
     _chk(lib().cav_debug_unit_roundtrip(_p(v), _p(out), v.size // 4, int(tag), C.byref(bad)), "cav_debug_unit_roundtrip")
     return out, bad.value
+
+
+def noalloc_max_n():
+    """Largest N cav_diag_noalloc accepts (its scratch is a fixed array inside the library)."""
+    return int(lib().cav_noalloc_max_n())
+
+
+def diag_noalloc(N, psi_dev, omega_dev, out4_dev, pitch=None, stream=0):
+    """cav_diag_noalloc: the a4 diagnostics of fields the caller holds on the device, for callers that may not allocate device
+    memory (no context, no cudaMalloc, no PyTorch allocator; see include/cavity.h for who that is and for the limits).
+    psi_dev, omega_dev, out4_dev: device addresses (int) or objects with data_ptr() (torch CUDA tensors of float64); pitch =
+    doubles per row (default N + 1: dense); stream = a cudaStream_t as an int (0 = default stream).  Only enqueues: out4_dev
+    (res_inf, res_l2, kinetic_energy, enstrophy) is valid once the stream has run that far.  Calls that can overlap on the GPU
+    race on the library's one scratch array; the first call on a device should precede any stream capture."""
+    def addr(x):
+        return C.c_void_p(int(x.data_ptr()) if hasattr(x, "data_ptr") else int(x))
+    _chk(lib().cav_diag_noalloc(int(N), int(N + 1 if pitch is None else pitch), addr(psi_dev), addr(omega_dev), addr(out4_dev),
+                                C.c_void_p(int(stream))), "cav_diag_noalloc")
 
 
 def plan_check(N, sweep="redblack", T=0, sms=148, smem_bytes=232448):

@@ -647,6 +647,7 @@ CAV_API const char* cav_strerror(int code) {
         case CAV_ENOMEM: return "out of memory";
         case CAV_ECUDA: return "CUDA error or no usable CUDA device";
         case CAV_ENOTSUP: return "engine not supported for this problem on this device";
+        case CAV_ELIMIT: return "problem larger than a fixed-size buffer of the library (cav_diag_noalloc: N > CAV_NOALLOC_MAX_N = 8192)";
         default: return "unknown error";
     }
 }
