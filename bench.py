@@ -404,7 +404,12 @@ def run_ours(args, wl, rank, world, local_rank):
 
 def run_stub(args, wl, rank, world):
     """CAV_BENCH_STUB=1 (tests only, CPU): the launch / rendezvous / combine logic of the N-rank path over gloo with a stubbed
-    step (a sleep of 10 ms x (rank + 1)); prints the same line shape with `"stub": true`.  No kernel runs: never a bench value."""
+    step (a sleep of 10 ms x (rank + 1)); prints a line of the same shape whose metric and unit say STUB and with `"stub": true`.
+    No kernel runs: never a bench value.  Refused (exit 2) outside a pytest run, so a leaked environment variable cannot
+    turn a driver run into a fake number."""
+    if "PYTEST_CURRENT_TEST" not in os.environ:
+        sys.stderr.write("bench.py: CAV_BENCH_STUB=1 is honoured only inside a pytest run; unset it\n")
+        raise SystemExit(2)
     import torch
     import torch.distributed as dist
     from paper_0809_3098_b200 import replicas
@@ -418,7 +423,7 @@ def run_stub(args, wl, rank, world):
     t_local = time.perf_counter() - t0
     units, t_max = replicas.combine(5.0 * (wl.N + 1) ** 2 * K, t_local, world, dist if world > 1 else None, torch.device("cpu"))
     if rank == 0:
-        print(json.dumps({"metric": METRIC, "value": units / t_max, "unit": UNIT, "n_gpus": world, "steps": K, "stub": True,
+        print(json.dumps({"metric": "STUB: no kernel ran, not a measurement", "value": units / t_max, "unit": "stub units/s", "n_gpus": world, "steps": K, "stub": True,
                           "ms_per_step": 1e3 * t_max / K, "config": {"workload": wl.name}}), flush=True)
     if world > 1:
         dist.destroy_process_group()

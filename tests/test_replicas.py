@@ -75,6 +75,11 @@ def test_bench_spawns_its_own_ranks_when_no_launcher_set_the_world():
     assert len(lines) == 1, out.stdout
     d = json.loads(lines[0])
     assert d["n_gpus"] == 2 and d["stub"] is True
+    assert "STUB" in d["metric"] and "stub" in d["unit"]          # cannot be mistaken for (or harvested as) the real metric
+    env.pop("PYTEST_CURRENT_TEST", None)                           # outside pytest the stub is refused
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "1", "--steps", "1"], env=env,
+                         capture_output=True, text=True, timeout=150)
+    assert out.returncode == 2 and not [l for l in out.stdout.splitlines() if l.startswith("{")]
     # rank 1 sleeps twice as long: the job time is the MAX over ranks, the units are the SUM
     assert 55.0 <= d["ms_per_step"] * 3 <= 400.0
     G = 1025 ** 2
