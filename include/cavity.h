@@ -94,9 +94,18 @@ int cav_get_fields(cav_ctx* ctx, double* psi_out, double* omega_out);
  * and the red-black sweeps the whole call is ONE kernel launch.
  * CAV_ECUDA from this or any later call of a resident-engine context can also mean that a tile of the persistent kernel waited
  * ~10 s for a neighbour's halo and gave up (it cannot happen on a healthy device: all tiles are co-resident; a debugger,
- * time-slicing or a sanitizer can stretch the wait).  The fields are then undefined; the condition is sticky until
- * cav_set_fields, cav_set_engine or cav_set_resident_plan, which clear it.  CAV_DEBUG=1 in the environment prints which
- * tile waited for which unit (and the CUDA error string behind any other CAV_ECUDA) to stderr. */
+ * time-slicing or a sanitizer can stretch the wait).  The fields are then undefined; the condition is sticky (cav_sync,
+ * cav_get_fields, cav_get_diag, cav_poisson, cav_step_res and cav_run_to_steady report it too) until cav_set_fields,
+ * cav_set_engine, cav_set_resident_plan or a cav_set_sweep that plans anew, which clear it.  CAV_DEBUG=1 in the environment
+ * prints which tile waited for which unit (and the CUDA error string behind any other CAV_ECUDA) to stderr.
+ * Two resident-engine contexts of one device must not have launches in flight at the same time: every launch wants all SMs
+ * for its co-resident tiles, so create them under the same stream (they then run one after the other) or cav_sync one before
+ * stepping the other.  A launch queued behind another context's long cav_step(n) on a DIFFERENT stream may start with only
+ * part of its tiles resident and trip the 10 s wait.
+ * Size limit of the resident engine: one tile per SM, tiles of at most 128 x 96 points including halos, so on a 148-SM B200
+ * there is a plan for every N <= 1200 with the 5-point sweeps (compact operator: every N <= 1133 and 1144 <= N <= 1200).
+ * Larger grids run on the streaming engine (10 S + 10 launches per step, several times slower per point); cav_describe
+ * says which engine a context uses. */
 int cav_step(cav_ctx* ctx, int nsteps);
 
 /* As cav_step but returns after enqueueing on the context's stream (no host synchronisation). */
@@ -117,7 +126,9 @@ int cav_poisson(cav_ctx* ctx, int nsweeps, double* res_inf_out);
  * first stage after cav_set_fields: the ring as given; reading N2).  The Jacobi sweeps run as one kernel per sweep
  * over global memory whatever the engine (inside a CUDA graph of the time step).  The compact sweeps run in the resident engine's
  * persistent kernel like the red-black ones (four colour passes per sweep, halo 4T deep; the tiling is planned anew when the
- * sweep kind changes), or, with CAV_ENGINE_STREAM, as four kernels per sweep over global memory; both agree bit for bit. */
+ * sweep kind changes: a T forced with cav_set_resident_plan is kept if the new operator has a plan with it, else dropped
+ * for the planner's own; the exchange buffers start afresh and the sticky error of cav_step is cleared), or, with
+ * CAV_ENGINE_STREAM, as four kernels per sweep over global memory; both agree bit for bit. */
 int cav_set_sweep(cav_ctx* ctx, int kind);
 
 /* One time step, and the paper's steady-state monitors of that step (eq 26-27):

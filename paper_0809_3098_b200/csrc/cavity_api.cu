@@ -50,6 +50,7 @@ struct cav_ctx {
     size_t field_doubles = 0;
     long long step = 0;
     long long launches = 0;
+    int forced_T = 0, forced_variant = -1;   // cav_set_resident_plan's request (0 / -1 = the planner's choice); kept across cav_set_sweep
     int engine_req = CAV_ENGINE_AUTO;
     int engine = CAV_ENGINE_STREAM;  // resolved
     cavk::ResidentPlan plan{};       // valid if plan.ok
@@ -376,7 +377,7 @@ CAV_API int cav_get_fields(cav_ctx* c, double* psi_out, double* omega_out) {
     if (psi_out) CK(cudaMemcpy2DAsync(psi_out, row, c->psi, dp, row, N + 1, cudaMemcpyDeviceToHost, c->st));
     if (omega_out) CK(cudaMemcpy2DAsync(omega_out, row, c->w[0], dp, row, N + 1, cudaMemcpyDeviceToHost, c->st));
     CK(cudaStreamSynchronize(c->st));
-    return CAV_OK;
+    return check_resident_error(c);      // after cav_step_async: fields of a launch whose tile gave up are undefined, say so
 }
 
 CAV_API int cav_step(cav_ctx* c, int nsteps) { return step_impl(c, nsteps, true); }
@@ -422,6 +423,7 @@ CAV_API int cav_get_diag(cav_ctx* c, cav_diag* out) {
     c->launches += nl;
     CK(cudaMemcpyAsync(r, c->out4, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
     CK(cudaStreamSynchronize(c->st));
+    { const int rc = check_resident_error(c); if (rc != CAV_OK) return rc; }
     out->t = (double)c->step * c->dt;
     out->step = c->step;
     out->res_inf = r[0]; out->res_l2 = r[1]; out->kinetic_energy = r[2]; out->enstrophy = r[3];
@@ -436,9 +438,14 @@ CAV_API int cav_set_sweep(cav_ctx* c, int kind) {
         c->sweep = kind;
         drop_graph(c);
         if (kind != CAV_SWEEP_JACOBI && c->plan.kind != plan_kind(kind)) {       // the halo depth per sweep differs: plan anew
-            c->plan = cavk::resident_plan(c->P, c->device, 0, -1, plan_kind(kind));
-            build_plan_buffers(c);
+            c->plan = cavk::resident_plan(c->P, c->device, c->forced_T, c->forced_variant, plan_kind(kind));
+            if (!c->plan.ok && (c->forced_T != 0 || c->forced_variant >= 0)) {   // no plan with the forced T for this operator: the planner's own
+                c->forced_T = 0; c->forced_variant = -1;
+                c->plan = cavk::resident_plan(c->P, c->device, 0, -1, plan_kind(kind));
+            }
+            build_plan_buffers(c);                                               // fresh exchange buffers
             resolve_engine(c);
+            return clear_resident_error(c);
         }
     }
     return CAV_OK;
@@ -513,6 +520,8 @@ CAV_API int cav_set_resident_plan(cav_ctx* c, int sweeps_per_exchange, int varia
     c->plan = pl;
     build_plan_buffers(c);
     if (!c->plan.ok) { c->plan = old; build_plan_buffers(c); resolve_engine(c); return CAV_ENOMEM; }
+    c->forced_T = sweeps_per_exchange;
+    c->forced_variant = variant < 0 ? -1 : variant;
     return clear_resident_error(c);
 }
 
@@ -520,7 +529,7 @@ CAV_API int cav_trace_sweeps(cav_ctx* c, int nsweeps, long long* stamps_out, int
     if (!c || nsweeps < 1 || !stamps_out || slots_per_tile < 2) return CAV_EINVAL;
     DeviceGuard dg(c->device);
     resolve_engine(c);
-    if (!resident_path(c)) return CAV_ENOTSUP;          // the red-black sweeps of the resident engine only
+    if (!resident_path(c) || c->sweep != CAV_SWEEP_REDBLACK) return CAV_ENOTSUP;   // the red-black sweeps of the resident engine only
     const size_t n = (size_t)c->plan.ntiles * (size_t)slots_per_tile;
     long long* dev = (long long*)dev_alloc(c, n * sizeof(long long));
     if (!dev) return CAV_ENOMEM;

@@ -1063,6 +1063,20 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
             }
             ++round;
             mark(a, tslot + 2);
+            if (a.nsteps == 0) {
+                // sweeps-only launches (cav_poisson, cav_trace_sweeps) never reach the once-per-stage reset below: put the
+                // registers of non-interior points back to +0.0 after every exchange round instead (outside the sweep loops)
+                const int z = opaque_zero();
+                const unsigned int dead = reinterpret_cast<const unsigned int*>(sm + edge_doubles + (((int)blockDim.y + z) * R + 1) * SW)
+                                              [2 * ((int)blockDim.y + z) * 32 + ((int)threadIdx.y + z) * 32 + (int)threadIdx.x];
+                if (dead != 0u) {
+#pragma unroll
+                    for (int rj = 0; rj < R; ++rj)
+#pragma unroll
+                        for (int ci = 0; ci < C; ++ci)
+                            if ((dead >> (rj * C + ci)) & 1u) p[rj][ci] = 0.0;
+                }
+            }
             publish_all<C, R, TOPOFF>(p, sB, fl);
             mark(a, tslot + 3);
         }

@@ -47,13 +47,18 @@ def relerr(a, b):
 def engines(cav, N):
     """engines that can run this grid on this device"""
     out = ["stream"]
+    rc, plan, _ = cav.plan_check(N)                  # host logic, B200 figures (148 SMs): is there a resident plan for this grid?
     c = cav.Cavity(N, 100.0, 1e-3, 1.5, 1)
     try:
         c.set_engine("resident")
         out.append("resident")
     except cav.CavityError:
-        pass
-    c.close()
+        # a planner regression must not quietly turn the callers into stream-only tests
+        assert rc != 0, "plan_check(%d) has a resident plan %r but the context refuses the resident engine" % (N, plan)
+    finally:
+        c.close()
+    if rc == 0:
+        assert "resident" in out
     return out
 
 
@@ -394,7 +399,7 @@ def test_trace_sweeps_reports_ordered_phases(cav):
     ref.set_fields(*W.initial_fields(wl))
     st = g.trace_sweeps(23, slots_per_tile=2 + 4 * 8)
     ref.poisson(23)
-    assert st.shape[0] == 140 or st.shape[0] > 1                     # one row of stamps per tile
+    assert st.shape[0] == 140                                        # one row of stamps per tile: 10 x 14 tiles at N = 1024
     used = st[:, :2 + 4 * 4]                                          # T = 5: rounds 0..3 exchange, round 4 is the last
     assert (used[:, 0] > 0).all() and (np.diff(used[:, :2 + 4 * 4], axis=1) >= 0).all()
     # the traced call is a real cav_poisson without the a2 pass: psi agrees with the streaming engine bit for bit
@@ -466,3 +471,97 @@ def test_exchange_unit_encoding_is_lossless_for_any_bit_pattern(cav):
         out, bad = cav.unit_roundtrip(vals, tag)
         assert bad == 0
         assert np.array_equal(out.view(np.uint64), bits), tag
+
+
+# ------------------------------------------------------------------------------------------------------
+# the benchmarked workloads themselves, in the launch configuration bench.py times (auto engine, the planner's own plan, S = 200):
+# full fields after two time steps, element by element against the oracle (a few seconds of one host core per mode)
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("k", [4, 5])
+def test_timed_configurations_direct_against_the_oracle(cav, orc, k):
+    wl = W.config(k)
+    psi0, w0 = W.initial_fields(wl)
+    pre = 200 if k == 5 else 0                       # config 5 starts with Poisson-only sweeps (G14); 200 of its 10 000 here
+    g = cav.Cavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage)
+    assert "engine resident" in g.describe(), g.describe()
+    g.set_fields(psi0, w0)
+    if pre:
+        g.poisson(pre)
+    g.step(2)
+    gp, gw = g.get_fields()
+    g.close()
+    for mode in (orc.MODE_FMA, orc.MODE_PLAIN):
+        o = orc.OracleCavity(wl.N, wl.Re, wl.dt, wl.sor_omega, wl.sweeps_per_stage, mode)
+        o.set_fields(psi0, w0)
+        if pre:
+            o.poisson(pre)
+        o.step(2)
+        op, ow = o.get_fields()
+        o.close()
+        if mode == orc.MODE_FMA:
+            assert np.array_equal(gp, op), (k, np.argwhere(gp != op)[:8])
+            assert np.array_equal(gw, ow), (k, np.argwhere(gw != ow)[:8])
+        else:
+            assert relerr(gp, op) <= TOL and relerr(gw, ow) <= TOL, (k, relerr(gp, op), relerr(gw, ow))
+
+
+# ------------------------------------------------------------------------------------------------------
+# the registers of non-interior points (wall columns, lanes and warps beyond a wall) are swept like live ones and only ever
+# read as 0 * value, so they must stay finite however long a launch sweeps: long sweeps-only launches and long stages at
+# beta -> 2 on plans whose tiles hold masked wall columns, bit for bit against the streaming engine (which has no such registers)
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("sweep,beta", [("redblack", 1.999), ("compact9", 1.999)])
+@pytest.mark.parametrize("N", [1022, 1023])
+def test_long_sweeps_only_launch_keeps_dead_registers_harmless(cav, N, sweep, beta):
+    psi0, w0 = random_fields(N, 4242 + N)
+    out = {}
+    for engine in ("resident", "stream"):
+        g = cav.Cavity(N, 1000.0, 0.4 / N, beta, 10, engine=engine)
+        g.set_sweep(sweep)
+        assert ("engine " + engine) in g.describe()
+        g.set_fields(psi0, w0)
+        res = g.poisson(20000)
+        out[engine] = (g.get_fields(), res)
+        g.close()
+    (rp, rw), rres = out["resident"]
+    (sp, sw_), sres = out["stream"]
+    assert np.all(np.isfinite(rp)) and np.isfinite(rres)
+    assert np.array_equal(rp, sp) and np.array_equal(rw, sw_), (N, sweep, np.argwhere(rp != sp)[:8])
+
+
+@pytest.mark.parametrize("N", [257, 513, 1021, 1024])
+def test_long_stages_near_beta_two_bit_exact(cav, orc, N):
+    S, beta = 1000, 1.999
+    psi0, w0 = random_fields(N, 999 + N)
+    out = {}
+    for engine in ("resident", "stream"):
+        g = cav.Cavity(N, 1000.0, 0.4 / N, beta, S, engine=engine)
+        g.set_fields(psi0, w0)
+        g.step(2)
+        out[engine] = g.get_fields()
+        g.close()
+    assert np.all(np.isfinite(out["resident"][0])) and np.all(np.isfinite(out["resident"][1]))
+    assert np.array_equal(out["resident"][0], out["stream"][0]) and np.array_equal(out["resident"][1], out["stream"][1]), N
+    if N == 257:
+        o = orc.OracleCavity(N, 1000.0, 0.4 / N, beta, S, orc.MODE_FMA)
+        o.set_fields(psi0, w0)
+        o.step(2)
+        op, ow = o.get_fields()
+        o.close()
+        assert np.array_equal(out["resident"][0], op) and np.array_equal(out["resident"][1], ow)
+
+
+def test_set_sweep_keeps_a_forced_exchange_period_and_trace_is_red_black_only(cav):
+    g = cav.Cavity(1024, 1000.0, 1e-4, 0.8, 6)
+    g.set_resident_plan(2)
+    assert "T=2" in g.describe()
+    g.set_sweep("compact9")                      # plans anew (halo 4T per sweep): the forced T survives
+    assert "compact" in g.describe() and "T=2" in g.describe(), g.describe()
+    g.set_fields(*random_fields(1024, 5))
+    with pytest.raises(cav.CavityError) as e:
+        g.trace_sweeps(4)
+    assert e.value.code == -4                    # CAV_ENOTSUP: the trace is of the red-black sweeps only
+    g.set_sweep("redblack")
+    assert "T=2" in g.describe()
+    assert g.trace_sweeps(4, slots_per_tile=2 + 4 * 4).shape[0] > 1
+    g.close()
