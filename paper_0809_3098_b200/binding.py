@@ -13,7 +13,7 @@ import numpy as np
 ENGINE_AUTO, ENGINE_STREAM, ENGINE_RESIDENT = 0, 1, 2
 _ENGINES = {"auto": ENGINE_AUTO, "stream": ENGINE_STREAM, "resident": ENGINE_RESIDENT}
 
-# every symbol include/cavity.h declares
+# every symbol include/cavity.h and include/cavity_debug.h declare
 SYMBOLS = ("cav_create", "cav_destroy", "cav_set_fields", "cav_get_fields", "cav_step", "cav_step_async", "cav_sync",
            "cav_poisson", "cav_get_diag", "cav_set_engine", "cav_set_resident_plan", "cav_trace_sweeps", "cav_describe", "cav_launch_count",
            "cav_last_elapsed_ms", "cav_strerror", "cav_set_sweep", "cav_step_res", "cav_run_to_steady", "cav_debug_set_epoch",
@@ -208,7 +208,7 @@ class Cavity:
         _chk(lib().cav_set_resident_plan(self._h, int(T), int(variant)), "cav_set_resident_plan")
 
     def trace_sweeps(self, nsweeps, slots_per_tile=64):
-        """(ntiles, slots) int64 array of %globaltimer stamps in ns (see include/cavity.h: cav_trace_sweeps)."""
+        """(ntiles, slots) int64 array of %globaltimer stamps in ns (see include/cavity_debug.h: cav_trace_sweeps)."""
         out = np.zeros((1024, slots_per_tile), dtype=np.int64)
         nt = C.c_int()
         _chk(lib().cav_trace_sweeps(self._h, int(nsweeps), out.ctypes.data_as(C.POINTER(C.c_longlong)),

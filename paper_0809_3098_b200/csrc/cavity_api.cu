@@ -1,4 +1,4 @@
-// cavity_api.cu — the C ABI of include/cavity.h: context, step scheduler, host <-> device copies.
+// cavity_api.cu — the C ABI of include/cavity.h and include/cavity_debug.h: context, step scheduler, host <-> device copies.
 //
 // PyTorch is used for exactly two things (BASELINE.json north_star): device memory comes from its CUDA
 // caching allocator and work is enqueued on its current stream.  No ATen operator does any arithmetic;
@@ -19,6 +19,7 @@
 #include <utility>
 
 #include "../../include/cavity.h"
+#include "../../include/cavity_debug.h"
 #include "cavity_kernels.cuh"
 #include "cavity_resident.cuh"
 

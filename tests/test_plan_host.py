@@ -1,4 +1,4 @@
-"""Host logic of the resident engine, no GPU: the tiling planner and the halo-exchange pattern (cav_plan_check, include/cavity.h).
+"""Host logic of the resident engine, no GPU: the tiling planner and the halo-exchange pattern (cav_plan_check, include/cavity_debug.h).
 
 Every unit of four grid points that a tile fetches from its ring must be stored by exactly one tile (the owner of those
 points), every stored unit must be fetched by some neighbour, and every tile must fit its thread grid: a mismatch would
