@@ -372,6 +372,20 @@ def run_ours(args, wl, rank, world, local_rank):
                                                        "GPSU_per_s": 5.0 * (w4.N + 1) ** 2 / min(ts), "ratio_to_5_point_path": min(ts) / step_s,
                                                        "steps_timed": 10, "plan": c9.describe()}
         c9.close()
+        # NEXT-3: damped Jacobi (beta 0.9) on the metric's config: one kernel per sweep over global memory inside a CUDA graph of the
+        # time step (every engine; the sweeps are not in the resident kernel), so that the line carries every sweep kind
+        cj = binding.Cavity(w4.N, w4.Re, w4.dt, 0.9, w4.sweeps_per_stage, engine=args.engine)
+        cj.set_sweep("jacobi")
+        cj.set_fields(*W.initial_fields(w4))
+        cj.step(2)
+        ts = []
+        for _ in range(3):
+            cj.step(5)
+            ts.append(cj.last_elapsed_ms() * 1e-3 / 5)
+        others["jacobi_" + "cfg%d" % args.config] = {"workload": w4.name + ", damped Jacobi sweeps (G21), beta 0.9", "ms_per_step": 1e3 * min(ts),
+                                                     "GPSU_per_s": 5.0 * (w4.N + 1) ** 2 / min(ts), "ratio_to_red_black_path": min(ts) / step_s,
+                                                     "steps_timed": 5, "plan": "one k_jacobi_sweep launch per sweep over global memory (ping-pong fields), CUDA graph of one time step"}
+        cj.close()
     else:
         cav.close()
 

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcavity.so")
 SOURCES = ["cavity_kernels.cu", "cavity_resident.cu", "cavity_noalloc.cu", "cavity_api.cu"]
-HEADERS = ["cavity_kernels.cuh", "cavity_resident.cuh", os.path.join("..", "..", "include", "cavity.h"),
+HEADERS = ["cavity_kernels.cuh", "cavity_resident.cuh", "cavity_scheme.cuh", os.path.join("..", "..", "include", "cavity.h"),
            os.path.join("..", "..", "include", "cavity_debug.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 

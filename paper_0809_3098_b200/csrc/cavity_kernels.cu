@@ -4,20 +4,13 @@
 // association is exactly the one DESIGN.md "Canonical arithmetic" states (and tests compare bit for bit).
 // P:n = /root/reference/PAPER.md line n.
 #include "cavity_kernels.cuh"
+#include "cavity_scheme.cuh"
 
 namespace cavk {
 
 namespace {
 
-// SSPRK(5,4) in Shu-Osher form, eq 9-13 P:85-108.  eq 9's constant is printed with 11 digits and eq 10's
-// second weight with a wrong digit (0.555626...); the values below are the 15-digit ones of the paper's
-// ref [23], which make every stage's weights sum to 1 (readings G1, G2).
-__device__ constexpr double RK1_C  = 0.391752226571890;
-__device__ constexpr double RK2_A0 = 0.444370493651235, RK2_A1 = 0.555629506348765, RK2_C = 0.368410593050371;
-__device__ constexpr double RK3_A0 = 0.620101851488403, RK3_A2 = 0.379898148511597, RK3_C = 0.251891774271694;
-__device__ constexpr double RK4_A0 = 0.178079954393132, RK4_A3 = 0.821920045606868, RK4_C = 0.544974750228521;
-__device__ constexpr double RK5_A2 = 0.517231671970585, RK5_A3 = 0.096059710526147, RK5_C3 = 0.063692468666290;
-__device__ constexpr double RK5_A4 = 0.386708617503269, RK5_C4 = 0.226007483236906;
+using namespace scheme;       // the SSPRK(5,4) table, Thom's formula, eq 8 / 22 and the stage combination: cavity_scheme.cuh
 
 inline int cdiv(int a, int b) { return (a + b - 1) / b; }
 
@@ -37,9 +30,6 @@ __global__ void k_scale_rhs(int N, int pitch, double cq, const double* __restric
 }
 
 // ---- a2: Thom ring, eq 25 P:161-169 ------------------------------------------------------------------
-__device__ __forceinline__ double thom_wall(double c2h2, double p_adj) { return -(c2h2 * p_adj); }
-__device__ __forceinline__ double thom_lid(double c2h2, double lid, double p_adj) { return -(c2h2 * p_adj) - lid; }
-
 __global__ void k_thom_ring(int N, int pitch, double c2h2, double lid, const double* __restrict__ psi,
                             double* __restrict__ w) {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -92,27 +82,10 @@ k_rk_stage(Params P, const double* __restrict__ psi, const double* __restrict__ 
     } else {
         wW = w_in[k - 1]; wE = w_in[k + 1]; wS = w_in[k - pitch]; wN = w_in[k + pitch];
     }
-    // eq 22: u = dpsi/dy, v = -dpsi/dx;  eq 8
-    const double u = (pN - pS) * P.i2h;
-    const double v = (pW - pE) * P.i2h;
-    const double wx = (wE - wW) * P.i2h;
-    const double wy = (wN - wS) * P.i2h;
-    const double lap = (((wW + wE) + (wS + wN)) - 4.0 * w0) * P.ih2;
-    const double L = fma(P.nu, lap, -fma(u, wx, v * wy));
-    const double dL = P.dt * L;
-
-    if (K == 1) {
-        w_out[k] = fma(RK1_C, dL, w0);                                              // eq 9
-    } else if (K == 2) {
-        w_out[k] = fma(RK2_C, dL, fma(RK2_A1, w0, RK2_A0 * a[k]));                  // eq 10 (w0 here is omega^(1))
-    } else if (K == 3) {
-        w_out[k] = fma(RK3_C, dL, fma(RK3_A2, w0, RK3_A0 * a[k]));                  // eq 11
-    } else if (K == 4) {
-        w_out[k] = fma(RK4_C, dL, fma(RK4_A3, w0, RK4_A0 * a[k]));                  // eq 12
-        t_out[k] = fma(RK5_C3, dL, fma(RK5_A3, w0, RK5_A2 * b[k]));                 // eq 13, first three terms
-    } else {
-        w_out[k] = fma(RK5_C4, dL, fma(RK5_A4, w0, a[k]));                          // eq 13, the rest (a = T)
-    }
+    const double dL = transport_dL(pW, pE, pS, pN, w0, wW, wE, wS, wN, P.i2h, P.ih2, P.nu, P.dt);   // eq 22, eq 8
+    // eq 9-13: w0 is the stage input; a = omega^n (stages 2-4) or T (stage 5); b = omega^(2) (stage 4)
+    w_out[k] = rk_stage_out(K, rk_c(K), rk_a1(K), rk_a0(K), dL, w0, K == 1 ? 0.0 : a[k]);
+    if (K == 4) t_out[k] = rk_T(dL, w0, b[k]);                                       // eq 13, first three terms
 }
 
 // ---- a4: diagnostics ----------------------------------------------------------------------------------

@@ -57,6 +57,7 @@
 // The kernel reads psi_in and writes psi_out (the API ping-pongs two fields), so no tile ever overwrites input a
 // neighbour has not loaded yet.
 #include "cavity_resident.cuh"
+#include "cavity_scheme.cuh"
 
 #include <algorithm>
 #include <cstdio>
@@ -80,14 +81,7 @@ constexpr long long SPIN_TIMEOUT_CYCLES = CAV_SPIN_TIMEOUT;
 #define CAV_QROWS 0             // rows of the micro-tile whose q lives in shared memory instead of registers (0: the register-to-register exchange left room for all of q)
 #endif
 
-// SSPRK(5,4) in Shu-Osher form, eq 9-13, readings G1 / G2 (the same table as cavity_kernels.cu, typed here again
-// because that one is file-local).
-__device__ constexpr double RK1_C  = 0.391752226571890;
-__device__ constexpr double RK2_A0 = 0.444370493651235, RK2_A1 = 0.555629506348765, RK2_C = 0.368410593050371;
-__device__ constexpr double RK3_A0 = 0.620101851488403, RK3_A2 = 0.379898148511597, RK3_C = 0.251891774271694;
-__device__ constexpr double RK4_A0 = 0.178079954393132, RK4_A3 = 0.821920045606868, RK4_C = 0.544974750228521;
-__device__ constexpr double RK5_A2 = 0.517231671970585, RK5_A3 = 0.096059710526147, RK5_C3 = 0.063692468666290;
-__device__ constexpr double RK5_A4 = 0.386708617503269, RK5_C4 = 0.226007483236906;
+using namespace scheme;       // the SSPRK(5,4) table, Thom's formula, eq 8 / 22 and the stage combination: cavity_scheme.cuh (shared with cavity_kernels.cu)
 
 struct ResArgs {
     int N, pitch;
@@ -725,8 +719,6 @@ __device__ __forceinline__ void qb_from_image(double (&q)[R][C], const double* _
     }
 }
 
-__device__ __forceinline__ double thom_wall(double c2h2, double p_adj) { return -(c2h2 * p_adj); }
-__device__ __forceinline__ double thom_lid(double c2h2, double lid, double p_adj) { return -(c2h2 * p_adj) - lid; }
 
 // a2 (eq 25) for the points of this thread's micro-tile that lie next to a wall and inside the tile's core
 // [X0, X1) x [Y0, Y1): the wall value goes into the image next to the point and, with TO_GLOBAL, into the ring of the stage
@@ -836,9 +828,7 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
     __syncthreads();
 
     // (2) eq 8 + eq 22 and the combination of eq 9-13 for the core points of this thread, row by row
-    const double rk_c = k == 1 ? RK1_C : (k == 2 ? RK2_C : (k == 3 ? RK3_C : (k == 4 ? RK4_C : RK5_C4)));
-    const double rk_a1 = k == 2 ? RK2_A1 : (k == 3 ? RK3_A2 : (k == 4 ? RK4_A3 : RK5_A4));
-    const double rk_a0 = k == 2 ? RK2_A0 : (k == 3 ? RK3_A0 : (k == 4 ? RK4_A0 : 1.0));
+    const double c_k = rk_c(k), a1_k = rk_a1(k), a0_k = rk_a0(k);
 #pragma unroll
     for (int rj = 0; rj < R; ++rj) {
         const int gy = gy0 + rj;
@@ -868,20 +858,11 @@ __device__ __forceinline__ void rhs_phase(const ResArgs& a, const double (&pp)[R
             const double pS = gy == 1 ? 0.0 : (rj > 0 ? pp[rj - 1][ci] : sB[TOPOFF + ci * 32]);      // psi = 0 on the wall y = 0; else the top row of the warp below
             const double pN = rj < R - 1 ? pp[rj + 1][ci] : sB[C * 32 + ci * 32];        // bottom row of the warp above
             const double w0 = wc[1 + ci], wW = wc[ci], wE = wc[2 + ci], wS = ws[ci], wN = wn[ci];
-            // eq 22: u = dpsi/dy, v = -dpsi/dx;  eq 8
-            const double u = (pN - pS) * a.i2h;
-            const double v = (pW - pE) * a.i2h;
-            const double wx = (wE - wW) * a.i2h;
-            const double wy = (wN - wS) * a.i2h;
-            const double lap = (((wW + wE) + (wS + wN)) - 4.0 * w0) * a.ih2;
-            const double L = fma(a.nu, lap, -fma(u, wx, v * wy));
-            const double dL = a.dt * L;
+            const double dL = transport_dL(pW, pE, pS, pN, w0, wW, wE, wS, wN, a.i2h, a.ih2, a.nu, a.dt);   // eq 22, eq 8
             const size_t gk = (size_t)gy * pitch + gx;
             const double av = ab[rj][ci];
-            // eq 9-13 in one form: out = fma(c, dL, fma(a1, w0, a0 av)) (eq 13: a0 = 1, av = T; eq 9: the inner term is w0 itself)
-            const double inner = k == 1 ? w0 : fma(rk_a1, w0, rk_a0 * av);
-            const double out = fma(rk_c, dL, inner);
-            if (k == 4) tbuf[gk] = fma(RK5_C3, dL, fma(RK5_A3, w0, RK5_A2 * w2b[gk]));      // eq 13, first three terms
+            const double out = rk_stage_out(k, c_k, a1_k, a0_k, dL, w0, av);                 // eq 9-13 (eq 13: a0 = 1, av = T)
+            if (k == 4) tbuf[gk] = rk_T(dL, w0, w2b[gk]);                                    // eq 13, first three terms
             wout[gk] = out;
             ab[rj][ci] = out;
         }
