@@ -47,9 +47,25 @@ SM_COUNT, FP64_LANES_PER_SM = 148, 64   # B200: 148 SMs x 64 fp64 lanes (DESIGN.
 FP64_INSTR_PER_POINT_SWEEP = 5     # 3 DADD + 2 DFMA
 FP64_INSTR_PER_POINT_STAGE = 30    # a2 + a3 ("5 S + 30 fp64 instructions per grid-point-stage")
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE k_resident launch (one time step of config 4) from the ncu --set full
-# capture summarised in profiles/ (cold L2 under ncu); None until that capture exists for the build
-NCU_DRAM_BYTES_PER_STEP_LAUNCH = 43.9e6
-NCU_DRAM_SOURCE = "profiles/r2c_final.md (ncu --set full, one launch = one time step of config 4)"
+# capture summarised in profiles/ (cold L2 under ncu).  The figure belongs to ONE build: it is reported only while the kernel's
+# sources still have the git blob ids the capture was taken on; after any change to them the line says traffic: null and why.
+NCU_DRAM_BYTES_PER_STEP_LAUNCH = 46.44e6
+NCU_DRAM_SOURCE = "profiles/r3_final.md (ncu --set full, one launch = one time step of config 4: 19.69 MB read + 26.75 MB written)"
+NCU_DRAM_BUILD = {"paper_0809_3098_b200/csrc/cavity_resident.cu": "483d2b762e5967d042d9e9bbe69bcaa3a9253215",
+                  "paper_0809_3098_b200/csrc/cavity_scheme.cuh": "2dc6c4f7694d00fc9620b710a2bde93d8820fc00"}
+
+
+def ncu_capture_is_current():
+    """True if the kernel sources are byte for byte those of the ncu capture (git blob id = sha1("blob <len>\\0" + content))."""
+    import hashlib
+    for rel, want in NCU_DRAM_BUILD.items():
+        try:
+            data = open(os.path.join(ROOT, rel), "rb").read()
+        except OSError:
+            return False
+        if hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest() != want:
+            return False
+    return True
 
 
 def parse():
@@ -306,9 +322,12 @@ def run_ours(args, wl, rank, world, local_rank):
         tsw += cav.last_elapsed_ms() * 1e-3
         lsw += cav.launch_count() - l1 - extra
     sweep_rate = ips * P * S * reps / tsw
-    traffic = NCU_DRAM_BYTES_PER_STEP_LAUNCH if (wl.N == 1024 and S == 200 and resident) else None
+    current = ncu_capture_is_current()
+    traffic = NCU_DRAM_BYTES_PER_STEP_LAUNCH if (wl.N == 1024 and S == 200 and resident and current) else None
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": dfma_peak / 1e12, "unit": "T fp64 instr/s",
-                "frac": achieved / dfma_peak, "traffic": traffic, "traffic_source": NCU_DRAM_SOURCE if traffic else None,
+                "frac": achieved / dfma_peak, "traffic": traffic,
+                "traffic_source": NCU_DRAM_SOURCE if traffic else (None if current else "null: the kernel sources changed since the ncu capture of "
+                                                                   + NCU_DRAM_SOURCE.split(" ")[0] + "; re-capture and update NCU_DRAM_* in bench.py"),
                 "dram_GBps": (traffic / step_s / 1e9) if traffic else None,
                 "peak_source": "measured in this run: DFMA-chain kernel, 16 warps per SM, 8 chains per thread (cav_measure_fp64_peak)",
                 "peak_nominal": fp64_nominal / 1e12, "peak_nominal_model": "148 SMs x 64 fp64 lanes x sm_max_mhz",

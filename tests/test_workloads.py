@@ -1,4 +1,6 @@
 """The seeded input generator (paper_0809_3098_b200/workloads.py): holds no arithmetic of the method."""
+import os
+
 import numpy as np
 
 from paper_0809_3098_b200 import workloads as W
@@ -45,3 +47,16 @@ def test_config5_smooth_part():
     w = W.initial_omega(64, 0.0, 1, smooth_amp=5.0)
     assert abs(w[16, 16] - 5.0) < 1e-12 and abs(w[48, 16] + 5.0) < 1e-12
     assert wl.smooth_amp == 5.0
+
+
+def test_bench_ncu_traffic_constant_is_tied_to_the_kernel_sources(tmp_path, monkeypatch):
+    # roofline.traffic is an ncu figure of ONE build: bench.py may report it only while the kernel sources are unchanged
+    import bench
+    assert set(bench.NCU_DRAM_BUILD) >= {"paper_0809_3098_b200/csrc/cavity_resident.cu"}
+    assert bench.ncu_capture_is_current() in (True, False)      # a changed kernel is not an error: bench.py then prints traffic: null
+    import hashlib
+    data = open(os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "README.md"), "rb").read()
+    monkeypatch.setattr(bench, "NCU_DRAM_BUILD", {"README.md": hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()})
+    assert bench.ncu_capture_is_current()                        # the id is git's blob id of the file's bytes
+    monkeypatch.setattr(bench, "NCU_DRAM_BUILD", {"paper_0809_3098_b200/csrc/cavity_resident.cu": "0" * 40})
+    assert not bench.ncu_capture_is_current()
