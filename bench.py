@@ -51,7 +51,9 @@ FP64_INSTR_PER_POINT_STAGE = 30    # a2 + a3 ("5 S + 30 fp6
 # sources still have the git blob ids the capture was taken on; after any change to them the line says traffic: null and why.
 NCU_DRAM_BYTES_PER_STEP_LAUNCH = 46.44e6
 NCU_DRAM_SOURCE = "profiles/r3_final.md (ncu --set full, one launch = one time step of config 4: 19.69 MB read + 26.75 MB written)"
-NCU_DRAM_BUILD = {"paper_0809_3098_b200/csrc/cavity_resident.cu": "483d2b762e5967d042d9e9bbe69bcaa3a9253215",
+# (cavity_resident.cu was captured as blob 483d2b76; the later blob 11118681 differs only in the compact-operator instances, KIND == 1:
+#  the SASS of the timed instance k_resident<4,6,16,false,0> is instruction for instruction the same, profiles/r3_sass.md)
+NCU_DRAM_BUILD = {"paper_0809_3098_b200/csrc/cavity_resident.cu": "11118681061ee6e44afb35f324e9f81df19fc72e",
                   "paper_0809_3098_b200/csrc/cavity_scheme.cuh": "2dc6c4f7694d00fc9620b710a2bde93d8820fc00"}
 
 
@@ -405,6 +407,30 @@ def run_ours(args, wl, rank, world, local_rank):
                                                      "GPSU_per_s": 5.0 * (w4.N + 1) ** 2 / min(ts), "ratio_to_red_black_path": min(ts) / step_s,
                                                      "steps_timed": 5, "plan": "one k_jacobi_sweep launch per sweep over global memory (ping-pong fields), CUDA graph of one time step"}
         cj.close()
+        # cav_diag_noalloc (the a4 reductions on caller-owned device buffers, no allocation): an HBM-bound kernel, timed alone on the
+        # largest grid it takes (N = 8192: 2 fields x 537 MB, larger than L2), CUDA events on the launching stream
+        nmax = binding.noalloc_max_n()
+        gen = torch.Generator(device=dev).manual_seed(8192)
+        pd = torch.randn((nmax + 1, nmax + 1), dtype=torch.float64, device=dev, generator=gen) * 0.05
+        wd = torch.randn((nmax + 1, nmax + 1), dtype=torch.float64, device=dev, generator=gen) * 3.0
+        o4 = torch.zeros(4, dtype=torch.float64, device=dev)
+        st_ = torch.cuda.current_stream(dev)
+        for _ in range(3):
+            binding.diag_noalloc(nmax, pd, wd, o4, stream=st_.cuda_stream)
+        ts = []
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st_)
+            binding.diag_noalloc(nmax, pd, wd, o4, stream=st_.cuda_stream)
+            e1.record(st_)
+            e1.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e-3)
+        nbytes = 2.0 * 8.0 * (nmax + 1) ** 2           # algorithmic bytes: psi and omega read once (16 B per grid point), 32 B written
+        others["diag_noalloc_%d" % (nmax + 1)] = {"workload": "a4 diagnostics of a %d x %d state in caller-owned device buffers (cav_diag_noalloc)" % (nmax + 1, nmax + 1),
+                                                  "ms_per_call": 1e3 * min(ts), "launches_per_call": 1, "bound": "hbm", "algorithmic_bytes": nbytes,
+                                                  "achieved_GBps": nbytes / min(ts) / 1e9, "peak_GBps": hbm_gbs, "frac": nbytes / min(ts) / 1e9 / hbm_gbs,
+                                                  "timing": "best of 5 calls, inputs larger than L2, includes the 256-byte counter clear"}
+        del pd, wd, o4
     else:
         cav.close()
 

@@ -1044,9 +1044,11 @@ __global__ void __launch_bounds__(32 * MAXW, 16 / MAXW) k_resident(const __grid_
             }
             ++round;
             mark(a, tslot + 2);
-            if (a.nsteps == 0) {
+            if (a.nsteps == 0 || KIND == 1) {
                 // sweeps-only launches (cav_poisson, cav_trace_sweeps) never reach the once-per-stage reset below: put the
-                // registers of non-interior points back to +0.0 after every exchange round instead (outside the sweep loops)
+                // registers of non-interior points back to +0.0 after every exchange round instead (outside the sweep loops).
+                // The compact operator does so in time-step launches too: its four colour passes per sweep let a dead register
+                // grow by up to 2.94^4 per sweep at beta -> 2, which over the sweeps of one stage reaches Inf (and 0 x Inf = NaN)
                 const int z = opaque_zero();
                 const unsigned int dead = reinterpret_cast<const unsigned int*>(sm + edge_doubles + (((int)blockDim.y + z) * R + 1) * SW)
                                               [2 * ((int)blockDim.y + z) * 32 + ((int)threadIdx.y + z) * 32 + (int)threadIdx.x];

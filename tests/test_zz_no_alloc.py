@@ -88,6 +88,15 @@ def test_noalloc_matches_get_diag_on_calls_in_a_row(cav):
         assert close(g, want[N]), (N, p, g, want[N])
         assert g[0] == want[N][0], "res_inf is a maximum: no rounding to differ by"
     assert np.array_equal(got[0], got[2]), "same input, same answer bit for bit, whatever ran in between"
+    # and against the CPU oracle's a4 (the definitions of struct cav_diag written out in plain loops), same tolerance
+    import oracle
+    for N in (64, 257):
+        o = oracle.OracleCavity(N, 100.0, 1e-3, 1.5, 1)
+        o.set_fields(*states[N])
+        od = o.diag()
+        o.close()
+        g = got[[c[0] for c in cases].index(N)]
+        assert close(g, np.array([od[k] for k in KEYS])), (N, g, od)
 
 
 @pytest.mark.gpu
